@@ -1,0 +1,144 @@
+/*
+ * cg.h — C ABI of libcg.so: the B200-native (sm_100a) hot path of the parallel
+ * kinetic Monte Carlo for Coulomb glasses of Ferrero, Kolton and Palassini
+ * (arXiv 1407.5026; citations are lines of /root/reference/PAPER.md).
+ *
+ * What the library computes: the "mixed PR algorithm" of PAPER.md:71-78 on an
+ * L x L periodic lattice at half filling —
+ *   1. M labelled proposals per iteration, each (i, j) drawn with probability
+ *      Gamma^T_ij / Gamma, Gamma^T_ij = exp(-2 r_ij / xi)
+ *   2. each accepted with probability theta_ij min[1, exp(-dH_ij/T)],
+ *      dH_ij = eps_j - eps_i - 1/r_ij - E dx_ij
+ *   3. the lowest accepting label q is executed, dP += dx_ij, every local
+ *      energy gets eps_l += 1/r_lj - 1/r_li, time advances by m/Gamma
+ *
+ * looped on the device without a host round trip per hop.  The random stream is
+ * Philox4x32-10 keyed by (seed, global attempt index), so the
+ * sequence of executed hops is identical to that of the serial mixed algorithm
+ * ("mathematically equivalent") and does not depend on M or on the
+ * launch shape.  DESIGN.md lists every reading of the paper this relies on.
+ *
+ * Conventions: site s = y*L + x (row-major, x = field direction), sites, labels
+ * and attempt indices 0-based.  All pointers are HOST pointers unless the name
+ * starts with dev_.  All functions return CG_OK (0) or a negative CG_E* code;
+ * none throws, aborts or prints.  A sim is not thread-safe; distinct sims are
+ * independent.  There is no CPU fallback: without a CUDA device every compute
+ * entry point fails with CG_ECUDA.
+ */
+#ifndef CG_H_
+#define CG_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct cg_sim cg_sim; /* opaque; owned by the library, released by cg_free */
+
+#define CG_OK            0
+#define CG_EINVAL       (-1)  /* bad argument (NULL, odd L, T<=0, xi<=0, M==0, range) */
+#define CG_ENOMEM       (-2)  /* host or device allocation failed / workspace too small */
+#define CG_ECUDA        (-3)  /* a CUDA call failed; text kept for cg_last_error       */
+#define CG_EUNSUPPORTED (-4)  /* valid problem the sm_100a path does not cover:
+                                 L not a power of two, L > 1024, or a tower too
+                                 long for shared memory (very large xi)            */
+
+/* Problem statement.  L: lattice side, N = L*L sites, a power
+ * of two in [4, 1024]; W: full width of the uniform disorder, phi_i in [-W/2, W/2);
+ * xi: localisation length; T: temperature (k_B = 1); E: field along +x in the
+ * sense of dH = ... - E dx; seed: Philox key; M >= 1: logical PR width (labels per
+ * iteration; may exceed the number of resident threads).
+ * Filling nu = 1/2 and the hop cut-off r <= L/2 are fixed.
+ * cg_init allocates its own device memory on the current device and uses the
+ * legacy default stream.  On failure *out is NULL. */
+int cg_init(cg_sim** out, int L, double W, double xi, double T, double E,
+            uint64_t seed, uint32_t M);
+
+/* Same, for callers that own device memory (e.g. a torch uint8 tensor) and a
+ * stream: dev_workspace must hold cg_workspace_bytes(L, M) bytes, be 256-byte
+ * aligned and outlive the sim; cuda_stream is a cudaStream_t (NULL = default). */
+size_t cg_workspace_bytes(int L, uint32_t M);
+int cg_init_ws(cg_sim** out, int L, double W, double xi, double T, double E,
+               uint64_t seed, uint32_t M,
+               void* dev_workspace, size_t bytes, void* cuda_stream);
+
+/* Advance exactly n_accepted_hops executed hops (not iterations) of the chain.
+ * One persistent cooperative kernel; asynchronous on the sim's stream.
+ * cg_run(a); cg_run(b) is the same chain as cg_run(a+b). */
+int cg_run(cg_sim* s, uint64_t n_accepted_hops);
+
+/* Synchronises the stream and copies out: occupations n[N] in {0,1}
+ * (PAPER.md:52), local energies eps[N], elapsed time
+ * t = attempts_consumed / Gamma in units of tau0 (deterministic increment
+ * m/Gamma, with m = (p-1)M + q), and the net
+ * charge displacement dP = sum of dx over executed hops.
+ * Any pointer may be NULL. */
+int cg_get_state(cg_sim* s, int8_t* n, double* eps, double* t_tau0, int64_t* dP);
+
+/* Restore a state previously read with cg_get_state / cg_get_counters
+ * (checkpoint): n[N] with sum N/2, eps[N], attempts consumed, hops, dP.
+ * iterations / proposals counters restart from zero. */
+int cg_set_state(cg_sim* s, const int8_t* n, const double* eps,
+                 uint64_t attempts, uint64_t hops, int64_t dP);
+
+/* Counters: attempts consumed (sum of m), proposals evaluated (M per
+ * iteration), PR iterations, executed hops.  Synchronises the stream. */
+int cg_get_counters(cg_sim* s, uint64_t* attempts, uint64_t* proposals_evaluated,
+                    uint64_t* iterations, uint64_t* hops);
+
+/* Hop log: (attempt index, i, j) of executed hops.  cg_enable_hop_log reserves
+ * room for `capacity` hops counted from the current hop; dev_buf (may be NULL:
+ * the library allocates) must hold 16*capacity bytes.  cg_get_hops copies hops
+ * [first, first+count) of the log (indices relative to the enabling point). */
+int cg_enable_hop_log(cg_sim* s, uint64_t capacity, void* dev_buf, size_t bytes);
+int cg_get_hops(cg_sim* s, uint64_t first, uint64_t count,
+                uint64_t* attempt, uint32_t* i, uint32_t* j);
+
+/* Recompute eps from its definition eps_i = phi_i + sum_{j!=i}(n_j - 1/2)/r_ij
+ * on the device and return max_i |eps_i - eps_i^incremental|. */
+int cg_recompute_eps(cg_sim* s, double* max_abs_dev);
+
+/* Step a6 alone: execute `count` scripted hops i[h] -> j[h] (occupations,
+ * dP and the O(N) update of PAPER.md:77; no acceptance test, no time) in one
+ * launch of the update kernel.  Used for parity of the update against the
+ * oracle and for its bandwidth measurement.  ms (may be NULL) receives the
+ * device time of the launch measured with CUDA events on the sim's stream. */
+int cg_apply_hops(cg_sim* s, uint64_t count, const uint32_t* i, const uint32_t* j, float* ms);
+
+/* Diagnostics of the one-time set-up (step a0): translation-invariant tables
+ * (PAPER.md:80).  K = number of displacements with 0 < r <= L/2 in the order
+ * (r^2, dy, dx); K_live = length of the prefix whose tower value is < 1 plus
+ * one (later entries can never be drawn by a uniform u < 1). */
+int cg_get_table_sizes(cg_sim* s, int64_t* K, int64_t* K_live);
+int cg_get_tables(cg_sim* s, int32_t* dy, int32_t* dx, double* cdf, double* invr_k, /* K_live each */
+                  double* S, double* Gamma);
+int cg_get_phi(cg_sim* s, double* phi /* N */);
+
+/* Launch shape of the persistent kernel: n_ctas in [1, co-resident maximum],
+ * threads in {256, 512, 1024}; 0 keeps the heuristic.  Results never depend on
+ * it.  cg_get_launch reports the shape in use. */
+int cg_set_launch(cg_sim* s, int n_ctas, int threads);
+int cg_get_launch(cg_sim* s, int* n_ctas, int* threads, int* smem_bytes);
+
+/* Device-side phase timers of CTA 0 accumulated over cg_run calls, in SM clock
+ * cycles: total, waiting at the grid exchange, update (W_U), propose+select
+ * (W_R) — the paper's split.  reset != 0 zeroes them. */
+int cg_get_phase_cycles(cg_sim* s, uint64_t* total, uint64_t* wait, uint64_t* update,
+                        uint64_t* propose, int reset);
+
+/* L2 roofline denominator: one kernel, all SMs,
+ * 16-byte L1-bypassing read-modify-write over a resident buffer of `bytes`
+ * repeated `reps` times inside the launch.  Returns GB/s counting
+ * 2*bytes*reps (read + write) over the best of `trials` launches. */
+int cg_bench_l2_rmw(size_t bytes, int reps, int trials, double* gbps);
+
+void cg_free(cg_sim* s);
+const char* cg_strerror(int code);
+const char* cg_last_error(cg_sim* s); /* text of the last CUDA failure, "" if none */
+
+#ifdef __cplusplus
+}
+#endif
+#endif

@@ -1,0 +1,44 @@
+"""Builds libcg.so (the C-ABI CUDA library, include/cg.h) in-tree with nvcc for sm_100a."""
+import os
+import shutil
+import subprocess
+import sys
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+ROOT = os.path.dirname(HERE)
+SRC = os.path.join(HERE, "csrc", "cg.cu")
+HDR = os.path.join(ROOT, "include", "cg.h")
+LIB = os.path.join(HERE, "libcg.so")
+
+NVCC_FLAGS = [
+    "-O3", "-std=c++17",
+    "-gencode", "arch=compute_100a,code=sm_100a",
+    "-lineinfo",
+    "-fmad=false",                      # no FMA contraction anywhere: decisions must match the serial chain
+    "-Xcompiler", "-fPIC,-ffp-contract=off,-O2",
+    "-shared", "-cudart", "static",
+]
+
+
+def nvcc():
+    return shutil.which("nvcc") or "/usr/local/cuda/bin/nvcc"
+
+
+def build(force=False, verbose=False):
+    stale = (not os.path.exists(LIB)
+             or os.path.getmtime(LIB) < max(os.path.getmtime(SRC), os.path.getmtime(HDR),
+                                            os.path.getmtime(__file__)))
+    if force or stale:
+        tmp = LIB + ".tmp.%d" % os.getpid()
+        cmd = [nvcc(), *NVCC_FLAGS, "-I", os.path.join(ROOT, "include"), "-o", tmp, SRC]
+        if verbose:
+            cmd.insert(1, "-Xptxas=-v")
+            print(" ".join(cmd))
+        subprocess.check_call(cmd)
+        os.replace(tmp, LIB)
+    return LIB
+
+
+if __name__ == "__main__":
+    build(force="--force" in sys.argv, verbose="-v" in sys.argv)
+    print(LIB)

@@ -1,0 +1,187 @@
+"""GPU parity: libcg.so (through its C ABI) against the CPU oracle, element by element.
+
+Bar (BASELINE.json north_star): hop log (attempt, i, j) and occupations bit-identical;
+eps within 1e-12 relative (expected bit-identical); incremental eps within 1e-9 of the
+from-scratch recomputation; counters (attempts, iterations, proposals) identical.
+"""
+import numpy as np
+import pytest
+
+import workloads
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def cg():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from paper_1407_5026_b200 import build
+    build.build()
+    import paper_1407_5026_b200 as pkg
+    return pkg
+
+
+def _compare(g, o, hops, check_eps_bits=True):
+    ga, gi, gj = g.hops(0, hops)
+    oa, oi, oj = o.hops(0, hops)
+    bad = np.flatnonzero((ga != oa) | (gi != oi) | (gj != oj))
+    assert bad.size == 0, "first divergence at hop %d: gpu %s oracle %s" % (
+        bad[0], (ga[bad[0]], gi[bad[0]], gj[bad[0]]), (oa[bad[0]], oi[bad[0]], oj[bad[0]]))
+    gn, ge, gt, gp = g.state()
+    on, oe, ot, op = o.state()
+    assert np.array_equal(gn, on) and gn.sum() == g.N // 2
+    assert gt == ot and gp == op
+    assert np.allclose(ge, oe, rtol=1e-12, atol=0)
+    if check_eps_bits:
+        assert np.array_equal(ge, oe)
+    assert g.counters() == o.counters()
+    assert o.near_ties() == 0          # O10 certificate: decisions did not depend on the libm
+
+
+@pytest.mark.parametrize("L", [4, 8, 16, 64, 256])
+def test_init_is_bit_identical(cg, oracle_lib, L):
+    """Step a0: tables, disorder, occupations and the full-sum eps."""
+    g = cg.CoulombGlass(L, W=1.0, xi=1.0, T=0.1, E=0.01, seed=40 + L, M=64)
+    o = oracle_lib.Oracle(L, W=1.0, xi=1.0, T=0.1, E=0.01, seed=40 + L, M=64)
+    tg, to = g.tables(), o.tables()
+    kl = tg["K_live"]
+    assert tg["K"] == to["K"] and tg["S"] == to["S"] and tg["Gamma"] == to["Gamma"]
+    for key in ("dy", "dx", "cdf", "invr_k"):
+        assert np.array_equal(tg[key], to[key][:kl]), key
+    assert np.all(to["cdf"][kl - 1:] == 1.0)           # entries past the live prefix can never be drawn
+    assert np.array_equal(g.phi(), o.phi())
+    gn, ge, gt, gp = g.state()
+    on, oe, _, _ = o.state()
+    assert np.array_equal(gn, on) and np.array_equal(ge, oe) and gt == 0.0 and gp == 0
+    assert g.recompute_eps() == 0.0
+
+
+CASES = [  # (name, index, hops compared) — prefixes the oracle finishes in seconds
+    ("cfg1_L16", 0, 100_000),
+    ("cfg2_L64", 0, 60_000),
+    ("cfg3_L128", 0, 20_000), ("cfg3_L128", 3, 20_000),
+    ("cfg4_L256", 1, 6_000),
+    ("cfg5_L512", 0, 3_000),
+]
+
+
+@pytest.mark.parametrize("name,idx,hops", CASES)
+def test_hop_log_matches_oracle(cg, oracle_lib, name, idx, hops):
+    kw = workloads.init_args(workloads.CONFIGS[name][idx])
+    g = cg.CoulombGlass(hop_log=hops, **kw)
+    o = oracle_lib.Oracle(**kw)
+    g.run(hops)
+    o.run(hops)
+    _compare(g, o, hops)
+    assert g.recompute_eps() < 1e-9
+
+
+def test_split_runs_continue_the_same_chain(cg, oracle_lib):
+    kw = workloads.init_args(workloads.CONFIGS["cfg2_L64"][0])
+    g = cg.CoulombGlass(hop_log=5000, **kw)
+    for part in (1, 7, 992, 4000):        # cg_run(a); cg_run(b) == cg_run(a+b)
+        g.run(part)
+    o = oracle_lib.Oracle(**kw)
+    o.run(5000)
+    _compare(g, o, 5000)
+
+
+@pytest.mark.parametrize("n_ctas,threads", [(1, 256), (3, 256), (8, 512), (37, 1024), (148, 512), (131, 1024)])
+def test_result_is_independent_of_launch_shape(cg, oracle_lib, n_ctas, threads):
+    kw = dict(L=64, T=0.05, E=0.02, seed=77, M=1000)     # M not a multiple of anything: ragged label tail
+    g = cg.CoulombGlass(hop_log=4000, **kw)
+    g.set_launch(n_ctas, threads)
+    assert g.launch()["n_ctas"] == n_ctas and g.launch()["threads"] == threads
+    g.run(4000)
+    o = oracle_lib.Oracle(**kw)
+    o.run(4000)
+    _compare(g, o, 4000)
+
+
+@pytest.mark.parametrize("M", [1, 2, 31, 33, 4096, 303104])
+def test_trajectory_is_independent_of_M(cg, oracle_lib, M):
+    """Reading G8: only the iteration bookkeeping depends on M; M=1 is the serial algorithm,
+    M = 148*2048 exceeds the resident threads."""
+    hops = 300 if M == 1 else 3000
+    kw = dict(L=32, T=0.08, E=0.01, seed=5, M=M)
+    g = cg.CoulombGlass(hop_log=hops, **kw)
+    g.run(hops)
+    o = oracle_lib.Oracle(**kw)
+    o.run(hops)
+    _compare(g, o, hops)
+    c = g.counters()
+    assert c["proposals_evaluated"] == M * c["iterations"]
+
+
+def test_smallest_lattice_and_hot_cold_limits(cg, oracle_lib):
+    for kw, hops in ((dict(L=4, T=0.5, E=0.0, seed=3, M=12), 20000),
+                     (dict(L=4, T=5.0, E=0.3, seed=4, M=5), 20000),      # hot: A ~ 1, q = 0 mostly
+                     (dict(L=16, T=0.01, E=0.0, seed=6, M=4096), 300),   # cold: many empty windows
+                     (dict(L=8, W=0.0, T=0.1, E=0.0, seed=9, M=64), 5000),   # no disorder
+                     (dict(L=32, W=2.0, xi=2.0, T=0.2, E=-0.05, seed=10, M=256), 5000)):  # paper's width, xi=2
+        g = cg.CoulombGlass(hop_log=hops, **kw)
+        g.run(hops)
+        o = oracle_lib.Oracle(**kw)
+        o.run(hops)
+        _compare(g, o, hops)
+
+
+def test_update_kernel_alone_on_scripted_hops(cg, oracle_lib):
+    """Step a6 by itself: eps bit-identical after scripted hops from an oracle log."""
+    for L, hops in ((16, 2000), (128, 1500), (512, 300)):
+        kw = dict(L=L, T=0.1, E=0.01, seed=90 + L, M=256)
+        o = oracle_lib.Oracle(**kw)
+        o.run(hops)
+        _, i, j = o.hops()
+        g = cg.CoulombGlass(**kw)
+        ms = g.apply_hops(i, j)
+        assert ms > 0
+        gn, ge, _, gp = g.state()
+        on, oe, _, op = o.state()
+        assert np.array_equal(gn, on) and np.array_equal(ge, oe) and gp == op
+        assert g.counters()["hops"] == hops
+        with pytest.raises(cg.CgError):           # a hop from an empty site violates theta_ij
+            empty = int(np.flatnonzero(gn == 0)[0]); occ = int(np.flatnonzero(gn == 1)[0])
+            g.apply_hops([empty], [occ])
+
+
+def test_checkpoint_restore(cg, oracle_lib):
+    kw = workloads.init_args(workloads.CONFIGS["cfg2_L64"][0])
+    g = cg.CoulombGlass(**kw)
+    g.run(3000)
+    n, eps, t, dP = g.state()
+    c = g.counters()
+    g2 = cg.CoulombGlass(hop_log=2000, **kw)
+    g2.set_state(n, eps, c["attempts"], c["hops"], dP)
+    g2.run(2000)
+    o = oracle_lib.Oracle(**kw)
+    o.run(5000)
+    oa, oi, oj = o.hops(3000, 2000)
+    ga, gi, gj = g2.hops(0, 2000)
+    assert np.array_equal(ga, oa) and np.array_equal(gi, oi) and np.array_equal(gj, oj)
+    assert np.array_equal(g2.state()[1], o.state()[1]) and g2.state()[3] == o.state()[3]
+
+
+def test_long_run_properties_at_headline_size(cg):
+    """Full-size config 5 in the launch shape bench.py times: properties that hold at any length."""
+    kw = workloads.init_args(workloads.CONFIGS["cfg5_L512"][0])
+    g = cg.CoulombGlass(hop_log=200_000, **kw)
+    g.run(200_000)
+    n, eps, t, dP = g.state()
+    c = g.counters()
+    assert n.sum() == g.N // 2 and c["hops"] == 200_000
+    assert g.recompute_eps() < 1e-9
+    assert abs(eps.sum() - g.phi().sum()) < 1e-6          # sum eps = sum phi at half filling
+    a, i, j = g.hops()
+    assert np.all(np.diff(a.astype(np.int64)) > 0) and a[-1] + 1 == c["attempts"]
+    assert t == c["attempts"] / g.tables()["Gamma"]
+    dx = (j.astype(np.int64) % 512 - i.astype(np.int64) % 512) % 512
+    dx = np.where(dx > 256, dx - 512, dx)
+    assert dP == dx.sum()
+    assert c["proposals_evaluated"] == kw["M"] * c["iterations"] and c["iterations"] >= c["hops"]
+    # replaying the log on the initial occupations gives the final occupations
+    g0 = cg.CoulombGlass(**kw)
+    n0 = g0.state()[0].astype(np.int64)
+    np.subtract.at(n0, i, 1); np.add.at(n0, j, 1)
+    assert np.array_equal(n0, n)

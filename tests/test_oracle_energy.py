@@ -138,3 +138,15 @@ def test_field_term_sign_and_size(oracle_lib):
     o2 = oracle_lib.Oracle(L, T=0.2, E=0.5, seed=3, M=8)
     o2.run(5000)
     assert o2.state()[3] > 500          # strong field: clear positive drift
+
+
+def test_half_lattice_hops_count_as_plus_half_L(oracle_lib):
+    """Reading G3: a hop of exactly L/2 along x has dx = +L/2 (components in (-L/2, L/2]);
+    on the 4x4 lattice such hops are frequent enough to pin the dP bookkeeping."""
+    L = 4
+    o = oracle_lib.Oracle(L, T=5.0, E=0.0, seed=12, M=2)
+    o.run(3000)
+    _, i, j = o.hops()
+    dx = np.array([min_image(int(b) % L - int(a) % L, L) for a, b in zip(i, j)])
+    assert (dx == 2).sum() > 10 and (dx == -2).sum() == 0
+    assert o.state()[3] == dx.sum()
