@@ -104,7 +104,13 @@ static int min_image(int d, int L)
     return d;
 }
 
-static int wrap(int v, int L) { return ((v % L) + L) % L; }
+/* Periodic wrap of a coordinate difference or sum, valid for -L <= v < 2L. */
+static int wrap(int v, int L)
+{
+    if (v < 0) v += L;
+    else if (v >= L) v -= L;
+    return v;
+}
 
 /* 1/r_ab under minimum image for sites a, b; 0 on the diagonal (O4). */
 static inline double invr_sites(const cgo_sim* s, uint32_t a, uint32_t b)
@@ -190,13 +196,19 @@ static int build_tables(cgo_sim* s)
  * summed in index order j = 0..N-1. */
 static void full_sum_eps(const cgo_sim* s, double* out)
 {
+    int L = s->L;
     int64_t N = (int64_t)s->N;
 #pragma omp parallel for schedule(static)
     for (int64_t a = 0; a < N; ++a) {
+        int ya = (int)(a / L), xa = (int)(a % L);
         double e = s->phi[a];
-        for (int64_t b = 0; b < N; ++b) {
-            if (b == a) continue;
-            e += ((double)s->n[b] - 0.5) * invr_sites(s, (uint32_t)a, (uint32_t)b);
+        for (int yb = 0; yb < L; ++yb) {                 /* b = yb*L + xb ascending */
+            const double* row = s->invr + (size_t)wrap(ya - yb, L) * (size_t)L;
+            const int8_t* nb = s->n + (size_t)yb * (size_t)L;
+            for (int xb = 0; xb < L; ++xb) {
+                if (yb == ya && xb == xa) continue;
+                e += ((double)nb[xb] - 0.5) * row[wrap(xa - xb, L)];
+            }
         }
         out[a] = e;
     }
