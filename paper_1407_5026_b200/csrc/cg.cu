@@ -35,6 +35,9 @@ typedef unsigned int u32;
 
 // ------------------------------------------------------------------ device --
 
+#define CG_SLOT_U64 32      // one exchange slot per CTA, 256-byte stride (own L2 slice), in u64 units
+#define CG_GUIDE 352        // tower guide: (43 + 1) binades x 8 sub-buckets of t = 2^43 - m
+
 struct CgCtl {              // device-resident control block (one per sim)
     u64 attempts;           // attempts consumed = next unused attempt index
     u64 hops;               // executed hops
@@ -42,27 +45,29 @@ struct CgCtl {              // device-resident control block (one per sim)
     u64 proposals;          // proposals evaluated (M per iteration)
     long long dP;           // sum of dx over executed hops
     u32 cur;                // eps buffer that holds the complete current state
-    u32 epoch;              // exchange epoch (one per PR iteration)
+    u32 bad_hops;           // scripted hops that violated theta_ij
+    u64 epoch;              // next exchange epoch; never reset, so stale slots can never match
     u64 log_base;           // hop count at which the hop log was enabled
     u64 cyc_total, cyc_wait, cyc_update, cyc_propose;
-    u32 bad_hops;           // scripted hops that violated theta_ij
-    u32 pad;
 };
 
 struct CgParams {           // kernel parameter block
     double* eps[2];         // double-buffered local energies, N each
     const double* tq;       // quarter table 1/r, (L/2+1) x (L/2+1)
     u32* nbits;             // occupations, bit s of word s/32
-    const double* cdf;      // live tower
+    const u64* cdfi;        // live tower as integer thresholds: u_d < cdf_k  <=>  m < cdfi_k
     const double* invr_k;   // 1/r of displacement k (live part)
+    const double* fld_k;    // E * dx of displacement k
     const int* disp;        // (dy << 16) | (dx & 0xffff)
-    ulonglong2* slots;      // one exchange slot per CTA
+    const u32* guide;       // tower guide: klo | khi << 16 per bucket
+    u64* slots;             // exchange slots, CG_SLOT_U64 per CTA
     CgCtl* ctl;
     u64* log_a; u32* log_i; u32* log_j; u64 log_cap;
     int L, lgL, pitch, Klive;
     u32 N, M;
     u32 seed_lo, seed_hi;
     double T, E;
+    float inv_T;            // (float)(1/T), pre-test of the Metropolis factor only
     u64 n_hops;
 };
 
@@ -83,14 +88,28 @@ __device__ __forceinline__ void philox4x32_10(u32 c0, u32 c1, u32 c2, u32 c3, u3
 
 __device__ __forceinline__ double ld_cg(const double* p) { return __ldcg(p); }
 
-__device__ __forceinline__ void slot_store(ulonglong2* p, u64 a, u64 b)
+__device__ __forceinline__ void slot_store(u64* p, u64 a, u64 b)
 {
     asm volatile("st.relaxed.gpu.global.v2.u64 [%0], {%1, %2};" ::"l"(p), "l"(a), "l"(b) : "memory");
 }
-__device__ __forceinline__ void slot_load(const ulonglong2* p, u64& a, u64& b)
+__device__ __forceinline__ void slot_load(const u64* p, u64& a, u64& b)
 {
     asm volatile("ld.relaxed.gpu.global.v2.u64 {%0, %1}, [%2];" : "=l"(a), "=l"(b) : "l"(p) : "memory");
 }
+__device__ __forceinline__ u64 ld_relaxed_u64(const u64* p)
+{
+    u64 v;
+    asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ void st_release_u64(u64* p, u64 v)
+{
+    asm volatile("st.release.gpu.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
+}
+__device__ __forceinline__ void fence_acquire_gpu() { asm volatile("fence.acquire.gpu;" ::: "memory"); }
+// named barrier 1: the warps that wrote eps arrive, the publishing warp waits for them
+__device__ __forceinline__ void bar1_arrive(int n) { asm volatile("bar.arrive 1, %0;" ::"r"(n) : "memory"); }
+__device__ __forceinline__ void bar1_sync(int n) { asm volatile("bar.sync 1, %0;" ::"r"(n) : "memory"); }
 
 // 1/r between site (y,x) and site (yb,xb) under minimum image, from
 // the quarter table; 0 on the diagonal.
@@ -110,66 +129,129 @@ __device__ __forceinline__ double hop_term(const double* __restrict__ tq, int pi
     return __dsub_rn(invr_at(tq, pitch, L, y, x, yj, xj), invr_at(tq, pitch, L, y, x, yi, xi));
 }
 
-// Update of a pair slab [pr0, pr1) (pairs of adjacent sites): dst = src + term.
-template <int THREADS>
-__device__ __forceinline__ void update_slab(const CgParams& p, const double* src,
-                                            double* dst, u32 pr0, u32 pr1,
-                                            u32 hi, u32 hj)
+// The two terms of a pair of adjacent sites (y, x), (y, x+1), x even: both rows once.
+__device__ __forceinline__ void hop_term2(const double* __restrict__ tq, int pitch, int L,
+                                          int y, int x, int yi, int xi, int yj, int xj,
+                                          double& c0, double& c1)
 {
-    const int L = p.L, lg = p.lgL, pitch = p.pitch;
-    const int yi = hi >> lg, xi = hi & (L - 1), yj = hj >> lg, xj = hj & (L - 1);
-    for (u32 pr = pr0 + threadIdx.x; pr < pr1; pr += THREADS) {
-        const u32 s = pr * 2;
-        const int y = s >> lg, x = s & (L - 1);
-        const double2 v = __ldcg(reinterpret_cast<const double2*>(src + s));
-        const double c0 = hop_term(p.tq, pitch, L, y, x, yi, xi, yj, xj);
-        const double c1 = hop_term(p.tq, pitch, L, y, x + 1, yi, xi, yj, xj);
-        double2 o;
-        o.x = __dadd_rn(v.x, c0);
-        o.y = __dadd_rn(v.y, c1);
-        __stcg(reinterpret_cast<double2*>(dst + s), o);
-    }
+    int dyj = (y - yj) & (L - 1); dyj = min(dyj, L - dyj);
+    int dyi = (y - yi) & (L - 1); dyi = min(dyi, L - dyi);
+    const double* __restrict__ rj = tq + dyj * pitch;
+    const double* __restrict__ ri = tq + dyi * pitch;
+    int aj = (x - xj) & (L - 1), bj = (aj + 1) & (L - 1);
+    int ai = (x - xi) & (L - 1), bi = (ai + 1) & (L - 1);
+    aj = min(aj, L - aj); bj = min(bj, L - bj); ai = min(ai, L - ai); bi = min(bi, L - bi);
+    const double j0 = __ldg(rj + aj), j1 = __ldg(rj + bj), i0 = __ldg(ri + ai), i1 = __ldg(ri + bi);
+    c0 = __dsub_rn(j0, i0);
+    c1 = __dsub_rn(j1, i1);
 }
 
+// eps slab of one CTA: pairs [pr0, pr1) of adjacent sites.  With RP > 0 thread t keeps pairs
+// pr0 + t + k*THREADS (k < RP) in registers across hops and writes every new value through to
+// global memory for the other CTAs' gathers; with RP == 0 the slab streams src -> dst.
+template <int THREADS, int RP>
+struct Slab {
+    double2 e[RP > 0 ? RP : 1];
+
+    __device__ __forceinline__ void load(const double* src, u32 pr0, u32 pr1)
+    {
+#pragma unroll
+        for (int k = 0; k < RP; ++k) {
+            const u32 pr = pr0 + threadIdx.x + k * THREADS;
+            if (pr < pr1) e[k] = __ldcg(reinterpret_cast<const double2*>(src + 2 * pr));
+        }
+    }
+
+    // dst = eps + (1/r_lj - 1/r_li) for every site l of the slab
+    __device__ __forceinline__ void update(const CgParams& p, const double* src, double* dst,
+                                           u32 pr0, u32 pr1, u32 hi, u32 hj)
+    {
+        const int L = p.L, lg = p.lgL, pitch = p.pitch;
+        const int yi = hi >> lg, xi = hi & (L - 1), yj = hj >> lg, xj = hj & (L - 1);
+        if (RP > 0) {
+            double c0[RP > 0 ? RP : 1], c1[RP > 0 ? RP : 1];
+#pragma unroll
+            for (int k = 0; k < RP; ++k) {            // all table gathers first
+                const u32 pr = pr0 + threadIdx.x + k * THREADS;
+                if (pr < pr1) {
+                    const u32 s = pr * 2;
+                    hop_term2(p.tq, pitch, L, s >> lg, s & (L - 1), yi, xi, yj, xj, c0[k], c1[k]);
+                }
+            }
+#pragma unroll
+            for (int k = 0; k < RP; ++k) {
+                const u32 pr = pr0 + threadIdx.x + k * THREADS;
+                if (pr < pr1) {
+                    e[k].x = __dadd_rn(e[k].x, c0[k]);
+                    e[k].y = __dadd_rn(e[k].y, c1[k]);
+                    __stcg(reinterpret_cast<double2*>(dst + 2 * pr), e[k]);
+                }
+            }
+        } else {
+            for (u32 pr = pr0 + threadIdx.x; pr < pr1; pr += THREADS) {
+                const u32 s = pr * 2;
+                const double2 v = __ldcg(reinterpret_cast<const double2*>(src + s));
+                double a0, a1;
+                hop_term2(p.tq, pitch, L, s >> lg, s & (L - 1), yi, xi, yj, xj, a0, a1);
+                double2 o;
+                o.x = __dadd_rn(v.x, a0);
+                o.y = __dadd_rn(v.y, a1);
+                __stcg(reinterpret_cast<double2*>(dst + s), o);
+            }
+        }
+    }
+};
+
 // The persistent kernel: steps 1, 2, 3a-3c of the mixed PR algorithm.
-template <int THREADS>
+template <int THREADS, int RP>
 __global__ void __launch_bounds__(THREADS, 1) cg_pr_persistent(const CgParams p)
 {
+    constexpr int NW = THREADS / 32;
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    double* s_cdf = reinterpret_cast<double*>(smem_raw);
-    double* s_invr = s_cdf + p.Klive;
-    int* s_disp = reinterpret_cast<int*>(s_invr + p.Klive);
-    u32* s_n = reinterpret_cast<u32*>(s_disp + p.Klive);
-    __shared__ u32 s_wlab[32], s_wi[32], s_wj[32];
-    __shared__ u32 s_win[3];
+    const int KL = p.Klive;
+    u64* s_cdfi = reinterpret_cast<u64*>(smem_raw);
+    double* s_invr = reinterpret_cast<double*>(s_cdfi + KL);
+    double* s_fld = s_invr + KL;
+    int* s_disp = reinterpret_cast<int*>(s_fld + KL);
+    u32* s_guide = reinterpret_cast<u32*>(s_disp + KL);
+    u32* s_n = s_guide + CG_GUIDE;
+    __shared__ u32 s_wlab[32], s_plab[32];
+    __shared__ u64 s_wpay[32], s_ppay[32];
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const u32 b = blockIdx.x, nb = gridDim.x;
     const int L = p.L, lg = p.lgL, pitch = p.pitch;
     const u32 N = p.N, M = p.M;
 
-    for (int k = tid; k < p.Klive; k += THREADS) {
-        s_cdf[k] = p.cdf[k]; s_invr[k] = p.invr_k[k]; s_disp[k] = p.disp[k];
+    for (int k = tid; k < KL; k += THREADS) {
+        s_cdfi[k] = p.cdfi[k]; s_invr[k] = p.invr_k[k]; s_fld[k] = p.fld_k[k]; s_disp[k] = p.disp[k];
     }
+    for (int k = tid; k < CG_GUIDE; k += THREADS) s_guide[k] = p.guide[k];
     for (u32 w = tid; w < (N + 31) / 32; w += THREADS) s_n[w] = p.nbits[w];
 
     // replicated, CTA-uniform control state
     u64 a0 = p.ctl->attempts, hops = p.ctl->hops, iters = p.ctl->iterations, props = p.ctl->proposals;
     long long dP = p.ctl->dP;
-    u32 base = p.ctl->cur, epoch = p.ctl->epoch;
+    u32 base = p.ctl->cur;
+    u64 epoch = p.ctl->epoch;
     const u64 log_base = p.ctl->log_base;
     const u64 target = hops + p.n_hops;
     bool pending = false;                 // hop whose term readers must add to eps[base]
+    u64 need_pub = 0;                     // epoch of the hop whose slabs must be complete before eps is read
     int pyi = 0, pxi = 0, pyj = 0, pxj = 0;
     u64 cyc_wait = 0, cyc_update = 0, cyc_propose = 0;
     const long long t_begin = clock64();
-    __syncthreads();
 
     const u32 per = (M + nb - 1) / nb;
     const u32 lab0 = min(M, b * per), lab1 = min(M, lab0 + per);
     const u32 pairs = N / 2, pper = (pairs + nb - 1) / nb;
     const u32 pr0 = min(pairs, b * pper), pr1 = min(pairs, pr0 + pper);
-    const int KL = p.Klive;
+    const u32 npw = min((u32)NW, (nb + 31) / 32);       // warps that poll the exchange slots
+    u64* const my_slot = p.slots + (size_t)b * CG_SLOT_U64;
+
+    Slab<THREADS, RP> slab;
+    slab.load(p.eps[base], pr0, pr1);
+    __syncthreads();
 
     while (hops < target) {
         const long long t0 = clock64();
@@ -182,11 +264,17 @@ __global__ void __launch_bounds__(THREADS, 1) cg_pr_persistent(const CgParams p)
             philox4x32_10((u32)a, (u32)(a >> 32), 0u, 0u, p.seed_lo, p.seed_hi, w0, w1, w2, w3);
             const u32 i = __umulhi(w0, N);                                   // uniform site
             if (!((s_n[i >> 5] >> (i & 31)) & 1u)) continue;                 // n_i = 1 ?
-            const double ud = (double)(((u64)w1 << 11) | (u64)(w2 >> 21)) * (1.0 / 8796093022208.0);
-            int lo = 0, hi = KL - 1;                                         // tower sampling
+            // tower sampling: smallest k with u_d < cdf_k, u_d = m 2^-43, as the
+            // equivalent integer test m < cdfi_k; the guide brackets k from the leading bits of 1 - u_d
+            const u64 m = ((u64)w1 << 11) | (u64)(w2 >> 21);
+            const u64 t = (1ull << 43) - m;
+            const int e = 63 - __clzll((long long)t);
+            const u32 mant = (e >= 3 ? (u32)(t >> (e - 3)) : (u32)(t << (3 - e))) & 7u;
+            const u32 g = s_guide[e * 8 + (int)mant];
+            int lo = (int)(g & 0xFFFFu), hi = (int)(g >> 16);
             while (lo < hi) {
                 const int mid = (lo + hi) >> 1;
-                if (ud < s_cdf[mid]) hi = mid; else lo = mid + 1;
+                if (m < s_cdfi[mid]) hi = mid; else lo = mid + 1;
             }
             const int d = s_disp[lo];
             const int dy = d >> 16, dx = (int)(short)(d & 0xFFFF);
@@ -200,63 +288,81 @@ __global__ void __launch_bounds__(THREADS, 1) cg_pr_persistent(const CgParams p)
                 ej = __dadd_rn(ej, hop_term(p.tq, pitch, L, yj, xj, pyi, pxi, pyj, pxj));
             }
             // dH_ij = eps_j - eps_i - 1/r_ij - E dx_ij
-            const double dE = __dsub_rn(__dsub_rn(__dsub_rn(ej, ei), s_invr[lo]),
-                                        __dmul_rn(p.E, (double)dx));
+            const double dE = __dsub_rn(__dsub_rn(__dsub_rn(ej, ei), s_invr[lo]), s_fld[lo]);
             bool acc = dE <= 0.0;
             if (!acc) {
-                const double ua = (double)(((u64)(w2 & 0x1FFFFFu) << 32) | (u64)w3)
-                                  * (1.0 / 9007199254740992.0);
-                acc = ua < exp(__ddiv_rn(-dE, p.T));                         // Eq.(2)
+                // Eq.(2): accept iff u_a < exp(-dE/T).  A float estimate with a 2^-10
+                // guard band decides all but near-ties; those take the double-precision path, so the
+                // decision is always that of the double comparison.
+                const u32 uh = ((w2 & 0x1FFFFFu) << 11) | (w3 >> 21);        // top 32 of the 53 bits
+                const float ul = (float)uh * 2.3283064365386963e-10f;        // u_a in [ul, ul + 2^-32)
+                const float xf = (float)(-dE) * p.inv_T;
+                const float pf = __expf(xf);
+                int dec = 0;                                                 // 0 undecided, 1 accept, 2 reject
+                if (ul > pf * 1.0009765625f) dec = 2;
+                else if (xf > -60.f && ul + 4.6566128730773926e-10f < pf * 0.9990234375f) dec = 1;
+                if (dec == 0) {
+                    const double ua = (double)(((u64)(w2 & 0x1FFFFFu) << 32) | (u64)w3)
+                                      * (1.0 / 9007199254740992.0);
+                    acc = ua < exp(__ddiv_rn(-dE, p.T));
+                } else acc = dec == 1;
             }
             if (acc) { best = l; bi = i; bj = j; break; }
         }
         const long long t1 = clock64();
-        // ---- step 3: lowest accepting label: warp, block, grid
+        // ---- step 3: lowest accepting label: warp, CTA, grid
         {
             const u32 wmin = __reduce_min_sync(CG_FULL, best);
             const int src = __ffs(__ballot_sync(CG_FULL, best == wmin)) - 1;
-            const u32 wi = __shfl_sync(CG_FULL, bi, src), wj = __shfl_sync(CG_FULL, bj, src);
-            if (lane == 0) { s_wlab[warp] = wmin; s_wi[warp] = wi; s_wj[warp] = wj; }
+            if (lane == src) { s_wlab[warp] = wmin; s_wpay[warp] = ((u64)bi << 32) | (u64)bj; }
         }
         __syncthreads();
         if (warp == 0) {
-            u32 lab = lane < THREADS / 32 ? s_wlab[lane] : CG_NONE;
-            u32 ii = lane < THREADS / 32 ? s_wi[lane] : 0u, jj = lane < THREADS / 32 ? s_wj[lane] : 0u;
-            u32 gmin = __reduce_min_sync(CG_FULL, lab);
-            int src = __ffs(__ballot_sync(CG_FULL, lab == gmin)) - 1;
-            ii = __shfl_sync(CG_FULL, ii, src); jj = __shfl_sync(CG_FULL, jj, src);
-            if (nb > 1) {
-                if (lane == 0) {
-                    __threadfence();      // release: this CTA's eps slab of the previous hop
-                    slot_store(p.slots + b, ((u64)epoch << 32) | gmin,
-                               ((u64)(epoch & 0xFFFFu) << 48) | ((u64)ii << 24) | (u64)jj);
-                }
-                for (;;) {
-                    u32 mlab = CG_NONE; u64 mpay = 0; bool ok = true;
-                    for (u32 c = lane; c < nb; c += 32) {
-                        u64 q0, q1;
-                        slot_load(p.slots + c, q0, q1);
-                        ok = ok && (u32)(q0 >> 32) == epoch && (u32)(q1 >> 48) == (epoch & 0xFFFFu);
-                        if ((u32)q0 < mlab) { mlab = (u32)q0; mpay = q1; }
-                    }
-                    if (__all_sync(CG_FULL, ok)) {
-                        gmin = __reduce_min_sync(CG_FULL, mlab);
-                        src = __ffs(__ballot_sync(CG_FULL, mlab == gmin)) - 1;
-                        mpay = __shfl_sync(CG_FULL, mpay, src);
-                        ii = (u32)(mpay >> 24) & 0xFFFFFFu; jj = (u32)mpay & 0xFFFFFFu;
-                        break;
-                    }
-                }
-                __threadfence();          // acquire: other CTAs' slabs
+            const u32 lab = lane < NW ? s_wlab[lane] : CG_NONE;
+            const u64 pay = lane < NW ? s_wpay[lane] : 0ull;
+            const u32 gmin = __reduce_min_sync(CG_FULL, lab);
+            const int src = __ffs(__ballot_sync(CG_FULL, lab == gmin)) - 1;
+            if (lane == src) {
+                if (nb > 1)
+                    slot_store(my_slot, ((u64)(u32)epoch << 32) | gmin,
+                               ((u64)((u32)epoch & 0xFFFFu) << 48) | ((pay >> 32) << 24) | (pay & 0xFFFFFFu));
+                else { s_plab[0] = gmin; s_ppay[0] = pay; }
             }
-            if (lane == 0) { s_win[0] = gmin; s_win[1] = ii; s_win[2] = jj; }
+        }
+        if (nb > 1 && warp < npw) {
+            // every slot is watched by one thread; the hop whose slabs the next gathers read must be
+            // published too (pub word, written by each CTA after its eps stores are fenced)
+            u32 plab = CG_NONE; u64 ppay = 0;
+            const u32 e32 = (u32)epoch, e16 = (u32)epoch & 0xFFFFu;
+            for (u32 c = tid; c < nb; c += THREADS) {
+                const u64* sl = p.slots + (size_t)c * CG_SLOT_U64;
+                u64 q0, q1;
+                for (;;) {
+                    slot_load(sl, q0, q1);
+                    const u64 pb = ld_relaxed_u64(sl + 2);
+                    if ((u32)(q0 >> 32) == e32 && (u32)(q1 >> 48) == e16 && pb >= need_pub) break;
+                }
+                if ((u32)q0 < plab) { plab = (u32)q0; ppay = ((q1 >> 24) & 0xFFFFFFull) << 32 | (q1 & 0xFFFFFFull); }
+            }
+            fence_acquire_gpu();
+            const u32 wmin = __reduce_min_sync(CG_FULL, plab);
+            const int src = __ffs(__ballot_sync(CG_FULL, plab == wmin)) - 1;
+            if (lane == src) { s_plab[warp] = wmin; s_ppay[warp] = ppay; }
         }
         __syncthreads();
-        const u32 q = s_win[0], hi_ = s_win[1], hj_ = s_win[2];
+        u32 q, hi_, hj_;
+        {
+            const u32 lab = (u32)lane < npw ? s_plab[lane] : CG_NONE;
+            const u64 pay = (u32)lane < npw ? s_ppay[lane] : 0ull;
+            q = __reduce_min_sync(CG_FULL, lab);
+            const int src = __ffs(__ballot_sync(CG_FULL, lab == q)) - 1;
+            const u64 wp = __shfl_sync(CG_FULL, pay, src);
+            hi_ = (u32)(wp >> 32); hj_ = (u32)wp;
+        }
         const long long t2 = clock64();
-        ++epoch; ++iters; props += M;
+        ++iters; props += M;
         cyc_propose += (u64)(t1 - t0); cyc_wait += (u64)(t2 - t1);
-        if (q == CG_NONE) { a0 += M; continue; }            // whole window rejected: p += 1
+        if (q == CG_NONE) { a0 += M; ++epoch; continue; }   // whole window rejected: p += 1
 
         // ---- step 3a: execute the hop of label q; m = (p-1)M + q attempts used
         const u64 a_hop = a0 + q;
@@ -273,11 +379,21 @@ __global__ void __launch_bounds__(THREADS, 1) cg_pr_persistent(const CgParams p)
             }
         }
         ++hops;
+        __syncthreads();
         // ---- step 3b: local energies of my slab, into the other buffer
         if (pending) base ^= 1u;
-        update_slab<THREADS>(p, p.eps[base], p.eps[base ^ 1u], pr0, pr1, hi_, hj_);
+        slab.update(p, p.eps[base], p.eps[base ^ 1u], pr0, pr1, hi_, hj_);
         pending = true; pyi = yi; pxi = xi; pyj = yj; pxj = xj;
-        __syncthreads();
+        need_pub = epoch;
+        if (nb > 1) {
+            // publish "my slab of this hop is written" off the critical path: the last warp waits for
+            // the others' stores (named barrier), fences them and releases the pub word
+            if (warp == NW - 1) {
+                bar1_sync(THREADS);
+                if (lane == 0) st_release_u64(my_slot + 2, epoch);
+            } else bar1_arrive(THREADS);
+        }
+        ++epoch;
         cyc_update += (u64)(clock64() - t2);
     }
 
@@ -294,7 +410,7 @@ __global__ void __launch_bounds__(THREADS, 1) cg_pr_persistent(const CgParams p)
 }
 
 // Step a6 alone: scripted hops, update in place (no readers), one launch.
-template <int THREADS>
+template <int THREADS, int RP>
 __global__ void __launch_bounds__(THREADS, 1)
 cg_update_scripted(const CgParams p, const u32* __restrict__ hop_i, const u32* __restrict__ hop_j, u64 count)
 {
@@ -302,8 +418,10 @@ cg_update_scripted(const CgParams p, const u32* __restrict__ hop_i, const u32* _
     const u32 pairs = p.N / 2, pper = (pairs + nb - 1) / nb;
     const u32 pr0 = min(pairs, b * pper), pr1 = min(pairs, pr0 + pper);
     double* e = p.eps[p.ctl->cur];
+    Slab<THREADS, RP> slab;
+    slab.load(e, pr0, pr1);
     for (u64 h = 0; h < count; ++h)
-        update_slab<THREADS>(p, e, e, pr0, pr1, __ldg(hop_i + h), __ldg(hop_j + h));
+        slab.update(p, e, e, pr0, pr1, __ldg(hop_i + h), __ldg(hop_j + h));
     if (b == 0 && threadIdx.x == 0) {       // occupations and dipole moment, in hop order
         long long dP = p.ctl->dP; u32 bad = 0;
         const int L = p.L;
@@ -410,7 +528,9 @@ struct cg_sim {
     // host tables (live part of the tower)
     int64_t K = 0, Klive = 0;
     std::vector<int32_t> dy, dx;
-    std::vector<double> cdf, invr_k;
+    std::vector<double> cdf, invr_k, fld_k;
+    std::vector<u64> cdfi;
+    std::vector<u32> guide;
     double S = 0, Gamma = 0;
     // device
     cudaStream_t stream = nullptr;
@@ -418,11 +538,12 @@ struct cg_sim {
     double* d_eps[2] = {nullptr, nullptr};
     double* d_scratch = nullptr; double* d_phi = nullptr;
     u32* d_nbits = nullptr; double* d_tq = nullptr;
-    double* d_cdf = nullptr; double* d_invr_k = nullptr; int* d_disp = nullptr;
-    ulonglong2* d_slots = nullptr; CgCtl* d_ctl = nullptr; u64* d_red = nullptr;
+    u64* d_cdfi = nullptr; double* d_invr_k = nullptr; double* d_fld_k = nullptr; int* d_disp = nullptr;
+    u32* d_guide = nullptr;
+    u64* d_slots = nullptr; CgCtl* d_ctl = nullptr; u64* d_red = nullptr;
     void* d_log = nullptr; bool own_log = false; u64 log_cap = 0;
     // launch shape
-    int num_sms = 0, n_ctas = 0, threads = 0, smem = 0;
+    int num_sms = 0, n_ctas = 0, threads = 0, smem = 0, rp = 0;
     std::string err;
 };
 
@@ -447,7 +568,8 @@ static bool valid_L(int L, int* lg)
     return true;
 }
 
-struct WsLayout { size_t eps0, eps1, scratch, phi, nbits, tq, cdf, invr_k, disp, slots, ctl, red, total; };
+struct WsLayout { size_t eps0, eps1, scratch, phi, nbits, tq, cdfi, invr_k, fld_k, disp, guide, slots, ctl, red, total; };
+#define CG_SLOT_BYTES ((size_t)8 * CG_SLOT_U64 * CG_MAX_CTAS)
 
 static WsLayout ws_layout(int L)
 {
@@ -459,10 +581,12 @@ static WsLayout ws_layout(int L)
     w.phi = o; o += align256(8 * N);
     w.nbits = o; o += align256(N / 8 + 4);
     w.tq = o; o += align256(8 * h * h);
-    w.cdf = o; o += align256(8 * N);            // tower can never be longer than N entries
+    w.cdfi = o; o += align256(8 * N);           // tower can never be longer than N entries
     w.invr_k = o; o += align256(8 * N);
+    w.fld_k = o; o += align256(8 * N);
     w.disp = o; o += align256(4 * N);
-    w.slots = o; o += align256(sizeof(ulonglong2) * CG_MAX_CTAS);
+    w.guide = o; o += align256(4 * CG_GUIDE);
+    w.slots = o; o += align256(CG_SLOT_BYTES);
     w.ctl = o; o += align256(sizeof(CgCtl));
     w.red = o; o += 256;
     w.total = o;
@@ -509,12 +633,32 @@ static void build_tables(cg_sim* s, std::vector<double>& tq)
     }
     s->Klive = (int64_t)live;
     s->dy.resize(live); s->dx.resize(live); s->cdf.resize(live); s->invr_k.resize(live);
+    s->fld_k.resize(live); s->cdfi.resize(live);
     for (size_t k = 0; k < live; ++k) {
         s->dy[k] = d[k].dy; s->dx[k] = d[k].dx;
         s->cdf[k] = (k + 1 == K) ? 1.0 : run[k] / acc;
         s->invr_k[k] = 1.0 / std::sqrt((double)d[k].r2);
+        s->fld_k[k] = s->E * (double)d[k].dx;              // the field term of dH
     }
     s->cdf[live - 1] = 1.0;
+    // u_d = m 2^-43 with integer m < 2^43, so u_d < cdf_k <=> m < ceil(cdf_k 2^43) (scaling by a power
+    // of two and ceil are exact in double)
+    for (size_t k = 0; k < live; ++k) s->cdfi[k] = (u64)std::ceil(std::ldexp(s->cdf[k], 43));
+    // Guide over t = 2^43 - m: bucket = (binade of t, next 3 bits).  The tail of the tower is geometric
+    // in r, so every bucket brackets only a few k; both ends found by the plain search.
+    auto kstar = [&](u64 m) { size_t k = 0; while (!(m < s->cdfi[k])) ++k; return (u32)k; };
+    s->guide.assign(CG_GUIDE, 0u);
+    for (int e = 0; e <= 43; ++e)
+        for (int mant = 0; mant < 8; ++mant) {
+            u64 tlo, thi;
+            if (e >= 3) { tlo = (u64)(8 + mant) << (e - 3); thi = (((u64)(8 + mant + 1)) << (e - 3)) - 1; }
+            else { if (mant & ((1 << (3 - e)) - 1)) continue; tlo = thi = (u64)(8 + mant) >> (3 - e); }
+            const u64 top = 1ull << 43;
+            if (tlo > top) continue;
+            if (thi > top) thi = top;
+            const u32 klo = kstar(top - thi), khi = kstar(top - tlo);
+            s->guide[(size_t)e * 8 + mant] = klo | (khi << 16);
+        }
     const int pitch = s->pitch;
     tq.assign((size_t)pitch * pitch, 0.0);
     for (int a = 0; a <= h; ++a)
@@ -524,14 +668,18 @@ static void build_tables(cg_sim* s, std::vector<double>& tq)
         }
 }
 
-static size_t smem_bytes(const cg_sim* s) { return (size_t)s->Klive * 20 + 4 * (((size_t)s->N + 31) / 32) + 16; }
+static size_t smem_bytes(const cg_sim* s)
+{
+    return (size_t)s->Klive * 28 + 4 * CG_GUIDE + 4 * (((size_t)s->N + 31) / 32) + 16;
+}
 
 static CgParams make_params(const cg_sim* s, u64 n_hops)
 {
     CgParams p;
     p.eps[0] = s->d_eps[0]; p.eps[1] = s->d_eps[1];
     p.tq = s->d_tq; p.nbits = s->d_nbits;
-    p.cdf = s->d_cdf; p.invr_k = s->d_invr_k; p.disp = s->d_disp;
+    p.cdfi = s->d_cdfi; p.invr_k = s->d_invr_k; p.fld_k = s->d_fld_k; p.disp = s->d_disp;
+    p.guide = s->d_guide;
     p.slots = s->d_slots; p.ctl = s->d_ctl;
     p.log_a = (u64*)s->d_log;
     p.log_i = s->d_log ? (u32*)((char*)s->d_log + 8 * s->log_cap) : nullptr;
@@ -540,26 +688,61 @@ static CgParams make_params(const cg_sim* s, u64 n_hops)
     p.L = s->L; p.lgL = s->lgL; p.pitch = s->pitch; p.Klive = (int)s->Klive;
     p.N = s->N; p.M = s->M;
     p.seed_lo = (u32)s->seed; p.seed_hi = (u32)(s->seed >> 32);
-    p.T = s->T; p.E = s->E; p.n_hops = n_hops;
+    p.T = s->T; p.E = s->E; p.inv_T = (float)(1.0 / s->T); p.n_hops = n_hops;
     return p;
 }
 
 typedef void (*persist_fn)(const CgParams);
 typedef void (*scripted_fn)(const CgParams, const u32*, const u32*, u64);
 
-static persist_fn persistent_kernel(int threads)
+// RP = eps pairs a thread keeps in registers (0: the slab streams through global memory)
+template <int THREADS>
+static persist_fn persistent_kernel_t(int rp)
+{
+    switch (rp) {
+        case 0: return cg_pr_persistent<THREADS, 0>;
+        case 1: return cg_pr_persistent<THREADS, 1>;
+        case 2: return cg_pr_persistent<THREADS, 2>;
+        case 4: return cg_pr_persistent<THREADS, 4>;
+        case 8: return cg_pr_persistent<THREADS, 8>;
+    }
+    return nullptr;
+}
+static persist_fn persistent_kernel(int threads, int rp)
 {
     switch (threads) {
-        case 256: return cg_pr_persistent<256>;
-        case 512: return cg_pr_persistent<512>;
-        case 1024: return cg_pr_persistent<1024>;
+        case 256: return persistent_kernel_t<256>(rp);
+        case 512: return persistent_kernel_t<512>(rp);
+        case 1024: return rp > 2 ? nullptr : persistent_kernel_t<1024>(rp);
+    }
+    return nullptr;
+}
+static scripted_fn scripted_kernel(int rp)
+{
+    switch (rp) {
+        case 0: return cg_update_scripted<512, 0>;
+        case 1: return cg_update_scripted<512, 1>;
+        case 2: return cg_update_scripted<512, 2>;
+        case 4: return cg_update_scripted<512, 4>;
+        case 8: return cg_update_scripted<512, 8>;
     }
     return nullptr;
 }
 
-static int max_coresident(cg_sim* s, int threads, int* out)
+// smallest supported register tiling that holds `pairs` pairs per CTA, else 0 (streaming)
+static int choose_rp(u64 pairs, int n_ctas, int threads)
 {
-    persist_fn f = persistent_kernel(threads);
+    const u64 per_cta = (pairs + n_ctas - 1) / n_ctas;
+    const u64 need = (per_cta + threads - 1) / threads;
+    const int cap = threads == 1024 ? 2 : 8;
+    for (int rp = 1; rp <= cap; rp *= 2)
+        if ((u64)rp >= need) return rp;
+    return 0;
+}
+
+static int max_coresident(cg_sim* s, int threads, int rp, int* out)
+{
+    persist_fn f = persistent_kernel(threads, rp);
     if (!f) return CG_EINVAL;
     CK(cudaFuncSetAttribute((const void*)f, cudaFuncAttributeMaxDynamicSharedMemorySize, s->smem));
     int per_sm = 0;
@@ -572,19 +755,29 @@ static int choose_launch(cg_sim* s, int n_ctas, int threads)
 {
     if (threads == 0) threads = 512;
     if (threads != 256 && threads != 512 && threads != 1024) return CG_EINVAL;
-    int cap = 0;
-    int rc = max_coresident(s, threads, &cap);
-    if (rc != CG_OK) return rc;
-    if (cap < 1) { s->err = "persistent kernel does not fit on an SM"; return CG_EUNSUPPORTED; }
-    if (n_ctas == 0) {
+    const bool heuristic = n_ctas == 0;
+    if (heuristic) {
         const u64 work = std::max<u64>(s->M, s->N / 2);
         n_ctas = (int)std::min<u64>((work + threads - 1) / threads, (u64)s->num_sms);
-        n_ctas = std::max(1, std::min(n_ctas, cap));
+        n_ctas = std::max(1, n_ctas);
     }
-    if (n_ctas < 1 || n_ctas > cap) return CG_EINVAL;
-    if (n_ctas != s->n_ctas)   // stale epochs of other grid shapes must not be mistaken for arrivals
-        CK(cudaMemsetAsync(s->d_slots, 0, sizeof(ulonglong2) * CG_MAX_CTAS, s->stream));
-    s->n_ctas = n_ctas; s->threads = threads;
+    if (n_ctas < 1 || n_ctas > CG_MAX_CTAS) return CG_EINVAL;
+    int rp = choose_rp(s->N / 2, n_ctas, threads);
+    int cap = 0;
+    int rc = max_coresident(s, threads, rp, &cap);
+    if (rc != CG_OK) return rc;
+    if (cap < 1) { s->err = "persistent kernel does not fit on an SM"; return CG_EUNSUPPORTED; }
+    if (n_ctas > cap) {
+        if (!heuristic) return CG_EINVAL;
+        n_ctas = cap;
+        rp = choose_rp(s->N / 2, n_ctas, threads);
+        rc = max_coresident(s, threads, rp, &cap);
+        if (rc != CG_OK) return rc;
+        if (n_ctas > cap) return CG_EUNSUPPORTED;
+    }
+    if (n_ctas != s->n_ctas)   // slots of CTAs that no longer exist must not look published
+        CK(cudaMemsetAsync(s->d_slots, 0, CG_SLOT_BYTES, s->stream));
+    s->n_ctas = n_ctas; s->threads = threads; s->rp = rp;
     return CG_OK;
 }
 
@@ -614,6 +807,7 @@ static int init_impl(cg_sim** out, int L, double W, double xi, double T, double 
 
     std::vector<double> tq;
     try { build_tables(s, tq); } catch (const std::bad_alloc&) { return CG_ENOMEM; }
+    if (s->Klive > 65535) return CG_EUNSUPPORTED;           // the guide packs k in 16 bits
     s->smem = (int)smem_bytes(s);
     if ((size_t)s->smem > (size_t)prop.sharedMemPerBlockOptin - 1024) return CG_EUNSUPPORTED;
 
@@ -630,18 +824,21 @@ static int init_impl(cg_sim** out, int L, double W, double xi, double T, double 
     s->d_eps[0] = (double*)(base + w.eps0); s->d_eps[1] = (double*)(base + w.eps1);
     s->d_scratch = (double*)(base + w.scratch); s->d_phi = (double*)(base + w.phi);
     s->d_nbits = (u32*)(base + w.nbits); s->d_tq = (double*)(base + w.tq);
-    s->d_cdf = (double*)(base + w.cdf); s->d_invr_k = (double*)(base + w.invr_k);
-    s->d_disp = (int*)(base + w.disp); s->d_slots = (ulonglong2*)(base + w.slots);
+    s->d_cdfi = (u64*)(base + w.cdfi); s->d_invr_k = (double*)(base + w.invr_k);
+    s->d_fld_k = (double*)(base + w.fld_k); s->d_guide = (u32*)(base + w.guide);
+    s->d_disp = (int*)(base + w.disp); s->d_slots = (u64*)(base + w.slots);
     s->d_ctl = (CgCtl*)(base + w.ctl); s->d_red = (u64*)(base + w.red);
 
     std::vector<int> disp((size_t)s->Klive);
     for (int64_t k = 0; k < s->Klive; ++k) disp[k] = (s->dy[k] << 16) | (s->dx[k] & 0xFFFF);
     cudaStream_t st = s->stream;
     CK(cudaMemcpyAsync(s->d_tq, tq.data(), 8 * tq.size(), cudaMemcpyHostToDevice, st));
-    CK(cudaMemcpyAsync(s->d_cdf, s->cdf.data(), 8 * (size_t)s->Klive, cudaMemcpyHostToDevice, st));
+    CK(cudaMemcpyAsync(s->d_cdfi, s->cdfi.data(), 8 * (size_t)s->Klive, cudaMemcpyHostToDevice, st));
     CK(cudaMemcpyAsync(s->d_invr_k, s->invr_k.data(), 8 * (size_t)s->Klive, cudaMemcpyHostToDevice, st));
+    CK(cudaMemcpyAsync(s->d_fld_k, s->fld_k.data(), 8 * (size_t)s->Klive, cudaMemcpyHostToDevice, st));
+    CK(cudaMemcpyAsync(s->d_guide, s->guide.data(), 4 * (size_t)CG_GUIDE, cudaMemcpyHostToDevice, st));
     CK(cudaMemcpyAsync(s->d_disp, disp.data(), 4 * (size_t)s->Klive, cudaMemcpyHostToDevice, st));
-    CK(cudaMemsetAsync(s->d_slots, 0, sizeof(ulonglong2) * CG_MAX_CTAS, st));
+    CK(cudaMemsetAsync(s->d_slots, 0, CG_SLOT_BYTES, st));
     CgCtl ctl; memset(&ctl, 0, sizeof ctl); ctl.epoch = 1;
     CK(cudaMemcpyAsync(s->d_ctl, &ctl, sizeof ctl, cudaMemcpyHostToDevice, st));
 
@@ -687,7 +884,8 @@ extern "C" int cg_run(cg_sim* s, uint64_t n_hops)
 {
     if (!s) return CG_EINVAL;
     if (n_hops == 0) return CG_OK;
-    persist_fn f = persistent_kernel(s->threads);
+    persist_fn f = persistent_kernel(s->threads, s->rp);
+    if (!f) return CG_EINVAL;
     CgParams p = make_params(s, n_hops);
     void* args[] = {&p};
     CK(cudaLaunchCooperativeKernel((const void*)f, dim3(s->n_ctas), dim3(s->threads), args, (size_t)s->smem, s->stream));
@@ -835,8 +1033,9 @@ extern "C" int cg_apply_hops(cg_sim* s, uint64_t count, const uint32_t* i, const
     CK(cudaEventCreate(&e0)); CK(cudaEventCreate(&e1));
     CgParams p = make_params(s, 0);
     const int grid = (int)std::max<u64>(1, std::min<u64>((s->N / 2 + 511) / 512, (u64)s->num_sms));
+    scripted_fn uf = scripted_kernel(choose_rp(s->N / 2, grid, 512));
     CK(cudaEventRecord(e0, s->stream));
-    cg_update_scripted<512><<<grid, 512, 0, s->stream>>>(p, d_ij, d_ij + count, count);
+    uf<<<grid, 512, 0, s->stream>>>(p, d_ij, d_ij + count, count);
     CK(cudaEventRecord(e1, s->stream));
     CK(cudaGetLastError());
     CK(cudaStreamSynchronize(s->stream));
