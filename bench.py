@@ -149,7 +149,7 @@ def run_reference(args):
     }))
 
 
-CTL_BYTES = 96  # sizeof(CgCtl) in csrc/cg.cu: the control block cg_set_state / cg_get_state move
+CTL_BYTES = 128  # sizeof(CgCtl) in csrc/cg.cu: the control block cg_set_state / cg_get_state move
 
 
 def run_ours(args):

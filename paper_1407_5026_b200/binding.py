@@ -19,7 +19,7 @@ EXPORTS = [
     "cg_init", "cg_workspace_bytes", "cg_init_ws", "cg_run", "cg_get_state", "cg_set_state",
     "cg_get_counters", "cg_enable_hop_log", "cg_get_hops", "cg_recompute_eps", "cg_apply_hops",
     "cg_get_table_sizes", "cg_get_tables", "cg_get_phi", "cg_set_launch", "cg_get_launch",
-    "cg_get_phase_cycles", "cg_bench_l2_rmw", "cg_free", "cg_strerror", "cg_last_error",
+    "cg_get_phase_cycles", "cg_set_trace", "cg_bench_l2_rmw", "cg_free", "cg_strerror", "cg_last_error",
 ]
 
 
@@ -59,6 +59,7 @@ def lib():
         "cg_set_launch": (ci, [vp, ci, ci]),
         "cg_get_launch": (ci, [vp, P(ci), P(ci), P(ci)]),
         "cg_get_phase_cycles": (ci, [vp, P(u64), P(u64), P(u64), P(u64), ci]),
+        "cg_set_trace": (ci, [vp, vp, sz, u32]),
         "cg_bench_l2_rmw": (ci, [sz, ci, ci, P(dbl)]),
         "cg_free": (None, [vp]),
         "cg_strerror": (C.c_char_p, [ci]),
@@ -230,6 +231,25 @@ class CoulombGlass:
         a, b, c = C.c_int(), C.c_int(), C.c_int()
         self._check(self._lib.cg_get_launch(self._h, C.byref(a), C.byref(b), C.byref(c)))
         return {"n_ctas": a.value, "threads": b.value, "smem_bytes": c.value}
+
+    def set_trace(self, iterations):
+        """Record %globaltimer events of the first `iterations` PR iterations of each following run."""
+        torch = self._torch
+        iterations = int(iterations)
+        if not iterations:
+            self._check(self._lib.cg_set_trace(self._h, None, 0, 0))
+            self._trace = None
+            return
+        self._trace = torch.zeros(24 * iterations * 1024, dtype=torch.int64, device=self.device)
+        self._trace_iters = iterations
+        self._check(self._lib.cg_set_trace(self._h, C.c_void_p(self._trace.data_ptr()),
+                                           self._trace.numel() * 8, iterations))
+
+    def trace(self):
+        """-> int64 array [n_ctas, iterations, 24] (see cg_set_trace in include/cg.h)."""
+        self._torch.cuda.synchronize(self.device)
+        n = self.launch()["n_ctas"]
+        return self._trace.view(1024, self._trace_iters, 24)[:n].cpu().numpy()
 
     def phase_cycles(self, reset=False):
         t, w, u, p = C.c_uint64(), C.c_uint64(), C.c_uint64(), C.c_uint64()

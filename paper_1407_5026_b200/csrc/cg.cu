@@ -36,6 +36,7 @@ typedef unsigned int u32;
 // ------------------------------------------------------------------ device --
 
 #define CG_SLOT_U64 32      // one exchange slot per CTA, 256-byte stride (own L2 slice), in u64 units
+#define CG_TRACE_EV 24      // events per iteration in the optional trace (cg_set_trace)
 #define CG_GUIDE 352        // tower guide: (43 + 1) binades x 8 sub-buckets of t = 2^43 - m
 
 struct CgCtl {              // device-resident control block (one per sim)
@@ -49,11 +50,14 @@ struct CgCtl {              // device-resident control block (one per sim)
     u64 epoch;              // next exchange epoch; never reset, so stale slots can never match
     u64 log_base;           // hop count at which the hop log was enabled
     u64 cyc_total, cyc_wait, cyc_update, cyc_propose;
+    u64 pub_count[2];       // slab publications: every CTA adds 1 per executed hop, to the counter of the
+                            // hop's parity within the launch (publications of two consecutive hops overlap)
+    u64 pub_base[2];        // values pub_count has when no launch is in flight
 };
 
 struct CgParams {           // kernel parameter block
-    double* eps[2];         // double-buffered local energies, N each
-    const double* tq;       // quarter table 1/r, (L/2+1) x (L/2+1)
+    double* eps[3];         // ring of local-energy buffers, N each (see "pending hops" below)
+    const double* tf;       // unfolded table 1/r, L rows of pitch 2L (see site_code)
     u32* nbits;             // occupations, bit s of word s/32
     const u64* cdfi;        // live tower as integer thresholds: u_d < cdf_k  <=>  m < cdfi_k
     const double* invr_k;   // 1/r of displacement k (live part)
@@ -65,10 +69,13 @@ struct CgParams {           // kernel parameter block
     u64* log_a; u32* log_i; u32* log_j; u64 log_cap;
     int L, lgL, pitch, Klive;
     u32 N, M;
+    u32 PL;                 // CACHED: threads per CTA that own attempts
     u32 seed_lo, seed_hi;
     double T, E;
     float inv_T;            // (float)(1/T), pre-test of the Metropolis factor only
     u64 n_hops;
+    u64* trace;             // optional event trace: [CTA][iteration][CG_TRACE_EV] globaltimer ns
+    u32 trace_iters;
 };
 
 // Philox4x32-10 (Salmon et al., SC'11): counter (c0..c3), key (k0,k1).
@@ -102,111 +109,189 @@ __device__ __forceinline__ u64 ld_relaxed_u64(const u64* p)
     asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
     return v;
 }
-__device__ __forceinline__ void st_release_u64(u64* p, u64 v)
+__device__ __forceinline__ void red_release_add_u64(u64* p, u64 v)
 {
-    asm volatile("st.release.gpu.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
+#ifdef CG_EXP_NOMEMBAR
+    asm volatile("red.relaxed.gpu.global.add.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
+#else
+    asm volatile("red.release.gpu.global.add.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
+#endif
 }
+__device__ __forceinline__ u64 global_ns()
+{
+    u64 t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    return t;
+}
+#ifdef CG_EXP_NOACQ
+__device__ __forceinline__ void fence_acquire_gpu() { }
+#else
 __device__ __forceinline__ void fence_acquire_gpu() { asm volatile("fence.acquire.gpu;" ::: "memory"); }
-// named barrier 1: the warps that wrote eps arrive, the publishing warp waits for them
-__device__ __forceinline__ void bar1_arrive(int n) { asm volatile("bar.arrive 1, %0;" ::"r"(n) : "memory"); }
-__device__ __forceinline__ void bar1_sync(int n) { asm volatile("bar.sync 1, %0;" ::"r"(n) : "memory"); }
+#endif
+// named barriers 1 and 2 (alternating by hop): the warps that wrote eps arrive, the service warp
+// waits for them; barrier 0 with an explicit count synchronises the worker warps only
+__device__ __forceinline__ void barN_arrive(int id, int n) { asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(n) : "memory"); }
+__device__ __forceinline__ void barN_sync(int id, int n) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(n) : "memory"); }
+__device__ __forceinline__ void bar0_sync(int n) { asm volatile("bar.sync 0, %0;" ::"r"(n) : "memory"); }
 
-// 1/r between site (y,x) and site (yb,xb) under minimum image, from
-// the quarter table; 0 on the diagonal.
-__device__ __forceinline__ double invr_at(const double* __restrict__ tq, int pitch, int L,
-                                          int y, int x, int yb, int xb)
-{
-    int dy = (y - yb) & (L - 1); dy = min(dy, L - dy);
-    int dx = (x - xb) & (L - 1); dx = min(dx, L - dx);
-    return __ldg(tq + dy * pitch + dx);
-}
+// ---- the unfolded 1/r table ------------------------------------------------------------
+// tf[dy * 2L + dx] = 1/r of the offset (dy, dx) under minimum image, dy in [0, L),
+// dx in [0, L] (dx = L repeats dx = 0, so the pair (dx, dx+1) never wraps); 0 at the origin.
+// A site s = y L + x is coded as c(s) = y 2L + x; with bit L (the spare bit between the fields) set
+// in the minuend, ONE subtraction and ONE mask give both periodic differences:
+//   ((c(s) | L) - c(t)) & mask  =  ((y_s - y_t) mod L) 2L + ((x_s - x_t) mod L).
+__device__ __forceinline__ u32 site_code(u32 s, int L) { return s + (s & ~(u32)(L - 1)); }
 
-// Step 3b of the mixed PR algorithm: what hop i->j adds to eps at (y,x):
-// 1/r_lj - 1/r_li (difference first, then ONE add by the caller).
-__device__ __forceinline__ double hop_term(const double* __restrict__ tq, int pitch, int L,
-                                           int y, int x, int yi, int xi, int yj, int xj)
+// Step 3b of the mixed PR algorithm: what hop i->j adds to eps at the site coded sc
+// (spare bit set): 1/r_lj - 1/r_li (difference first, then ONE add by the caller).
+__device__ __forceinline__ double hop_term(const double* __restrict__ tf, u32 mask, u32 sc, u32 ci, u32 cj)
 {
-    return __dsub_rn(invr_at(tq, pitch, L, y, x, yj, xj), invr_at(tq, pitch, L, y, x, yi, xi));
-}
-
-// The two terms of a pair of adjacent sites (y, x), (y, x+1), x even: both rows once.
-__device__ __forceinline__ void hop_term2(const double* __restrict__ tq, int pitch, int L,
-                                          int y, int x, int yi, int xi, int yj, int xj,
-                                          double& c0, double& c1)
-{
-    int dyj = (y - yj) & (L - 1); dyj = min(dyj, L - dyj);
-    int dyi = (y - yi) & (L - 1); dyi = min(dyi, L - dyi);
-    const double* __restrict__ rj = tq + dyj * pitch;
-    const double* __restrict__ ri = tq + dyi * pitch;
-    int aj = (x - xj) & (L - 1), bj = (aj + 1) & (L - 1);
-    int ai = (x - xi) & (L - 1), bi = (ai + 1) & (L - 1);
-    aj = min(aj, L - aj); bj = min(bj, L - bj); ai = min(ai, L - ai); bi = min(bi, L - bi);
-    const double j0 = __ldg(rj + aj), j1 = __ldg(rj + bj), i0 = __ldg(ri + ai), i1 = __ldg(ri + bi);
-    c0 = __dsub_rn(j0, i0);
-    c1 = __dsub_rn(j1, i1);
+    return __dsub_rn(__ldg(tf + ((sc - cj) & mask)), __ldg(tf + ((sc - ci) & mask)));
 }
 
 // eps slab of one CTA: pairs [pr0, pr1) of adjacent sites.  With RP > 0 thread t keeps pairs
 // pr0 + t + k*THREADS (k < RP) in registers across hops and writes every new value through to
 // global memory for the other CTAs' gathers; with RP == 0 the slab streams src -> dst.
-template <int THREADS, int RP>
+// issue() starts the table gathers of a hop, finish() adds and stores: the caller puts
+// independent work between the two.
+template <int TW, int RP>
 struct Slab {
-    double2 e[RP > 0 ? RP : 1];
+    static constexpr int R = RP > 0 ? RP : 1;
+    double2 e[R];
+    double tj0[R], tj1[R], ti0[R], ti1[R];
+    u32 sc[R];
+    u32 hci, hcj;
 
-    __device__ __forceinline__ void load(const double* src, u32 pr0, u32 pr1)
+    __device__ __forceinline__ void load(const double* src, u32 pr0, u32 pr1, int L)
     {
 #pragma unroll
         for (int k = 0; k < RP; ++k) {
-            const u32 pr = pr0 + threadIdx.x + k * THREADS;
+            const u32 pr = pr0 + threadIdx.x + k * TW;
+            sc[k] = site_code(2 * pr, L) | (u32)L;
             if (pr < pr1) e[k] = __ldcg(reinterpret_cast<const double2*>(src + 2 * pr));
         }
     }
 
-    // dst = eps + (1/r_lj - 1/r_li) for every site l of the slab (PAPER.md:77)
-    __device__ __forceinline__ void update(const CgParams& p, const double* src, double* dst,
-                                           u32 pr0, u32 pr1, u32 hi, u32 hj)
+    __device__ __forceinline__ void issue(const double* __restrict__ tf, u32 mask, u32 pr0, u32 pr1, u32 ci, u32 cj)
     {
-        const int L = p.L, lg = p.lgL, pitch = p.pitch;
-        const int yi = hi >> lg, xi = hi & (L - 1), yj = hj >> lg, xj = hj & (L - 1);
-        if (RP > 0) {
-            double c0[RP > 0 ? RP : 1], c1[RP > 0 ? RP : 1];
+        hci = ci; hcj = cj;
 #pragma unroll
-            for (int k = 0; k < RP; ++k) {            // all table gathers first
-                const u32 pr = pr0 + threadIdx.x + k * THREADS;
-                if (pr < pr1) {
-                    const u32 s = pr * 2;
-                    hop_term2(p.tq, pitch, L, s >> lg, s & (L - 1), yi, xi, yj, xj, c0[k], c1[k]);
-                }
+        for (int k = 0; k < RP; ++k) {
+            const u32 pr = pr0 + threadIdx.x + k * TW;
+            if (pr < pr1) {
+                const double* aj = tf + ((sc[k] - cj) & mask);
+                const double* ai = tf + ((sc[k] - ci) & mask);
+                tj0[k] = __ldg(aj); tj1[k] = __ldg(aj + 1);
+                ti0[k] = __ldg(ai); ti1[k] = __ldg(ai + 1);
             }
+        }
+    }
+
+    // dst = eps + (1/r_lj - 1/r_li) for every site l of the slab (PAPER.md:77)
+    __device__ __forceinline__ void finish(const double* __restrict__ tf, u32 mask, int L, const double* src,
+                                           double* dst, u32 pr0, u32 pr1)
+    {
+        if (RP > 0) {
 #pragma unroll
             for (int k = 0; k < RP; ++k) {
-                const u32 pr = pr0 + threadIdx.x + k * THREADS;
+                const u32 pr = pr0 + threadIdx.x + k * TW;
                 if (pr < pr1) {
-                    e[k].x = __dadd_rn(e[k].x, c0[k]);
-                    e[k].y = __dadd_rn(e[k].y, c1[k]);
+                    e[k].x = __dadd_rn(e[k].x, __dsub_rn(tj0[k], ti0[k]));
+                    e[k].y = __dadd_rn(e[k].y, __dsub_rn(tj1[k], ti1[k]));
                     __stcg(reinterpret_cast<double2*>(dst + 2 * pr), e[k]);
                 }
             }
         } else {
-            for (u32 pr = pr0 + threadIdx.x; pr < pr1; pr += THREADS) {
-                const u32 s = pr * 2;
-                const double2 v = __ldcg(reinterpret_cast<const double2*>(src + s));
-                double a0, a1;
-                hop_term2(p.tq, pitch, L, s >> lg, s & (L - 1), yi, xi, yj, xj, a0, a1);
+            for (u32 pr = pr0 + threadIdx.x; pr < pr1; pr += TW) {
+                const u32 c = site_code(2 * pr, L) | (u32)L;
+                const double* aj = tf + ((c - hcj) & mask);
+                const double* ai = tf + ((c - hci) & mask);
+                const double2 v = __ldcg(reinterpret_cast<const double2*>(src + 2 * pr));
+                const double j0 = __ldg(aj), j1 = __ldg(aj + 1), i0 = __ldg(ai), i1 = __ldg(ai + 1);
                 double2 o;
-                o.x = __dadd_rn(v.x, a0);
-                o.y = __dadd_rn(v.y, a1);
-                __stcg(reinterpret_cast<double2*>(dst + s), o);
+                o.x = __dadd_rn(v.x, __dsub_rn(j0, i0));
+                o.y = __dadd_rn(v.y, __dsub_rn(j1, i1));
+                __stcg(reinterpret_cast<double2*>(dst + 2 * pr), o);
             }
         }
     }
 };
 
+struct Prop {               // one decoded attempt (a pure function of seed and attempt index)
+    u32 i, j, k;            // sites and tower index
+    u32 uh, ul;             // the 53 acceptance bits: u_a = (uh 2^32 + ul) 2^-53, uh < 2^21
+};
+
+struct Tables {             // shared-memory views
+    const u64* cdfi; const double* invr; const double* fld; const int* disp; const u32* guide;
+};
+
+// Tower sampling: smallest k with u_d < cdf_k, u_d = m 2^-43, as the equivalent integer
+// test m < cdfi_k; the guide brackets k from the leading bits of t = 2^43 - m (the tail of the tower is
+// geometric, so a binade of t holds only a few k).
+__device__ __forceinline__ u32 tower_search(const Tables& t, u64 m)
+{
+    const u64 tt = (1ull << 43) - m;
+    const int e = 63 - __clzll((long long)tt);
+    const u32 mant = (e >= 3 ? (u32)(tt >> (e - 3)) : (u32)(tt << (3 - e))) & 7u;
+    const u32 g = t.guide[e * 8 + (int)mant];
+    u32 lo = g & 0xFFFFu, hi = g >> 16;
+    while (lo < hi) {
+        const u32 mid = (lo + hi) >> 1;
+        if (m < t.cdfi[mid]) hi = mid; else lo = mid + 1;
+    }
+    return lo;
+}
+
+__device__ __forceinline__ u32 hop_target(const Tables& t, u32 i, u32 k, int L, int lg)
+{
+    const int d = t.disp[k];
+    const int dy = d >> 16, dx = (int)(short)(d & 0xFFFF);
+    const int yj = ((int)(i >> lg) + dy) & (L - 1), xj = ((int)(i & (L - 1)) + dx) & (L - 1);
+    return ((u32)yj << lg) | (u32)xj;
+}
+
+// Attempt a -> proposal (reading G9): one Philox block, i = (w0 N) >> 32,
+// displacement from 43 bits, acceptance uniform from the remaining 53.
+__device__ __forceinline__ Prop decode_attempt(const Tables& t, const CgParams& p, u64 a)
+{
+    u32 w0, w1, w2, w3;
+    philox4x32_10((u32)a, (u32)(a >> 32), 0u, 0u, p.seed_lo, p.seed_hi, w0, w1, w2, w3);
+    Prop r;
+    r.i = __umulhi(w0, p.N);
+    r.k = tower_search(t, ((u64)w1 << 11) | (u64)(w2 >> 21));
+    r.j = hop_target(t, r.i, r.k, p.L, p.lgL);
+    r.uh = w2 & 0x1FFFFFu; r.ul = w3;
+    return r;
+}
+
+// Eq.(2): for dE > 0 accept iff u_a < exp(-dE/T).  A float estimate with a 2^-10 guard
+// band decides all but near-ties; those take the double-precision path, so the decision is always
+// that of the double comparison.
+__device__ __forceinline__ bool metropolis(double dE, u32 uh, u32 ul, double T, float inv_T)
+{
+    if (dE <= 0.0) return true;
+    const u32 top = (uh << 11) | (ul >> 21);                       // top 32 of the 53 bits
+    const float lo = (float)top * 2.3283064365386963e-10f;         // u_a in [lo, lo + 2^-32)
+    const float xf = (float)(-dE) * inv_T;
+    const float pf = __expf(xf);
+    if (lo > pf * 1.0009765625f) return false;
+    if (xf > -60.f && lo + 4.6566128730773926e-10f < pf * 0.9990234375f) return true;
+    const double ua = (double)(((u64)uh << 32) | (u64)ul) * (1.0 / 9007199254740992.0);
+    return ua < exp(__ddiv_rn(-dE, T));
+}
+
+#define BIT(sn, s) (((sn)[(s) >> 5] >> ((s) & 31)) & 1u)
+
 // The persistent kernel: steps 1, 2, 3a-3c of the mixed PR algorithm.
-template <int THREADS, int RP>
+// CACHED: thread g of the grid owns the attempts a = g (mod P), P = gridDim.x * PL >= M, and keeps
+// its current and its next proposal decoded in registers; an iteration only re-tests them on the
+// current state.  Otherwise CTA b evaluates labels [b per, (b+1) per) from scratch.
+template <int THREADS, int RP, bool CACHED>
 __global__ void __launch_bounds__(THREADS, 1) cg_pr_persistent(const CgParams p)
 {
-    constexpr int NW = THREADS / 32;
+    constexpr int TW = THREADS - 32;      // worker threads; the last warp only publishes slab updates
+    constexpr int NW = TW / 32;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int KL = p.Klive;
     u64* s_cdfi = reinterpret_cast<u64*>(smem_raw);
@@ -215,13 +300,16 @@ __global__ void __launch_bounds__(THREADS, 1) cg_pr_persistent(const CgParams p)
     int* s_disp = reinterpret_cast<int*>(s_fld + KL);
     u32* s_guide = reinterpret_cast<u32*>(s_disp + KL);
     u32* s_n = s_guide + CG_GUIDE;
-    __shared__ u32 s_wlab[32], s_plab[32];
-    __shared__ u64 s_wpay[32], s_ppay[32];
+    __shared__ u32 s_wlab[2][32], s_plab[2];    // indexed by iteration parity: one barrier per iteration
+    __shared__ u64 s_wpay[2][32], s_ppay[2];
+    const Tables tb = {s_cdfi, s_invr, s_fld, s_disp, s_guide};
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const u32 b = blockIdx.x, nb = gridDim.x;
-    const int L = p.L, lg = p.lgL, pitch = p.pitch;
+    const int L = p.L, lg = p.lgL;
     const u32 N = p.N, M = p.M;
+    const u32 mask = ((u32)(L - 1) << (lg + 1)) | (u32)(L - 1);
+    const double* __restrict__ tf = p.tf;
 
     for (int k = tid; k < KL; k += THREADS) {
         s_cdfi[k] = p.cdfi[k]; s_invr[k] = p.invr_k[k]; s_fld[k] = p.fld_k[k]; s_disp[k] = p.disp[k];
@@ -232,177 +320,300 @@ __global__ void __launch_bounds__(THREADS, 1) cg_pr_persistent(const CgParams p)
     // replicated, CTA-uniform control state
     u64 a0 = p.ctl->attempts, hops = p.ctl->hops, iters = p.ctl->iterations, props = p.ctl->proposals;
     long long dP = p.ctl->dP;
-    u32 base = p.ctl->cur;
-    u64 epoch = p.ctl->epoch;
+    const u64 epoch0 = p.ctl->epoch;
     const u64 log_base = p.ctl->log_base;
     const u64 target = hops + p.n_hops;
-    bool pending = false;                 // hop whose term readers must add to eps[base]
-    u64 need_pub = 0;                     // epoch of the hop whose slabs must be complete before eps is read
-    int pyi = 0, pxi = 0, pyj = 0, pxj = 0;
+    // Pending hops.  eps lives in a ring of three buffers: hop h writes eps_h (each CTA its own slab)
+    // into the buffer after the one hop h-1 wrote.  Proposals never read the two newest buffers, which
+    // other CTAs may still be writing: they read eps_{h-2} (buffer rbuf, complete on every CTA: checked
+    // against pub_count) and add the terms 1/r_lj - 1/r_li of the npend <= 2 newest hops themselves, in
+    // hop order - the same single rounded adds the update performs, so the values are bit-identical.
+    u32 rbuf = p.ctl->cur, wbuf = p.ctl->cur;
+    int npend = 0;
+    u32 pci0 = 0, pcj0 = 0, pci1 = 0, pcj1 = 0;   // coded sites of the pending hops, oldest first
+    bool upd = false;                     // slab update issued, not yet finished
+    u32 upd_parity = 0;                   // hops finished in this launch (selects the named barrier)
+    const u64 hops0 = hops;
+    const u64 pub_base0 = p.ctl->pub_base[0], pub_base1 = p.ctl->pub_base[1];
+    // hop number hl of this launch (1-based) is published on counter hl & 1; all CTAs have published it
+    // once that counter reaches its base + nb * ((hl + 1) / 2)
+    u64 need_pub = 0;                     // ... for the hop whose buffer becomes rbuf at the next executed hop
+    u32 need_par = 0;
     u64 cyc_wait = 0, cyc_update = 0, cyc_propose = 0;
     const long long t_begin = clock64();
 
-    const u32 per = (M + nb - 1) / nb;
+    // labels: CTA-blocked (scan order = CTA order) or, CACHED, cyclic in the global thread index
+    const u32 per = CACHED ? p.PL : (M + nb - 1) / nb;
     const u32 lab0 = min(M, b * per), lab1 = min(M, lab0 + per);
+    const u32 P = nb * per;               // CACHED: attempts a = g (mod P) belong to thread g
+    u32 g0 = CACHED ? (u32)(a0 % P) : 0u; // global thread index that holds attempt a0
+    u32 c_first = CACHED ? g0 / per : 0u; // CTA at scan position 0 and the offset of a0 in it
+    u32 t0r = CACHED ? g0 - c_first * per : 0u;
+    u64 a_cur = 0;
+    Prop cur = {0, 0, 0, 0, 0}, nxt = {0, 0, 0, 0, 0};
+    bool nxt_valid = false;
+    const bool has_label = CACHED && (u32)tid < per;
+    __syncthreads();
+    if (warp == NW) {
+        // service warp: once per executed hop, wait until every worker has stored its part of the
+        // slab (named barrier), fence those stores and bump the publication counter - off the
+        // workers' critical path.  Workers run at most two hops ahead of it (the exchange of hop h+2
+        // waits for the publication of hop h by every CTA, this one included), hence two barriers.
+        if (nb > 1)
+            for (u64 h = 0; h < p.n_hops; ++h) {
+                barN_sync(1 + (int)(h & 1), THREADS);
+                if (lane == 0) red_release_add_u64(&p.ctl->pub_count[(h + 1) & 1], 1ull);
+            }
+        return;
+    }
+    if (has_label) {
+        const u32 g = b * per + (u32)tid;
+        a_cur = a0 + (u64)((g + P - g0) % P);
+        cur = decode_attempt(tb, p, a_cur);
+    }
+
     const u32 pairs = N / 2, pper = (pairs + nb - 1) / nb;
     const u32 pr0 = min(pairs, b * pper), pr1 = min(pairs, pr0 + pper);
-    const u32 npw = min((u32)NW, (nb + 31) / 32);       // warps that poll the exchange slots
     u64* const my_slot = p.slots + (size_t)b * CG_SLOT_U64;
 
-    Slab<THREADS, RP> slab;
-    slab.load(p.eps[base], pr0, pr1);
-    __syncthreads();
+    Slab<TW, RP> slab;
+    slab.load(p.eps[rbuf], pr0, pr1, L);
+
+    // finish the issued slab update and hand it to the service warp for publication
+    auto finish_update = [&]() {
+        const u32 src = wbuf == 0 ? 2u : wbuf - 1u;
+        slab.finish(tf, mask, L, p.eps[src], p.eps[wbuf], pr0, pr1);
+        if (nb > 1) barN_arrive(1 + (int)(upd_parity & 1u), THREADS);
+        ++upd_parity;
+        upd = false;
+    };
+
+    u32 it_local = 0;
+    auto trace = [&](int ev, u64 extra) {       // thread 0 of every CTA, first trace_iters iterations
+        if (p.trace && tid == 0 && it_local < p.trace_iters)
+            p.trace[((size_t)b * p.trace_iters + it_local) * CG_TRACE_EV + ev] = ev == 7 ? extra : global_ns();
+    };
 
     while (hops < target) {
         const long long t0 = clock64();
-        const double* __restrict__ erd = p.eps[base];
+        trace(0, 0);
+        const u32 par = it_local & 1u;
+        const u64 epoch = epoch0 + it_local;
+        const double* __restrict__ erd = p.eps[rbuf];
+        const u32 kb = b >= c_first ? b - c_first : b + nb - c_first;    // my scan position
+        u64 pc = 0;
+        if (nb > 1 && tid == 0) pc = ld_relaxed_u64(&p.ctl->pub_count[need_par]);   // checked before the barrier below
         // ---- steps 1-2: propose and test, state untouched
         u32 best = CG_NONE, bi = 0, bj = 0;
-        for (u32 l = lab0 + tid; l < lab1; l += THREADS) {
-            const u64 a = a0 + l;
-            u32 w0, w1, w2, w3;
-            philox4x32_10((u32)a, (u32)(a >> 32), 0u, 0u, p.seed_lo, p.seed_hi, w0, w1, w2, w3);
-            const u32 i = __umulhi(w0, N);                                   // uniform site
-            if (!((s_n[i >> 5] >> (i & 31)) & 1u)) continue;                 // n_i = 1 ?
-            // tower sampling: smallest k with u_d < cdf_k, u_d = m 2^-43, as the
-            // equivalent integer test m < cdfi_k; the guide brackets k from the leading bits of 1 - u_d
-            const u64 m = ((u64)w1 << 11) | (u64)(w2 >> 21);
-            const u64 t = (1ull << 43) - m;
-            const int e = 63 - __clzll((long long)t);
-            const u32 mant = (e >= 3 ? (u32)(t >> (e - 3)) : (u32)(t << (3 - e))) & 7u;
-            const u32 g = s_guide[e * 8 + (int)mant];
-            int lo = (int)(g & 0xFFFFu), hi = (int)(g >> 16);
-            while (lo < hi) {
-                const int mid = (lo + hi) >> 1;
-                if (m < s_cdfi[mid]) hi = mid; else lo = mid + 1;
+        if (CACHED) {
+            const u64 lab = a_cur - a0;
+            const bool th = has_label && lab < (u64)M && BIT(s_n, cur.i) && !BIT(s_n, cur.j);
+            double ei = 0, ej = 0, a_i0 = 0, b_i0 = 0, a_j0 = 0, b_j0 = 0, a_i1 = 0, b_i1 = 0, a_j1 = 0, b_j1 = 0;
+            if (th) {                      // gathers first ...
+                ei = ld_cg(erd + cur.i); ej = ld_cg(erd + cur.j);
+                const u32 sci = site_code(cur.i, L) | (u32)L, scj = site_code(cur.j, L) | (u32)L;
+                if (npend > 0) {
+                    a_i0 = __ldg(tf + ((sci - pcj0) & mask)); b_i0 = __ldg(tf + ((sci - pci0) & mask));
+                    a_j0 = __ldg(tf + ((scj - pcj0) & mask)); b_j0 = __ldg(tf + ((scj - pci0) & mask));
+                }
+                if (npend > 1) {
+                    a_i1 = __ldg(tf + ((sci - pcj1) & mask)); b_i1 = __ldg(tf + ((sci - pci1) & mask));
+                    a_j1 = __ldg(tf + ((scj - pcj1) & mask)); b_j1 = __ldg(tf + ((scj - pci1) & mask));
+                }
             }
-            const int d = s_disp[lo];
-            const int dy = d >> 16, dx = (int)(short)(d & 0xFFFF);
-            const int yi = i >> lg, xi = i & (L - 1);
-            const int yj = (yi + dy) & (L - 1), xj = (xi + dx) & (L - 1);
-            const u32 j = ((u32)yj << lg) | (u32)xj;
-            if ((s_n[j >> 5] >> (j & 31)) & 1u) continue;                    // n_j = 0 ?
-            double ei = ld_cg(erd + i), ej = ld_cg(erd + j);
-            if (pending) {
-                ei = __dadd_rn(ei, hop_term(p.tq, pitch, L, yi, xi, pyi, pxi, pyj, pxj));
-                ej = __dadd_rn(ej, hop_term(p.tq, pitch, L, yj, xj, pyi, pxi, pyj, pxj));
+            if (upd) finish_update();      // ... the slab of the previous hop while they are in flight
+            trace(1, 0);
+            // ... and, while another CTA holds the start of the window (this one only waits for it),
+            // the decode one attempt ahead (state-independent)
+            if (has_label && !nxt_valid && kb != 0) { nxt = decode_attempt(tb, p, a_cur + P); nxt_valid = true; }
+            if (th) {
+                if (npend > 0) { ei = __dadd_rn(ei, __dsub_rn(a_i0, b_i0)); ej = __dadd_rn(ej, __dsub_rn(a_j0, b_j0)); }
+                if (npend > 1) { ei = __dadd_rn(ei, __dsub_rn(a_i1, b_i1)); ej = __dadd_rn(ej, __dsub_rn(a_j1, b_j1)); }
+                // dH_ij = eps_j - eps_i - 1/r_ij - E dx_ij
+                const double dE = __dsub_rn(__dsub_rn(__dsub_rn(ej, ei), s_invr[cur.k]), s_fld[cur.k]);
+                if (metropolis(dE, cur.uh, cur.ul, p.T, p.inv_T)) { best = (u32)lab; bi = cur.i; bj = cur.j; }
             }
-            // dH_ij = eps_j - eps_i - 1/r_ij - E dx_ij
-            const double dE = __dsub_rn(__dsub_rn(__dsub_rn(ej, ei), s_invr[lo]), s_fld[lo]);
-            bool acc = dE <= 0.0;
-            if (!acc) {
-                // Eq.(2): accept iff u_a < exp(-dE/T).  A float estimate with a 2^-10
-                // guard band decides all but near-ties; those take the double-precision path, so the
-                // decision is always that of the double comparison.
-                const u32 uh = ((w2 & 0x1FFFFFu) << 11) | (w3 >> 21);        // top 32 of the 53 bits
-                const float ul = (float)uh * 2.3283064365386963e-10f;        // u_a in [ul, ul + 2^-32)
-                const float xf = (float)(-dE) * p.inv_T;
-                const float pf = __expf(xf);
-                int dec = 0;                                                 // 0 undecided, 1 accept, 2 reject
-                if (ul > pf * 1.0009765625f) dec = 2;
-                else if (xf > -60.f && ul + 4.6566128730773926e-10f < pf * 0.9990234375f) dec = 1;
-                if (dec == 0) {
-                    const double ua = (double)(((u64)(w2 & 0x1FFFFFu) << 32) | (u64)w3)
-                                      * (1.0 / 9007199254740992.0);
-                    acc = ua < exp(__ddiv_rn(-dE, p.T));
-                } else acc = dec == 1;
+        } else {
+            if (upd) finish_update();
+            trace(1, 0);
+            for (u32 l = lab0 + tid; l < lab1; l += TW) {
+                const u64 a = a0 + l;
+                u32 w0, w1, w2, w3;
+                philox4x32_10((u32)a, (u32)(a >> 32), 0u, 0u, p.seed_lo, p.seed_hi, w0, w1, w2, w3);
+                const u32 i = __umulhi(w0, N);                                   // uniform site
+                if (!BIT(s_n, i)) continue;                                      // n_i = 1 ?
+                const u32 k = tower_search(tb, ((u64)w1 << 11) | (u64)(w2 >> 21));
+                const u32 j = hop_target(tb, i, k, L, lg);
+                if (BIT(s_n, j)) continue;                                       // n_j = 0 ?
+                double ei = ld_cg(erd + i), ej = ld_cg(erd + j);
+                const u32 sci = site_code(i, L) | (u32)L, scj = site_code(j, L) | (u32)L;
+                if (npend > 0) {
+                    ei = __dadd_rn(ei, hop_term(tf, mask, sci, pci0, pcj0));
+                    ej = __dadd_rn(ej, hop_term(tf, mask, scj, pci0, pcj0));
+                }
+                if (npend > 1) {
+                    ei = __dadd_rn(ei, hop_term(tf, mask, sci, pci1, pcj1));
+                    ej = __dadd_rn(ej, hop_term(tf, mask, scj, pci1, pcj1));
+                }
+                const double dE = __dsub_rn(__dsub_rn(__dsub_rn(ej, ei), s_invr[k]), s_fld[k]);
+                if (metropolis(dE, w2 & 0x1FFFFFu, w3, p.T, p.inv_T)) { best = l; bi = i; bj = j; break; }
             }
-            if (acc) { best = l; bi = i; bj = j; break; }
         }
         const long long t1 = clock64();
+        trace(2, 0);
+        // the buffer the NEXT iterations gather from must be complete on every CTA before this
+        // CTA passes the barrier below (one thread checks; everybody waits for it there)
+        if (nb > 1 && tid == 0) {
+            while (pc < need_pub) pc = ld_relaxed_u64(&p.ctl->pub_count[need_par]);
+            fence_acquire_gpu();
+        }
         // ---- step 3: lowest accepting label: warp, CTA, grid
         {
             const u32 wmin = __reduce_min_sync(CG_FULL, best);
             const int src = __ffs(__ballot_sync(CG_FULL, best == wmin)) - 1;
-            if (lane == src) { s_wlab[warp] = wmin; s_wpay[warp] = ((u64)bi << 32) | (u64)bj; }
+            if (lane == src) { s_wlab[par][warp] = wmin; s_wpay[par][warp] = ((u64)bi << 32) | (u64)bj; }
         }
-        __syncthreads();
-        if (warp == 0) {
-            const u32 lab = lane < NW ? s_wlab[lane] : CG_NONE;
-            const u64 pay = lane < NW ? s_wpay[lane] : 0ull;
-            const u32 gmin = __reduce_min_sync(CG_FULL, lab);
-            const int src = __ffs(__ballot_sync(CG_FULL, lab == gmin)) - 1;
-            if (lane == src) {
-                if (nb > 1)
-                    slot_store(my_slot, ((u64)(u32)epoch << 32) | gmin,
-                               ((u64)((u32)epoch & 0xFFFFu) << 48) | ((pay >> 32) << 24) | (pay & 0xFFFFFFu));
-                else { s_plab[0] = gmin; s_ppay[0] = pay; }
-            }
-        }
-        if (nb > 1 && warp < npw) {
-            // every slot is watched by one thread; the hop whose slabs the next gathers read must be
-            // published too (pub word, written by each CTA after its eps stores are fenced)
-            u32 plab = CG_NONE; u64 ppay = 0;
-            const u32 e32 = (u32)epoch, e16 = (u32)epoch & 0xFFFFu;
-            for (u32 c = tid; c < nb; c += THREADS) {
-                const u64* sl = p.slots + (size_t)c * CG_SLOT_U64;
-                u64 q0, q1;
-                for (;;) {
-                    slot_load(sl, q0, q1);
-                    const u64 pb = ld_relaxed_u64(sl + 2);
-                    if ((u32)(q0 >> 32) == e32 && (u32)(q1 >> 48) == e16 && pb >= need_pub) break;
-                }
-                if ((u32)q0 < plab) { plab = (u32)q0; ppay = ((q1 >> 24) & 0xFFFFFFull) << 32 | (q1 & 0xFFFFFFull); }
-            }
-            fence_acquire_gpu();
-            const u32 wmin = __reduce_min_sync(CG_FULL, plab);
-            const int src = __ffs(__ballot_sync(CG_FULL, plab == wmin)) - 1;
-            if (lane == src) { s_plab[warp] = wmin; s_ppay[warp] = ppay; }
-        }
-        __syncthreads();
-        u32 q, hi_, hj_;
+        if (p.trace && lane == 0 && it_local < p.trace_iters)     // per-warp "proposals tested" times
+            p.trace[((size_t)b * p.trace_iters + it_local) * CG_TRACE_EV + 8 + (warp & 15)] = global_ns();
+        bar0_sync(TW);
+        // CTA minimum, in every warp
+        u32 gmin; u64 gpay;
         {
-            const u32 lab = (u32)lane < npw ? s_plab[lane] : CG_NONE;
-            const u64 pay = (u32)lane < npw ? s_ppay[lane] : 0ull;
-            q = __reduce_min_sync(CG_FULL, lab);
-            const int src = __ffs(__ballot_sync(CG_FULL, lab == q)) - 1;
-            const u64 wp = __shfl_sync(CG_FULL, pay, src);
-            hi_ = (u32)(wp >> 32); hj_ = (u32)wp;
+            const u32 lab = lane < NW ? s_wlab[par][lane] : CG_NONE;
+            const u64 pay = lane < NW ? s_wpay[par][lane] : 0ull;
+            gmin = __reduce_min_sync(CG_FULL, lab);
+            const int src = __ffs(__ballot_sync(CG_FULL, lab == gmin)) - 1;
+            gpay = __shfl_sync(CG_FULL, pay, src);
         }
+        trace(3, 0);
+        // The grid.  In scan order (CTA order starting at the CTA that holds attempt a0) every CTA holds
+        // lower labels than the next one, except that CACHED the first CTA also holds the end of the
+        // window in its threads below a0's ("tail" labels).  The winner is the first non-tail accept in
+        // scan order; the scan stops there: slots of later CTAs are never waited for (their proposals
+        // cannot win), and the first CTA, when it accepts, waits for nobody.
+        const u32 tail0 = CACHED ? per - t0r : CG_NONE;            // position 0: labels >= tail0 are tail labels
+        const bool own_low = gmin != CG_NONE && (!CACHED || kb != 0 || gmin < tail0);
+        // A CTA can be up to three exchanges ahead of the slowest reader of its slot (bounded by the
+        // publication check and by every fully rejected window, which needs all slots): ring of four.
+        const u32 ring = ((u32)epoch & 3u) * 2u;
+        if (nb > 1 && tid == 0)
+            slot_store(my_slot + ring, ((u64)(u32)epoch << 32) | gmin,
+                       ((u64)((u32)epoch & 0xFFFFu) << 48) | ((gpay >> 32) << 24) | (gpay & 0xFFFFFFu));
+        u32 q = gmin; u64 wp = gpay;
+        if (!(own_low && kb == 0) && nb > 1) {
+            if (warp == 0) {
+                u32 wlab = gmin; u64 wpay = gpay;                      // result if nobody beats it
+                u32 tlab = CG_NONE; u64 tpay = 0;                      // tail accept of position 0
+                const u32 e32 = (u32)epoch, e16 = (u32)epoch & 0xFFFFu;
+                const u32 k_end = own_low ? kb : nb;    // an accept of my own: only earlier CTAs can beat it
+                u32 k0 = 0, width = 4;                  // the winner is almost always in the first CTAs
+                bool found = false;
+                while (!found && k0 < k_end) {
+                    const u32 k = k0 + lane;
+                    const bool mine = k < k_end && (u32)lane < width && k != kb;
+                    u32 c = c_first + k; if (c >= nb) c -= nb;
+                    const u64* sl = p.slots + (size_t)(mine ? c : b) * CG_SLOT_U64 + ring;
+                    bool ready = !mine; u32 l = CG_NONE; u64 q1 = 0;
+                    for (;;) {
+                        if (!ready) {
+                            u64 q0;
+                            slot_load(sl, q0, q1);
+                            if ((u32)(q0 >> 32) == e32 && (u32)(q1 >> 48) == e16) {
+                                ready = true; l = (u32)q0;
+                                if (CACHED && k == 0 && l != CG_NONE && l >= tail0) { tlab = l; tpay = q1; l = CG_NONE; }
+                            }
+                        }
+                        const u32 racc = __ballot_sync(CG_FULL, ready && l != CG_NONE);
+                        const u32 rnot = __ballot_sync(CG_FULL, !ready);
+                        const int fa = racc ? __ffs(racc) - 1 : 32;
+                        const int fn = rnot ? __ffs(rnot) - 1 : 32;
+                        if (fa < fn) {                  // first accepting slot, everything before it rejected
+                            wlab = __shfl_sync(CG_FULL, l, fa);
+                            wpay = __shfl_sync(CG_FULL, q1, fa);
+                            wpay = ((wpay >> 24) & 0xFFFFFFull) << 32 | (wpay & 0xFFFFFFull);
+                            found = true;
+                            break;
+                        }
+                        if (!rnot) break;               // whole chunk rejected: next chunk
+                    }
+                    if (k0 == 0) {                      // position 0 sits in lane 0 of the first chunk
+                        tlab = __shfl_sync(CG_FULL, tlab, 0); tpay = __shfl_sync(CG_FULL, tpay, 0);
+                    }
+                    k0 += width; width = 32;
+                }
+                if (!found && !own_low && kb != 0 && tlab != CG_NONE) {   // only the tail of the window accepted
+                    wlab = tlab; wpay = ((tpay >> 24) & 0xFFFFFFull) << 32 | (tpay & 0xFFFFFFull);
+                }
+                if (lane == 0) { s_plab[par] = wlab; s_ppay[par] = wpay; }
+            }
+            bar0_sync(TW);
+            q = s_plab[par]; wp = s_ppay[par];
+        }
+        const u32 hi_ = (u32)(wp >> 32), hj_ = (u32)wp;
         const long long t2 = clock64();
+        trace(4, 0);
+        trace(7, ((u64)kb << 32) | q);
         ++iters; props += M;
         cyc_propose += (u64)(t1 - t0); cyc_wait += (u64)(t2 - t1);
-        if (q == CG_NONE) { a0 += M; ++epoch; continue; }   // whole window rejected: p += 1
-
-        // ---- step 3a: execute the hop of label q; m = (p-1)M + q attempts used
-        const u64 a_hop = a0 + q;
-        a0 = a_hop + 1;
-        const int yi = hi_ >> lg, xi = hi_ & (L - 1), yj = hj_ >> lg, xj = hj_ & (L - 1);
-        int ddx = (xj - xi) & (L - 1); if (ddx > L / 2) ddx -= L;   // minimum image, tie -> +L/2
-        dP += ddx;                                                   // step 3b: dP = dx (PAPER.md:77)
-        if (tid == 0) {
-            s_n[hi_ >> 5] &= ~(1u << (hi_ & 31));
-            s_n[hj_ >> 5] |= (1u << (hj_ & 31));
-            if (b == 0 && hops - log_base < p.log_cap) {
-                const u64 h = hops - log_base;
-                p.log_a[h] = a_hop; p.log_i[h] = hi_; p.log_j[h] = hj_;
+        // attempts consumed: m = (p-1)M + q per executed hop
+        const u32 used = q == CG_NONE ? M : q + 1;
+        a0 += used;
+        if (CACHED) {
+            if (t0r + used < per) t0r += used;
+            else {
+                g0 = c_first * per + t0r + used; if (g0 >= P) g0 -= P;      // used <= M <= P
+                c_first = g0 / per; t0r = g0 - c_first * per;
+            }
+            if (has_label && a_cur < a0) {          // my attempt was consumed: take the next one
+                if (!nxt_valid) nxt = decode_attempt(tb, p, a_cur + P);
+                cur = nxt; a_cur += P; nxt_valid = false;
             }
         }
-        ++hops;
-        __syncthreads();
-        // ---- step 3b: local energies of my slab, into the other buffer
-        if (pending) base ^= 1u;
-        slab.update(p, p.eps[base], p.eps[base ^ 1u], pr0, pr1, hi_, hj_);
-        pending = true; pyi = yi; pxi = xi; pyj = yj; pxj = xj;
-        need_pub = epoch;
-        if (nb > 1) {
-            // publish "my slab of this hop is written" off the critical path: the last warp waits for
-            // the others' stores (named barrier), fences them and releases the pub word
-            if (warp == NW - 1) {
-                bar1_sync(THREADS);
-                if (lane == 0) st_release_u64(my_slot + 2, epoch);
-            } else bar1_arrive(THREADS);
+        ++it_local;
+        if (q == CG_NONE) continue;                 // whole window rejected: p += 1
+
+        // ---- step 3a: execute the hop of label q
+        const int xi = hi_ & (L - 1), xj = hj_ & (L - 1);
+        int ddx = (xj - xi) & (L - 1); if (ddx > L / 2) ddx -= L;   // minimum image, tie -> +L/2
+        dP += ddx;                                                   // step 3b: dP = dx (PAPER.md:77)
+        if (lane == 0) {                            // every warp flips the bits itself (idempotent), so its
+            atomicAnd(&s_n[hi_ >> 5], ~(1u << (hi_ & 31)));      // own lanes see them without a CTA barrier
+            atomicOr(&s_n[hj_ >> 5], 1u << (hj_ & 31));
+            if (b == 0 && tid == 0 && hops - log_base < p.log_cap) {
+                const u64 h = hops - log_base;
+                p.log_a[h] = a0 - 1; p.log_i[h] = hi_; p.log_j[h] = hj_;
+            }
         }
-        ++epoch;
+        __syncwarp();
+        ++hops;
+        // ---- step 3b: local energies of my slab, into the next buffer of the ring
+        const u32 ci = site_code(hi_, L), cj = site_code(hj_, L);
+        wbuf = wbuf == 2 ? 0u : wbuf + 1u;
+        if (npend == 2) { rbuf = rbuf == 2 ? 0u : rbuf + 1u; pci0 = pci1; pcj0 = pcj1; pci1 = ci; pcj1 = cj; }
+        else if (npend == 1) { pci1 = ci; pcj1 = cj; npend = 2; }
+        else { pci0 = ci; pcj0 = cj; npend = 1; }
+        slab.issue(tf, mask, pr0, pr1, ci, cj);
+        upd = true;
+        {   // all slabs of the hop before this one: they are read (as rbuf) once the NEXT hop is
+            // executed, and awaited before that
+            const u64 hl = hops - hops0 - 1;  // launch-relative number of the hop before this one
+            need_par = (u32)hl & 1u;
+            need_pub = hl == 0 ? 0 : (need_par ? pub_base1 : pub_base0) + (u64)nb * ((hl + 1) / 2);
+        }
         cyc_update += (u64)(clock64() - t2);
+        trace(5, 0);
     }
+    if (upd) finish_update();
 
     if (b == 0) {
-        for (u32 w = tid; w < (N + 31) / 32; w += THREADS) p.nbits[w] = s_n[w];
+        for (u32 w = tid; w < (N + 31) / 32; w += TW) p.nbits[w] = s_n[w];
         if (tid == 0) {
             CgCtl* c = p.ctl;
             c->attempts = a0; c->hops = hops; c->iterations = iters; c->proposals = props;
-            c->dP = dP; c->cur = pending ? (base ^ 1u) : base; c->epoch = epoch;
+            c->dP = dP; c->cur = wbuf; c->epoch = epoch0 + it_local;
+            const u64 H = hops - hops0;
+            c->pub_base[0] = pub_base0 + (u64)nb * (H / 2);
+            c->pub_base[1] = pub_base1 + (u64)nb * ((H + 1) / 2);
             c->cyc_total += (u64)(clock64() - t_begin);
             c->cyc_wait += cyc_wait; c->cyc_update += cyc_update; c->cyc_propose += cyc_propose;
         }
@@ -415,16 +626,19 @@ __global__ void __launch_bounds__(THREADS, 1)
 cg_update_scripted(const CgParams p, const u32* __restrict__ hop_i, const u32* __restrict__ hop_j, u64 count)
 {
     const u32 b = blockIdx.x, nb = gridDim.x;
+    const int L = p.L;
+    const u32 mask = ((u32)(L - 1) << (p.lgL + 1)) | (u32)(L - 1);
     const u32 pairs = p.N / 2, pper = (pairs + nb - 1) / nb;
     const u32 pr0 = min(pairs, b * pper), pr1 = min(pairs, pr0 + pper);
     double* e = p.eps[p.ctl->cur];
     Slab<THREADS, RP> slab;
-    slab.load(e, pr0, pr1);
-    for (u64 h = 0; h < count; ++h)
-        slab.update(p, e, e, pr0, pr1, __ldg(hop_i + h), __ldg(hop_j + h));
+    slab.load(e, pr0, pr1, L);
+    for (u64 h = 0; h < count; ++h) {
+        slab.issue(p.tf, mask, pr0, pr1, site_code(__ldg(hop_i + h), L), site_code(__ldg(hop_j + h), L));
+        slab.finish(p.tf, mask, L, e, e, pr0, pr1);
+    }
     if (b == 0 && threadIdx.x == 0) {       // occupations and dipole moment, in hop order
         long long dP = p.ctl->dP; u32 bad = 0;
-        const int L = p.L;
         for (u64 h = 0; h < count; ++h) {
             const u32 i = hop_i[h], j = hop_j[h];
             const u32 wi = p.nbits[i >> 5], wj = p.nbits[j >> 5];
@@ -435,6 +649,17 @@ cg_update_scripted(const CgParams p, const u32* __restrict__ hop_i, const u32* _
             dP += ddx;
         }
         p.ctl->dP = dP; p.ctl->hops += count; p.ctl->bad_hops += bad;
+    }
+}
+
+// tf from the quarter table (one-time set-up)
+__global__ void cg_build_tf(const double* __restrict__ tq, double* __restrict__ tf, int L, int pitch)
+{
+    const int dy = blockIdx.x;
+    const int fy = min(dy, L - dy);
+    for (int dx = threadIdx.x; dx <= L; dx += blockDim.x) {
+        const int w = dx & (L - 1), fx = min(w, L - w);
+        tf[(size_t)dy * 2 * L + dx] = tq[fy * pitch + fx];
     }
 }
 
@@ -535,15 +760,16 @@ struct cg_sim {
     // device
     cudaStream_t stream = nullptr;
     void* ws = nullptr; bool own_ws = false;
-    double* d_eps[2] = {nullptr, nullptr};
+    double* d_eps[3] = {nullptr, nullptr, nullptr};
     double* d_scratch = nullptr; double* d_phi = nullptr;
-    u32* d_nbits = nullptr; double* d_tq = nullptr;
+    u32* d_nbits = nullptr; double* d_tq = nullptr; double* d_tf = nullptr;
     u64* d_cdfi = nullptr; double* d_invr_k = nullptr; double* d_fld_k = nullptr; int* d_disp = nullptr;
     u32* d_guide = nullptr;
     u64* d_slots = nullptr; CgCtl* d_ctl = nullptr; u64* d_red = nullptr;
     void* d_log = nullptr; bool own_log = false; u64 log_cap = 0;
+    u64* d_trace = nullptr; u32 trace_iters = 0;
     // launch shape
-    int num_sms = 0, n_ctas = 0, threads = 0, smem = 0, rp = 0;
+    int num_sms = 0, n_ctas = 0, threads = 0, smem = 0, rp = 0, pl = 0;   // pl > 0: cached proposals
     std::string err;
 };
 
@@ -568,7 +794,7 @@ static bool valid_L(int L, int* lg)
     return true;
 }
 
-struct WsLayout { size_t eps0, eps1, scratch, phi, nbits, tq, cdfi, invr_k, fld_k, disp, guide, slots, ctl, red, total; };
+struct WsLayout { size_t eps0, eps1, eps2, scratch, phi, nbits, tq, tf, cdfi, invr_k, fld_k, disp, guide, slots, ctl, red, total; };
 #define CG_SLOT_BYTES ((size_t)8 * CG_SLOT_U64 * CG_MAX_CTAS)
 
 static WsLayout ws_layout(int L)
@@ -577,10 +803,12 @@ static WsLayout ws_layout(int L)
     WsLayout w; size_t o = 0;
     w.eps0 = o; o += align256(8 * N);
     w.eps1 = o; o += align256(8 * N);
+    w.eps2 = o; o += align256(8 * N);
     w.scratch = o; o += align256(8 * N);
     w.phi = o; o += align256(8 * N);
     w.nbits = o; o += align256(N / 8 + 4);
     w.tq = o; o += align256(8 * h * h);
+    w.tf = o; o += align256(16 * N);
     w.cdfi = o; o += align256(8 * N);           // tower can never be longer than N entries
     w.invr_k = o; o += align256(8 * N);
     w.fld_k = o; o += align256(8 * N);
@@ -676,8 +904,8 @@ static size_t smem_bytes(const cg_sim* s)
 static CgParams make_params(const cg_sim* s, u64 n_hops)
 {
     CgParams p;
-    p.eps[0] = s->d_eps[0]; p.eps[1] = s->d_eps[1];
-    p.tq = s->d_tq; p.nbits = s->d_nbits;
+    p.eps[0] = s->d_eps[0]; p.eps[1] = s->d_eps[1]; p.eps[2] = s->d_eps[2];
+    p.tf = s->d_tf; p.nbits = s->d_nbits;
     p.cdfi = s->d_cdfi; p.invr_k = s->d_invr_k; p.fld_k = s->d_fld_k; p.disp = s->d_disp;
     p.guide = s->d_guide;
     p.slots = s->d_slots; p.ctl = s->d_ctl;
@@ -686,9 +914,10 @@ static CgParams make_params(const cg_sim* s, u64 n_hops)
     p.log_j = s->d_log ? (u32*)((char*)s->d_log + 12 * s->log_cap) : nullptr;
     p.log_cap = s->d_log ? s->log_cap : 0;
     p.L = s->L; p.lgL = s->lgL; p.pitch = s->pitch; p.Klive = (int)s->Klive;
-    p.N = s->N; p.M = s->M;
+    p.N = s->N; p.M = s->M; p.PL = (u32)s->pl;
     p.seed_lo = (u32)s->seed; p.seed_hi = (u32)(s->seed >> 32);
     p.T = s->T; p.E = s->E; p.inv_T = (float)(1.0 / s->T); p.n_hops = n_hops;
+    p.trace = s->d_trace; p.trace_iters = s->trace_iters;
     return p;
 }
 
@@ -696,24 +925,25 @@ typedef void (*persist_fn)(const CgParams);
 typedef void (*scripted_fn)(const CgParams, const u32*, const u32*, u64);
 
 // RP = eps pairs a thread keeps in registers (0: the slab streams through global memory)
-template <int THREADS>
+template <int THREADS, bool CACHED>
 static persist_fn persistent_kernel_t(int rp)
 {
     switch (rp) {
-        case 0: return cg_pr_persistent<THREADS, 0>;
-        case 1: return cg_pr_persistent<THREADS, 1>;
-        case 2: return cg_pr_persistent<THREADS, 2>;
-        case 4: return cg_pr_persistent<THREADS, 4>;
-        case 8: return cg_pr_persistent<THREADS, 8>;
+        case 0: return cg_pr_persistent<THREADS, 0, CACHED>;
+        case 1: return cg_pr_persistent<THREADS, 1, CACHED>;
+        case 2: return cg_pr_persistent<THREADS, 2, CACHED>;
+        case 4: return cg_pr_persistent<THREADS, 4, CACHED>;
+        case 8: return cg_pr_persistent<THREADS, 8, CACHED>;
     }
     return nullptr;
 }
-static persist_fn persistent_kernel(int threads, int rp)
+static persist_fn persistent_kernel(int threads, int rp, bool cached)
 {
     switch (threads) {
-        case 256: return persistent_kernel_t<256>(rp);
-        case 512: return persistent_kernel_t<512>(rp);
-        case 1024: return rp > 2 ? nullptr : persistent_kernel_t<1024>(rp);
+        case 256: return cached ? persistent_kernel_t<256, true>(rp) : persistent_kernel_t<256, false>(rp);
+        case 512: return cached ? persistent_kernel_t<512, true>(rp) : persistent_kernel_t<512, false>(rp);
+        case 1024: if (rp > 2) return nullptr;
+                   return cached ? persistent_kernel_t<1024, true>(rp) : persistent_kernel_t<1024, false>(rp);
     }
     return nullptr;
 }
@@ -733,22 +963,29 @@ static scripted_fn scripted_kernel(int rp)
 static int choose_rp(u64 pairs, int n_ctas, int threads)
 {
     const u64 per_cta = (pairs + n_ctas - 1) / n_ctas;
-    const u64 need = (per_cta + threads - 1) / threads;
+    const u64 workers = (u64)threads - 32;               // the last warp of a CTA holds no eps
+    const u64 need = (per_cta + workers - 1) / workers;
     const int cap = threads == 1024 ? 2 : 8;
     for (int rp = 1; rp <= cap; rp *= 2)
         if ((u64)rp >= need) return rp;
     return 0;
 }
 
-static int max_coresident(cg_sim* s, int threads, int rp, int* out)
+static int max_coresident(cg_sim* s, int threads, int rp, bool cached, int* out)
 {
-    persist_fn f = persistent_kernel(threads, rp);
+    persist_fn f = persistent_kernel(threads, rp, cached);
     if (!f) return CG_EINVAL;
     CK(cudaFuncSetAttribute((const void*)f, cudaFuncAttributeMaxDynamicSharedMemorySize, s->smem));
     int per_sm = 0;
     CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, (const void*)f, threads, s->smem));
     *out = std::min(per_sm * s->num_sms, CG_MAX_CTAS);
     return CG_OK;
+}
+
+// threads per CTA that own attempts when the proposals can be cached (M <= n_ctas * pl), else 0
+static int choose_pl(u64 M, int n_ctas, int threads)
+{
+    return M <= (u64)n_ctas * (u64)(threads - 32) ? threads - 32 : 0;
 }
 
 static int choose_launch(cg_sim* s, int n_ctas, int threads)
@@ -762,22 +999,22 @@ static int choose_launch(cg_sim* s, int n_ctas, int threads)
         n_ctas = std::max(1, n_ctas);
     }
     if (n_ctas < 1 || n_ctas > CG_MAX_CTAS) return CG_EINVAL;
-    int rp = choose_rp(s->N / 2, n_ctas, threads);
+    int rp = choose_rp(s->N / 2, n_ctas, threads), pl = choose_pl(s->M, n_ctas, threads);
     int cap = 0;
-    int rc = max_coresident(s, threads, rp, &cap);
+    int rc = max_coresident(s, threads, rp, pl > 0, &cap);
     if (rc != CG_OK) return rc;
     if (cap < 1) { s->err = "persistent kernel does not fit on an SM"; return CG_EUNSUPPORTED; }
     if (n_ctas > cap) {
         if (!heuristic) return CG_EINVAL;
         n_ctas = cap;
-        rp = choose_rp(s->N / 2, n_ctas, threads);
-        rc = max_coresident(s, threads, rp, &cap);
+        rp = choose_rp(s->N / 2, n_ctas, threads); pl = choose_pl(s->M, n_ctas, threads);
+        rc = max_coresident(s, threads, rp, pl > 0, &cap);
         if (rc != CG_OK) return rc;
         if (n_ctas > cap) return CG_EUNSUPPORTED;
     }
     if (n_ctas != s->n_ctas)   // slots of CTAs that no longer exist must not look published
         CK(cudaMemsetAsync(s->d_slots, 0, CG_SLOT_BYTES, s->stream));
-    s->n_ctas = n_ctas; s->threads = threads; s->rp = rp;
+    s->n_ctas = n_ctas; s->threads = threads; s->rp = rp; s->pl = pl;
     return CG_OK;
 }
 
@@ -822,8 +1059,9 @@ static int init_impl(cg_sim** out, int L, double W, double xi, double T, double 
     }
     char* base = (char*)s->ws;
     s->d_eps[0] = (double*)(base + w.eps0); s->d_eps[1] = (double*)(base + w.eps1);
+    s->d_eps[2] = (double*)(base + w.eps2);
     s->d_scratch = (double*)(base + w.scratch); s->d_phi = (double*)(base + w.phi);
-    s->d_nbits = (u32*)(base + w.nbits); s->d_tq = (double*)(base + w.tq);
+    s->d_nbits = (u32*)(base + w.nbits); s->d_tq = (double*)(base + w.tq); s->d_tf = (double*)(base + w.tf);
     s->d_cdfi = (u64*)(base + w.cdfi); s->d_invr_k = (double*)(base + w.invr_k);
     s->d_fld_k = (double*)(base + w.fld_k); s->d_guide = (u32*)(base + w.guide);
     s->d_disp = (int*)(base + w.disp); s->d_slots = (u64*)(base + w.slots);
@@ -833,6 +1071,7 @@ static int init_impl(cg_sim** out, int L, double W, double xi, double T, double 
     for (int64_t k = 0; k < s->Klive; ++k) disp[k] = (s->dy[k] << 16) | (s->dx[k] & 0xFFFF);
     cudaStream_t st = s->stream;
     CK(cudaMemcpyAsync(s->d_tq, tq.data(), 8 * tq.size(), cudaMemcpyHostToDevice, st));
+    cg_build_tf<<<L, 256, 0, st>>>(s->d_tq, s->d_tf, L, s->pitch);
     CK(cudaMemcpyAsync(s->d_cdfi, s->cdfi.data(), 8 * (size_t)s->Klive, cudaMemcpyHostToDevice, st));
     CK(cudaMemcpyAsync(s->d_invr_k, s->invr_k.data(), 8 * (size_t)s->Klive, cudaMemcpyHostToDevice, st));
     CK(cudaMemcpyAsync(s->d_fld_k, s->fld_k.data(), 8 * (size_t)s->Klive, cudaMemcpyHostToDevice, st));
@@ -884,7 +1123,7 @@ extern "C" int cg_run(cg_sim* s, uint64_t n_hops)
 {
     if (!s) return CG_EINVAL;
     if (n_hops == 0) return CG_OK;
-    persist_fn f = persistent_kernel(s->threads, s->rp);
+    persist_fn f = persistent_kernel(s->threads, s->rp, s->pl > 0);
     if (!f) return CG_EINVAL;
     CgParams p = make_params(s, n_hops);
     void* args[] = {&p};
@@ -905,7 +1144,7 @@ extern "C" int cg_get_state(cg_sim* s, int8_t* n, double* eps, double* t_tau0, i
     CgCtl c;
     int rc = read_ctl(s, &c);
     if (rc != CG_OK) return rc;
-    if (eps) CK(cudaMemcpyAsync(eps, s->d_eps[c.cur & 1], 8 * (size_t)s->N, cudaMemcpyDeviceToHost, s->stream));
+    if (eps) CK(cudaMemcpyAsync(eps, s->d_eps[c.cur % 3], 8 * (size_t)s->N, cudaMemcpyDeviceToHost, s->stream));
     if (n) {
         std::vector<u32> bits((s->N + 31) / 32);
         CK(cudaMemcpyAsync(bits.data(), s->d_nbits, 4 * bits.size(), cudaMemcpyDeviceToHost, s->stream));
@@ -1006,7 +1245,7 @@ extern "C" int cg_recompute_eps(cg_sim* s, double* max_abs_dev)
     cg_full_sum_eps<<<(s->N + 127) / 128, 128, 0, s->stream>>>(s->d_phi, s->d_nbits, s->d_tq, s->d_scratch,
                                                                s->L, s->lgL, s->pitch, s->N);
     CK(cudaMemsetAsync(s->d_red, 0, 8, s->stream));
-    cg_max_abs_diff<<<std::max(1u, std::min(s->N / 256, 1024u)), 256, 0, s->stream>>>(s->d_scratch, s->d_eps[c.cur & 1],
+    cg_max_abs_diff<<<std::max(1u, std::min(s->N / 256, 1024u)), 256, 0, s->stream>>>(s->d_scratch, s->d_eps[c.cur % 3],
                                                                                      s->N, s->d_red);
     CK(cudaGetLastError());
     u64 bits = 0;
@@ -1097,6 +1336,16 @@ extern "C" int cg_get_launch(cg_sim* s, int* n_ctas, int* threads, int* smem)
     if (n_ctas) *n_ctas = s->n_ctas;
     if (threads) *threads = s->threads;
     if (smem) *smem = s->smem;
+    return CG_OK;
+}
+
+extern "C" int cg_set_trace(cg_sim* s, void* dev_buf, size_t bytes, uint32_t iterations)
+{
+    if (!s) return CG_EINVAL;
+    CK(cudaStreamSynchronize(s->stream));
+    if (!dev_buf || !iterations) { s->d_trace = nullptr; s->trace_iters = 0; return CG_OK; }
+    if (((uintptr_t)dev_buf & 7) || bytes < (size_t)8 * CG_TRACE_EV * iterations * CG_MAX_CTAS) return CG_EINVAL;
+    s->d_trace = (u64*)dev_buf; s->trace_iters = iterations;
     return CG_OK;
 }
 
