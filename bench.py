@@ -245,9 +245,8 @@ def run_ours(args):
         "clocks": clk.summary(),
     }
     tot = max(ph["total"], 1)
-    out["phases"] = {k: ph[k] / tot for k in ("wait", "update", "propose")}
-    out["phases"]["W_U_us_per_hop"] = 1e3 * ms_rank * ph["update"] / tot / c["hops"]
-    out["phases"]["W_R_us_per_hop"] = 1e3 * ms_rank * (ph["propose"] + ph["wait"]) / tot / c["hops"]
+    if ph["update"]:                      # phase timers exist only in a -DCG_TRACE build of the library
+        out["phases"] = {k: ph[k] / tot for k in ("wait", "update", "propose")}
 
     # ---- roofline of the eps update (16 N algorithmic bytes per hop, L2-resident)
     l2_peak = pkg.bench_l2_rmw(16 * N, reps=2000, trials=10)      # 4 MiB = both eps buffers
@@ -276,8 +275,6 @@ def run_ours(args):
     out["roofline_update_kernel"] = {
         "bound": "l2", "kernel": "cg_update_scripted (step a6 alone, %d scripted hops per launch)" % si.size,
         "achieved": upd, "peak": l2_peak, "unit": "GB/s", "frac": upd / l2_peak, "us_per_hop": 1e3 * best / si.size}
-    out["roofline"]["update_phase_achieved"] = 16.0 * N / (out["phases"]["W_U_us_per_hop"] * 1e-6) / 1e9
-    out["roofline"]["update_phase_frac"] = out["roofline"]["update_phase_achieved"] / l2_peak
 
     if world == 1 and not args.no_cpu_baseline:
         r = time_oracle(cfg, args.cpu_seconds, 250)

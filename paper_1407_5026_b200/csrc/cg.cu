@@ -35,6 +35,7 @@ typedef unsigned int u32;
 
 // ------------------------------------------------------------------ device --
 
+#define CG_RING 5           // eps buffers: eps_{h-3} .. eps_{h+1} can be live at the same time
 #define CG_SLOT_U64 32      // one exchange slot per CTA, 256-byte stride (own L2 slice), in u64 units
 #define CG_TRACE_EV 24      // events per iteration in the optional trace (cg_set_trace)
 #define CG_GUIDE 352        // tower guide: (43 + 1) binades x 8 sub-buckets of t = 2^43 - m
@@ -56,7 +57,7 @@ struct CgCtl {              // device-resident control block (one per sim)
 };
 
 struct CgParams {           // kernel parameter block
-    double* eps[3];         // ring of local-energy buffers, N each (see "pending hops" below)
+    double* eps[CG_RING];   // ring of local-energy buffers, N each (see "pending hops" below)
     const double* tf;       // unfolded table 1/r, L rows of pitch 2L (see site_code)
     u32* nbits;             // occupations, bit s of word s/32
     const u64* cdfi;        // live tower as integer thresholds: u_d < cdf_k  <=>  m < cdfi_k
@@ -130,8 +131,16 @@ __device__ __forceinline__ void fence_acquire_gpu() { asm volatile("fence.acquir
 #endif
 // named barriers 1 and 2 (alternating by hop): the warps that wrote eps arrive, the service warp
 // waits for them; barrier 0 with an explicit count synchronises the worker warps only
-__device__ __forceinline__ void barN_arrive(int id, int n) { asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(n) : "memory"); }
-__device__ __forceinline__ void barN_sync(int id, int n) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(n) : "memory"); }
+__device__ __forceinline__ void barN_arrive(bool second, int n)
+{
+    if (second) asm volatile("bar.arrive 2, %0;" ::"r"(n) : "memory");
+    else asm volatile("bar.arrive 1, %0;" ::"r"(n) : "memory");
+}
+__device__ __forceinline__ void barN_sync(bool second, int n)
+{
+    if (second) asm volatile("bar.sync 2, %0;" ::"r"(n) : "memory");
+    else asm volatile("bar.sync 1, %0;" ::"r"(n) : "memory");
+}
 __device__ __forceinline__ void bar0_sync(int n) { asm volatile("bar.sync 0, %0;" ::"r"(n) : "memory"); }
 
 // ---- the unfolded 1/r table ------------------------------------------------------------
@@ -283,10 +292,19 @@ __device__ __forceinline__ bool metropolis(double dE, u32 uh, u32 ul, double T, 
 
 #define BIT(sn, s) (((sn)[(s) >> 5] >> ((s) & 31)) & 1u)
 
+#ifdef CG_TRACE
+#define TRACE(ev, extra) do { if (p.trace && tid == 0 && it_local < p.trace_iters) \
+    p.trace[((size_t)b * p.trace_iters + it_local) * CG_TRACE_EV + (ev)] = (ev) == 7 ? (u64)(extra) : global_ns(); } while (0)
+#else
+#define TRACE(ev, extra) do { } while (0)
+#endif
+
 // The persistent kernel: steps 1, 2, 3a-3c of the mixed PR algorithm.
-// CACHED: thread g of the grid owns the attempts a = g (mod P), P = gridDim.x * PL >= M, and keeps
-// its current and its next proposal decoded in registers; an iteration only re-tests them on the
-// current state.  Otherwise CTA b evaluates labels [b per, (b+1) per) from scratch.
+// CACHED: thread g of the grid owns the attempts a = g (mod P), P = gridDim.x * PL >= M, keeps its
+// current and its next proposal decoded in registers (a proposal is a pure function of the seed and
+// the attempt index) and, while theta_ij = 1, also the two local energies it needs, to which it adds
+// the term of every executed hop itself; an iteration then only re-tests the proposal on the current
+// state.  Otherwise CTA b evaluates labels [b per, (b+1) per) from scratch.
 template <int THREADS, int RP, bool CACHED>
 __global__ void __launch_bounds__(THREADS, 1) cg_pr_persistent(const CgParams p)
 {
@@ -317,41 +335,41 @@ __global__ void __launch_bounds__(THREADS, 1) cg_pr_persistent(const CgParams p)
     for (int k = tid; k < CG_GUIDE; k += THREADS) s_guide[k] = p.guide[k];
     for (u32 w = tid; w < (N + 31) / 32; w += THREADS) s_n[w] = p.nbits[w];
 
-    // replicated, CTA-uniform control state
-    u64 a0 = p.ctl->attempts, hops = p.ctl->hops, iters = p.ctl->iterations, props = p.ctl->proposals;
-    long long dP = p.ctl->dP;
-    const u64 epoch0 = p.ctl->epoch;
-    const u64 log_base = p.ctl->log_base;
-    const u64 target = hops + p.n_hops;
-    // Pending hops.  eps lives in a ring of three buffers: hop h writes eps_h (each CTA its own slab)
-    // into the buffer after the one hop h-1 wrote.  Proposals never read the two newest buffers, which
-    // other CTAs may still be writing: they read eps_{h-2} (buffer rbuf, complete on every CTA: checked
-    // against pub_count) and add the terms 1/r_lj - 1/r_li of the npend <= 2 newest hops themselves, in
-    // hop order - the same single rounded adds the update performs, so the values are bit-identical.
+    // replicated, CTA-uniform control state; 64-bit totals are formed once, after the loop
+    const u64 a_start = p.ctl->attempts;
+    const u64 log_base = p.ctl->log_base, hops_start = p.ctl->hops;
+    const u32 e_start = (u32)p.ctl->epoch;
+    u64 used_sum = 0, hl = 0;             // attempts consumed and hops executed in this launch
+    long long dP = 0;
+    u32 it_local = 0;                     // PR iterations of this launch
+    // Pending hops.  eps lives in a ring of CG_RING buffers: hop h writes eps_h (each CTA its own slab)
+    // into the buffer after the one hop h-1 wrote.  Nobody reads the two newest buffers, which other
+    // CTAs may still be writing: a proposal that starts to follow a pair of sites reads eps_{h-2}
+    // (buffer rbuf, complete on every CTA: checked against pub_count) and adds the terms
+    // 1/r_lj - 1/r_li of the npend <= 2 newest hops itself, in hop order - the same single rounded adds
+    // the update performs, so the values are bit-identical.  A CTA writes eps_{h+1} only when every CTA
+    // has published hop h-1, i.e. reads eps_{h-3} or newer: five buffers are never written while read.
     u32 rbuf = p.ctl->cur, wbuf = p.ctl->cur;
     int npend = 0;
     u32 pci0 = 0, pcj0 = 0, pci1 = 0, pcj1 = 0;   // coded sites of the pending hops, oldest first
     bool upd = false;                     // slab update issued, not yet finished
-    u32 upd_parity = 0;                   // hops finished in this launch (selects the named barrier)
-    const u64 hops0 = hops;
-    const u64 pub_base0 = p.ctl->pub_base[0], pub_base1 = p.ctl->pub_base[1];
-    // hop number hl of this launch (1-based) is published on counter hl & 1; all CTAs have published it
-    // once that counter reaches its base + nb * ((hl + 1) / 2)
+    bool newhop = false;                  // the previous iteration executed a hop
+    // hop number hl of this launch (1-based) is published on counter hl & 1; every CTA has published it
+    // once that counter reaches cnt0 / cnt1 (advanced by nb when the hop is executed)
+    u64 cnt0 = p.ctl->pub_base[0], cnt1 = p.ctl->pub_base[1];
     u64 need_pub = 0;                     // ... for the hop whose buffer becomes rbuf at the next executed hop
     u32 need_par = 0;
+#ifdef CG_TRACE
     u64 cyc_wait = 0, cyc_update = 0, cyc_propose = 0;
+#endif
     const long long t_begin = clock64();
 
     // labels: CTA-blocked (scan order = CTA order) or, CACHED, cyclic in the global thread index
     const u32 per = CACHED ? p.PL : (M + nb - 1) / nb;
     const u32 lab0 = min(M, b * per), lab1 = min(M, lab0 + per);
     const u32 P = nb * per;               // CACHED: attempts a = g (mod P) belong to thread g
-    u32 g0 = CACHED ? (u32)(a0 % P) : 0u; // global thread index that holds attempt a0
-    u32 c_first = CACHED ? g0 / per : 0u; // CTA at scan position 0 and the offset of a0 in it
-    u32 t0r = CACHED ? g0 - c_first * per : 0u;
-    u64 a_cur = 0;
-    Prop cur = {0, 0, 0, 0, 0}, nxt = {0, 0, 0, 0, 0};
-    bool nxt_valid = false;
+    u32 c_first = 0, t0r = 0;             // CACHED: CTA at scan position 0 and the offset of a0 in it
+    if (CACHED) { const u32 g0 = (u32)(a_start % P); c_first = g0 / per; t0r = g0 - c_first * per; }
     const bool has_label = CACHED && (u32)tid < per;
     __syncthreads();
     if (warp == NW) {
@@ -361,15 +379,31 @@ __global__ void __launch_bounds__(THREADS, 1) cg_pr_persistent(const CgParams p)
         // waits for the publication of hop h by every CTA, this one included), hence two barriers.
         if (nb > 1)
             for (u64 h = 0; h < p.n_hops; ++h) {
-                barN_sync(1 + (int)(h & 1), THREADS);
+                barN_sync((h & 1) != 0, THREADS);
                 if (lane == 0) red_release_add_u64(&p.ctl->pub_count[(h + 1) & 1], 1ull);
             }
         return;
     }
+    // CACHED per-thread state: label of my attempt relative to the window start, the decoded proposal
+    // and what its test needs; the attempt after it, decoded ahead when there is idle time
+    u32 lab = CG_NONE;
+    u64 a_cur = 0;
+    u32 ci_ = 0, cj_ = 0, sci = 0, scj = 0, cuh = 0, cul = 0;
+    double c_invr = 0, c_fld = 0, ei = 0, ej = 0;
+    bool tracked = false;                 // ei, ej hold the current local energies of my two sites
+    Prop nxt = {0, 0, 0, 0, 0};
+    bool nxt_valid = false;
+    auto take = [&](const Prop& q) {
+        ci_ = q.i; cj_ = q.j; cuh = q.uh; cul = q.ul;
+        sci = site_code(q.i, L) | (u32)L; scj = site_code(q.j, L) | (u32)L;
+        c_invr = s_invr[q.k]; c_fld = s_fld[q.k];
+        tracked = false;
+    };
     if (has_label) {
-        const u32 g = b * per + (u32)tid;
-        a_cur = a0 + (u64)((g + P - g0) % P);
-        cur = decode_attempt(tb, p, a_cur);
+        const u32 g = b * per + (u32)tid, g0 = c_first * per + t0r;
+        lab = g >= g0 ? g - g0 : g + P - g0;
+        a_cur = a_start + lab;
+        take(decode_attempt(tb, p, a_cur));
     }
 
     const u32 pairs = N / 2, pper = (pairs + nb - 1) / nb;
@@ -381,24 +415,19 @@ __global__ void __launch_bounds__(THREADS, 1) cg_pr_persistent(const CgParams p)
 
     // finish the issued slab update and hand it to the service warp for publication
     auto finish_update = [&]() {
-        const u32 src = wbuf == 0 ? 2u : wbuf - 1u;
+        const u32 src = wbuf == 0 ? CG_RING - 1u : wbuf - 1u;
         slab.finish(tf, mask, L, p.eps[src], p.eps[wbuf], pr0, pr1);
-        if (nb > 1) barN_arrive(1 + (int)(upd_parity & 1u), THREADS);
-        ++upd_parity;
+        if (nb > 1) barN_arrive((hl & 1) == 0, THREADS);         // hop hl (1-based) on barrier 1 + ((hl - 1) & 1)
         upd = false;
     };
 
-    u32 it_local = 0;
-    auto trace = [&](int ev, u64 extra) {       // thread 0 of every CTA, first trace_iters iterations
-        if (p.trace && tid == 0 && it_local < p.trace_iters)
-            p.trace[((size_t)b * p.trace_iters + it_local) * CG_TRACE_EV + ev] = ev == 7 ? extra : global_ns();
-    };
-
-    while (hops < target) {
+    while (hl < p.n_hops) {
+#ifdef CG_TRACE
         const long long t0 = clock64();
-        trace(0, 0);
+#endif
+        TRACE(0, 0);
         const u32 par = it_local & 1u;
-        const u64 epoch = epoch0 + it_local;
+        const u32 e32 = e_start + it_local;
         const double* __restrict__ erd = p.eps[rbuf];
         const u32 kb = b >= c_first ? b - c_first : b + nb - c_first;    // my scan position
         u64 pc = 0;
@@ -406,38 +435,50 @@ __global__ void __launch_bounds__(THREADS, 1) cg_pr_persistent(const CgParams p)
         // ---- steps 1-2: propose and test, state untouched
         u32 best = CG_NONE, bi = 0, bj = 0;
         if (CACHED) {
-            const u64 lab = a_cur - a0;
-            const bool th = has_label && lab < (u64)M && BIT(s_n, cur.i) && !BIT(s_n, cur.j);
-            double ei = 0, ej = 0, a_i0 = 0, b_i0 = 0, a_j0 = 0, b_j0 = 0, a_i1 = 0, b_i1 = 0, a_j1 = 0, b_j1 = 0;
+            const bool th = lab < M && BIT(s_n, ci_) && !BIT(s_n, cj_);   // theta_ij, inside the window
+            double ga = 0, gb = 0, a_i0 = 0, b_i0 = 0, a_j0 = 0, b_j0 = 0, a_i1 = 0, b_i1 = 0, a_j1 = 0, b_j1 = 0;
             if (th) {                      // gathers first ...
-                ei = ld_cg(erd + cur.i); ej = ld_cg(erd + cur.j);
-                const u32 sci = site_code(cur.i, L) | (u32)L, scj = site_code(cur.j, L) | (u32)L;
-                if (npend > 0) {
-                    a_i0 = __ldg(tf + ((sci - pcj0) & mask)); b_i0 = __ldg(tf + ((sci - pci0) & mask));
-                    a_j0 = __ldg(tf + ((scj - pcj0) & mask)); b_j0 = __ldg(tf + ((scj - pci0) & mask));
-                }
-                if (npend > 1) {
-                    a_i1 = __ldg(tf + ((sci - pcj1) & mask)); b_i1 = __ldg(tf + ((sci - pci1) & mask));
-                    a_j1 = __ldg(tf + ((scj - pcj1) & mask)); b_j1 = __ldg(tf + ((scj - pci1) & mask));
+                if (tracked) {
+                    if (newhop) {          // the term of the hop executed last iteration
+                        const u32 hc_i = npend > 1 ? pci1 : pci0, hc_j = npend > 1 ? pcj1 : pcj0;
+                        a_i0 = __ldg(tf + ((sci - hc_j) & mask)); b_i0 = __ldg(tf + ((sci - hc_i) & mask));
+                        a_j0 = __ldg(tf + ((scj - hc_j) & mask)); b_j0 = __ldg(tf + ((scj - hc_i) & mask));
+                    }
+                } else {                   // start to follow (i, j): complete buffer + all pending hops
+                    ga = ld_cg(erd + ci_); gb = ld_cg(erd + cj_);
+                    if (npend > 0) {
+                        a_i0 = __ldg(tf + ((sci - pcj0) & mask)); b_i0 = __ldg(tf + ((sci - pci0) & mask));
+                        a_j0 = __ldg(tf + ((scj - pcj0) & mask)); b_j0 = __ldg(tf + ((scj - pci0) & mask));
+                    }
+                    if (npend > 1) {
+                        a_i1 = __ldg(tf + ((sci - pcj1) & mask)); b_i1 = __ldg(tf + ((sci - pci1) & mask));
+                        a_j1 = __ldg(tf + ((scj - pcj1) & mask)); b_j1 = __ldg(tf + ((scj - pci1) & mask));
+                    }
                 }
             }
             if (upd) finish_update();      // ... the slab of the previous hop while they are in flight
-            trace(1, 0);
+            TRACE(1, 0);
             // ... and, while another CTA holds the start of the window (this one only waits for it),
-            // the decode one attempt ahead (state-independent)
+            // the decode one attempt ahead
             if (has_label && !nxt_valid && kb != 0) { nxt = decode_attempt(tb, p, a_cur + P); nxt_valid = true; }
             if (th) {
-                if (npend > 0) { ei = __dadd_rn(ei, __dsub_rn(a_i0, b_i0)); ej = __dadd_rn(ej, __dsub_rn(a_j0, b_j0)); }
-                if (npend > 1) { ei = __dadd_rn(ei, __dsub_rn(a_i1, b_i1)); ej = __dadd_rn(ej, __dsub_rn(a_j1, b_j1)); }
+                if (tracked) {
+                    if (newhop) { ei = __dadd_rn(ei, __dsub_rn(a_i0, b_i0)); ej = __dadd_rn(ej, __dsub_rn(a_j0, b_j0)); }
+                } else {
+                    ei = ga; ej = gb;
+                    if (npend > 0) { ei = __dadd_rn(ei, __dsub_rn(a_i0, b_i0)); ej = __dadd_rn(ej, __dsub_rn(a_j0, b_j0)); }
+                    if (npend > 1) { ei = __dadd_rn(ei, __dsub_rn(a_i1, b_i1)); ej = __dadd_rn(ej, __dsub_rn(a_j1, b_j1)); }
+                    tracked = true;
+                }
                 // dH_ij = eps_j - eps_i - 1/r_ij - E dx_ij
-                const double dE = __dsub_rn(__dsub_rn(__dsub_rn(ej, ei), s_invr[cur.k]), s_fld[cur.k]);
-                if (metropolis(dE, cur.uh, cur.ul, p.T, p.inv_T)) { best = (u32)lab; bi = cur.i; bj = cur.j; }
-            }
+                const double dE = __dsub_rn(__dsub_rn(__dsub_rn(ej, ei), c_invr), c_fld);
+                if (metropolis(dE, cuh, cul, p.T, p.inv_T)) { best = lab; bi = ci_; bj = cj_; }
+            } else tracked = false;
         } else {
             if (upd) finish_update();
-            trace(1, 0);
+            TRACE(1, 0);
             for (u32 l = lab0 + tid; l < lab1; l += TW) {
-                const u64 a = a0 + l;
+                const u64 a = a_start + used_sum + l;
                 u32 w0, w1, w2, w3;
                 philox4x32_10((u32)a, (u32)(a >> 32), 0u, 0u, p.seed_lo, p.seed_hi, w0, w1, w2, w3);
                 const u32 i = __umulhi(w0, N);                                   // uniform site
@@ -445,24 +486,26 @@ __global__ void __launch_bounds__(THREADS, 1) cg_pr_persistent(const CgParams p)
                 const u32 k = tower_search(tb, ((u64)w1 << 11) | (u64)(w2 >> 21));
                 const u32 j = hop_target(tb, i, k, L, lg);
                 if (BIT(s_n, j)) continue;                                       // n_j = 0 ?
-                double ei = ld_cg(erd + i), ej = ld_cg(erd + j);
-                const u32 sci = site_code(i, L) | (u32)L, scj = site_code(j, L) | (u32)L;
+                double vi = ld_cg(erd + i), vj = ld_cg(erd + j);
+                const u32 si = site_code(i, L) | (u32)L, sj = site_code(j, L) | (u32)L;
                 if (npend > 0) {
-                    ei = __dadd_rn(ei, hop_term(tf, mask, sci, pci0, pcj0));
-                    ej = __dadd_rn(ej, hop_term(tf, mask, scj, pci0, pcj0));
+                    vi = __dadd_rn(vi, hop_term(tf, mask, si, pci0, pcj0));
+                    vj = __dadd_rn(vj, hop_term(tf, mask, sj, pci0, pcj0));
                 }
                 if (npend > 1) {
-                    ei = __dadd_rn(ei, hop_term(tf, mask, sci, pci1, pcj1));
-                    ej = __dadd_rn(ej, hop_term(tf, mask, scj, pci1, pcj1));
+                    vi = __dadd_rn(vi, hop_term(tf, mask, si, pci1, pcj1));
+                    vj = __dadd_rn(vj, hop_term(tf, mask, sj, pci1, pcj1));
                 }
-                const double dE = __dsub_rn(__dsub_rn(__dsub_rn(ej, ei), s_invr[k]), s_fld[k]);
+                const double dE = __dsub_rn(__dsub_rn(__dsub_rn(vj, vi), s_invr[k]), s_fld[k]);
                 if (metropolis(dE, w2 & 0x1FFFFFu, w3, p.T, p.inv_T)) { best = l; bi = i; bj = j; break; }
             }
         }
+#ifdef CG_TRACE
         const long long t1 = clock64();
-        trace(2, 0);
-        // the buffer the NEXT iterations gather from must be complete on every CTA before this
-        // CTA passes the barrier below (one thread checks; everybody waits for it there)
+#endif
+        TRACE(2, 0);
+        // the buffer that becomes rbuf at the next executed hop must be complete on every CTA before
+        // this CTA passes the barrier below (one thread checks; everybody waits for it there)
         if (nb > 1 && tid == 0) {
             while (pc < need_pub) pc = ld_relaxed_u64(&p.ctl->pub_count[need_par]);
             fence_acquire_gpu();
@@ -473,19 +516,21 @@ __global__ void __launch_bounds__(THREADS, 1) cg_pr_persistent(const CgParams p)
             const int src = __ffs(__ballot_sync(CG_FULL, best == wmin)) - 1;
             if (lane == src) { s_wlab[par][warp] = wmin; s_wpay[par][warp] = ((u64)bi << 32) | (u64)bj; }
         }
+#ifdef CG_TRACE
         if (p.trace && lane == 0 && it_local < p.trace_iters)     // per-warp "proposals tested" times
             p.trace[((size_t)b * p.trace_iters + it_local) * CG_TRACE_EV + 8 + (warp & 15)] = global_ns();
+#endif
         bar0_sync(TW);
         // CTA minimum, in every warp
         u32 gmin; u64 gpay;
         {
-            const u32 lab = lane < NW ? s_wlab[par][lane] : CG_NONE;
+            const u32 l_ = lane < NW ? s_wlab[par][lane] : CG_NONE;
             const u64 pay = lane < NW ? s_wpay[par][lane] : 0ull;
-            gmin = __reduce_min_sync(CG_FULL, lab);
-            const int src = __ffs(__ballot_sync(CG_FULL, lab == gmin)) - 1;
+            gmin = __reduce_min_sync(CG_FULL, l_);
+            const int src = __ffs(__ballot_sync(CG_FULL, l_ == gmin)) - 1;
             gpay = __shfl_sync(CG_FULL, pay, src);
         }
-        trace(3, 0);
+        TRACE(3, 0);
         // The grid.  In scan order (CTA order starting at the CTA that holds attempt a0) every CTA holds
         // lower labels than the next one, except that CACHED the first CTA also holds the end of the
         // window in its threads below a0's ("tail" labels).  The winner is the first non-tail accept in
@@ -495,16 +540,16 @@ __global__ void __launch_bounds__(THREADS, 1) cg_pr_persistent(const CgParams p)
         const bool own_low = gmin != CG_NONE && (!CACHED || kb != 0 || gmin < tail0);
         // A CTA can be up to three exchanges ahead of the slowest reader of its slot (bounded by the
         // publication check and by every fully rejected window, which needs all slots): ring of four.
-        const u32 ring = ((u32)epoch & 3u) * 2u;
+        const u32 ring = (e32 & 3u) * 2u;
         if (nb > 1 && tid == 0)
-            slot_store(my_slot + ring, ((u64)(u32)epoch << 32) | gmin,
-                       ((u64)((u32)epoch & 0xFFFFu) << 48) | ((gpay >> 32) << 24) | (gpay & 0xFFFFFFu));
+            slot_store(my_slot + ring, ((u64)e32 << 32) | gmin,
+                       ((u64)(e32 & 0xFFFFu) << 48) | ((gpay >> 32) << 24) | (gpay & 0xFFFFFFu));
         u32 q = gmin; u64 wp = gpay;
         if (!(own_low && kb == 0) && nb > 1) {
             if (warp == 0) {
                 u32 wlab = gmin; u64 wpay = gpay;                      // result if nobody beats it
                 u32 tlab = CG_NONE; u64 tpay = 0;                      // tail accept of position 0
-                const u32 e32 = (u32)epoch, e16 = (u32)epoch & 0xFFFFu;
+                const u32 e16 = e32 & 0xFFFFu;
                 const u32 k_end = own_low ? kb : nb;    // an accept of my own: only earlier CTAs can beat it
                 u32 k0 = 0, width = 4;                  // the winner is almost always in the first CTAs
                 bool found = false;
@@ -550,27 +595,33 @@ __global__ void __launch_bounds__(THREADS, 1) cg_pr_persistent(const CgParams p)
             q = s_plab[par]; wp = s_ppay[par];
         }
         const u32 hi_ = (u32)(wp >> 32), hj_ = (u32)wp;
+#ifdef CG_TRACE
         const long long t2 = clock64();
-        trace(4, 0);
-        trace(7, ((u64)kb << 32) | q);
-        ++iters; props += M;
         cyc_propose += (u64)(t1 - t0); cyc_wait += (u64)(t2 - t1);
+#endif
+        TRACE(4, 0);
+        TRACE(7, ((u64)kb << 32) | q);
         // attempts consumed: m = (p-1)M + q per executed hop
         const u32 used = q == CG_NONE ? M : q + 1;
-        a0 += used;
+        used_sum += used;
+        ++it_local;
         if (CACHED) {
             if (t0r + used < per) t0r += used;
             else {
-                g0 = c_first * per + t0r + used; if (g0 >= P) g0 -= P;      // used <= M <= P
+                u32 g0 = c_first * per + t0r + used; if (g0 >= P) g0 -= P;      // used <= M <= P
                 c_first = g0 / per; t0r = g0 - c_first * per;
             }
-            if (has_label && a_cur < a0) {          // my attempt was consumed: take the next one
-                if (!nxt_valid) nxt = decode_attempt(tb, p, a_cur + P);
-                cur = nxt; a_cur += P; nxt_valid = false;
+            if (has_label) {
+                if (lab >= used) lab -= used;
+                else {                              // my attempt was consumed: take the next one
+                    lab += P - used;
+                    if (!nxt_valid) nxt = decode_attempt(tb, p, a_cur + P);
+                    take(nxt); a_cur += P; nxt_valid = false;
+                }
             }
         }
-        ++it_local;
-        if (q == CG_NONE) continue;                 // whole window rejected: p += 1
+        newhop = q != CG_NONE;
+        if (!newhop) continue;                      // whole window rejected: p += 1
 
         // ---- step 3a: execute the hop of label q
         const int xi = hi_ & (L - 1), xj = hj_ & (L - 1);
@@ -579,29 +630,29 @@ __global__ void __launch_bounds__(THREADS, 1) cg_pr_persistent(const CgParams p)
         if (lane == 0) {                            // every warp flips the bits itself (idempotent), so its
             atomicAnd(&s_n[hi_ >> 5], ~(1u << (hi_ & 31)));      // own lanes see them without a CTA barrier
             atomicOr(&s_n[hj_ >> 5], 1u << (hj_ & 31));
-            if (b == 0 && tid == 0 && hops - log_base < p.log_cap) {
-                const u64 h = hops - log_base;
-                p.log_a[h] = a0 - 1; p.log_i[h] = hi_; p.log_j[h] = hj_;
+            if (b == 0 && tid == 0 && hops_start + hl - log_base < p.log_cap) {
+                const u64 h = hops_start + hl - log_base;
+                p.log_a[h] = a_start + used_sum - 1; p.log_i[h] = hi_; p.log_j[h] = hj_;
             }
         }
         __syncwarp();
-        ++hops;
+        ++hl;
         // ---- step 3b: local energies of my slab, into the next buffer of the ring
         const u32 ci = site_code(hi_, L), cj = site_code(hj_, L);
-        wbuf = wbuf == 2 ? 0u : wbuf + 1u;
-        if (npend == 2) { rbuf = rbuf == 2 ? 0u : rbuf + 1u; pci0 = pci1; pcj0 = pcj1; pci1 = ci; pcj1 = cj; }
+        wbuf = wbuf == CG_RING - 1 ? 0u : wbuf + 1u;
+        if (npend == 2) { rbuf = rbuf == CG_RING - 1 ? 0u : rbuf + 1u; pci0 = pci1; pcj0 = pcj1; pci1 = ci; pcj1 = cj; }
         else if (npend == 1) { pci1 = ci; pcj1 = cj; npend = 2; }
         else { pci0 = ci; pcj0 = cj; npend = 1; }
         slab.issue(tf, mask, pr0, pr1, ci, cj);
         upd = true;
-        {   // all slabs of the hop before this one: they are read (as rbuf) once the NEXT hop is
-            // executed, and awaited before that
-            const u64 hl = hops - hops0 - 1;  // launch-relative number of the hop before this one
-            need_par = (u32)hl & 1u;
-            need_pub = hl == 0 ? 0 : (need_par ? pub_base1 : pub_base0) + (u64)nb * ((hl + 1) / 2);
-        }
+        // all slabs of the hop before this one: they are read (as rbuf) once the NEXT hop is executed,
+        // and awaited before that
+        if (hl & 1) { cnt1 += nb; need_pub = cnt0; need_par = 0; }
+        else { cnt0 += nb; need_pub = cnt1; need_par = 1; }
+#ifdef CG_TRACE
         cyc_update += (u64)(clock64() - t2);
-        trace(5, 0);
+#endif
+        TRACE(5, 0);
     }
     if (upd) finish_update();
 
@@ -609,13 +660,14 @@ __global__ void __launch_bounds__(THREADS, 1) cg_pr_persistent(const CgParams p)
         for (u32 w = tid; w < (N + 31) / 32; w += TW) p.nbits[w] = s_n[w];
         if (tid == 0) {
             CgCtl* c = p.ctl;
-            c->attempts = a0; c->hops = hops; c->iterations = iters; c->proposals = props;
-            c->dP = dP; c->cur = wbuf; c->epoch = epoch0 + it_local;
-            const u64 H = hops - hops0;
-            c->pub_base[0] = pub_base0 + (u64)nb * (H / 2);
-            c->pub_base[1] = pub_base1 + (u64)nb * ((H + 1) / 2);
+            c->attempts = a_start + used_sum; c->hops = hops_start + hl;
+            c->iterations += it_local; c->proposals += (u64)M * it_local;
+            c->dP += dP; c->cur = wbuf; c->epoch += it_local;
+            c->pub_base[0] = cnt0; c->pub_base[1] = cnt1;
             c->cyc_total += (u64)(clock64() - t_begin);
+#ifdef CG_TRACE
             c->cyc_wait += cyc_wait; c->cyc_update += cyc_update; c->cyc_propose += cyc_propose;
+#endif
         }
     }
 }
@@ -760,7 +812,7 @@ struct cg_sim {
     // device
     cudaStream_t stream = nullptr;
     void* ws = nullptr; bool own_ws = false;
-    double* d_eps[3] = {nullptr, nullptr, nullptr};
+    double* d_eps[CG_RING] = {};
     double* d_scratch = nullptr; double* d_phi = nullptr;
     u32* d_nbits = nullptr; double* d_tq = nullptr; double* d_tf = nullptr;
     u64* d_cdfi = nullptr; double* d_invr_k = nullptr; double* d_fld_k = nullptr; int* d_disp = nullptr;
@@ -794,16 +846,14 @@ static bool valid_L(int L, int* lg)
     return true;
 }
 
-struct WsLayout { size_t eps0, eps1, eps2, scratch, phi, nbits, tq, tf, cdfi, invr_k, fld_k, disp, guide, slots, ctl, red, total; };
+struct WsLayout { size_t eps0, scratch, phi, nbits, tq, tf, cdfi, invr_k, fld_k, disp, guide, slots, ctl, red, total; };
 #define CG_SLOT_BYTES ((size_t)8 * CG_SLOT_U64 * CG_MAX_CTAS)
 
 static WsLayout ws_layout(int L)
 {
     const size_t N = (size_t)L * L, h = (size_t)L / 2 + 1;
     WsLayout w; size_t o = 0;
-    w.eps0 = o; o += align256(8 * N);
-    w.eps1 = o; o += align256(8 * N);
-    w.eps2 = o; o += align256(8 * N);
+    w.eps0 = o; o += CG_RING * align256(8 * N);
     w.scratch = o; o += align256(8 * N);
     w.phi = o; o += align256(8 * N);
     w.nbits = o; o += align256(N / 8 + 4);
@@ -904,7 +954,7 @@ static size_t smem_bytes(const cg_sim* s)
 static CgParams make_params(const cg_sim* s, u64 n_hops)
 {
     CgParams p;
-    p.eps[0] = s->d_eps[0]; p.eps[1] = s->d_eps[1]; p.eps[2] = s->d_eps[2];
+    for (int k = 0; k < CG_RING; ++k) p.eps[k] = s->d_eps[k];
     p.tf = s->d_tf; p.nbits = s->d_nbits;
     p.cdfi = s->d_cdfi; p.invr_k = s->d_invr_k; p.fld_k = s->d_fld_k; p.disp = s->d_disp;
     p.guide = s->d_guide;
@@ -1058,8 +1108,7 @@ static int init_impl(cg_sim** out, int L, double W, double xi, double T, double 
         s->ws = dev_ws;
     }
     char* base = (char*)s->ws;
-    s->d_eps[0] = (double*)(base + w.eps0); s->d_eps[1] = (double*)(base + w.eps1);
-    s->d_eps[2] = (double*)(base + w.eps2);
+    for (int k = 0; k < CG_RING; ++k) s->d_eps[k] = (double*)(base + w.eps0 + (size_t)k * align256(8 * (size_t)s->N));
     s->d_scratch = (double*)(base + w.scratch); s->d_phi = (double*)(base + w.phi);
     s->d_nbits = (u32*)(base + w.nbits); s->d_tq = (double*)(base + w.tq); s->d_tf = (double*)(base + w.tf);
     s->d_cdfi = (u64*)(base + w.cdfi); s->d_invr_k = (double*)(base + w.invr_k);
@@ -1144,7 +1193,7 @@ extern "C" int cg_get_state(cg_sim* s, int8_t* n, double* eps, double* t_tau0, i
     CgCtl c;
     int rc = read_ctl(s, &c);
     if (rc != CG_OK) return rc;
-    if (eps) CK(cudaMemcpyAsync(eps, s->d_eps[c.cur % 3], 8 * (size_t)s->N, cudaMemcpyDeviceToHost, s->stream));
+    if (eps) CK(cudaMemcpyAsync(eps, s->d_eps[c.cur % CG_RING], 8 * (size_t)s->N, cudaMemcpyDeviceToHost, s->stream));
     if (n) {
         std::vector<u32> bits((s->N + 31) / 32);
         CK(cudaMemcpyAsync(bits.data(), s->d_nbits, 4 * bits.size(), cudaMemcpyDeviceToHost, s->stream));
@@ -1245,7 +1294,7 @@ extern "C" int cg_recompute_eps(cg_sim* s, double* max_abs_dev)
     cg_full_sum_eps<<<(s->N + 127) / 128, 128, 0, s->stream>>>(s->d_phi, s->d_nbits, s->d_tq, s->d_scratch,
                                                                s->L, s->lgL, s->pitch, s->N);
     CK(cudaMemsetAsync(s->d_red, 0, 8, s->stream));
-    cg_max_abs_diff<<<std::max(1u, std::min(s->N / 256, 1024u)), 256, 0, s->stream>>>(s->d_scratch, s->d_eps[c.cur % 3],
+    cg_max_abs_diff<<<std::max(1u, std::min(s->N / 256, 1024u)), 256, 0, s->stream>>>(s->d_scratch, s->d_eps[c.cur % CG_RING],
                                                                                      s->N, s->d_red);
     CK(cudaGetLastError());
     u64 bits = 0;
@@ -1344,6 +1393,9 @@ extern "C" int cg_set_trace(cg_sim* s, void* dev_buf, size_t bytes, uint32_t ite
     if (!s) return CG_EINVAL;
     CK(cudaStreamSynchronize(s->stream));
     if (!dev_buf || !iterations) { s->d_trace = nullptr; s->trace_iters = 0; return CG_OK; }
+#ifndef CG_TRACE
+    return CG_EUNSUPPORTED;                   // the library was built without -DCG_TRACE
+#endif
     if (((uintptr_t)dev_buf & 7) || bytes < (size_t)8 * CG_TRACE_EV * iterations * CG_MAX_CTAS) return CG_EINVAL;
     s->d_trace = (u64*)dev_buf; s->trace_iters = iterations;
     return CG_OK;
