@@ -128,14 +128,14 @@ int cg_get_launch(cg_sim* s, int* n_ctas, int* threads, int* smem_bytes);
 int cg_get_phase_cycles(cg_sim* s, uint64_t* total, uint64_t* wait, uint64_t* update,
                         uint64_t* propose, int reset);
 
-/* Optional event trace of the persistent kernel (diagnostic; NULL / 0 switches it off):
- * during the first `iterations` PR iterations of every following cg_run, thread 0 of CTA b
- * writes dev_buf[(b*iterations + it)*24 + ev] = %globaltimer in ns for the events
- * 0 iteration start, 1 slab of the previous hop stored, 2 proposals tested, 3 winner known
- * (exchange scanned), 4 slabs of the previous hop complete on all CTAs, 5 winner broadcast in
- * the CTA, 6 table gathers of the new hop issued; entry 7 = (scan position of the CTA << 32) |
- * winning label; entries 8 + w: event 2 as seen by lane 0 of warp w (w < 16).  dev_buf: device
- * memory, 8-byte aligned, 8*24*iterations*1024 bytes. */
+/* Optional segment timers of the persistent kernel (diagnostic; needs a library built with
+ * -DCG_TRACE, else CG_EUNSUPPORTED; NULL / 0 switches it off).  Every following cg_run adds, for
+ * CTA b, to dev_buf[b*32 + c*16 + k] the SM cycles thread 0 spent in segment k of the iterations in
+ * which the CTA held the start of the window (c = 0) or not (c = 1): 0 loop bookkeeping, 1 until the
+ * slab of the previous hop is stored, 2 until its own proposals are tested, 6 waiting for the
+ * publication counter, 3 until the CTA minimum is known (CTA barrier), 4 until the winner is known
+ * (exchange), 5 executing the hop and issuing the table gathers; k = 15 counts the iterations.
+ * dev_buf: zeroed device memory, 8-byte aligned, 8*32*1024 bytes; `iterations` must be non-zero. */
 int cg_set_trace(cg_sim* s, void* dev_buf, size_t bytes, uint32_t iterations);
 
 /* L2 roofline denominator: one kernel, all SMs,

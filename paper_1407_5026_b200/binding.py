@@ -232,24 +232,22 @@ class CoulombGlass:
         self._check(self._lib.cg_get_launch(self._h, C.byref(a), C.byref(b), C.byref(c)))
         return {"n_ctas": a.value, "threads": b.value, "smem_bytes": c.value}
 
-    def set_trace(self, iterations):
-        """Record %globaltimer events of the first `iterations` PR iterations of each following run."""
+    def set_trace(self, on=True):
+        """Segment timers of the persistent kernel (library built with -DCG_TRACE); see cg_set_trace."""
         torch = self._torch
-        iterations = int(iterations)
-        if not iterations:
+        if not on:
             self._check(self._lib.cg_set_trace(self._h, None, 0, 0))
             self._trace = None
             return
-        self._trace = torch.zeros(24 * iterations * 1024, dtype=torch.int64, device=self.device)
-        self._trace_iters = iterations
+        self._trace = torch.zeros(32 * 1024, dtype=torch.int64, device=self.device)
         self._check(self._lib.cg_set_trace(self._h, C.c_void_p(self._trace.data_ptr()),
-                                           self._trace.numel() * 8, iterations))
+                                           self._trace.numel() * 8, 1))
 
     def trace(self):
-        """-> int64 array [n_ctas, iterations, 24] (see cg_set_trace in include/cg.h)."""
+        """-> int64 array [n_ctas, 2, 16] of SM cycles (see cg_set_trace in include/cg.h)."""
         self._torch.cuda.synchronize(self.device)
         n = self.launch()["n_ctas"]
-        return self._trace.view(1024, self._trace_iters, 24)[:n].cpu().numpy()
+        return self._trace.view(1024, 2, 16)[:n].cpu().numpy()
 
     def phase_cycles(self, reset=False):
         t, w, u, p = C.c_uint64(), C.c_uint64(), C.c_uint64(), C.c_uint64()

@@ -35,7 +35,11 @@ typedef unsigned int u32;
 
 // ------------------------------------------------------------------ device --
 
-#define CG_RING 5           // eps buffers: eps_{h-3} .. eps_{h+1} can be live at the same time
+#define CG_DEPTH 4          // pending hops: proposals read eps_{h-DEPTH} and add the newer hops' terms themselves
+#define CG_RING (2 * CG_DEPTH + 1)   // eps buffers: eps_{h+1-2 DEPTH} .. eps_{h+1} can be live at the same time
+#define CG_SRING 8          // exchange slots per CTA: a CTA posts up to DEPTH exchanges ahead of the slowest reader
+#define CG_SLOT_REP 1       // replicas of every exchange slot (more did not make the polls faster)
+#define CG_PUB_U64 16       // offset of a CTA's publication word in its slot line (u64 units)
 #define CG_SLOT_U64 32      // one exchange slot per CTA, 256-byte stride (own L2 slice), in u64 units
 #define CG_TRACE_EV 24      // events per iteration in the optional trace (cg_set_trace)
 #define CG_GUIDE 352        // tower guide: (43 + 1) binades x 8 sub-buckets of t = 2^43 - m
@@ -51,9 +55,10 @@ struct CgCtl {              // device-resident control block (one per sim)
     u64 epoch;              // next exchange epoch; never reset, so stale slots can never match
     u64 log_base;           // hop count at which the hop log was enabled
     u64 cyc_total, cyc_wait, cyc_update, cyc_propose;
-    u64 pub_count[2];       // slab publications: every CTA adds 1 per executed hop, to the counter of the
-                            // hop's parity within the launch (publications of two consecutive hops overlap)
-    u64 pub_base[2];        // values pub_count has when no launch is in flight
+    u64 pub_base;           // publication sequence number of the last hop of the previous launch: CTA c
+                            // stores pub_base + h into its pub word once its slab of hop h of a launch is
+                            // written (never reset, so stale words of other launch shapes are always smaller)
+    u64 pub_pad[3];
 };
 
 struct CgParams {           // kernel parameter block
@@ -110,12 +115,12 @@ __device__ __forceinline__ u64 ld_relaxed_u64(const u64* p)
     asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
     return v;
 }
-__device__ __forceinline__ void red_release_add_u64(u64* p, u64 v)
+__device__ __forceinline__ void st_release_u64(u64* p, u64 v)
 {
 #ifdef CG_EXP_NOMEMBAR
-    asm volatile("red.relaxed.gpu.global.add.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
+    asm volatile("st.relaxed.gpu.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
 #else
-    asm volatile("red.release.gpu.global.add.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
+    asm volatile("st.release.gpu.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
 #endif
 }
 __device__ __forceinline__ u64 global_ns()
@@ -129,19 +134,30 @@ __device__ __forceinline__ void fence_acquire_gpu() { }
 #else
 __device__ __forceinline__ void fence_acquire_gpu() { asm volatile("fence.acquire.gpu;" ::: "memory"); }
 #endif
-// named barriers 1 and 2 (alternating by hop): the warps that wrote eps arrive, the service warp
-// waits for them; barrier 0 with an explicit count synchronises the worker warps only
-__device__ __forceinline__ void barN_arrive(bool second, int n)
+// named barriers 1 .. CG_DEPTH (cyclic in the hop number): the warps that wrote eps arrive, the
+// service warp waits for them; barrier 0 with an explicit count synchronises the worker warps only
+__device__ __forceinline__ void barN_arrive(u32 k, int n)      // barrier 1 + k, k < 4
 {
-    if (second) asm volatile("bar.arrive 2, %0;" ::"r"(n) : "memory");
-    else asm volatile("bar.arrive 1, %0;" ::"r"(n) : "memory");
+    switch (k) {
+        case 0: asm volatile("bar.arrive 1, %0;" ::"r"(n) : "memory"); break;
+        case 1: asm volatile("bar.arrive 2, %0;" ::"r"(n) : "memory"); break;
+        case 2: asm volatile("bar.arrive 3, %0;" ::"r"(n) : "memory"); break;
+        default: asm volatile("bar.arrive 4, %0;" ::"r"(n) : "memory"); break;
+    }
 }
-__device__ __forceinline__ void barN_sync(bool second, int n)
+__device__ __forceinline__ void barN_sync(u32 k, int n)
 {
-    if (second) asm volatile("bar.sync 2, %0;" ::"r"(n) : "memory");
-    else asm volatile("bar.sync 1, %0;" ::"r"(n) : "memory");
+    switch (k) {
+        case 0: asm volatile("bar.sync 1, %0;" ::"r"(n) : "memory"); break;
+        case 1: asm volatile("bar.sync 2, %0;" ::"r"(n) : "memory"); break;
+        case 2: asm volatile("bar.sync 3, %0;" ::"r"(n) : "memory"); break;
+        default: asm volatile("bar.sync 4, %0;" ::"r"(n) : "memory"); break;
+    }
 }
-__device__ __forceinline__ void bar0_sync(int n) { asm volatile("bar.sync 0, %0;" ::"r"(n) : "memory"); }
+__device__ __forceinline__ void barX_sync(int n) { asm volatile("bar.sync 0, %0;" ::"r"(n) : "memory"); }
+// barrier 5: second CTA barrier of an iteration; the control warp only arrives
+__device__ __forceinline__ void barB_sync(int n) { asm volatile("bar.sync 5, %0;" ::"r"(n) : "memory"); }
+__device__ __forceinline__ void barB_arrive(int n) { asm volatile("bar.arrive 5, %0;" ::"r"(n) : "memory"); }
 
 // ---- the unfolded 1/r table ------------------------------------------------------------
 // tf[dy * 2L + dx] = 1/r of the offset (dy, dx) under minimum image, dy in [0, L),
@@ -293,11 +309,27 @@ __device__ __forceinline__ bool metropolis(double dE, u32 uh, u32 ul, double T, 
 #define BIT(sn, s) (((sn)[(s) >> 5] >> ((s) & 31)) & 1u)
 
 #ifdef CG_TRACE
-#define TRACE(ev, extra) do { if (p.trace && tid == 0 && it_local < p.trace_iters) \
-    p.trace[((size_t)b * p.trace_iters + it_local) * CG_TRACE_EV + (ev)] = (ev) == 7 ? (u64)(extra) : global_ns(); } while (0)
+// segment timers of thread 0 (SM cycles), summed over the launch, separately for iterations in which
+// this CTA held the start of the window (class 0) or not (class 1): p.trace[b*32 + class*16 + segment]
+#define TRACE(ev, extra) do { if (lane == 0) { const long long now_ = clock64(); \
+    s_seg[(kb == 0 ? 0 : 16) + (ev)] += (u64)(now_ - t_prev); t_prev = now_; } } while (0)
 #else
 #define TRACE(ev, extra) do { } while (0)
 #endif
+
+// What warp 0 tells the other warps of its CTA about an exchange (written before the second barrier).
+struct Desc {
+    u32 used;               // attempts consumed: q + 1, or M when the whole window was rejected
+    u32 hop;                // 1: a hop was executed
+    u32 ci, cj;             // its coded sites (site_code)
+    u32 ahead;              // 1: another CTA holds the start of the next window (time to decode ahead)
+    u32 pad[3];
+};
+struct Pend {               // pending hops, for threads that start to follow a pair of sites
+    u32 npend, rbuf, head;  // entry k (oldest first) is c[(head + k) % CG_DEPTH]
+    u32 c[CG_DEPTH][2];     // coded sites (i, j)
+};
+static_assert(CG_DEPTH <= 4 && CG_DEPTH < CG_SRING, "named barriers 1..4, slot ring");
 
 // The persistent kernel: steps 1, 2, 3a-3c of the mixed PR algorithm.
 // CACHED: thread g of the grid owns the attempts a = g (mod P), P = gridDim.x * PL >= M, keeps its
@@ -305,11 +337,14 @@ __device__ __forceinline__ bool metropolis(double dE, u32 uh, u32 ul, double T, 
 // the attempt index) and, while theta_ij = 1, also the two local energies it needs, to which it adds
 // the term of every executed hop itself; an iteration then only re-tests the proposal on the current
 // state.  Otherwise CTA b evaluates labels [b per, (b+1) per) from scratch.
+// Warp 0 of every CTA does the exchange and all bookkeeping; the other worker warps only test their
+// proposals and update their part of the eps slab, and learn the outcome from a small descriptor.
 template <int THREADS, int RP, bool CACHED>
 __global__ void __launch_bounds__(THREADS, 1) cg_pr_persistent(const CgParams p)
 {
-    constexpr int TW = THREADS - 32;      // worker threads; the last warp only publishes slab updates
-    constexpr int NW = TW / 32;
+    constexpr int TW = THREADS - 64;      // worker threads; then the control warp and the service warp
+    constexpr int NWK = TW / 32;          // index of the control warp
+    constexpr int TB = TW + 32;           // threads at the two CTA barriers of an iteration
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int KL = p.Klive;
     u64* s_cdfi = reinterpret_cast<u64*>(smem_raw);
@@ -318,9 +353,16 @@ __global__ void __launch_bounds__(THREADS, 1) cg_pr_persistent(const CgParams p)
     int* s_disp = reinterpret_cast<int*>(s_fld + KL);
     u32* s_guide = reinterpret_cast<u32*>(s_disp + KL);
     u32* s_n = s_guide + CG_GUIDE;
-    __shared__ u32 s_wlab[2][32], s_plab[2];    // indexed by iteration parity: one barrier per iteration
-    __shared__ u64 s_wpay[2][32], s_ppay[2];
+    __shared__ u32 s_wlab[32];
+    __shared__ u64 s_wpay[32];
+    __shared__ __align__(16) Desc s_desc;
+    __shared__ __align__(8) Pend s_pend;
     const Tables tb = {s_cdfi, s_invr, s_fld, s_disp, s_guide};
+#ifdef CG_TRACE
+    __shared__ u64 s_seg[32];
+    if (threadIdx.x < 32) s_seg[threadIdx.x] = 0;
+    long long t_prev = 0;
+#endif
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const u32 b = blockIdx.x, nb = gridDim.x;
@@ -334,34 +376,17 @@ __global__ void __launch_bounds__(THREADS, 1) cg_pr_persistent(const CgParams p)
     }
     for (int k = tid; k < CG_GUIDE; k += THREADS) s_guide[k] = p.guide[k];
     for (u32 w = tid; w < (N + 31) / 32; w += THREADS) s_n[w] = p.nbits[w];
+    if (tid == 0) {
+        s_pend.npend = 0; s_pend.rbuf = p.ctl->cur; s_pend.head = 0;
+    }
 
-    // replicated, CTA-uniform control state; 64-bit totals are formed once, after the loop
-    const u64 a_start = p.ctl->attempts;
-    const u64 log_base = p.ctl->log_base, hops_start = p.ctl->hops;
-    const u32 e_start = (u32)p.ctl->epoch;
-    u64 used_sum = 0, hl = 0;             // attempts consumed and hops executed in this launch
-    long long dP = 0;
-    u32 it_local = 0;                     // PR iterations of this launch
-    // Pending hops.  eps lives in a ring of CG_RING buffers: hop h writes eps_h (each CTA its own slab)
-    // into the buffer after the one hop h-1 wrote.  Nobody reads the two newest buffers, which other
-    // CTAs may still be writing: a proposal that starts to follow a pair of sites reads eps_{h-2}
-    // (buffer rbuf, complete on every CTA: checked against pub_count) and adds the terms
-    // 1/r_lj - 1/r_li of the npend <= 2 newest hops itself, in hop order - the same single rounded adds
-    // the update performs, so the values are bit-identical.  A CTA writes eps_{h+1} only when every CTA
-    // has published hop h-1, i.e. reads eps_{h-3} or newer: five buffers are never written while read.
-    u32 rbuf = p.ctl->cur, wbuf = p.ctl->cur;
-    int npend = 0;
-    u32 pci0 = 0, pcj0 = 0, pci1 = 0, pcj1 = 0;   // coded sites of the pending hops, oldest first
+    const u64 a_start = p.ctl->attempts, pub_base = p.ctl->pub_base;
+    u64 hl = 0;                           // hops executed in this launch
+    u32 wbuf = p.ctl->cur;                // buffer of the ring that holds the newest eps
     bool upd = false;                     // slab update issued, not yet finished
-    bool newhop = false;                  // the previous iteration executed a hop
-    // hop number hl of this launch (1-based) is published on counter hl & 1; every CTA has published it
-    // once that counter reaches cnt0 / cnt1 (advanced by nb when the hop is executed)
-    u64 cnt0 = p.ctl->pub_base[0], cnt1 = p.ctl->pub_base[1];
-    u64 need_pub = 0;                     // ... for the hop whose buffer becomes rbuf at the next executed hop
-    u32 need_par = 0;
-#ifdef CG_TRACE
-    u64 cyc_wait = 0, cyc_update = 0, cyc_propose = 0;
-#endif
+    bool newhop = false;                  // the previous iteration executed a hop ...
+    u32 hci = 0, hcj = 0;                 // ... with these coded sites
+    bool ahead = false;                   // another CTA holds the start of the window
     const long long t_begin = clock64();
 
     // labels: CTA-blocked (scan order = CTA order) or, CACHED, cyclic in the global thread index
@@ -372,15 +397,16 @@ __global__ void __launch_bounds__(THREADS, 1) cg_pr_persistent(const CgParams p)
     if (CACHED) { const u32 g0 = (u32)(a_start % P); c_first = g0 / per; t0r = g0 - c_first * per; }
     const bool has_label = CACHED && (u32)tid < per;
     __syncthreads();
-    if (warp == NW) {
+    if (warp == NWK + 1) {
         // service warp: once per executed hop, wait until every worker has stored its part of the
         // slab (named barrier), fence those stores and bump the publication counter - off the
-        // workers' critical path.  Workers run at most two hops ahead of it (the exchange of hop h+2
-        // waits for the publication of hop h by every CTA, this one included), hence two barriers.
+        // workers' critical path.  Workers run at most CG_DEPTH hops ahead of it (the exchange of hop
+        // h+DEPTH waits for the publication of hop h by every CTA, this one included), hence as many
+        // barriers.
         if (nb > 1)
             for (u64 h = 0; h < p.n_hops; ++h) {
-                barN_sync((h & 1) != 0, THREADS);
-                if (lane == 0) red_release_add_u64(&p.ctl->pub_count[(h + 1) & 1], 1ull);
+                barN_sync((u32)(h % CG_DEPTH), TB);
+                if (lane == 0) st_release_u64(p.slots + (size_t)b * (CG_SLOT_REP * CG_SLOT_U64) + CG_PUB_U64, pub_base + h + 1);
             }
         return;
     }
@@ -405,159 +431,94 @@ __global__ void __launch_bounds__(THREADS, 1) cg_pr_persistent(const CgParams p)
         a_cur = a_start + lab;
         take(decode_attempt(tb, p, a_cur));
     }
+    ahead = CACHED && c_first != b;
 
     const u32 pairs = N / 2, pper = (pairs + nb - 1) / nb;
     const u32 pr0 = min(pairs, b * pper), pr1 = min(pairs, pr0 + pper);
-    u64* const my_slot = p.slots + (size_t)b * CG_SLOT_U64;
+    u64* const my_slot = p.slots + (size_t)b * (CG_SLOT_REP * CG_SLOT_U64);   // replica r at + r * CG_SLOT_U64
 
-    Slab<TW, RP> slab;
-    slab.load(p.eps[rbuf], pr0, pr1, L);
-
-    // finish the issued slab update and hand it to the service warp for publication
-    auto finish_update = [&]() {
-        const u32 src = wbuf == 0 ? CG_RING - 1u : wbuf - 1u;
-        slab.finish(tf, mask, L, p.eps[src], p.eps[wbuf], pr0, pr1);
-        if (nb > 1) barN_arrive((hl & 1) == 0, THREADS);         // hop hl (1-based) on barrier 1 + ((hl - 1) & 1)
-        upd = false;
-    };
-
-    while (hl < p.n_hops) {
+    if (warp == NWK) {
+        // ------------------------------------------------------------------ control warp ----
+        // Exchange and bookkeeping of the CTA; it holds no labels and no eps.
+        const u64 log_base = p.ctl->log_base, hops_start = p.ctl->hops;
+        const u32 e_start = (u32)p.ctl->epoch;
+        u64 used_sum = 0;                 // attempts consumed in this launch
+        long long dP = 0;
+        u32 it_local = 0;                 // PR iterations of this launch
+        // Pending hops.  eps lives in a ring of CG_RING buffers: hop h writes eps_h (each CTA its own
+        // slab) into the buffer after the one hop h-1 wrote.  Nobody reads the two newest buffers, which
+        // other CTAs may still be writing: a proposal that starts to follow a pair of sites reads
+        // eps_{h-2} (buffer rbuf, complete on every CTA: checked against pub_count) and adds the terms
+        // 1/r_lj - 1/r_li of the npend <= 2 newest hops itself, in hop order - the same single rounded
+        // adds the update performs, so the values are bit-identical.  A CTA writes eps_{h+1} only when
+        // every CTA has published hop h-1, i.e. reads eps_{h-3} or newer: five buffers are never
+        // written while read.
+        u32 rbuf = wbuf, npend = 0, head = 0;     // as in s_pend
+        // CTA c has published hop number h of this launch once its pub word is >= pub_base + h
+        u64 need_pub = 0;                 // ... for the hop whose buffer becomes rbuf at the next executed hop
+        while (hl < p.n_hops) {
+            const u32 e32 = e_start + it_local;
+            const u32 kb = b >= c_first ? b - c_first : b + nb - c_first;    // my scan position
 #ifdef CG_TRACE
-        const long long t0 = clock64();
+            if (lane == 0) { if (t_prev == 0) t_prev = clock64(); s_seg[(kb == 0 ? 0 : 16) + 15] += 1; }
 #endif
-        TRACE(0, 0);
-        const u32 par = it_local & 1u;
-        const u32 e32 = e_start + it_local;
-        const double* __restrict__ erd = p.eps[rbuf];
-        const u32 kb = b >= c_first ? b - c_first : b + nb - c_first;    // my scan position
-        u64 pc = 0;
-        if (nb > 1 && tid == 0) pc = ld_relaxed_u64(&p.ctl->pub_count[need_par]);   // checked before the barrier below
-        // ---- steps 1-2: propose and test, state untouched (PAPER.md:73-74)
-        u32 best = CG_NONE, bi = 0, bj = 0;
-        if (CACHED) {
-            const bool th = lab < M && BIT(s_n, ci_) && !BIT(s_n, cj_);   // theta_ij, inside the window
-            double ga = 0, gb = 0, a_i0 = 0, b_i0 = 0, a_j0 = 0, b_j0 = 0, a_i1 = 0, b_i1 = 0, a_j1 = 0, b_j1 = 0;
-            if (th) {                      // gathers first ...
-                if (tracked) {
-                    if (newhop) {          // the term of the hop executed last iteration
-                        const u32 hc_i = npend > 1 ? pci1 : pci0, hc_j = npend > 1 ? pcj1 : pcj0;
-                        a_i0 = __ldg(tf + ((sci - hc_j) & mask)); b_i0 = __ldg(tf + ((sci - hc_i) & mask));
-                        a_j0 = __ldg(tf + ((scj - hc_j) & mask)); b_j0 = __ldg(tf + ((scj - hc_i) & mask));
+            // The buffer that becomes rbuf at the next executed hop must be complete on every CTA before the
+            // workers of this CTA are let into the next iteration: one publication word per CTA, each in its
+            // own L2 slice.  This warp is idle while the workers test their proposals, so the check is free.
+            if (nb > 1) {
+                for (;;) {
+                    bool ok = true;
+                    for (u32 c0 = lane; c0 < nb; c0 += 32 * 8) {        // eight independent loads in flight
+                        u64 v[8];
+#pragma unroll
+                        for (int k = 0; k < 8; ++k) {
+                            const u32 c = c0 + 32 * k;
+                            v[k] = c < nb ? ld_relaxed_u64(p.slots + (size_t)c * (CG_SLOT_REP * CG_SLOT_U64) + CG_PUB_U64) : ~0ull;
+                        }
+#pragma unroll
+                        for (int k = 0; k < 8; ++k) ok = ok && v[k] >= need_pub;
                     }
-                } else {                   // start to follow (i, j): complete buffer + all pending hops
-                    ga = ld_cg(erd + ci_); gb = ld_cg(erd + cj_);
-                    if (npend > 0) {
-                        a_i0 = __ldg(tf + ((sci - pcj0) & mask)); b_i0 = __ldg(tf + ((sci - pci0) & mask));
-                        a_j0 = __ldg(tf + ((scj - pcj0) & mask)); b_j0 = __ldg(tf + ((scj - pci0) & mask));
-                    }
-                    if (npend > 1) {
-                        a_i1 = __ldg(tf + ((sci - pcj1) & mask)); b_i1 = __ldg(tf + ((sci - pci1) & mask));
-                        a_j1 = __ldg(tf + ((scj - pcj1) & mask)); b_j1 = __ldg(tf + ((scj - pci1) & mask));
-                    }
+                    if (__all_sync(CG_FULL, ok)) break;
                 }
+                fence_acquire_gpu();
             }
-            if (upd) finish_update();      // ... the slab of the previous hop while they are in flight
-            TRACE(1, 0);
-            // ... and, while another CTA holds the start of the window (this one only waits for it),
-            // the decode one attempt ahead
-            if (has_label && !nxt_valid && kb != 0) { nxt = decode_attempt(tb, p, a_cur + P); nxt_valid = true; }
-            if (th) {
-                if (tracked) {
-                    if (newhop) { ei = __dadd_rn(ei, __dsub_rn(a_i0, b_i0)); ej = __dadd_rn(ej, __dsub_rn(a_j0, b_j0)); }
-                } else {
-                    ei = ga; ej = gb;
-                    if (npend > 0) { ei = __dadd_rn(ei, __dsub_rn(a_i0, b_i0)); ej = __dadd_rn(ej, __dsub_rn(a_j0, b_j0)); }
-                    if (npend > 1) { ei = __dadd_rn(ei, __dsub_rn(a_i1, b_i1)); ej = __dadd_rn(ej, __dsub_rn(a_j1, b_j1)); }
-                    tracked = true;
-                }
-                // dH_ij = eps_j - eps_i - 1/r_ij - E dx_ij (PAPER.md:63)
-                const double dE = __dsub_rn(__dsub_rn(__dsub_rn(ej, ei), c_invr), c_fld);
-                if (metropolis(dE, cuh, cul, p.T, p.inv_T)) { best = lab; bi = ci_; bj = cj_; }
-            } else tracked = false;
-        } else {
-            if (upd) finish_update();
-            TRACE(1, 0);
-            for (u32 l = lab0 + tid; l < lab1; l += TW) {
-                const u64 a = a_start + used_sum + l;
-                u32 w0, w1, w2, w3;
-                philox4x32_10((u32)a, (u32)(a >> 32), 0u, 0u, p.seed_lo, p.seed_hi, w0, w1, w2, w3);
-                const u32 i = __umulhi(w0, N);                                   // uniform site
-                if (!BIT(s_n, i)) continue;                                      // n_i = 1 ?
-                const u32 k = tower_search(tb, ((u64)w1 << 11) | (u64)(w2 >> 21));
-                const u32 j = hop_target(tb, i, k, L, lg);
-                if (BIT(s_n, j)) continue;                                       // n_j = 0 ?
-                double vi = ld_cg(erd + i), vj = ld_cg(erd + j);
-                const u32 si = site_code(i, L) | (u32)L, sj = site_code(j, L) | (u32)L;
-                if (npend > 0) {
-                    vi = __dadd_rn(vi, hop_term(tf, mask, si, pci0, pcj0));
-                    vj = __dadd_rn(vj, hop_term(tf, mask, sj, pci0, pcj0));
-                }
-                if (npend > 1) {
-                    vi = __dadd_rn(vi, hop_term(tf, mask, si, pci1, pcj1));
-                    vj = __dadd_rn(vj, hop_term(tf, mask, sj, pci1, pcj1));
-                }
-                const double dE = __dsub_rn(__dsub_rn(__dsub_rn(vj, vi), s_invr[k]), s_fld[k]);
-                if (metropolis(dE, w2 & 0x1FFFFFu, w3, p.T, p.inv_T)) { best = l; bi = i; bj = j; break; }
+            TRACE(6, 0);
+            barX_sync(TB);                // [A] the workers have tested their proposals
+            TRACE(3, 0);
+            // ---- step 3: lowest accepting label: CTA, then grid
+            u32 gmin; u64 gpay;
+            {
+                const u32 l_ = lane < NWK ? s_wlab[lane] : CG_NONE;
+                const u64 pay = lane < NWK ? s_wpay[lane] : 0ull;
+                gmin = __reduce_min_sync(CG_FULL, l_);
+                const int src = __ffs(__ballot_sync(CG_FULL, l_ == gmin)) - 1;
+                gpay = __shfl_sync(CG_FULL, pay, src);
             }
-        }
-#ifdef CG_TRACE
-        const long long t1 = clock64();
-#endif
-        TRACE(2, 0);
-        // the buffer that becomes rbuf at the next executed hop must be complete on every CTA before
-        // this CTA passes the barrier below (one thread checks; everybody waits for it there)
-        if (nb > 1 && tid == 0) {
-            while (pc < need_pub) pc = ld_relaxed_u64(&p.ctl->pub_count[need_par]);
-            fence_acquire_gpu();
-        }
-        // ---- step 3: lowest accepting label: warp, CTA, grid
-        {
-            const u32 wmin = __reduce_min_sync(CG_FULL, best);
-            const int src = __ffs(__ballot_sync(CG_FULL, best == wmin)) - 1;
-            if (lane == src) { s_wlab[par][warp] = wmin; s_wpay[par][warp] = ((u64)bi << 32) | (u64)bj; }
-        }
-#ifdef CG_TRACE
-        if (p.trace && lane == 0 && it_local < p.trace_iters)     // per-warp "proposals tested" times
-            p.trace[((size_t)b * p.trace_iters + it_local) * CG_TRACE_EV + 8 + (warp & 15)] = global_ns();
-#endif
-        bar0_sync(TW);
-        // CTA minimum, in every warp
-        u32 gmin; u64 gpay;
-        {
-            const u32 l_ = lane < NW ? s_wlab[par][lane] : CG_NONE;
-            const u64 pay = lane < NW ? s_wpay[par][lane] : 0ull;
-            gmin = __reduce_min_sync(CG_FULL, l_);
-            const int src = __ffs(__ballot_sync(CG_FULL, l_ == gmin)) - 1;
-            gpay = __shfl_sync(CG_FULL, pay, src);
-        }
-        TRACE(3, 0);
-        // The grid.  In scan order (CTA order starting at the CTA that holds attempt a0) every CTA holds
-        // lower labels than the next one, except that CACHED the first CTA also holds the end of the
-        // window in its threads below a0's ("tail" labels).  The winner is the first non-tail accept in
-        // scan order; the scan stops there: slots of later CTAs are never waited for (their proposals
-        // cannot win), and the first CTA, when it accepts, waits for nobody.
-        const u32 tail0 = CACHED ? per - t0r : CG_NONE;            // position 0: labels >= tail0 are tail labels
-        const bool own_low = gmin != CG_NONE && (!CACHED || kb != 0 || gmin < tail0);
-        // A CTA can be up to three exchanges ahead of the slowest reader of its slot (bounded by the
-        // publication check and by every fully rejected window, which needs all slots): ring of four.
-        const u32 ring = (e32 & 3u) * 2u;
-        if (nb > 1 && tid == 0)
-            slot_store(my_slot + ring, ((u64)e32 << 32) | gmin,
-                       ((u64)(e32 & 0xFFFFu) << 48) | ((gpay >> 32) << 24) | (gpay & 0xFFFFFFu));
-        u32 q = gmin; u64 wp = gpay;
-        if (!(own_low && kb == 0) && nb > 1) {
-            if (warp == 0) {
-                u32 wlab = gmin; u64 wpay = gpay;                      // result if nobody beats it
+            // In scan order (CTA order starting at the CTA that holds attempt a0) every CTA holds lower
+            // labels than the next one, except that CACHED the first CTA also holds the end of the window
+            // in its threads below a0's ("tail" labels).  The winner is the first non-tail accept in scan
+            // order; the scan stops there: slots of later CTAs are never waited for (their proposals
+            // cannot win), and the first CTA, when it accepts, waits for nobody.
+            const u32 tail0 = CACHED ? per - t0r : CG_NONE;            // position 0: labels >= tail0 are tail labels
+            const bool own_low = gmin != CG_NONE && (!CACHED || kb != 0 || gmin < tail0);
+            // A CTA can be up to three exchanges ahead of the slowest reader of its slot (bounded by the
+            // publication check and by every fully rejected window, which needs all slots): ring of four.
+            const u32 ring = (e32 & (CG_SRING - 1u)) * 2u;
+            if (nb > 1 && lane < CG_SLOT_REP)
+                slot_store(my_slot + lane * CG_SLOT_U64 + ring, ((u64)e32 << 32) | gmin,
+                           ((u64)(e32 & 0xFFFFu) << 48) | ((gpay >> 32) << 24) | (gpay & 0xFFFFFFu));
+            u32 q = gmin; u64 wp = gpay;
+            if (!(own_low && kb == 0) && nb > 1) {
                 u32 tlab = CG_NONE; u64 tpay = 0;                      // tail accept of position 0
                 const u32 e16 = e32 & 0xFFFFu;
                 const u32 k_end = own_low ? kb : nb;    // an accept of my own: only earlier CTAs can beat it
-                u32 k0 = 0, width = 4;                  // the winner is almost always in the first CTAs
+                u32 k0 = 0, width = 2;                  // the winner is almost always in the first CTAs
                 bool found = false;
                 while (!found && k0 < k_end) {
                     const u32 k = k0 + lane;
                     const bool mine = k < k_end && (u32)lane < width && k != kb;
                     u32 c = c_first + k; if (c >= nb) c -= nb;
-                    const u64* sl = p.slots + (size_t)(mine ? c : b) * CG_SLOT_U64 + ring;
+                    const u64* sl = p.slots + ((size_t)(mine ? c : b) * CG_SLOT_REP + (b & (CG_SLOT_REP - 1))) * CG_SLOT_U64 + ring;
                     bool ready = !mine; u32 l = CG_NONE; u64 q1 = 0;
                     for (;;) {
                         if (!ready) {
@@ -573,9 +534,9 @@ __global__ void __launch_bounds__(THREADS, 1) cg_pr_persistent(const CgParams p)
                         const int fa = racc ? __ffs(racc) - 1 : 32;
                         const int fn = rnot ? __ffs(rnot) - 1 : 32;
                         if (fa < fn) {                  // first accepting slot, everything before it rejected
-                            wlab = __shfl_sync(CG_FULL, l, fa);
-                            wpay = __shfl_sync(CG_FULL, q1, fa);
-                            wpay = ((wpay >> 24) & 0xFFFFFFull) << 32 | (wpay & 0xFFFFFFull);
+                            q = __shfl_sync(CG_FULL, l, fa);
+                            wp = __shfl_sync(CG_FULL, q1, fa);
+                            wp = ((wp >> 24) & 0xFFFFFFull) << 32 | (wp & 0xFFFFFFull);
                             found = true;
                             break;
                         }
@@ -587,89 +548,178 @@ __global__ void __launch_bounds__(THREADS, 1) cg_pr_persistent(const CgParams p)
                     k0 += width; width = 32;
                 }
                 if (!found && !own_low && kb != 0 && tlab != CG_NONE) {   // only the tail of the window accepted
-                    wlab = tlab; wpay = ((tpay >> 24) & 0xFFFFFFull) << 32 | (tpay & 0xFFFFFFull);
+                    q = tlab; wp = ((tpay >> 24) & 0xFFFFFFull) << 32 | (tpay & 0xFFFFFFull);
                 }
-                if (lane == 0) { s_plab[par] = wlab; s_ppay[par] = wpay; }
             }
-            bar0_sync(TW);
-            q = s_plab[par]; wp = s_ppay[par];
+            TRACE(4, 0);
+            // ---- what the workers need: attempts consumed (m = (p-1)M + q per executed hop, PAPER.md:39,
+            // 78), the hop (step 3a), occupations, pending list
+            const u32 used = q == CG_NONE ? M : q + 1;
+            if (CACHED) {
+                if (t0r + used < per) t0r += used;
+                else {
+                    u32 g0 = c_first * per + t0r + used; if (g0 >= P) g0 -= P;      // used <= M <= P
+                    c_first = g0 / per; t0r = g0 - c_first * per;
+                }
+            }
+            const u32 hi_ = (u32)(wp >> 32), hj_ = (u32)wp;
+            const u32 ci = site_code(hi_, L), cj = site_code(hj_, L);
+            if (q != CG_NONE) {
+                const u32 pos = npend < CG_DEPTH ? (head + npend) % CG_DEPTH : head;
+                if (npend < CG_DEPTH) ++npend;
+                else { head = (head + 1) % CG_DEPTH; rbuf = rbuf == CG_RING - 1 ? 0u : rbuf + 1u; }
+                if (lane == 0) {              // the workers are between the two barriers: nobody reads these
+                    s_n[hi_ >> 5] &= ~(1u << (hi_ & 31));
+                    s_n[hj_ >> 5] |= 1u << (hj_ & 31);
+                    s_pend.c[pos][0] = ci; s_pend.c[pos][1] = cj;
+                    s_pend.npend = npend; s_pend.rbuf = rbuf; s_pend.head = head;
+                }
+            }
+            if (lane == 0) {
+                *reinterpret_cast<uint4*>(&s_desc) = make_uint4(used, q != CG_NONE, ci, cj);
+                s_desc.ahead = CACHED && c_first != b;
+            }
+            TRACE(5, 0);
+            barB_arrive(TB);              // [B] the workers may read the descriptor; this warp goes on
+            // ---- the rest of the bookkeeping, while the workers run
+            used_sum += used;
+            ++it_local;
+            if (q != CG_NONE) {
+                const int xi = hi_ & (L - 1), xj = hj_ & (L - 1);
+                int ddx = (xj - xi) & (L - 1); if (ddx > L / 2) ddx -= L;   // minimum image, tie -> +L/2
+                dP += ddx;                                                   // step 3b: dP = dx
+                if (lane == 0 && b == 0 && hops_start + hl - log_base < p.log_cap) {
+                    const u64 h = hops_start + hl - log_base;
+                    p.log_a[h] = a_start + used_sum - 1; p.log_i[h] = hi_; p.log_j[h] = hj_;
+                }
+                ++hl;
+                // all slabs of hop hl - DEPTH + 1: they are read (as rbuf) once the NEXT hop is executed,
+                // and awaited before that
+                need_pub = hl >= CG_DEPTH ? pub_base + hl - CG_DEPTH + 1 : 0;
+            }
+            TRACE(0, 0);
         }
-        const u32 hi_ = (u32)(wp >> 32), hj_ = (u32)wp;
 #ifdef CG_TRACE
-        const long long t2 = clock64();
-        cyc_propose += (u64)(t1 - t0); cyc_wait += (u64)(t2 - t1);
+        __syncwarp();
+        if (p.trace) p.trace[(size_t)b * 32 + lane] += s_seg[lane];
 #endif
-        TRACE(4, 0);
-        TRACE(7, ((u64)kb << 32) | q);
-        // attempts consumed: m = (p-1)M + q per executed hop
-        const u32 used = q == CG_NONE ? M : q + 1;
-        used_sum += used;
-        ++it_local;
+        if (b == 0 && lane == 0) {
+            CgCtl* c = p.ctl;
+            c->attempts = a_start + used_sum; c->hops = hops_start + hl;
+            c->iterations += it_local; c->proposals += (u64)M * it_local;
+            c->dP += dP; c->cur = rbuf + npend >= CG_RING ? rbuf + npend - CG_RING : rbuf + npend; c->epoch += it_local;
+            c->pub_base = pub_base + hl;
+            c->cyc_total += (u64)(clock64() - t_begin);
+        }
+        return;
+    }
+
+    Slab<TW, RP> slab;
+    slab.load(p.eps[wbuf], pr0, pr1, L);
+
+    // finish the issued slab update and hand it to the service warp for publication
+    auto finish_update = [&]() {
+        const u32 src = wbuf == 0 ? CG_RING - 1u : wbuf - 1u;
+        slab.finish(tf, mask, L, p.eps[src], p.eps[wbuf], pr0, pr1);
+        if (nb > 1) barN_arrive((u32)((hl - 1) % CG_DEPTH), TB);   // hop hl (1-based) on barrier 1 + (hl - 1) % DEPTH
+        upd = false;
+    };
+
+    // ---------------------------------------------------------------------- worker warps ----
+    // One loop body = outcome of the previous exchange (descriptor) -> table gathers of its hop ->
+    // proposals -> slab update: gathers and update sit in the same body, so the gathers stay in flight
+    // during the whole propose phase.
+    u64 a0 = a_start;                     // first attempt of the window (used when labels are not cached)
+    uint4 d4 = make_uint4(0u, 0u, 0u, 0u);       // used, hop, ci, cj of the previous exchange
+    for (;;) {
         if (CACHED) {
-            if (t0r + used < per) t0r += used;
-            else {
-                u32 g0 = c_first * per + t0r + used; if (g0 >= P) g0 -= P;      // used <= M <= P
-                c_first = g0 / per; t0r = g0 - c_first * per;
-            }
-            if (has_label) {
-                if (lab >= used) lab -= used;
+            if (has_label && d4.x) {
+                if (lab >= d4.x) lab -= d4.x;
                 else {                              // my attempt was consumed: take the next one
-                    lab += P - used;
+                    lab += P - d4.x;
                     if (!nxt_valid) nxt = decode_attempt(tb, p, a_cur + P);
                     take(nxt); a_cur += P; nxt_valid = false;
                 }
             }
+        } else a0 += d4.x;
+        newhop = d4.y != 0;
+        if (newhop) {
+            // step 3b: local energies of my slab, into the next buffer of the ring
+            ++hl;
+            hci = d4.z; hcj = d4.w;
+            wbuf = wbuf == CG_RING - 1 ? 0u : wbuf + 1u;
+            slab.issue(tf, mask, pr0, pr1, hci, hcj);
+            upd = true;
         }
-        newhop = q != CG_NONE;
-        if (!newhop) continue;                      // whole window rejected: p += 1
-
-        // ---- step 3a: execute the hop of label q
-        const int xi = hi_ & (L - 1), xj = hj_ & (L - 1);
-        int ddx = (xj - xi) & (L - 1); if (ddx > L / 2) ddx -= L;   // minimum image, tie -> +L/2
-        dP += ddx;                                                   // step 3b: dP = dx
-        if (lane == 0) {                            // every warp flips the bits itself (idempotent), so its
-            atomicAnd(&s_n[hi_ >> 5], ~(1u << (hi_ & 31)));      // own lanes see them without a CTA barrier
-            atomicOr(&s_n[hj_ >> 5], 1u << (hj_ & 31));
-            if (b == 0 && tid == 0 && hops_start + hl - log_base < p.log_cap) {
-                const u64 h = hops_start + hl - log_base;
-                p.log_a[h] = a_start + used_sum - 1; p.log_i[h] = hi_; p.log_j[h] = hj_;
+        if (hl >= p.n_hops) break;
+        // ---- steps 1-2: propose and test, state untouched (PAPER.md:73-74)
+        u32 best = CG_NONE, bi = 0, bj = 0;
+        if (CACHED) {
+            const bool th = lab < M && BIT(s_n, ci_) && !BIT(s_n, cj_);   // theta_ij, inside the window
+            if (th) {
+                if (!tracked) {            // start to follow (i, j): complete buffer + all pending hops
+                    const u32 np = s_pend.npend;
+                    const double* __restrict__ erd = p.eps[s_pend.rbuf];
+                    ei = ld_cg(erd + ci_); ej = ld_cg(erd + cj_);
+                    for (u32 k = 0; k < np; ++k) {
+                        const u32 e_ = (s_pend.head + k) % CG_DEPTH;
+                        const u32 ki = s_pend.c[e_][0], kj = s_pend.c[e_][1];
+                        ei = __dadd_rn(ei, hop_term(tf, mask, sci, ki, kj));
+                        ej = __dadd_rn(ej, hop_term(tf, mask, scj, ki, kj));
+                    }
+                    tracked = true;
+                } else if (newhop) {       // the term of the hop executed last iteration
+                    const double a_i = __ldg(tf + ((sci - hcj) & mask)), b_i = __ldg(tf + ((sci - hci) & mask));
+                    const double a_j = __ldg(tf + ((scj - hcj) & mask)), b_j = __ldg(tf + ((scj - hci) & mask));
+                    ei = __dadd_rn(ei, __dsub_rn(a_i, b_i)); ej = __dadd_rn(ej, __dsub_rn(a_j, b_j));
+                }
+                // dH_ij = eps_j - eps_i - 1/r_ij - E dx_ij (PAPER.md:63)
+                const double dE = __dsub_rn(__dsub_rn(__dsub_rn(ej, ei), c_invr), c_fld);
+                if (metropolis(dE, cuh, cul, p.T, p.inv_T)) { best = lab; bi = ci_; bj = cj_; }
+            } else tracked = false;
+        } else {
+            const u32 np = s_pend.npend;
+            const double* __restrict__ erd = p.eps[s_pend.rbuf];
+            for (u32 l = lab0 + tid; l < lab1; l += TW) {
+                const u64 a = a0 + l;
+                u32 w0, w1, w2, w3;
+                philox4x32_10((u32)a, (u32)(a >> 32), 0u, 0u, p.seed_lo, p.seed_hi, w0, w1, w2, w3);
+                const u32 i = __umulhi(w0, N);                                   // uniform site
+                if (!BIT(s_n, i)) continue;                                      // n_i = 1 ?
+                const u32 k = tower_search(tb, ((u64)w1 << 11) | (u64)(w2 >> 21));
+                const u32 j = hop_target(tb, i, k, L, lg);
+                if (BIT(s_n, j)) continue;                                       // n_j = 0 ?
+                double vi = ld_cg(erd + i), vj = ld_cg(erd + j);
+                const u32 si = site_code(i, L) | (u32)L, sj = site_code(j, L) | (u32)L;
+                for (u32 t = 0; t < np; ++t) {
+                    const u32 e_ = (s_pend.head + t) % CG_DEPTH;
+                    const u32 ki = s_pend.c[e_][0], kj = s_pend.c[e_][1];
+                    vi = __dadd_rn(vi, hop_term(tf, mask, si, ki, kj));
+                    vj = __dadd_rn(vj, hop_term(tf, mask, sj, ki, kj));
+                }
+                const double dE = __dsub_rn(__dsub_rn(__dsub_rn(vj, vi), s_invr[k]), s_fld[k]);
+                if (metropolis(dE, w2 & 0x1FFFFFu, w3, p.T, p.inv_T)) { best = l; bi = i; bj = j; break; }
             }
         }
-        __syncwarp();
-        ++hl;
-        // ---- step 3b: local energies of my slab, into the next buffer of the ring
-        const u32 ci = site_code(hi_, L), cj = site_code(hj_, L);
-        wbuf = wbuf == CG_RING - 1 ? 0u : wbuf + 1u;
-        if (npend == 2) { rbuf = rbuf == CG_RING - 1 ? 0u : rbuf + 1u; pci0 = pci1; pcj0 = pcj1; pci1 = ci; pcj1 = cj; }
-        else if (npend == 1) { pci1 = ci; pcj1 = cj; npend = 2; }
-        else { pci0 = ci; pcj0 = cj; npend = 1; }
-        slab.issue(tf, mask, pr0, pr1, ci, cj);
-        upd = true;
-        // all slabs of the hop before this one: they are read (as rbuf) once the NEXT hop is executed,
-        // and awaited before that
-        if (hl & 1) { cnt1 += nb; need_pub = cnt0; need_par = 0; }
-        else { cnt0 += nb; need_pub = cnt1; need_par = 1; }
-#ifdef CG_TRACE
-        cyc_update += (u64)(clock64() - t2);
-#endif
-        TRACE(5, 0);
+        // ---- step 3: lowest accepting label: warp, then the control warp
+        {
+            const u32 wmin = __reduce_min_sync(CG_FULL, best);
+            const int src = __ffs(__ballot_sync(CG_FULL, best == wmin)) - 1;
+            if (lane == src) { s_wlab[warp] = wmin; s_wpay[warp] = ((u64)bi << 32) | (u64)bj; }
+        }
+        barX_sync(TB);                    // [A]
+        // while the control warp does the exchange: the slab of the previous hop (its table gathers,
+        // issued when that hop was executed, have had the whole propose phase to arrive) and, if another
+        // CTA holds the start of the window, the decode one attempt ahead
+        if (upd) finish_update();
+        if (has_label && !nxt_valid && ahead) { nxt = decode_attempt(tb, p, a_cur + P); nxt_valid = true; }
+        barB_sync(TB);                    // [B] the control warp has written the descriptor
+        d4 = *reinterpret_cast<const uint4*>(&s_desc);      // used, hop, ci, cj
+        ahead = s_desc.ahead != 0;
     }
     if (upd) finish_update();
-
-    if (b == 0) {
+    if (b == 0)
         for (u32 w = tid; w < (N + 31) / 32; w += TW) p.nbits[w] = s_n[w];
-        if (tid == 0) {
-            CgCtl* c = p.ctl;
-            c->attempts = a_start + used_sum; c->hops = hops_start + hl;
-            c->iterations += it_local; c->proposals += (u64)M * it_local;
-            c->dP += dP; c->cur = wbuf; c->epoch += it_local;
-            c->pub_base[0] = cnt0; c->pub_base[1] = cnt1;
-            c->cyc_total += (u64)(clock64() - t_begin);
-#ifdef CG_TRACE
-            c->cyc_wait += cyc_wait; c->cyc_update += cyc_update; c->cyc_propose += cyc_propose;
-#endif
-        }
-    }
 }
 
 // Step a6 alone: scripted hops, update in place (no readers), one launch.
@@ -847,7 +897,7 @@ static bool valid_L(int L, int* lg)
 }
 
 struct WsLayout { size_t eps0, scratch, phi, nbits, tq, tf, cdfi, invr_k, fld_k, disp, guide, slots, ctl, red, total; };
-#define CG_SLOT_BYTES ((size_t)8 * CG_SLOT_U64 * CG_MAX_CTAS)
+#define CG_SLOT_BYTES ((size_t)8 * CG_SLOT_U64 * CG_SLOT_REP * CG_MAX_CTAS)
 
 static WsLayout ws_layout(int L)
 {
@@ -1013,7 +1063,7 @@ static scripted_fn scripted_kernel(int rp)
 static int choose_rp(u64 pairs, int n_ctas, int threads)
 {
     const u64 per_cta = (pairs + n_ctas - 1) / n_ctas;
-    const u64 workers = (u64)threads - 32;               // the last warp of a CTA holds no eps
+    const u64 workers = (u64)threads - 64;               // the last two warps of a CTA hold no eps
     const u64 need = (per_cta + workers - 1) / workers;
     const int cap = threads == 1024 ? 2 : 8;
     for (int rp = 1; rp <= cap; rp *= 2)
@@ -1035,7 +1085,7 @@ static int max_coresident(cg_sim* s, int threads, int rp, bool cached, int* out)
 // threads per CTA that own attempts when the proposals can be cached (M <= n_ctas * pl), else 0
 static int choose_pl(u64 M, int n_ctas, int threads)
 {
-    return M <= (u64)n_ctas * (u64)(threads - 32) ? threads - 32 : 0;
+    return M <= (u64)n_ctas * (u64)(threads - 64) ? threads - 64 : 0;
 }
 
 static int choose_launch(cg_sim* s, int n_ctas, int threads)
@@ -1396,7 +1446,7 @@ extern "C" int cg_set_trace(cg_sim* s, void* dev_buf, size_t bytes, uint32_t ite
 #ifndef CG_TRACE
     return CG_EUNSUPPORTED;                   // the library was built without -DCG_TRACE
 #endif
-    if (((uintptr_t)dev_buf & 7) || bytes < (size_t)8 * CG_TRACE_EV * iterations * CG_MAX_CTAS) return CG_EINVAL;
+    if (((uintptr_t)dev_buf & 7) || bytes < (size_t)8 * 32 * CG_MAX_CTAS) return CG_EINVAL;
     s->d_trace = (u64*)dev_buf; s->trace_iters = iterations;
     return CG_OK;
 }
