@@ -21,6 +21,7 @@
 #include <algorithm>
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <string>
@@ -64,6 +65,7 @@ struct CgCtl {              // device-resident control block (one per sim)
 struct CgParams {           // kernel parameter block
     double* eps[CG_RING];   // ring of local-energy buffers, N each (see "pending hops" below)
     const double* tf;       // unfolded table 1/r, L rows of pitch 2L (see site_code)
+    const double* tq;       // quarter table 1/r, (L/2+1) x (L/2+1), indexed by the folded offsets
     u32* nbits;             // occupations, bit s of word s/32
     const u64* cdfi;        // live tower as integer thresholds: u_d < cdf_k  <=>  m < cdfi_k
     const double* invr_k;   // 1/r of displacement k (live part)
@@ -174,26 +176,35 @@ __device__ __forceinline__ double hop_term(const double* __restrict__ tf, u32 ma
     return __dsub_rn(__ldg(tf + ((sc - cj) & mask)), __ldg(tf + ((sc - ci) & mask)));
 }
 
-// eps slab of one CTA: pairs [pr0, pr1) of adjacent sites.  With RP > 0 thread t keeps pairs
-// pr0 + t + k*THREADS (k < RP) in registers across hops and writes every new value through to
-// global memory for the other CTAs' gathers; with RP == 0 the slab streams src -> dst.
-// issue() starts the table gathers of a hop, finish() adds and stores: the caller puts
-// independent work between the two.
+// eps slab of one CTA: sites [2 pr0, 2 pr1).  With RP > 0 warp w keeps the blocks of 64 consecutive
+// sites number w, w + TW/32, ... (RP of them) in registers across hops - lane l holds sites l and
+// 32 + l of a block, so that every load and store of the warp covers 256 contiguous bytes (the L1
+// wavefront rate, not L2 bandwidth, bounds this kernel) - and writes every new value through to global
+// memory for the other CTAs' gathers; with RP == 0 the slab streams src -> dst.
+// issue() starts the table gathers of a hop, finish() adds and stores: the caller puts independent
+// work between the two.
 template <int TW, int RP>
 struct Slab {
     static constexpr int R = RP > 0 ? RP : 1;
-    double2 e[R];
-    double tj0[R], tj1[R], ti0[R], ti1[R];
-    u32 sc[R];
+    double ea[R], eb[R];
+    double ja[R], ia[R], jb[R], ib[R];
+    u32 sca[R], scb[R];                  // coded sites (spare bit set); 0 marks a site outside the slab
     u32 hci, hcj;
+
+    __device__ __forceinline__ u32 site_a(u32 pr0, int k) const
+    {
+        return 2u * (pr0 + (u32)k * TW + (threadIdx.x & ~31u)) + (threadIdx.x & 31u);
+    }
 
     __device__ __forceinline__ void load(const double* src, u32 pr0, u32 pr1, int L)
     {
 #pragma unroll
         for (int k = 0; k < RP; ++k) {
-            const u32 pr = pr0 + threadIdx.x + k * TW;
-            sc[k] = site_code(2 * pr, L) | (u32)L;
-            if (pr < pr1) e[k] = __ldcg(reinterpret_cast<const double2*>(src + 2 * pr));
+            const u32 sa = site_a(pr0, k), sb = sa + 32u;
+            sca[k] = sa < 2u * pr1 ? site_code(sa, L) | (u32)L : 0u;
+            scb[k] = sb < 2u * pr1 ? site_code(sb, L) | (u32)L : 0u;
+            if (sca[k]) ea[k] = __ldcg(src + sa);
+            if (scb[k]) eb[k] = __ldcg(src + sb);
         }
     }
 
@@ -202,13 +213,8 @@ struct Slab {
         hci = ci; hcj = cj;
 #pragma unroll
         for (int k = 0; k < RP; ++k) {
-            const u32 pr = pr0 + threadIdx.x + k * TW;
-            if (pr < pr1) {
-                const double* aj = tf + ((sc[k] - cj) & mask);
-                const double* ai = tf + ((sc[k] - ci) & mask);
-                tj0[k] = __ldg(aj); tj1[k] = __ldg(aj + 1);
-                ti0[k] = __ldg(ai); ti1[k] = __ldg(ai + 1);
-            }
+            if (sca[k]) { ja[k] = __ldg(tf + ((sca[k] - cj) & mask)); ia[k] = __ldg(tf + ((sca[k] - ci) & mask)); }
+            if (scb[k]) { jb[k] = __ldg(tf + ((scb[k] - cj) & mask)); ib[k] = __ldg(tf + ((scb[k] - ci) & mask)); }
         }
     }
 
@@ -219,24 +225,16 @@ struct Slab {
         if (RP > 0) {
 #pragma unroll
             for (int k = 0; k < RP; ++k) {
-                const u32 pr = pr0 + threadIdx.x + k * TW;
-                if (pr < pr1) {
-                    e[k].x = __dadd_rn(e[k].x, __dsub_rn(tj0[k], ti0[k]));
-                    e[k].y = __dadd_rn(e[k].y, __dsub_rn(tj1[k], ti1[k]));
-                    __stcg(reinterpret_cast<double2*>(dst + 2 * pr), e[k]);
-                }
+                const u32 sa = site_a(pr0, k);
+                if (sca[k]) { ea[k] = __dadd_rn(ea[k], __dsub_rn(ja[k], ia[k])); __stcg(dst + sa, ea[k]); }
+                if (scb[k]) { eb[k] = __dadd_rn(eb[k], __dsub_rn(jb[k], ib[k])); __stcg(dst + sa + 32u, eb[k]); }
             }
         } else {
-            for (u32 pr = pr0 + threadIdx.x; pr < pr1; pr += TW) {
-                const u32 c = site_code(2 * pr, L) | (u32)L;
-                const double* aj = tf + ((c - hcj) & mask);
-                const double* ai = tf + ((c - hci) & mask);
-                const double2 v = __ldcg(reinterpret_cast<const double2*>(src + 2 * pr));
-                const double j0 = __ldg(aj), j1 = __ldg(aj + 1), i0 = __ldg(ai), i1 = __ldg(ai + 1);
-                double2 o;
-                o.x = __dadd_rn(v.x, __dsub_rn(j0, i0));
-                o.y = __dadd_rn(v.y, __dsub_rn(j1, i1));
-                __stcg(reinterpret_cast<double2*>(dst + 2 * pr), o);
+            for (u32 s = 2u * pr0 + threadIdx.x; s < 2u * pr1; s += TW) {
+                const u32 c = site_code(s, L) | (u32)L;
+                const double v = __ldcg(src + s);
+                const double tj = __ldg(tf + ((c - hcj) & mask)), ti = __ldg(tf + ((c - hci) & mask));
+                __stcg(dst + s, __dadd_rn(v, __dsub_rn(tj, ti)));
             }
         }
     }
@@ -1005,7 +1003,7 @@ static CgParams make_params(const cg_sim* s, u64 n_hops)
 {
     CgParams p;
     for (int k = 0; k < CG_RING; ++k) p.eps[k] = s->d_eps[k];
-    p.tf = s->d_tf; p.nbits = s->d_nbits;
+    p.tf = s->d_tf; p.tq = s->d_tq; p.nbits = s->d_nbits;
     p.cdfi = s->d_cdfi; p.invr_k = s->d_invr_k; p.fld_k = s->d_fld_k; p.disp = s->d_disp;
     p.guide = s->d_guide;
     p.slots = s->d_slots; p.ctl = s->d_ctl;
@@ -1370,10 +1368,13 @@ extern "C" int cg_apply_hops(cg_sim* s, uint64_t count, const uint32_t* i, const
     cudaEvent_t e0, e1;
     CK(cudaEventCreate(&e0)); CK(cudaEventCreate(&e1));
     CgParams p = make_params(s, 0);
+    // several small CTAs per SM (one block of 64 sites per warp) keep enough requests in flight to make
+    // the stand-alone update throughput-bound; larger lattices fall back to one CTA per SM
+    const u64 g1 = (s->N / 2 + 255) / 256;
     const int grid = (int)std::max<u64>(1, std::min<u64>((s->N / 2 + 511) / 512, (u64)s->num_sms));
-    scripted_fn uf = scripted_kernel(choose_rp(s->N / 2, grid, 512));
     CK(cudaEventRecord(e0, s->stream));
-    uf<<<grid, 512, 0, s->stream>>>(p, d_ij, d_ij + count, count);
+    if (g1 <= (u64)s->num_sms * 6) cg_update_scripted<256, 1><<<(int)g1, 256, 0, s->stream>>>(p, d_ij, d_ij + count, count);
+    else scripted_kernel(choose_rp(s->N / 2, grid, 512))<<<grid, 512, 0, s->stream>>>(p, d_ij, d_ij + count, count);
     CK(cudaEventRecord(e1, s->stream));
     CK(cudaGetLastError());
     CK(cudaStreamSynchronize(s->stream));
