@@ -64,3 +64,12 @@ def test_product_path_never_touches_the_oracle():
         text = open(os.path.join(ROOT, "oracle", f)).read()
         assert "import paper_1407_5026_b200" not in text and "from paper_1407_5026_b200" not in text
         assert "libcg.so" not in text and '#include "cg.h"' not in text
+
+
+def test_diagnostic_entry_points_validate_arguments(cg):
+    lib = cg.lib()
+    assert lib.cg_set_trace(None, None, 0, 0) == cg.binding.CG_EINVAL
+    assert lib.cg_set_launch(None, 0, 0) == cg.binding.CG_EINVAL
+    assert lib.cg_get_counters(None, None, None, None, None) == cg.binding.CG_EINVAL
+    out = C.c_double()
+    assert lib.cg_bench_l2_rmw(100, 1, 1, C.byref(out)) == cg.binding.CG_EINVAL      # too small a buffer

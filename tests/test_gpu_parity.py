@@ -185,3 +185,61 @@ def test_long_run_properties_at_headline_size(cg):
     n0 = g0.state()[0].astype(np.int64)
     np.subtract.at(n0, i, 1); np.add.at(n0, j, 1)
     assert np.array_equal(n0, n)
+
+
+def test_launch_shape_may_change_between_runs(cg, oracle_lib):
+    """The exchange slots, publication words and the eps ring carry over from one launch shape to the
+    next: the chain must not notice (stale words of other shapes are never mistaken for arrivals)."""
+    kw = dict(L=128, T=0.1, E=0.01, seed=21, M=4096)
+    g = cg.CoulombGlass(hop_log=6000, **kw)
+    for n_ctas, threads, hops in ((0, 0, 1500), (37, 256, 1000), (148, 1024, 1500), (5, 512, 500), (0, 0, 1500)):
+        g.set_launch(n_ctas, threads)
+        g.run(hops)
+    o = oracle_lib.Oracle(**kw)
+    o.run(6000)
+    _compare(g, o, 6000)
+    assert g.recompute_eps() < 1e-9
+
+
+@pytest.mark.parametrize("n_ctas,threads,M", [(148, 512, 303104), (148, 256, 65536), (20, 1024, 65536), (148, 1024, 65536)])
+def test_labels_recomputed_or_cached(cg, oracle_lib, n_ctas, threads, M):
+    """M larger than the label-owning threads of the grid takes the path that decodes every label in
+    every iteration; otherwise proposals are cached.  Both must give the serial chain."""
+    kw = dict(L=256, T=0.05, E=0.01, seed=31, M=M)
+    g = cg.CoulombGlass(hop_log=3000, **kw)
+    g.set_launch(n_ctas, threads)
+    g.run(3000)
+    o = oracle_lib.Oracle(**kw)
+    o.run(3000)
+    _compare(g, o, 3000)
+
+
+def test_config4_M_sweep_is_one_trajectory(cg):
+    """Config 4 of BASELINE.json (L=256, T=0.02): the hop log must be the same for every M (reading G8),
+    including M = resident threads of the chip; only iterations and proposals differ."""
+    import torch
+    sms = torch.cuda.get_device_properties(0).multi_processor_count
+    logs = []
+    for cfg in workloads.CONFIGS["cfg4_L256"]:
+        kw = workloads.init_args(cfg, sms * 2048)
+        g = cg.CoulombGlass(hop_log=20000, **kw)
+        g.run(20000)
+        c = g.counters()
+        assert c["proposals_evaluated"] == kw["M"] * c["iterations"]
+        logs.append((g.hops(), g.state(), c["attempts"]))
+    for (h, st, a) in logs[1:]:
+        for x, y in zip(h, logs[0][0]):
+            assert np.array_equal(x, y)
+        assert np.array_equal(st[0], logs[0][1][0]) and np.array_equal(st[1], logs[0][1][1]) and a == logs[0][2]
+
+
+def test_largest_supported_lattice(cg, oracle_lib):
+    """L = 1024 (N = 2^20): init bit-identical, a short prefix of the chain, drift of the update."""
+    kw = dict(L=1024, T=0.05, E=0.01, seed=12, M=65536)
+    g = cg.CoulombGlass(hop_log=400, **kw)
+    o = oracle_lib.Oracle(**kw)
+    assert np.array_equal(g.state()[1], o.state()[1])
+    g.run(400)
+    o.run(400)
+    _compare(g, o, 400)
+    assert g.recompute_eps() < 1e-9
