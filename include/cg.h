@@ -122,20 +122,24 @@ int cg_get_phi(cg_sim* s, double* phi /* N */);
 int cg_set_launch(cg_sim* s, int n_ctas, int threads);
 int cg_get_launch(cg_sim* s, int* n_ctas, int* threads, int* smem_bytes);
 
-/* Device-side phase timers of CTA 0 accumulated over cg_run calls, in SM clock
- * cycles: total, waiting at the grid exchange, update (W_U), propose+select
- * (W_R) — the paper's split.  reset != 0 zeroes them. */
+/* SM clock cycles CTA 0 spent inside the persistent kernel, accumulated over cg_run calls
+ * (*total).  The propose and update phases of a hop overlap, so there is no meaningful split
+ * into the paper's W_R and W_U inside this kernel: *wait, *update and *propose
+ * are returned as 0; use cg_apply_hops for the update alone and cg_set_trace for a breakdown.
+ * reset != 0 zeroes the counter. */
 int cg_get_phase_cycles(cg_sim* s, uint64_t* total, uint64_t* wait, uint64_t* update,
                         uint64_t* propose, int reset);
 
 /* Optional segment timers of the persistent kernel (diagnostic; needs a library built with
  * -DCG_TRACE, else CG_EUNSUPPORTED; NULL / 0 switches it off).  Every following cg_run adds, for
- * CTA b, to dev_buf[b*32 + c*16 + k] the SM cycles thread 0 spent in segment k of the iterations in
- * which the CTA held the start of the window (c = 0) or not (c = 1): 0 loop bookkeeping, 1 until the
- * slab of the previous hop is stored, 2 until its own proposals are tested, 6 waiting for the
- * publication counter, 3 until the CTA minimum is known (CTA barrier), 4 until the winner is known
- * (exchange), 5 executing the hop and issuing the table gathers; k = 15 counts the iterations.
- * dev_buf: zeroed device memory, 8-byte aligned, 8*32*1024 bytes; `iterations` must be non-zero. */
+ * CTA b, to dev_buf[b*64 + c*16 + k] the SM cycles the CTA's control warp spent in segment k of
+ * the iterations in which the CTA was at scan position 0 (c = 0: it holds the start of the window),
+ * position 1 (c = 2), the last position (c = 3) or elsewhere (c = 1): 6 publication check,
+ * 3 waiting for its workers, 10 CTA minimum and posting it, 4 scanning other CTAs' slots,
+ * 5 what the workers wait for of the bookkeeping, 0 the rest of it; k = 15 counts iterations,
+ * 8 passes of the publication check, 9 scans, 11-14, 1, 2 a histogram of the scan time
+ * (< 500, 1000, 2000, 4000, 8000 cycles, more).
+ * dev_buf: zeroed device memory, 8-byte aligned, 8*64*1024 bytes; `iterations` must be non-zero. */
 int cg_set_trace(cg_sim* s, void* dev_buf, size_t bytes, uint32_t iterations);
 
 /* L2 roofline denominator: one kernel, all SMs,

@@ -239,15 +239,15 @@ class CoulombGlass:
             self._check(self._lib.cg_set_trace(self._h, None, 0, 0))
             self._trace = None
             return
-        self._trace = torch.zeros(32 * 1024, dtype=torch.int64, device=self.device)
+        self._trace = torch.zeros(64 * 1024, dtype=torch.int64, device=self.device)
         self._check(self._lib.cg_set_trace(self._h, C.c_void_p(self._trace.data_ptr()),
                                            self._trace.numel() * 8, 1))
 
     def trace(self):
-        """-> int64 array [n_ctas, 2, 16] of SM cycles (see cg_set_trace in include/cg.h)."""
+        """-> int64 array [n_ctas, 4, 16] of SM cycles (see cg_set_trace in include/cg.h)."""
         self._torch.cuda.synchronize(self.device)
         n = self.launch()["n_ctas"]
-        return self._trace.view(1024, 2, 16)[:n].cpu().numpy()
+        return self._trace.view(1024, 4, 16)[:n].cpu().numpy()
 
     def phase_cycles(self, reset=False):
         t, w, u, p = C.c_uint64(), C.c_uint64(), C.c_uint64(), C.c_uint64()

@@ -4,15 +4,22 @@
 // The ABI is declared and documented in include/cg.h.  DESIGN.md explains the
 // kernel design; the short version:
 //   * one persistent cooperative kernel runs the whole propose -> select ->
-//     apply -> update loop; there is ONE grid-wide exchange per
-//     PR iteration, which carries both the lowest accepting label and the
-//     "all local-energy slabs are written" guarantee;
-//   * eps is double-buffered: after hop h every CTA writes eps_h for its own slab
-//     into the other buffer while proposals read eps_{h-1} and add the pending
-//     correction 1/r_lj - 1/r_li of hop h themselves (same single rounded add as
-//     the update, so the values are bit-identical to the serial algorithm);
+//     apply -> update loop, one CTA per SM; in each CTA 14 worker
+//     warps test proposals and update eps, a control warp does the exchange and the
+//     bookkeeping, a service warp publishes finished slab updates;
+//   * the grid exchange is one-way most of the time: slots are scanned in label
+//     order and the scan stops at the first accepting CTA, so the CTA that holds
+//     the start of the window never waits for the others;
+//   * every thread owns the attempts a = g (mod P), keeps its proposal decoded and,
+//     while theta_ij = 1, follows the two local energies it needs in registers by
+//     adding every executed hop's term itself (the same rounded adds as the update);
+//   * each CTA keeps its eps slab in registers and writes it through to a ring of
+//     buffers; readers only touch a buffer that every CTA has published and add the
+//     terms of the (at most CG_DEPTH) newer hops in hop order, so no reader ever
+//     waits for a writer and every value is bit-identical to the serial algorithm;
 //   * occupations live as a bitmap in every CTA's shared memory, next to the live
-//     part of the tower; 1/r comes from a quarter table in L2.
+//     part of the tower and its guide table; 1/r comes from an
+//     unfolded table in L2 indexed with one subtraction and one mask.
 // Nothing in this file is shared with oracle/ (the CPU reference).
 #include "cg.h"
 
@@ -21,7 +28,6 @@
 #include <algorithm>
 #include <cmath>
 #include <cstdio>
-#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <string>
@@ -36,13 +42,13 @@ typedef unsigned int u32;
 
 // ------------------------------------------------------------------ device --
 
+#ifndef CG_DEPTH
 #define CG_DEPTH 4          // pending hops: proposals read eps_{h-DEPTH} and add the newer hops' terms themselves
+#endif
 #define CG_RING (2 * CG_DEPTH + 1)   // eps buffers: eps_{h+1-2 DEPTH} .. eps_{h+1} can be live at the same time
-#define CG_SRING 8          // exchange slots per CTA: a CTA posts up to DEPTH exchanges ahead of the slowest reader
-#define CG_SLOT_REP 1       // replicas of every exchange slot (more did not make the polls faster)
-#define CG_PUB_U64 16       // offset of a CTA's publication word in its slot line (u64 units)
-#define CG_SLOT_U64 32      // one exchange slot per CTA, 256-byte stride (own L2 slice), in u64 units
-#define CG_TRACE_EV 24      // events per iteration in the optional trace (cg_set_trace)
+#define CG_SRING 16         // exchange slots per CTA: a CTA posts up to DEPTH exchanges ahead of the slowest reader
+#define CG_PUB_U64 32       // offset of a CTA's publication word in its slot block (u64 units)
+#define CG_SLOT_U64 64      // one block per CTA, 512-byte stride: the slot ring in the first half, the pub word after it
 #define CG_GUIDE 352        // tower guide: (43 + 1) binades x 8 sub-buckets of t = 2^43 - m
 
 struct CgCtl {              // device-resident control block (one per sim)
@@ -82,7 +88,7 @@ struct CgParams {           // kernel parameter block
     double T, E;
     float inv_T;            // (float)(1/T), pre-test of the Metropolis factor only
     u64 n_hops;
-    u64* trace;             // optional event trace: [CTA][iteration][CG_TRACE_EV] globaltimer ns
+    u64* trace;             // optional segment timers (cg_set_trace), 64 words per CTA
     u32 trace_iters;
 };
 
@@ -119,11 +125,7 @@ __device__ __forceinline__ u64 ld_relaxed_u64(const u64* p)
 }
 __device__ __forceinline__ void st_release_u64(u64* p, u64 v)
 {
-#ifdef CG_EXP_NOMEMBAR
-    asm volatile("st.relaxed.gpu.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
-#else
     asm volatile("st.release.gpu.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
-#endif
 }
 __device__ __forceinline__ u64 global_ns()
 {
@@ -131,31 +133,20 @@ __device__ __forceinline__ u64 global_ns()
     asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
     return t;
 }
-#ifdef CG_EXP_NOACQ
-__device__ __forceinline__ void fence_acquire_gpu() { }
-#else
 __device__ __forceinline__ void fence_acquire_gpu() { asm volatile("fence.acquire.gpu;" ::: "memory"); }
-#endif
 // named barriers 1 .. CG_DEPTH (cyclic in the hop number): the warps that wrote eps arrive, the
 // service warp waits for them; barrier 0 with an explicit count synchronises the worker warps only
-__device__ __forceinline__ void barN_arrive(u32 k, int n)      // barrier 1 + k, k < 4
-{
-    switch (k) {
-        case 0: asm volatile("bar.arrive 1, %0;" ::"r"(n) : "memory"); break;
-        case 1: asm volatile("bar.arrive 2, %0;" ::"r"(n) : "memory"); break;
-        case 2: asm volatile("bar.arrive 3, %0;" ::"r"(n) : "memory"); break;
-        default: asm volatile("bar.arrive 4, %0;" ::"r"(n) : "memory"); break;
-    }
-}
-__device__ __forceinline__ void barN_sync(u32 k, int n)
-{
-    switch (k) {
-        case 0: asm volatile("bar.sync 1, %0;" ::"r"(n) : "memory"); break;
-        case 1: asm volatile("bar.sync 2, %0;" ::"r"(n) : "memory"); break;
-        case 2: asm volatile("bar.sync 3, %0;" ::"r"(n) : "memory"); break;
-        default: asm volatile("bar.sync 4, %0;" ::"r"(n) : "memory"); break;
-    }
-}
+#define CG_BARN(OP) switch (k) { \
+        case 0: asm volatile(OP " 1, %0;" ::"r"(n) : "memory"); break; \
+        case 1: asm volatile(OP " 2, %0;" ::"r"(n) : "memory"); break; \
+        case 2: asm volatile(OP " 3, %0;" ::"r"(n) : "memory"); break; \
+        case 3: asm volatile(OP " 4, %0;" ::"r"(n) : "memory"); break; \
+        case 4: asm volatile(OP " 6, %0;" ::"r"(n) : "memory"); break; \
+        case 5: asm volatile(OP " 7, %0;" ::"r"(n) : "memory"); break; \
+        case 6: asm volatile(OP " 8, %0;" ::"r"(n) : "memory"); break; \
+        default: asm volatile(OP " 9, %0;" ::"r"(n) : "memory"); break; }
+__device__ __forceinline__ void barN_arrive(u32 k, int n) { CG_BARN("bar.arrive") }   // k < CG_DEPTH <= 8
+__device__ __forceinline__ void barN_sync(u32 k, int n) { CG_BARN("bar.sync") }
 __device__ __forceinline__ void barX_sync(int n) { asm volatile("bar.sync 0, %0;" ::"r"(n) : "memory"); }
 // barrier 5: second CTA barrier of an iteration; the control warp only arrives
 __device__ __forceinline__ void barB_sync(int n) { asm volatile("bar.sync 5, %0;" ::"r"(n) : "memory"); }
@@ -309,8 +300,9 @@ __device__ __forceinline__ bool metropolis(double dE, u32 uh, u32 ul, double T, 
 #ifdef CG_TRACE
 // segment timers of thread 0 (SM cycles), summed over the launch, separately for iterations in which
 // this CTA held the start of the window (class 0) or not (class 1): p.trace[b*32 + class*16 + segment]
+#define CLS_ (kb == 0 ? 0 : kb == 1 ? 32 : kb == nb - 1 ? 48 : 16)
 #define TRACE(ev, extra) do { if (lane == 0) { const long long now_ = clock64(); \
-    s_seg[(kb == 0 ? 0 : 16) + (ev)] += (u64)(now_ - t_prev); t_prev = now_; } } while (0)
+    s_seg[CLS_ + (ev)] += (u64)(now_ - t_prev); t_prev = now_; } } while (0)
 #else
 #define TRACE(ev, extra) do { } while (0)
 #endif
@@ -327,7 +319,7 @@ struct Pend {               // pending hops, for threads that start to follow a 
     u32 npend, rbuf, head;  // entry k (oldest first) is c[(head + k) % CG_DEPTH]
     u32 c[CG_DEPTH][2];     // coded sites (i, j)
 };
-static_assert(CG_DEPTH <= 4 && CG_DEPTH < CG_SRING, "named barriers 1..4, slot ring");
+static_assert(CG_DEPTH <= 8 && CG_DEPTH < CG_SRING, "named barriers, slot ring");
 
 // The persistent kernel: steps 1, 2, 3a-3c of the mixed PR algorithm.
 // CACHED: thread g of the grid owns the attempts a = g (mod P), P = gridDim.x * PL >= M, keeps its
@@ -357,8 +349,8 @@ __global__ void __launch_bounds__(THREADS, 1) cg_pr_persistent(const CgParams p)
     __shared__ __align__(8) Pend s_pend;
     const Tables tb = {s_cdfi, s_invr, s_fld, s_disp, s_guide};
 #ifdef CG_TRACE
-    __shared__ u64 s_seg[32];
-    if (threadIdx.x < 32) s_seg[threadIdx.x] = 0;
+    __shared__ u64 s_seg[64];
+    if (threadIdx.x < 64) s_seg[threadIdx.x] = 0;
     long long t_prev = 0;
 #endif
 
@@ -404,7 +396,7 @@ __global__ void __launch_bounds__(THREADS, 1) cg_pr_persistent(const CgParams p)
         if (nb > 1)
             for (u64 h = 0; h < p.n_hops; ++h) {
                 barN_sync((u32)(h % CG_DEPTH), TB);
-                if (lane == 0) st_release_u64(p.slots + (size_t)b * (CG_SLOT_REP * CG_SLOT_U64) + CG_PUB_U64, pub_base + h + 1);
+                if (lane == 0) st_release_u64(p.slots + (size_t)b * CG_SLOT_U64 + CG_PUB_U64, pub_base + h + 1);
             }
         return;
     }
@@ -433,7 +425,7 @@ __global__ void __launch_bounds__(THREADS, 1) cg_pr_persistent(const CgParams p)
 
     const u32 pairs = N / 2, pper = (pairs + nb - 1) / nb;
     const u32 pr0 = min(pairs, b * pper), pr1 = min(pairs, pr0 + pper);
-    u64* const my_slot = p.slots + (size_t)b * (CG_SLOT_REP * CG_SLOT_U64);   // replica r at + r * CG_SLOT_U64
+    u64* const my_slot = p.slots + (size_t)b * CG_SLOT_U64;
 
     if (warp == NWK) {
         // ------------------------------------------------------------------ control warp ----
@@ -458,7 +450,7 @@ __global__ void __launch_bounds__(THREADS, 1) cg_pr_persistent(const CgParams p)
             const u32 e32 = e_start + it_local;
             const u32 kb = b >= c_first ? b - c_first : b + nb - c_first;    // my scan position
 #ifdef CG_TRACE
-            if (lane == 0) { if (t_prev == 0) t_prev = clock64(); s_seg[(kb == 0 ? 0 : 16) + 15] += 1; }
+            if (lane == 0) { if (t_prev == 0) t_prev = clock64(); s_seg[CLS_ + 15] += 1; }
 #endif
             // The buffer that becomes rbuf at the next executed hop must be complete on every CTA before the
             // workers of this CTA are let into the next iteration: one publication word per CTA, each in its
@@ -471,11 +463,14 @@ __global__ void __launch_bounds__(THREADS, 1) cg_pr_persistent(const CgParams p)
 #pragma unroll
                         for (int k = 0; k < 8; ++k) {
                             const u32 c = c0 + 32 * k;
-                            v[k] = c < nb ? ld_relaxed_u64(p.slots + (size_t)c * (CG_SLOT_REP * CG_SLOT_U64) + CG_PUB_U64) : ~0ull;
+                            v[k] = c < nb ? ld_relaxed_u64(p.slots + (size_t)c * CG_SLOT_U64 + CG_PUB_U64) : ~0ull;
                         }
 #pragma unroll
                         for (int k = 0; k < 8; ++k) ok = ok && v[k] >= need_pub;
                     }
+#ifdef CG_TRACE
+                    if (lane == 0) s_seg[CLS_ + 8] += 1;      // passes of the publication check
+#endif
                     if (__all_sync(CG_FULL, ok)) break;
                 }
                 fence_acquire_gpu();
@@ -502,11 +497,15 @@ __global__ void __launch_bounds__(THREADS, 1) cg_pr_persistent(const CgParams p)
             // A CTA can be up to three exchanges ahead of the slowest reader of its slot (bounded by the
             // publication check and by every fully rejected window, which needs all slots): ring of four.
             const u32 ring = (e32 & (CG_SRING - 1u)) * 2u;
-            if (nb > 1 && lane < CG_SLOT_REP)
-                slot_store(my_slot + lane * CG_SLOT_U64 + ring, ((u64)e32 << 32) | gmin,
+            if (nb > 1 && lane == 0)
+                slot_store(my_slot + ring, ((u64)e32 << 32) | gmin,
                            ((u64)(e32 & 0xFFFFu) << 48) | ((gpay >> 32) << 24) | (gpay & 0xFFFFFFu));
             u32 q = gmin; u64 wp = gpay;
+            TRACE(10, 0);
             if (!(own_low && kb == 0) && nb > 1) {
+#ifdef CG_TRACE
+                if (lane == 0) s_seg[CLS_ + 9] += 1;      // scans
+#endif
                 u32 tlab = CG_NONE; u64 tpay = 0;                      // tail accept of position 0
                 const u32 e16 = e32 & 0xFFFFu;
                 const u32 k_end = own_low ? kb : nb;    // an accept of my own: only earlier CTAs can beat it
@@ -516,7 +515,7 @@ __global__ void __launch_bounds__(THREADS, 1) cg_pr_persistent(const CgParams p)
                     const u32 k = k0 + lane;
                     const bool mine = k < k_end && (u32)lane < width && k != kb;
                     u32 c = c_first + k; if (c >= nb) c -= nb;
-                    const u64* sl = p.slots + ((size_t)(mine ? c : b) * CG_SLOT_REP + (b & (CG_SLOT_REP - 1))) * CG_SLOT_U64 + ring;
+                    const u64* sl = p.slots + (size_t)(mine ? c : b) * CG_SLOT_U64 + ring;
                     bool ready = !mine; u32 l = CG_NONE; u64 q1 = 0;
                     for (;;) {
                         if (!ready) {
@@ -549,6 +548,13 @@ __global__ void __launch_bounds__(THREADS, 1) cg_pr_persistent(const CgParams p)
                     q = tlab; wp = ((tpay >> 24) & 0xFFFFFFull) << 32 | (tpay & 0xFFFFFFull);
                 }
             }
+#ifdef CG_TRACE
+            if (lane == 0 && !(own_low && kb == 0) && nb > 1) {       // histogram of the scan time
+                const long long dt = clock64() - t_prev;
+                const int bin = dt < 500 ? 11 : dt < 1000 ? 12 : dt < 2000 ? 13 : dt < 4000 ? 14 : dt < 8000 ? 1 : 2;
+                s_seg[CLS_ + bin] += 1;
+            }
+#endif
             TRACE(4, 0);
             // ---- what the workers need: attempts consumed (m = (p-1)M + q per executed hop, PAPER.md:39,
             // 78), the hop (step 3a), occupations, pending list
@@ -599,7 +605,7 @@ __global__ void __launch_bounds__(THREADS, 1) cg_pr_persistent(const CgParams p)
         }
 #ifdef CG_TRACE
         __syncwarp();
-        if (p.trace) p.trace[(size_t)b * 32 + lane] += s_seg[lane];
+        if (p.trace) { p.trace[(size_t)b * 64 + lane] += s_seg[lane]; p.trace[(size_t)b * 64 + 32 + lane] += s_seg[32 + lane]; }
 #endif
         if (b == 0 && lane == 0) {
             CgCtl* c = p.ctl;
@@ -895,7 +901,7 @@ static bool valid_L(int L, int* lg)
 }
 
 struct WsLayout { size_t eps0, scratch, phi, nbits, tq, tf, cdfi, invr_k, fld_k, disp, guide, slots, ctl, red, total; };
-#define CG_SLOT_BYTES ((size_t)8 * CG_SLOT_U64 * CG_SLOT_REP * CG_MAX_CTAS)
+#define CG_SLOT_BYTES ((size_t)8 * CG_SLOT_U64 * CG_MAX_CTAS)
 
 static WsLayout ws_layout(int L)
 {
@@ -1447,7 +1453,7 @@ extern "C" int cg_set_trace(cg_sim* s, void* dev_buf, size_t bytes, uint32_t ite
 #ifndef CG_TRACE
     return CG_EUNSUPPORTED;                   // the library was built without -DCG_TRACE
 #endif
-    if (((uintptr_t)dev_buf & 7) || bytes < (size_t)8 * 32 * CG_MAX_CTAS) return CG_EINVAL;
+    if (((uintptr_t)dev_buf & 7) || bytes < (size_t)8 * 64 * CG_MAX_CTAS) return CG_EINVAL;
     s->d_trace = (u64*)dev_buf; s->trace_iters = iterations;
     return CG_OK;
 }
