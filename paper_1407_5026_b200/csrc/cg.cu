@@ -476,6 +476,32 @@ __global__ void __launch_bounds__(THREADS, 1) cg_pr_persistent(const CgParams p)
                 fence_acquire_gpu();
             }
             TRACE(6, 0);
+            // A CTA that does not hold the start of the window usually runs behind the one that does: the
+            // winner of this exchange may already be posted.  One look at the first two scan positions
+            // before the barrier takes that round trip off the path between the two barriers.
+            const u32 tail0 = CACHED ? per - t0r : CG_NONE;            // position 0: labels >= tail0 are tail labels
+            const u32 ring = (e32 & (CG_SRING - 1u)) * 2u;
+            const u32 e16 = e32 & 0xFFFFu;
+            u32 eq = CG_NONE; u64 ewp = 0;
+            if (nb > 1 && kb != 0) {
+                const bool mine = lane < 2 && (u32)lane < kb;
+                u32 c = c_first + lane; if (c >= nb) c -= nb;
+                u32 l = CG_NONE; u64 q0 = 0, q1 = 0; bool ready = false;
+                if (mine) {
+                    slot_load(p.slots + (size_t)c * CG_SLOT_U64 + ring, q0, q1);
+                    ready = (u32)(q0 >> 32) == e32 && (u32)(q1 >> 48) == e16;
+                    l = ready ? (u32)q0 : CG_NONE;
+                    if (CACHED && lane == 0 && l != CG_NONE && l >= tail0) l = CG_NONE;    // tail labels never win early
+                }
+                const u32 racc = __ballot_sync(CG_FULL, mine && ready && l != CG_NONE);
+                const u32 rnot = __ballot_sync(CG_FULL, mine && !ready);
+                const int fa = racc ? __ffs(racc) - 1 : 32, fn = rnot ? __ffs(rnot) - 1 : 32;
+                if (fa < fn) {
+                    eq = __shfl_sync(CG_FULL, l, fa);
+                    ewp = __shfl_sync(CG_FULL, q1, fa);
+                    ewp = ((ewp >> 24) & 0xFFFFFFull) << 32 | (ewp & 0xFFFFFFull);
+                }
+            }
             barX_sync(TB);                // [A] the workers have tested their proposals
             TRACE(3, 0);
             // ---- step 3: lowest accepting label: CTA, then grid
@@ -492,22 +518,26 @@ __global__ void __launch_bounds__(THREADS, 1) cg_pr_persistent(const CgParams p)
             // in its threads below a0's ("tail" labels).  The winner is the first non-tail accept in scan
             // order; the scan stops there: slots of later CTAs are never waited for (their proposals
             // cannot win), and the first CTA, when it accepts, waits for nobody.
-            const u32 tail0 = CACHED ? per - t0r : CG_NONE;            // position 0: labels >= tail0 are tail labels
             const bool own_low = gmin != CG_NONE && (!CACHED || kb != 0 || gmin < tail0);
-            // A CTA can be up to three exchanges ahead of the slowest reader of its slot (bounded by the
-            // publication check and by every fully rejected window, which needs all slots): ring of four.
-            const u32 ring = (e32 & (CG_SRING - 1u)) * 2u;
+            // A CTA can be up to DEPTH + 1 exchanges ahead of the slowest reader of its slot (bounded by the
+            // publication check and by every fully rejected window, which needs all slots): ring of CG_SRING.
             if (nb > 1 && lane == 0)
                 slot_store(my_slot + ring, ((u64)e32 << 32) | gmin,
                            ((u64)(e32 & 0xFFFFu) << 48) | ((gpay >> 32) << 24) | (gpay & 0xFFFFFFu));
             u32 q = gmin; u64 wp = gpay;
             TRACE(10, 0);
-            if (!(own_low && kb == 0) && nb > 1) {
+#ifdef CG_TRACE_EVENTS
+            if (p.trace && lane == 0 && it_local < 4096) {
+                u64* ev = p.trace + 64 * 1024 + ((size_t)it_local * 1024 + b) * 4;
+                ev[0] = global_ns(); ev[1] = ((u64)kb << 32) | gmin;
+            }
+#endif
+            if (eq != CG_NONE) { q = eq; wp = ewp; }                   // answered before the barrier
+            else if (!(own_low && kb == 0) && nb > 1) {
 #ifdef CG_TRACE
                 if (lane == 0) s_seg[CLS_ + 9] += 1;      // scans
 #endif
                 u32 tlab = CG_NONE; u64 tpay = 0;                      // tail accept of position 0
-                const u32 e16 = e32 & 0xFFFFu;
                 const u32 k_end = own_low ? kb : nb;    // an accept of my own: only earlier CTAs can beat it
                 u32 k0 = 0, width = 2;                  // the winner is almost always in the first CTAs
                 bool found = false;
@@ -553,6 +583,12 @@ __global__ void __launch_bounds__(THREADS, 1) cg_pr_persistent(const CgParams p)
                 const long long dt = clock64() - t_prev;
                 const int bin = dt < 500 ? 11 : dt < 1000 ? 12 : dt < 2000 ? 13 : dt < 4000 ? 14 : dt < 8000 ? 1 : 2;
                 s_seg[CLS_ + bin] += 1;
+            }
+#endif
+#ifdef CG_TRACE_EVENTS
+            if (p.trace && lane == 0 && it_local < 4096) {
+                u64* ev = p.trace + 64 * 1024 + ((size_t)it_local * 1024 + b) * 4;
+                ev[2] = global_ns(); ev[3] = q;
             }
 #endif
             TRACE(4, 0);
