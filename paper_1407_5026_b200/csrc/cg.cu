@@ -1134,8 +1134,9 @@ static int choose_launch(cg_sim* s, int n_ctas, int threads)
     if (threads != 256 && threads != 512 && threads != 1024) return CG_EINVAL;
     const bool heuristic = n_ctas == 0;
     if (heuristic) {
-        const u64 work = std::max<u64>(s->M, s->N / 2);
-        n_ctas = (int)std::min<u64>((work + threads - 1) / threads, (u64)s->num_sms);
+        const u64 work = std::max<u64>(s->M, s->N / 2);        // labels or pairs of sites, per worker thread
+        const u64 workers = (u64)threads - 64;
+        n_ctas = (int)std::min<u64>((work + workers - 1) / workers, (u64)s->num_sms);
         n_ctas = std::max(1, n_ctas);
     }
     if (n_ctas < 1 || n_ctas > CG_MAX_CTAS) return CG_EINVAL;
