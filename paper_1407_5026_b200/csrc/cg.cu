@@ -46,9 +46,6 @@ typedef unsigned int u32;
 #define CG_DEPTH 4          // pending hops: proposals read eps_{h-DEPTH} and add the newer hops' terms themselves
 #endif
 #define CG_RING (2 * CG_DEPTH + 1)   // eps buffers: eps_{h+1-2 DEPTH} .. eps_{h+1} can be live at the same time
-#ifndef CG_WATCH_SLEEP
-#define CG_WATCH_SLEEP 100  // ns between two looks at another CTA's slot
-#endif
 #define CG_SRING 16         // exchange slots per CTA: a CTA posts up to DEPTH exchanges ahead of the slowest reader
 #define CG_PUB_U64 32       // offset of a CTA's publication word in its slot block (u64 units)
 #define CG_SLOT_U64 64      // one block per CTA, 512-byte stride: the slot ring in the first half, the pub word after it
@@ -348,7 +345,6 @@ __global__ void __launch_bounds__(THREADS, 1) cg_pr_persistent(const CgParams p)
     u32* s_n = s_guide + CG_GUIDE;
     __shared__ u32 s_wlab[32];
     __shared__ u64 s_wpay[32];
-    __shared__ u32 s_arrived;             // worker warps that have delivered their minimum, summed over iterations
     __shared__ __align__(16) Desc s_desc;
     __shared__ __align__(8) Pend s_pend;
     const Tables tb = {s_cdfi, s_invr, s_fld, s_disp, s_guide};
@@ -371,7 +367,6 @@ __global__ void __launch_bounds__(THREADS, 1) cg_pr_persistent(const CgParams p)
     for (int k = tid; k < CG_GUIDE; k += THREADS) s_guide[k] = p.guide[k];
     for (u32 w = tid; w < (N + 31) / 32; w += THREADS) s_n[w] = p.nbits[w];
     if (tid == 0) {
-        s_arrived = 0;
         s_pend.npend = 0; s_pend.rbuf = p.ctl->cur; s_pend.head = 0;
     }
 
@@ -482,44 +477,32 @@ __global__ void __launch_bounds__(THREADS, 1) cg_pr_persistent(const CgParams p)
             }
             TRACE(6, 0);
             // A CTA that does not hold the start of the window usually runs behind the one that does: the
-            // winner of this exchange may be posted before this CTA's workers are done.  While waiting for
-            // them (a counter in shared memory instead of a hardware barrier, so that this warp can do
-            // something meanwhile) the first two scan positions are watched; an answer found here takes the
-            // exchange round trip off the path between the workers' two synchronisation points.
+            // winner of this exchange may already be posted.  One look at the first two scan positions
+            // before the barrier takes that round trip off the path between the two barriers.
             const u32 tail0 = CACHED ? per - t0r : CG_NONE;            // position 0: labels >= tail0 are tail labels
             const u32 ring = (e32 & (CG_SRING - 1u)) * 2u;
             const u32 e16 = e32 & 0xFFFFu;
             u32 eq = CG_NONE; u64 ewp = 0;
-            {
-                const u32 target = (u32)NWK * (it_local + 1u);
-                const bool watch = nb > 1 && kb != 0;
+            if (nb > 1 && kb != 0) {
                 const bool mine = lane < 2 && (u32)lane < kb;
                 u32 c = c_first + lane; if (c >= nb) c -= nb;
-                const u64* sl = p.slots + (size_t)(mine ? c : b) * CG_SLOT_U64 + ring;
-                for (;;) {
-                    const bool arrived = *(volatile u32*)&s_arrived == target;
-                    if (watch && eq == CG_NONE) {
-                        u32 l = CG_NONE; u64 q0 = 0, q1 = 0; bool ready = false;
-                        if (mine) {
-                            slot_load(sl, q0, q1);
-                            ready = (u32)(q0 >> 32) == e32 && (u32)(q1 >> 48) == e16;
-                            l = ready ? (u32)q0 : CG_NONE;
-                            if (CACHED && lane == 0 && l != CG_NONE && l >= tail0) l = CG_NONE;   // tail labels never win early
-                        }
-                        const u32 racc = __ballot_sync(CG_FULL, mine && ready && l != CG_NONE);
-                        const u32 rnot = __ballot_sync(CG_FULL, mine && !ready);
-                        const int fa = racc ? __ffs(racc) - 1 : 32, fn = rnot ? __ffs(rnot) - 1 : 32;
-                        if (fa < fn) {
-                            eq = __shfl_sync(CG_FULL, l, fa);
-                            ewp = __shfl_sync(CG_FULL, q1, fa);
-                            ewp = ((ewp >> 24) & 0xFFFFFFull) << 32 | (ewp & 0xFFFFFFull);
-                        }
-                    }
-                    if (__all_sync(CG_FULL, arrived)) break;        // [A] the workers have tested their proposals
-                    if (eq == CG_NONE) __nanosleep(CG_WATCH_SLEEP);     // ~150 CTAs watch the same slot: do not hammer it
+                u32 l = CG_NONE; u64 q0 = 0, q1 = 0; bool ready = false;
+                if (mine) {
+                    slot_load(p.slots + (size_t)c * CG_SLOT_U64 + ring, q0, q1);
+                    ready = (u32)(q0 >> 32) == e32 && (u32)(q1 >> 48) == e16;
+                    l = ready ? (u32)q0 : CG_NONE;
+                    if (CACHED && lane == 0 && l != CG_NONE && l >= tail0) l = CG_NONE;    // tail labels never win early
                 }
-                __threadfence_block();
+                const u32 racc = __ballot_sync(CG_FULL, mine && ready && l != CG_NONE);
+                const u32 rnot = __ballot_sync(CG_FULL, mine && !ready);
+                const int fa = racc ? __ffs(racc) - 1 : 32, fn = rnot ? __ffs(rnot) - 1 : 32;
+                if (fa < fn) {
+                    eq = __shfl_sync(CG_FULL, l, fa);
+                    ewp = __shfl_sync(CG_FULL, q1, fa);
+                    ewp = ((ewp >> 24) & 0xFFFFFFull) << 32 | (ewp & 0xFFFFFFull);
+                }
             }
+            barX_sync(TB);                // [A] the workers have tested their proposals
             TRACE(3, 0);
             // ---- step 3: lowest accepting label: CTA, then grid
             u32 gmin; u64 gpay;
@@ -764,8 +747,7 @@ __global__ void __launch_bounds__(THREADS, 1) cg_pr_persistent(const CgParams p)
             const int src = __ffs(__ballot_sync(CG_FULL, best == wmin)) - 1;
             if (lane == src) { s_wlab[warp] = wmin; s_wpay[warp] = ((u64)bi << 32) | (u64)bj; }
         }
-        __syncwarp();
-        if (lane == 0) { __threadfence_block(); atomicAdd(&s_arrived, 1u); }     // [A] tells the control warp
+        barX_sync(TB);                    // [A]
         // while the control warp does the exchange: the slab of the previous hop (its table gathers,
         // issued when that hop was executed, have had the whole propose phase to arrive) and, if another
         // CTA holds the start of the window, the decode one attempt ahead
