@@ -526,12 +526,6 @@ __global__ void __launch_bounds__(THREADS, 1) cg_pr_persistent(const CgParams p)
                            ((u64)(e32 & 0xFFFFu) << 48) | ((gpay >> 32) << 24) | (gpay & 0xFFFFFFu));
             u32 q = gmin; u64 wp = gpay;
             TRACE(10, 0);
-#ifdef CG_TRACE_EVENTS
-            if (p.trace && lane == 0 && it_local < 4096) {
-                u64* ev = p.trace + 64 * 1024 + ((size_t)it_local * 1024 + b) * 4;
-                ev[0] = global_ns(); ev[1] = ((u64)kb << 32) | gmin;
-            }
-#endif
             if (eq != CG_NONE) { q = eq; wp = ewp; }                   // answered before the barrier
             else if (!(own_low && kb == 0) && nb > 1) {
 #ifdef CG_TRACE
@@ -583,12 +577,6 @@ __global__ void __launch_bounds__(THREADS, 1) cg_pr_persistent(const CgParams p)
                 const long long dt = clock64() - t_prev;
                 const int bin = dt < 500 ? 11 : dt < 1000 ? 12 : dt < 2000 ? 13 : dt < 4000 ? 14 : dt < 8000 ? 1 : 2;
                 s_seg[CLS_ + bin] += 1;
-            }
-#endif
-#ifdef CG_TRACE_EVENTS
-            if (p.trace && lane == 0 && it_local < 4096) {
-                u64* ev = p.trace + 64 * 1024 + ((size_t)it_local * 1024 + b) * 4;
-                ev[2] = global_ns(); ev[3] = q;
             }
 #endif
             TRACE(4, 0);

@@ -243,3 +243,19 @@ def test_largest_supported_lattice(cg, oracle_lib):
     o.run(400)
     _compare(g, o, 400)
     assert g.recompute_eps() < 1e-9
+
+
+def test_replicas_on_separate_streams_run_concurrently_and_independently(cg, oracle_lib):
+    """Independent samples (the paper's recommended use of more hardware): config 3's four
+    temperatures as four sims on four streams, launched back to back; each must be its own serial chain."""
+    import torch
+    sims = []
+    for cfg in workloads.CONFIGS["cfg3_L128"]:
+        kw = workloads.init_args(cfg)
+        sims.append((kw, cg.CoulombGlass(hop_log=5000, stream=torch.cuda.Stream(), **kw)))
+    for _, g in sims:
+        g.run(5000)                       # asynchronous: the four persistent kernels overlap
+    for kw, g in sims:
+        o = oracle_lib.Oracle(**kw)
+        o.run(5000)
+        _compare(g, o, 5000)
