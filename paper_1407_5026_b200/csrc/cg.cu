@@ -676,7 +676,6 @@ __global__ void __launch_bounds__(THREADS, 1) cg_pr_persistent(const CgParams p)
             ++hl;
             hci = d4.z; hcj = d4.w;
             wbuf = wbuf == CG_RING - 1 ? 0u : wbuf + 1u;
-            slab.issue(tf, mask, pr0, pr1, hci, hcj);
             upd = true;
         }
         if (hl >= p.n_hops) break;
@@ -739,13 +738,13 @@ __global__ void __launch_bounds__(THREADS, 1) cg_pr_persistent(const CgParams p)
         // while the control warp does the exchange: the slab of the previous hop (its table gathers,
         // issued when that hop was executed, have had the whole propose phase to arrive) and, if another
         // CTA holds the start of the window, the decode one attempt ahead
-        if (upd) finish_update();
+        if (upd) { slab.issue(tf, mask, pr0, pr1, hci, hcj); finish_update(); }
         if (has_label && !nxt_valid && ahead) { nxt = decode_attempt(tb, p, a_cur + P); nxt_valid = true; }
         barB_sync(TB);                    // [B] the control warp has written the descriptor
         d4 = *reinterpret_cast<const uint4*>(&s_desc);      // used, hop, ci, cj
         ahead = s_desc.ahead != 0;
     }
-    if (upd) finish_update();
+    if (upd) { slab.issue(tf, mask, pr0, pr1, hci, hcj); finish_update(); }
     if (b == 0)
         for (u32 w = tid; w < (N + 31) / 32; w += TW) p.nbits[w] = s_n[w];
 }
