@@ -533,11 +533,11 @@ __global__ void __launch_bounds__(THREADS, 1) cg_pr_persistent(const CgParams p)
 #endif
                 u32 tlab = CG_NONE; u64 tpay = 0;                      // tail accept of position 0
                 const u32 k_end = own_low ? kb : nb;    // an accept of my own: only earlier CTAs can beat it
-                u32 k0 = 0, width = 2;                  // the winner is almost always in the first CTAs
+                u32 k0 = 0;                             // 32 scan positions at a time (measured best)
                 bool found = false;
                 while (!found && k0 < k_end) {
                     const u32 k = k0 + lane;
-                    const bool mine = k < k_end && (u32)lane < width && k != kb;
+                    const bool mine = k < k_end && k != kb;
                     u32 c = c_first + k; if (c >= nb) c -= nb;
                     const u64* sl = p.slots + (size_t)(mine ? c : b) * CG_SLOT_U64 + ring;
                     bool ready = !mine; u32 l = CG_NONE; u64 q1 = 0;
@@ -566,7 +566,7 @@ __global__ void __launch_bounds__(THREADS, 1) cg_pr_persistent(const CgParams p)
                     if (k0 == 0) {                      // position 0 sits in lane 0 of the first chunk
                         tlab = __shfl_sync(CG_FULL, tlab, 0); tpay = __shfl_sync(CG_FULL, tpay, 0);
                     }
-                    k0 += width; width = 32;
+                    k0 += 32;
                 }
                 if (!found && !own_low && kb != 0 && tlab != CG_NONE) {   // only the tail of the window accepted
                     q = tlab; wp = ((tpay >> 24) & 0xFFFFFFull) << 32 | (tpay & 0xFFFFFFull);
