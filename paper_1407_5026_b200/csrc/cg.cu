@@ -1398,12 +1398,13 @@ extern "C" int cg_apply_hops(cg_sim* s, uint64_t count, const uint32_t* i, const
     cudaEvent_t e0, e1;
     CK(cudaEventCreate(&e0)); CK(cudaEventCreate(&e1));
     CgParams p = make_params(s, 0);
-    // several small CTAs per SM (one block of 64 sites per warp) keep enough requests in flight to make
-    // the stand-alone update throughput-bound; larger lattices fall back to one CTA per SM
-    const u64 g1 = (s->N / 2 + 255) / 256;
+    // many small CTAs per SM (one block of 64 sites per warp; 128 threads measured best) keep enough
+    // requests in flight to make the stand-alone update throughput-bound; larger lattices fall back to
+    // one CTA per SM
+    const u64 g1 = (s->N / 2 + 127) / 128;
     const int grid = (int)std::max<u64>(1, std::min<u64>((s->N / 2 + 511) / 512, (u64)s->num_sms));
     CK(cudaEventRecord(e0, s->stream));
-    if (g1 <= (u64)s->num_sms * 6) cg_update_scripted<256, 1><<<(int)g1, 256, 0, s->stream>>>(p, d_ij, d_ij + count, count);
+    if (g1 <= (u64)s->num_sms * 12) cg_update_scripted<128, 1><<<(int)g1, 128, 0, s->stream>>>(p, d_ij, d_ij + count, count);
     else scripted_kernel(choose_rp(s->N / 2, grid, 512))<<<grid, 512, 0, s->stream>>>(p, d_ij, d_ij + count, count);
     CK(cudaEventRecord(e1, s->stream));
     CK(cudaGetLastError());

@@ -259,3 +259,26 @@ def test_replicas_on_separate_streams_run_concurrently_and_independently(cg, ora
         o = oracle_lib.Oracle(**kw)
         o.run(5000)
         _compare(g, o, 5000)
+
+
+FULL = [("cfg1_L16", 0), ("cfg2_L64", 0), ("cfg3_L128", 0), ("cfg3_L128", 1), ("cfg3_L128", 2), ("cfg3_L128", 3),
+        ("cfg4_L256", 2), ("cfg5_L512", 0)]
+
+
+@pytest.mark.slow
+@pytest.mark.parametrize("name,idx", FULL)
+def test_full_length_configs(cg, oracle_lib, name, idx):
+    """BASELINE.json's configs at their FULL hop counts (1e5 / 1e6 hops), hop log element by element.
+    About ten minutes of single-core oracle time: runs only with CG_FULL_PARITY=1."""
+    import os
+    if os.environ.get("CG_FULL_PARITY") != "1":
+        pytest.skip("set CG_FULL_PARITY=1 to run the full-length parity check")
+    cfg = workloads.CONFIGS[name][idx]
+    kw = workloads.init_args(cfg)
+    hops = cfg["hops"]
+    g = cg.CoulombGlass(hop_log=hops, **kw)
+    g.run(hops)
+    o = oracle_lib.Oracle(**kw)
+    o.run(hops)
+    _compare(g, o, hops)
+    assert g.recompute_eps() < 1e-9
