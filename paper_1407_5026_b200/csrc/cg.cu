@@ -28,6 +28,7 @@
 #include <algorithm>
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <string>
@@ -181,14 +182,16 @@ struct Slab {
     double ja[R], ia[R], jb[R], ib[R];
     u32 sca[R], scb[R];                  // coded sites (spare bit set); 0 marks a site outside the slab
     u32 hci, hcj;
+    u32 tix;                             // index of this thread among the TW threads that hold the slab
 
     __device__ __forceinline__ u32 site_a(u32 pr0, int k) const
     {
-        return 2u * (pr0 + (u32)k * TW + (threadIdx.x & ~31u)) + (threadIdx.x & 31u);
+        return 2u * (pr0 + (u32)k * TW + (tix & ~31u)) + (tix & 31u);
     }
 
-    __device__ __forceinline__ void load(const double* src, u32 pr0, u32 pr1, int L)
+    __device__ __forceinline__ void load(const double* src, u32 pr0, u32 pr1, int L, u32 t)
     {
+        tix = t;
 #pragma unroll
         for (int k = 0; k < RP; ++k) {
             const u32 sa = site_a(pr0, k), sb = sa + 32u;
@@ -221,7 +224,7 @@ struct Slab {
                 if (scb[k]) { eb[k] = __dadd_rn(eb[k], __dsub_rn(jb[k], ib[k])); __stcg(dst + sa + 32u, eb[k]); }
             }
         } else {
-            for (u32 s = 2u * pr0 + threadIdx.x; s < 2u * pr1; s += TW) {
+            for (u32 s = 2u * pr0 + tix; s < 2u * pr1; s += TW) {
                 const u32 c = site_code(s, L) | (u32)L;
                 const double v = __ldcg(src + s);
                 const double tj = __ldg(tf + ((c - hcj) & mask)), ti = __ldg(tf + ((c - hci) & mask));
@@ -303,6 +306,8 @@ __device__ __forceinline__ bool metropolis(double dE, u32 uh, u32 ul, double T, 
 #define CLS_ (kb == 0 ? 0 : kb == 1 ? 32 : kb == nb - 1 ? 48 : 16)
 #define TRACE(ev, extra) do { if (lane == 0) { const long long now_ = clock64(); \
     s_seg[CLS_ + (ev)] += (u64)(now_ - t_prev); t_prev = now_; } } while (0)
+#elif defined(CG_TRACE_W)
+#define TRACE(ev, extra) do { const long long now_ = clock64(); cw[ev] += (u64)(now_ - cprev); cprev = now_; } while (0)
 #else
 #define TRACE(ev, extra) do { } while (0)
 #endif
@@ -329,12 +334,19 @@ static_assert(CG_DEPTH <= 8 && CG_DEPTH < CG_SRING, "named barriers, slot ring")
 // state.  Otherwise CTA b evaluates labels [b per, (b+1) per) from scratch.
 // Warp 0 of every CTA does the exchange and all bookkeeping; the other worker warps only test their
 // proposals and update their part of the eps slab, and learn the outcome from a small descriptor.
-template <int THREADS, int RP, bool CACHED>
+// SPLIT: the first half of the worker warps only tests proposals, the second half only updates the slab
+// (one hop behind, synchronised with the others at the second barrier only), so that the two overlap.
+template <int THREADS, int RP, bool CACHED, bool SPLIT>
 __global__ void __launch_bounds__(THREADS, 1) cg_pr_persistent(const CgParams p)
 {
     constexpr int TW = THREADS - 64;      // worker threads; then the control warp and the service warp
     constexpr int NWK = TW / 32;          // index of the control warp
-    constexpr int TB = TW + 32;           // threads at the two CTA barriers of an iteration
+    constexpr int TT = SPLIT ? TW / 2 : TW;   // threads that test proposals (the first ones)
+    constexpr int TU = TW - (SPLIT ? TT : 0); // threads that hold the eps slab (the last ones)
+    constexpr int NTW = TT / 32;          // testing warps
+    constexpr int TA = TT + 32;           // threads at the first CTA barrier of an iteration (testers + control)
+    constexpr int TB = TW + 32;           // ... at the second (workers + control)
+    constexpr int TS = TU + 32;           // ... at the service warp's barriers (slab holders + service)
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int KL = p.Klive;
     u64* s_cdfi = reinterpret_cast<u64*>(smem_raw);
@@ -345,6 +357,7 @@ __global__ void __launch_bounds__(THREADS, 1) cg_pr_persistent(const CgParams p)
     u32* s_n = s_guide + CG_GUIDE;
     __shared__ u32 s_wlab[32];
     __shared__ u64 s_wpay[32];
+    __shared__ u64 s_verified;            // newest publication sequence number seen from ALL CTAs (service warp)
     __shared__ __align__(16) Desc s_desc;
     __shared__ __align__(8) Pend s_pend;
     const Tables tb = {s_cdfi, s_invr, s_fld, s_disp, s_guide};
@@ -367,6 +380,7 @@ __global__ void __launch_bounds__(THREADS, 1) cg_pr_persistent(const CgParams p)
     for (int k = tid; k < CG_GUIDE; k += THREADS) s_guide[k] = p.guide[k];
     for (u32 w = tid; w < (N + 31) / 32; w += THREADS) s_n[w] = p.nbits[w];
     if (tid == 0) {
+        s_verified = p.ctl->pub_base;
         s_pend.npend = 0; s_pend.rbuf = p.ctl->cur; s_pend.head = 0;
     }
 
@@ -385,7 +399,7 @@ __global__ void __launch_bounds__(THREADS, 1) cg_pr_persistent(const CgParams p)
     const u32 P = nb * per;               // CACHED: attempts a = g (mod P) belong to thread g
     u32 c_first = 0, t0r = 0;             // CACHED: CTA at scan position 0 and the offset of a0 in it
     if (CACHED) { const u32 g0 = (u32)(a_start % P); c_first = g0 / per; t0r = g0 - c_first * per; }
-    const bool has_label = CACHED && (u32)tid < per;
+    const bool has_label = CACHED && tid < TT && (u32)tid < per;
     __syncthreads();
     if (warp == NWK + 1) {
         // service warp: once per executed hop, wait until every worker has stored its part of the
@@ -393,10 +407,28 @@ __global__ void __launch_bounds__(THREADS, 1) cg_pr_persistent(const CgParams p)
         // workers' critical path.  Workers run at most CG_DEPTH hops ahead of it (the exchange of hop
         // h+DEPTH waits for the publication of hop h by every CTA, this one included), hence as many
         // barriers.
+        // After publishing it looks at every CTA's publication word once and leaves the newest hop that
+        // ALL of them have published in shared memory: the control warp, which must know that before it
+        // lets a hop through, then rarely has to look itself.
         if (nb > 1)
             for (u64 h = 0; h < p.n_hops; ++h) {
-                barN_sync((u32)(h % CG_DEPTH), TB);
+                barN_sync((u32)(h % CG_DEPTH), TS);
                 if (lane == 0) st_release_u64(p.slots + (size_t)b * CG_SLOT_U64 + CG_PUB_U64, pub_base + h + 1);
+                u64 vmin = ~0ull;
+                for (u32 c0 = lane; c0 < nb; c0 += 32 * 8) {            // eight independent loads in flight
+                    u64 v[8];
+#pragma unroll
+                    for (int k = 0; k < 8; ++k) {
+                        const u32 c = c0 + 32 * k;
+                        v[k] = c < nb ? ld_relaxed_u64(p.slots + (size_t)c * CG_SLOT_U64 + CG_PUB_U64) : ~0ull;
+                    }
+#pragma unroll
+                    for (int k = 0; k < 8; ++k) vmin = min(vmin, v[k]);
+                }
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1) vmin = min(vmin, __shfl_xor_sync(CG_FULL, vmin, o));
+                fence_acquire_gpu();
+                if (lane == 0 && vmin > pub_base) *(volatile u64*)&s_verified = vmin;    // stale words are smaller
             }
         return;
     }
@@ -446,6 +478,9 @@ __global__ void __launch_bounds__(THREADS, 1) cg_pr_persistent(const CgParams p)
         u32 rbuf = wbuf, npend = 0, head = 0;     // as in s_pend
         // CTA c has published hop number h of this launch once its pub word is >= pub_base + h
         u64 need_pub = 0;                 // ... for the hop whose buffer becomes rbuf at the next executed hop
+#ifdef CG_TRACE_W
+        u64 cw[16] = {}; long long cprev = clock64();
+#endif
         while (hl < p.n_hops) {
             const u32 e32 = e_start + it_local;
             const u32 kb = b >= c_first ? b - c_first : b + nb - c_first;    // my scan position
@@ -455,7 +490,7 @@ __global__ void __launch_bounds__(THREADS, 1) cg_pr_persistent(const CgParams p)
             // The buffer that becomes rbuf at the next executed hop must be complete on every CTA before the
             // workers of this CTA are let into the next iteration: one publication word per CTA, each in its
             // own L2 slice.  This warp is idle while the workers test their proposals, so the check is free.
-            if (nb > 1) {
+            if (nb > 1 && *(volatile u64*)&s_verified < need_pub) {     // rarely: the service warp has usually seen it
                 for (;;) {
                     bool ok = true;
                     for (u32 c0 = lane; c0 < nb; c0 += 32 * 8) {        // eight independent loads in flight
@@ -502,13 +537,17 @@ __global__ void __launch_bounds__(THREADS, 1) cg_pr_persistent(const CgParams p)
                     ewp = ((ewp >> 24) & 0xFFFFFFull) << 32 | (ewp & 0xFFFFFFull);
                 }
             }
-            barX_sync(TB);                // [A] the workers have tested their proposals
+            TRACE(7, 0);
+#ifdef CG_TRACE_W
+            cw[15] += 1; if (eq != CG_NONE) cw[14] += 1; if (kb == 0) cw[13] += 1;
+#endif
+            barX_sync(TA);                // [A] the workers have tested their proposals
             TRACE(3, 0);
             // ---- step 3: lowest accepting label: CTA, then grid
             u32 gmin; u64 gpay;
             {
-                const u32 l_ = lane < NWK ? s_wlab[lane] : CG_NONE;
-                const u64 pay = lane < NWK ? s_wpay[lane] : 0ull;
+                const u32 l_ = lane < NTW ? s_wlab[lane] : CG_NONE;
+                const u64 pay = lane < NTW ? s_wpay[lane] : 0ull;
                 gmin = __reduce_min_sync(CG_FULL, l_);
                 const int src = __ffs(__ballot_sync(CG_FULL, l_ == gmin)) - 1;
                 gpay = __shfl_sync(CG_FULL, pay, src);
@@ -631,6 +670,9 @@ __global__ void __launch_bounds__(THREADS, 1) cg_pr_persistent(const CgParams p)
         __syncwarp();
         if (p.trace) { p.trace[(size_t)b * 64 + lane] += s_seg[lane]; p.trace[(size_t)b * 64 + 32 + lane] += s_seg[32 + lane]; }
 #endif
+#ifdef CG_TRACE_W
+        if (p.trace && lane == 0) for (int k = 0; k < 16; ++k) p.trace[32768 + (size_t)b * 16 + k] = cw[k];
+#endif
         if (b == 0 && lane == 0) {
             CgCtl* c = p.ctl;
             c->attempts = a_start + used_sum; c->hops = hops_start + hl;
@@ -642,14 +684,14 @@ __global__ void __launch_bounds__(THREADS, 1) cg_pr_persistent(const CgParams p)
         return;
     }
 
-    Slab<TW, RP> slab;
-    slab.load(p.eps[wbuf], pr0, pr1, L);
+    Slab<TU, RP> slab;
+    slab.load(p.eps[wbuf], tid >= TW - TU ? pr0 : pr1, pr1, L, (u32)tid - (u32)(TW - TU));   // testers hold nothing
 
     // finish the issued slab update and hand it to the service warp for publication
     auto finish_update = [&]() {
         const u32 src = wbuf == 0 ? CG_RING - 1u : wbuf - 1u;
         slab.finish(tf, mask, L, p.eps[src], p.eps[wbuf], pr0, pr1);
-        if (nb > 1) barN_arrive((u32)((hl - 1) % CG_DEPTH), TB);   // hop hl (1-based) on barrier 1 + (hl - 1) % DEPTH
+        if (nb > 1) barN_arrive((u32)((hl - 1) % CG_DEPTH), TS);   // hop hl (1-based) on barrier 1 + (hl - 1) % DEPTH
         upd = false;
     };
 
@@ -657,6 +699,25 @@ __global__ void __launch_bounds__(THREADS, 1) cg_pr_persistent(const CgParams p)
     // One loop body = outcome of the previous exchange (descriptor) -> table gathers of its hop ->
     // proposals -> slab update: gathers and update sit in the same body, so the gathers stay in flight
     // during the whole propose phase.
+    if (SPLIT && tid >= TT) {
+        // ---- slab warps: per executed hop gather, add, store through, hand to the service warp; they meet
+        // the others at the second barrier of every iteration only, and work while the testers test
+        for (;;) {
+            barB_sync(TB);
+            const uint4 d = *reinterpret_cast<const uint4*>(&s_desc);      // used, hop, ci, cj
+            if (d.y) {
+                ++hl;
+                wbuf = wbuf == CG_RING - 1 ? 0u : wbuf + 1u;
+                slab.issue(tf, mask, pr0, pr1, d.z, d.w);
+                finish_update();
+            }
+            if (hl >= p.n_hops) break;
+        }
+        return;
+    }
+#ifdef CG_TRACE_W
+    u64 tw[7] = {}; long long wprev = 0;
+#endif
     u64 a0 = a_start;                     // first attempt of the window (used when labels are not cached)
     uint4 d4 = make_uint4(0u, 0u, 0u, 0u);       // used, hop, ci, cj of the previous exchange
     for (;;) {
@@ -676,9 +737,12 @@ __global__ void __launch_bounds__(THREADS, 1) cg_pr_persistent(const CgParams p)
             ++hl;
             hci = d4.z; hcj = d4.w;
             wbuf = wbuf == CG_RING - 1 ? 0u : wbuf + 1u;
-            upd = true;
+            upd = !SPLIT;
         }
         if (hl >= p.n_hops) break;
+#ifdef CG_TRACE_W
+        const long long w0 = clock64();
+#endif
         // ---- steps 1-2: propose and test, state untouched
         u32 best = CG_NONE, bi = 0, bj = 0;
         if (CACHED) {
@@ -707,7 +771,7 @@ __global__ void __launch_bounds__(THREADS, 1) cg_pr_persistent(const CgParams p)
         } else {
             const u32 np = s_pend.npend;
             const double* __restrict__ erd = p.eps[s_pend.rbuf];
-            for (u32 l = lab0 + tid; l < lab1; l += TW) {
+            for (u32 l = lab0 + tid; l < lab1; l += TT) {
                 const u64 a = a0 + l;
                 u32 w0, w1, w2, w3;
                 philox4x32_10((u32)a, (u32)(a >> 32), 0u, 0u, p.seed_lo, p.seed_hi, w0, w1, w2, w3);
@@ -728,25 +792,48 @@ __global__ void __launch_bounds__(THREADS, 1) cg_pr_persistent(const CgParams p)
                 if (metropolis(dE, w2 & 0x1FFFFFu, w3, p.T, p.inv_T)) { best = l; bi = i; bj = j; break; }
             }
         }
+#ifdef CG_TRACE_W
+        const long long w1 = clock64();
+#endif
         // ---- step 3: lowest accepting label: warp, then the control warp
         {
             const u32 wmin = __reduce_min_sync(CG_FULL, best);
             const int src = __ffs(__ballot_sync(CG_FULL, best == wmin)) - 1;
             if (lane == src) { s_wlab[warp] = wmin; s_wpay[warp] = ((u64)bi << 32) | (u64)bj; }
         }
-        barX_sync(TB);                    // [A]
+#ifdef CG_TRACE_W
+        const long long w2 = clock64();
+#endif
+        barX_sync(TA);                    // [A]
+#ifdef CG_TRACE_W
+        const long long w3 = clock64();
+#endif
         // while the control warp does the exchange: the slab of the previous hop (its table gathers,
         // issued when that hop was executed, have had the whole propose phase to arrive) and, if another
         // CTA holds the start of the window, the decode one attempt ahead
         if (upd) { slab.issue(tf, mask, pr0, pr1, hci, hcj); finish_update(); }
         if (has_label && !nxt_valid && ahead) { nxt = decode_attempt(tb, p, a_cur + P); nxt_valid = true; }
+#ifdef CG_TRACE_W
+        const long long w4 = clock64();
+#endif
         barB_sync(TB);                    // [B] the control warp has written the descriptor
+#ifdef CG_TRACE_W
+        {
+            const long long w5 = clock64();
+            tw[0] += (u64)(w1 - w0); tw[1] += (u64)(w2 - w1); tw[2] += (u64)(w3 - w2); tw[3] += (u64)(w4 - w3); tw[4] += (u64)(w5 - w4);
+            if (wprev) tw[5] += (u64)(w0 - wprev);
+            wprev = w5; ++tw[6];
+        }
+#endif
         d4 = *reinterpret_cast<const uint4*>(&s_desc);      // used, hop, ci, cj
         ahead = s_desc.ahead != 0;
     }
+#ifdef CG_TRACE_W
+    if (p.trace && lane == 0) for (int k = 0; k < 7; ++k) p.trace[((size_t)b * 16 + warp) * 8 + k] = tw[k];
+#endif
     if (upd) { slab.issue(tf, mask, pr0, pr1, hci, hcj); finish_update(); }
     if (b == 0)
-        for (u32 w = tid; w < (N + 31) / 32; w += TW) p.nbits[w] = s_n[w];
+        for (u32 w = tid; w < (N + 31) / 32; w += TT) p.nbits[w] = s_n[w];
 }
 
 // Step a6 alone: scripted hops, update in place (no readers), one launch.
@@ -761,7 +848,7 @@ cg_update_scripted(const CgParams p, const u32* __restrict__ hop_i, const u32* _
     const u32 pr0 = min(pairs, b * pper), pr1 = min(pairs, pr0 + pper);
     double* e = p.eps[p.ctl->cur];
     Slab<THREADS, RP> slab;
-    slab.load(e, pr0, pr1, L);
+    slab.load(e, pr0, pr1, L, threadIdx.x);
     for (u64 h = 0; h < count; ++h) {
         slab.issue(p.tf, mask, pr0, pr1, site_code(__ldg(hop_i + h), L), site_code(__ldg(hop_j + h), L));
         slab.finish(p.tf, mask, L, e, e, pr0, pr1);
@@ -898,6 +985,7 @@ struct cg_sim {
     void* d_log = nullptr; bool own_log = false; u64 log_cap = 0;
     u64* d_trace = nullptr; u32 trace_iters = 0;
     // launch shape
+    bool split = false;
     int num_sms = 0, n_ctas = 0, threads = 0, smem = 0, rp = 0, pl = 0;   // pl > 0: cached proposals
     std::string err;
 };
@@ -1056,16 +1144,25 @@ template <int THREADS, bool CACHED>
 static persist_fn persistent_kernel_t(int rp)
 {
     switch (rp) {
-        case 0: return cg_pr_persistent<THREADS, 0, CACHED>;
-        case 1: return cg_pr_persistent<THREADS, 1, CACHED>;
-        case 2: return cg_pr_persistent<THREADS, 2, CACHED>;
-        case 4: return cg_pr_persistent<THREADS, 4, CACHED>;
-        case 8: return cg_pr_persistent<THREADS, 8, CACHED>;
+        case 0: return cg_pr_persistent<THREADS, 0, CACHED, false>;
+        case 1: return cg_pr_persistent<THREADS, 1, CACHED, false>;
+        case 2: return cg_pr_persistent<THREADS, 2, CACHED, false>;
+        case 4: return cg_pr_persistent<THREADS, 4, CACHED, false>;
+        case 8: return cg_pr_persistent<THREADS, 8, CACHED, false>;
     }
     return nullptr;
 }
-static persist_fn persistent_kernel(int threads, int rp, bool cached)
+static persist_fn persistent_kernel(int threads, int rp, bool cached, bool split = false)
 {
+    if (split) {            // 512 threads, cached labels only
+        switch (rp) {
+            case 1: return cg_pr_persistent<512, 1, true, true>;
+            case 2: return cg_pr_persistent<512, 2, true, true>;
+            case 4: return cg_pr_persistent<512, 4, true, true>;
+            case 8: return cg_pr_persistent<512, 8, true, true>;
+        }
+        return nullptr;
+    }
     switch (threads) {
         case 256: return cached ? persistent_kernel_t<256, true>(rp) : persistent_kernel_t<256, false>(rp);
         case 512: return cached ? persistent_kernel_t<512, true>(rp) : persistent_kernel_t<512, false>(rp);
@@ -1142,7 +1239,18 @@ static int choose_launch(cg_sim* s, int n_ctas, int threads)
     }
     if (n_ctas != s->n_ctas)   // slots of CTAs that no longer exist must not look published
         CK(cudaMemsetAsync(s->d_slots, 0, CG_SLOT_BYTES, s->stream));
-    s->n_ctas = n_ctas; s->threads = threads; s->rp = rp; s->pl = pl;
+    s->n_ctas = n_ctas; s->threads = threads; s->rp = rp; s->pl = pl; s->split = false;
+    // prototype: half of the workers test, half update (needs half as many labels per CTA)
+    if (getenv("CG_SPLIT") && threads == 512 && s->M <= (u64)n_ctas * 224) {
+        const u64 per_cta = (s->N / 2 + n_ctas - 1) / n_ctas, need = (per_cta + 223) / 224;
+        int r2 = 0;
+        for (int r = 1; r <= 8; r *= 2) if ((u64)r >= need) { r2 = r; break; }
+        if (r2) {
+            persist_fn f = persistent_kernel(512, r2, true, true);
+            CK(cudaFuncSetAttribute((const void*)f, cudaFuncAttributeMaxDynamicSharedMemorySize, s->smem));
+            s->rp = r2; s->pl = 224; s->split = true;
+        }
+    }
     return CG_OK;
 }
 
@@ -1250,7 +1358,7 @@ extern "C" int cg_run(cg_sim* s, uint64_t n_hops)
 {
     if (!s) return CG_EINVAL;
     if (n_hops == 0) return CG_OK;
-    persist_fn f = persistent_kernel(s->threads, s->rp, s->pl > 0);
+    persist_fn f = persistent_kernel(s->threads, s->rp, s->pl > 0, s->split);
     if (!f) return CG_EINVAL;
     CgParams p = make_params(s, n_hops);
     void* args[] = {&p};
@@ -1475,7 +1583,7 @@ extern "C" int cg_set_trace(cg_sim* s, void* dev_buf, size_t bytes, uint32_t ite
     if (!s) return CG_EINVAL;
     CK(cudaStreamSynchronize(s->stream));
     if (!dev_buf || !iterations) { s->d_trace = nullptr; s->trace_iters = 0; return CG_OK; }
-#ifndef CG_TRACE
+#if !defined(CG_TRACE) && !defined(CG_TRACE_W)
     return CG_EUNSUPPORTED;                   // the library was built without -DCG_TRACE
 #endif
     if (((uintptr_t)dev_buf & 7) || bytes < (size_t)8 * 64 * CG_MAX_CTAS) return CG_EINVAL;
