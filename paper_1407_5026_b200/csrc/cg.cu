@@ -622,33 +622,32 @@ __global__ void __launch_bounds__(THREADS, 1) cg_pr_persistent(const CgParams p)
             // ---- what the workers need: attempts consumed (m = (p-1)M + q per executed hop, PAPER.md:39,
             // 78), the hop (step 3a), occupations, pending list
             const u32 used = q == CG_NONE ? M : q + 1;
+            const u32 hi_ = (u32)(wp >> 32), hj_ = (u32)wp;
+            const u32 ci = site_code(hi_, L), cj = site_code(hj_, L);
+            if (lane == 0) *reinterpret_cast<uint4*>(&s_desc) = make_uint4(used, q != CG_NONE, ci, cj);
+            if (q != CG_NONE) {
+                const u32 pos = npend < CG_DEPTH ? (head + npend) % CG_DEPTH : head;
+                if (npend < CG_DEPTH) ++npend;
+                else { head = (head + 1) % CG_DEPTH; rbuf = rbuf == CG_RING - 1 ? 0u : rbuf + 1u; }
+                if (lane == 0) {              // the workers are between the two barriers: nobody reads these
+                    atomicAnd(&s_n[hi_ >> 5], ~(1u << (hi_ & 31)));     // no return value: fire and forget
+                    atomicOr(&s_n[hj_ >> 5], 1u << (hj_ & 31));
+                    s_pend.c[pos][0] = ci; s_pend.c[pos][1] = cj;
+                    s_pend.npend = npend; s_pend.rbuf = rbuf; s_pend.head = head;
+                }
+            }
+            TRACE(5, 0);
+            barB_arrive(TB);              // [B] the workers may read the descriptor; this warp goes on
+            // ---- the rest of the bookkeeping, while the workers run
             if (CACHED) {
                 if (t0r + used < per) t0r += used;
                 else {
                     u32 g0 = c_first * per + t0r + used; if (g0 >= P) g0 -= P;      // used <= M <= P
                     c_first = g0 / per; t0r = g0 - c_first * per;
                 }
+                // a hint only (time to decode ahead): the workers may still see the previous value
+                if (lane == 0) s_desc.ahead = c_first != b;
             }
-            const u32 hi_ = (u32)(wp >> 32), hj_ = (u32)wp;
-            const u32 ci = site_code(hi_, L), cj = site_code(hj_, L);
-            if (q != CG_NONE) {
-                const u32 pos = npend < CG_DEPTH ? (head + npend) % CG_DEPTH : head;
-                if (npend < CG_DEPTH) ++npend;
-                else { head = (head + 1) % CG_DEPTH; rbuf = rbuf == CG_RING - 1 ? 0u : rbuf + 1u; }
-                if (lane == 0) {              // the workers are between the two barriers: nobody reads these
-                    s_n[hi_ >> 5] &= ~(1u << (hi_ & 31));
-                    s_n[hj_ >> 5] |= 1u << (hj_ & 31);
-                    s_pend.c[pos][0] = ci; s_pend.c[pos][1] = cj;
-                    s_pend.npend = npend; s_pend.rbuf = rbuf; s_pend.head = head;
-                }
-            }
-            if (lane == 0) {
-                *reinterpret_cast<uint4*>(&s_desc) = make_uint4(used, q != CG_NONE, ci, cj);
-                s_desc.ahead = CACHED && c_first != b;
-            }
-            TRACE(5, 0);
-            barB_arrive(TB);              // [B] the workers may read the descriptor; this warp goes on
-            // ---- the rest of the bookkeeping, while the workers run
             used_sum += used;
             ++it_local;
             if (q != CG_NONE) {
