@@ -28,7 +28,6 @@
 #include <algorithm>
 #include <cmath>
 #include <cstdio>
-#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <string>
@@ -334,19 +333,12 @@ static_assert(CG_DEPTH <= 8 && CG_DEPTH < CG_SRING, "named barriers, slot ring")
 // state.  Otherwise CTA b evaluates labels [b per, (b+1) per) from scratch.
 // Warp 0 of every CTA does the exchange and all bookkeeping; the other worker warps only test their
 // proposals and update their part of the eps slab, and learn the outcome from a small descriptor.
-// SPLIT: the first half of the worker warps only tests proposals, the second half only updates the slab
-// (one hop behind, synchronised with the others at the second barrier only), so that the two overlap.
-template <int THREADS, int RP, bool CACHED, bool SPLIT>
+template <int THREADS, int RP, bool CACHED>
 __global__ void __launch_bounds__(THREADS, 1) cg_pr_persistent(const CgParams p)
 {
     constexpr int TW = THREADS - 64;      // worker threads; then the control warp and the service warp
-    constexpr int NWK = TW / 32;          // index of the control warp
-    constexpr int TT = SPLIT ? TW / 2 : TW;   // threads that test proposals (the first ones)
-    constexpr int TU = TW - (SPLIT ? TT : 0); // threads that hold the eps slab (the last ones)
-    constexpr int NTW = TT / 32;          // testing warps
-    constexpr int TA = TT + 32;           // threads at the first CTA barrier of an iteration (testers + control)
-    constexpr int TB = TW + 32;           // ... at the second (workers + control)
-    constexpr int TS = TU + 32;           // ... at the service warp's barriers (slab holders + service)
+    constexpr int NWK = TW / 32;          // worker warps = index of the control warp
+    constexpr int TB = TW + 32;           // threads at the CTA barriers of an iteration (workers + control)
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int KL = p.Klive;
     u64* s_cdfi = reinterpret_cast<u64*>(smem_raw);
@@ -399,7 +391,7 @@ __global__ void __launch_bounds__(THREADS, 1) cg_pr_persistent(const CgParams p)
     const u32 P = nb * per;               // CACHED: attempts a = g (mod P) belong to thread g
     u32 c_first = 0, t0r = 0;             // CACHED: CTA at scan position 0 and the offset of a0 in it
     if (CACHED) { const u32 g0 = (u32)(a_start % P); c_first = g0 / per; t0r = g0 - c_first * per; }
-    const bool has_label = CACHED && tid < TT && (u32)tid < per;
+    const bool has_label = CACHED && (u32)tid < per;
     __syncthreads();
     if (warp == NWK + 1) {
         // service warp: once per executed hop, wait until every worker has stored its part of the
@@ -412,7 +404,7 @@ __global__ void __launch_bounds__(THREADS, 1) cg_pr_persistent(const CgParams p)
         // lets a hop through, then rarely has to look itself.
         if (nb > 1)
             for (u64 h = 0; h < p.n_hops; ++h) {
-                barN_sync((u32)(h % CG_DEPTH), TS);
+                barN_sync((u32)(h % CG_DEPTH), TB);
                 if (lane == 0) st_release_u64(p.slots + (size_t)b * CG_SLOT_U64 + CG_PUB_U64, pub_base + h + 1);
                 u64 vmin = ~0ull;
                 for (u32 c0 = lane; c0 < nb; c0 += 32 * 8) {            // eight independent loads in flight
@@ -541,13 +533,13 @@ __global__ void __launch_bounds__(THREADS, 1) cg_pr_persistent(const CgParams p)
 #ifdef CG_TRACE_W
             cw[15] += 1; if (eq != CG_NONE) cw[14] += 1; if (kb == 0) cw[13] += 1;
 #endif
-            barX_sync(TA);                // [A] the workers have tested their proposals
+            barX_sync(TB);                // [A] the workers have tested their proposals
             TRACE(3, 0);
             // ---- step 3: lowest accepting label: CTA, then grid
             u32 gmin; u64 gpay;
             {
-                const u32 l_ = lane < NTW ? s_wlab[lane] : CG_NONE;
-                const u64 pay = lane < NTW ? s_wpay[lane] : 0ull;
+                const u32 l_ = lane < NWK ? s_wlab[lane] : CG_NONE;
+                const u64 pay = lane < NWK ? s_wpay[lane] : 0ull;
                 gmin = __reduce_min_sync(CG_FULL, l_);
                 const int src = __ffs(__ballot_sync(CG_FULL, l_ == gmin)) - 1;
                 gpay = __shfl_sync(CG_FULL, pay, src);
@@ -683,14 +675,14 @@ __global__ void __launch_bounds__(THREADS, 1) cg_pr_persistent(const CgParams p)
         return;
     }
 
-    Slab<TU, RP> slab;
-    slab.load(p.eps[wbuf], tid >= TW - TU ? pr0 : pr1, pr1, L, (u32)tid - (u32)(TW - TU));   // testers hold nothing
+    Slab<TW, RP> slab;
+    slab.load(p.eps[wbuf], pr0, pr1, L, (u32)tid);
 
     // finish the issued slab update and hand it to the service warp for publication
     auto finish_update = [&]() {
         const u32 src = wbuf == 0 ? CG_RING - 1u : wbuf - 1u;
         slab.finish(tf, mask, L, p.eps[src], p.eps[wbuf], pr0, pr1);
-        if (nb > 1) barN_arrive((u32)((hl - 1) % CG_DEPTH), TS);   // hop hl (1-based) on barrier 1 + (hl - 1) % DEPTH
+        if (nb > 1) barN_arrive((u32)((hl - 1) % CG_DEPTH), TB);   // hop hl (1-based) on barrier 1 + (hl - 1) % DEPTH
         upd = false;
     };
 
@@ -698,22 +690,6 @@ __global__ void __launch_bounds__(THREADS, 1) cg_pr_persistent(const CgParams p)
     // One loop body = outcome of the previous exchange (descriptor) -> table gathers of its hop ->
     // proposals -> slab update: gathers and update sit in the same body, so the gathers stay in flight
     // during the whole propose phase.
-    if (SPLIT && tid >= TT) {
-        // ---- slab warps: per executed hop gather, add, store through, hand to the service warp; they meet
-        // the others at the second barrier of every iteration only, and work while the testers test
-        for (;;) {
-            barB_sync(TB);
-            const uint4 d = *reinterpret_cast<const uint4*>(&s_desc);      // used, hop, ci, cj
-            if (d.y) {
-                ++hl;
-                wbuf = wbuf == CG_RING - 1 ? 0u : wbuf + 1u;
-                slab.issue(tf, mask, pr0, pr1, d.z, d.w);
-                finish_update();
-            }
-            if (hl >= p.n_hops) break;
-        }
-        return;
-    }
 #ifdef CG_TRACE_W
     u64 tw[7] = {}; long long wprev = 0;
 #endif
@@ -736,7 +712,7 @@ __global__ void __launch_bounds__(THREADS, 1) cg_pr_persistent(const CgParams p)
             ++hl;
             hci = d4.z; hcj = d4.w;
             wbuf = wbuf == CG_RING - 1 ? 0u : wbuf + 1u;
-            upd = !SPLIT;
+            upd = true;
         }
         if (hl >= p.n_hops) break;
 #ifdef CG_TRACE_W
@@ -770,7 +746,7 @@ __global__ void __launch_bounds__(THREADS, 1) cg_pr_persistent(const CgParams p)
         } else {
             const u32 np = s_pend.npend;
             const double* __restrict__ erd = p.eps[s_pend.rbuf];
-            for (u32 l = lab0 + tid; l < lab1; l += TT) {
+            for (u32 l = lab0 + tid; l < lab1; l += TW) {
                 const u64 a = a0 + l;
                 u32 w0, w1, w2, w3;
                 philox4x32_10((u32)a, (u32)(a >> 32), 0u, 0u, p.seed_lo, p.seed_hi, w0, w1, w2, w3);
@@ -803,7 +779,7 @@ __global__ void __launch_bounds__(THREADS, 1) cg_pr_persistent(const CgParams p)
 #ifdef CG_TRACE_W
         const long long w2 = clock64();
 #endif
-        barX_sync(TA);                    // [A]
+        barX_sync(TB);                    // [A]
 #ifdef CG_TRACE_W
         const long long w3 = clock64();
 #endif
@@ -832,7 +808,7 @@ __global__ void __launch_bounds__(THREADS, 1) cg_pr_persistent(const CgParams p)
 #endif
     if (upd) { slab.issue(tf, mask, pr0, pr1, hci, hcj); finish_update(); }
     if (b == 0)
-        for (u32 w = tid; w < (N + 31) / 32; w += TT) p.nbits[w] = s_n[w];
+        for (u32 w = tid; w < (N + 31) / 32; w += TW) p.nbits[w] = s_n[w];
 }
 
 // Step a6 alone: scripted hops, update in place (no readers), one launch.
@@ -984,7 +960,6 @@ struct cg_sim {
     void* d_log = nullptr; bool own_log = false; u64 log_cap = 0;
     u64* d_trace = nullptr; u32 trace_iters = 0;
     // launch shape
-    bool split = false;
     int num_sms = 0, n_ctas = 0, threads = 0, smem = 0, rp = 0, pl = 0;   // pl > 0: cached proposals
     std::string err;
 };
@@ -1143,25 +1118,16 @@ template <int THREADS, bool CACHED>
 static persist_fn persistent_kernel_t(int rp)
 {
     switch (rp) {
-        case 0: return cg_pr_persistent<THREADS, 0, CACHED, false>;
-        case 1: return cg_pr_persistent<THREADS, 1, CACHED, false>;
-        case 2: return cg_pr_persistent<THREADS, 2, CACHED, false>;
-        case 4: return cg_pr_persistent<THREADS, 4, CACHED, false>;
-        case 8: return cg_pr_persistent<THREADS, 8, CACHED, false>;
+        case 0: return cg_pr_persistent<THREADS, 0, CACHED>;
+        case 1: return cg_pr_persistent<THREADS, 1, CACHED>;
+        case 2: return cg_pr_persistent<THREADS, 2, CACHED>;
+        case 4: return cg_pr_persistent<THREADS, 4, CACHED>;
+        case 8: return cg_pr_persistent<THREADS, 8, CACHED>;
     }
     return nullptr;
 }
-static persist_fn persistent_kernel(int threads, int rp, bool cached, bool split = false)
+static persist_fn persistent_kernel(int threads, int rp, bool cached)
 {
-    if (split) {            // 512 threads, cached labels only
-        switch (rp) {
-            case 1: return cg_pr_persistent<512, 1, true, true>;
-            case 2: return cg_pr_persistent<512, 2, true, true>;
-            case 4: return cg_pr_persistent<512, 4, true, true>;
-            case 8: return cg_pr_persistent<512, 8, true, true>;
-        }
-        return nullptr;
-    }
     switch (threads) {
         case 256: return cached ? persistent_kernel_t<256, true>(rp) : persistent_kernel_t<256, false>(rp);
         case 512: return cached ? persistent_kernel_t<512, true>(rp) : persistent_kernel_t<512, false>(rp);
@@ -1238,18 +1204,7 @@ static int choose_launch(cg_sim* s, int n_ctas, int threads)
     }
     if (n_ctas != s->n_ctas)   // slots of CTAs that no longer exist must not look published
         CK(cudaMemsetAsync(s->d_slots, 0, CG_SLOT_BYTES, s->stream));
-    s->n_ctas = n_ctas; s->threads = threads; s->rp = rp; s->pl = pl; s->split = false;
-    // prototype: half of the workers test, half update (needs half as many labels per CTA)
-    if (getenv("CG_SPLIT") && threads == 512 && s->M <= (u64)n_ctas * 224) {
-        const u64 per_cta = (s->N / 2 + n_ctas - 1) / n_ctas, need = (per_cta + 223) / 224;
-        int r2 = 0;
-        for (int r = 1; r <= 8; r *= 2) if ((u64)r >= need) { r2 = r; break; }
-        if (r2) {
-            persist_fn f = persistent_kernel(512, r2, true, true);
-            CK(cudaFuncSetAttribute((const void*)f, cudaFuncAttributeMaxDynamicSharedMemorySize, s->smem));
-            s->rp = r2; s->pl = 224; s->split = true;
-        }
-    }
+    s->n_ctas = n_ctas; s->threads = threads; s->rp = rp; s->pl = pl;
     return CG_OK;
 }
 
@@ -1357,7 +1312,7 @@ extern "C" int cg_run(cg_sim* s, uint64_t n_hops)
 {
     if (!s) return CG_EINVAL;
     if (n_hops == 0) return CG_OK;
-    persist_fn f = persistent_kernel(s->threads, s->rp, s->pl > 0, s->split);
+    persist_fn f = persistent_kernel(s->threads, s->rp, s->pl > 0);
     if (!f) return CG_EINVAL;
     CgParams p = make_params(s, n_hops);
     void* args[] = {&p};
