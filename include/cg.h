@@ -139,6 +139,13 @@ int cg_get_phase_cycles(cg_sim* s, uint64_t* total, uint64_t* wait, uint64_t* up
  * 5 what the workers wait for of the bookkeeping, 0 the rest of it; k = 15 counts iterations,
  * 8 passes of the publication check, 9 scans, 11-14, 1, 2 a histogram of the scan time
  * (< 500, 1000, 2000, 4000, 8000 cycles, more).
+ * A library built with -DCG_TRACE_W instead keeps cheap clock64 sums in registers (no measurable
+ * slow-down): dev_buf[(b*16 + w)*8 + k] for worker warp w of CTA b, k = 0 test phase, 1 warp minimum,
+ * 2 first barrier, 3 slab update, 4 second barrier, 5 descriptor and labels, 6 iterations; and
+ * dev_buf[32768 + b*16 + k] for the control warp, k = 6 publication check, 7 early look, 3 first
+ * barrier, 10 CTA minimum and post, 4 scan, 5 before and 0 after the second barrier, 15 iterations,
+ * 14 early looks that found the winner, 13 iterations at scan position 0.  (A barrier's wait shows
+ * up in the segment AFTER it: the clock is read when the barrier instruction issues.)
  * dev_buf: zeroed device memory, 8-byte aligned, 8*64*1024 bytes; `iterations` must be non-zero. */
 int cg_set_trace(cg_sim* s, void* dev_buf, size_t bytes, uint32_t iterations);
 
