@@ -254,7 +254,7 @@ def run_ours(args):
     out["roofline"] = {
         "bound": "l2", "kernel": "cg_pr_persistent (the whole hop: propose, select, apply, update; one launch per step)",
         "achieved": achieved, "peak": l2_peak, "unit": "GB/s", "frac": achieved / l2_peak,
-        # ncu --set full (profiles/r1i_ncu_pr_persistent.txt): 0.71 KB of DRAM traffic and 6.5 MB of L2 sectors
+        # ncu --set full (profiles/r1j_ncu_pr_persistent.txt): 0.71 KB of DRAM traffic and 6.5 MB of L2 sectors
         # (4.4 read + 2.1 written) per hop - the state is L2-resident, so DRAM bytes are not the bound
         "traffic": 710.0 * c["hops"] / K, "traffic_source": "ncu dram__bytes per hop x hops per launch",
         "l2_bytes_per_hop_ncu": 6.54e6,
