@@ -1,0 +1,138 @@
+"""Per-config throughput report and replica packing (§8f-2), through the Python binding.
+
+    python -m paper_1407_5026_b200.report --configs [--hops 200000] [--warm 2000]
+    python -m paper_1407_5026_b200.report --replicas [--hops 100000]
+
+--configs: every workload of BASELINE.json (workloads.CONFIGS), a bounded prefix of its chain, one line each:
+accepted hops/s, window proposals evaluated/s (M per PR iteration), attempts consumed/s
+(m = (p-1)M + q per hop), mean p and mean q (0-based label of the executed proposal),
+acceptance A = hops/attempts over the run and over its last 10 %, the paper's split of the time per hop
+ W_U = the eps update alone (`cg_apply_hops` on the hops just executed and their reversal) and
+W_R = time per hop - W_U (in the persistent kernel the two overlap, so W_R is what the update does not
+explain), the update's algorithmic GB/s (16 N bytes per hop) and the drift of the incremental eps against a
+full-sum recomputation.
+
+--replicas: independent sims on separate CUDA streams, persistent kernels side by side on one GPU.
+
+Needs a CUDA device; nothing here computes on the host.
+"""
+import argparse
+import os
+import sys
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np      # noqa: E402
+import torch            # noqa: E402
+
+import workloads        # noqa: E402
+from . import binding   # noqa: E402
+
+
+def _timed(fn):
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    fn()
+    e1.record()
+    torch.cuda.synchronize()
+    return e0.elapsed_time(e1)
+
+
+def update_alone_us(kw, n_script=1000):
+    """W_U: microseconds per hop of step a6 alone at this lattice, on hops of its own chain."""
+    u = binding.CoulombGlass(hop_log=n_script, **kw)
+    u.run(n_script)
+    _, hi, hj = u.hops()
+    v = binding.CoulombGlass(**kw)
+    si = np.concatenate([hi, hj[::-1]])
+    sj = np.concatenate([hj, hi[::-1]])
+    best = min(v.apply_hops(si, sj) for _ in range(3))
+    return 1e3 * best / si.size
+
+
+def report_configs(hops, warm):
+    sms = torch.cuda.get_device_properties(0).multi_processor_count
+    print("# %s, %d SMs; %d warm-up hops, then min(config's hops, %d) timed in 10 chunks" % (
+        torch.cuda.get_device_name(0), sms, warm, hops))
+    for name, cfgs in workloads.CONFIGS.items():
+        for cfg in cfgs:
+            kw = workloads.init_args(cfg, sms * 2048)
+            N, M = kw["L"] ** 2, kw["M"]
+            g = binding.CoulombGlass(**kw)
+            H = min(cfg["hops"], hops)
+            chunk = H // 10
+            g.run(warm)
+            torch.cuda.synchronize()
+            c0 = g.counters()
+            ms, cs = 0.0, [c0]
+            for _ in range(10):
+                ms += _timed(lambda: g.run(chunk))
+                cs.append(g.counters())
+            c, c9 = cs[-1], cs[-2]
+            Hd = c["hops"] - c0["hops"]
+            it = c["iterations"] - c0["iterations"]
+            at = c["attempts"] - c0["attempts"]
+            mean_q = (at - (it - Hd) * M) / Hd - 1.0
+            A_all = Hd / at
+            A_last = (c["hops"] - c9["hops"]) / (c["attempts"] - c9["attempts"])
+            us_hop = 1e3 * ms / Hd
+            w_u = update_alone_us(kw)
+            ln = g.launch()
+            print("%-9s T=%-5g M=%-6d %3d CTAs x %d: %7.0f hops/s  %.2e proposals/s  %.2e attempts/s  "
+                  "p=%.3f q=%8.1f  A=%.2e (last 10%%: %.2e)  %5.2f us/hop = W_U %.3f + W_R %.2f  "
+                  "update alone %6.0f GB/s  drift %.1e" % (
+                      name, kw["T"], M, ln["n_ctas"], ln["threads"], Hd / ms * 1e3, M * it / ms * 1e3,
+                      at / ms * 1e3, it / Hd, mean_q, A_all, A_last, us_hop, w_u, us_hop - w_u,
+                      16.0 * N / w_u / 1e3, g.recompute_eps()))
+            sys.stdout.flush()
+
+
+def report_replicas(hops):
+    def run(name, idxs, copies):
+        sims = []
+        for r in range(copies):
+            for i in idxs:
+                kw = workloads.init_args(workloads.CONFIGS[name][i])
+                kw["seed"] += 100 * r
+                sims.append(binding.CoulombGlass(stream=torch.cuda.Stream(), **kw))
+        for g in sims:
+            g.run(1000)
+        torch.cuda.synchronize()
+
+        def go():
+            for g in sims:
+                g.run(hops)
+            for g in sims:
+                torch.cuda.current_stream().wait_stream(g._stream)
+        ms = _timed(go)
+        print("%s x%d replicas (%d CTAs each): %.0f hops/s aggregate, %.0f per replica" % (
+            name, len(sims), sims[0].launch()["n_ctas"], len(sims) * hops / ms * 1e3, hops / ms * 1e3))
+        sys.stdout.flush()
+
+    run("cfg3_L128", [0, 1, 2, 3], 1)     # the temperature sweep of config 3 as one replica set
+    run("cfg3_L128", [0, 1, 2, 3], 2)
+    run("cfg1_L16", [0], 1)
+    run("cfg1_L16", [0], 32)
+    run("cfg1_L16", [0], 148)
+    run("cfg2_L64", [0], 29)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--configs", action="store_true")
+    ap.add_argument("--replicas", action="store_true")
+    ap.add_argument("--hops", type=int, default=0)
+    ap.add_argument("--warm", type=int, default=2000)
+    a = ap.parse_args()
+    if not torch.cuda.is_available():
+        raise SystemExit("report needs a CUDA device: the hot path has no CPU fallback")
+    if a.configs:
+        report_configs(a.hops or 200_000, a.warm)
+    if a.replicas:
+        report_replicas(a.hops or 100_000)
+
+
+if __name__ == "__main__":
+    main()
