@@ -69,6 +69,17 @@ int cg_init_ws(cg_sim** out, int L, double W, double xi, double T, double E,
  * cg_run(a); cg_run(b) is the same chain as cg_run(a+b). */
 int cg_run(cg_sim* s, uint64_t n_accepted_hops);
 
+/* Replica packing (averaging many samples at intermediate L is the
+ * recommended use): advance EACH of the n_sims independent sims by
+ * n_accepted_hops executed hops in ONE persistent launch, every sim on its own
+ * CTAs side by side; each chain is exactly the one cg_run would produce.
+ * sims[] is a host array of distinct sims that share device, stream and launch
+ * shape (512 threads, same register tiling and label caching: true for sims of
+ * equal L whose M fits their CTAs; see cg_get_launch / cg_set_launch); the sum of
+ * their CTA counts must fit on the device at once, else CG_EUNSUPPORTED.
+ * Asynchronous on that stream; the array is not referenced after the call. */
+int cg_run_many(cg_sim* const* sims, int n_sims, uint64_t n_accepted_hops);
+
 /* Synchronises the stream and copies out: occupations n[N] in {0,1}
  * (PAPER.md:52), local energies eps[N], elapsed time
  * t = attempts_consumed / Gamma in units of tau0 (deterministic increment

@@ -16,7 +16,7 @@ _lib = None
 CG_OK, CG_EINVAL, CG_ENOMEM, CG_ECUDA, CG_EUNSUPPORTED = 0, -1, -2, -3, -4
 
 EXPORTS = [
-    "cg_init", "cg_workspace_bytes", "cg_init_ws", "cg_run", "cg_get_state", "cg_set_state",
+    "cg_init", "cg_workspace_bytes", "cg_init_ws", "cg_run", "cg_run_many", "cg_get_state", "cg_set_state",
     "cg_get_counters", "cg_enable_hop_log", "cg_get_hops", "cg_recompute_eps", "cg_apply_hops",
     "cg_get_table_sizes", "cg_get_tables", "cg_get_phi", "cg_set_launch", "cg_get_launch",
     "cg_get_phase_cycles", "cg_set_trace", "cg_bench_l2_rmw", "cg_free", "cg_strerror", "cg_last_error",
@@ -46,6 +46,7 @@ def lib():
         "cg_workspace_bytes": (sz, [ci, u32]),
         "cg_init_ws": (ci, [P(vp), ci, dbl, dbl, dbl, dbl, u64, u32, vp, sz, vp]),
         "cg_run": (ci, [vp, u64]),
+        "cg_run_many": (ci, [P(vp), ci, u64]),
         "cg_get_state": (ci, [vp, vp, vp, P(dbl), P(i64)]),
         "cg_set_state": (ci, [vp, vp, vp, u64, u64, i64]),
         "cg_get_counters": (ci, [vp, P(u64), P(u64), P(u64), P(u64)]),
@@ -83,6 +84,17 @@ def bench_l2_rmw(nbytes, reps=1000, trials=10):
     if rc != 0:
         raise CgError(rc, lib().cg_strerror(rc).decode())
     return out.value
+
+
+def run_many(sims, n_accepted_hops):
+    """cg_run_many: every sim of `sims` advances by n_accepted_hops in ONE persistent launch."""
+    sims = list(sims)
+    arr = (C.c_void_p * len(sims))(*[g._h for g in sims])
+    with sims[0]._torch.cuda.device(sims[0].device):
+        rc = lib().cg_run_many(arr, len(sims), int(n_accepted_hops))
+    if rc != 0:
+        text = lib().cg_last_error(sims[0]._h).decode() or lib().cg_strerror(rc).decode()
+        raise CgError(rc, text)
 
 
 class CoulombGlass:

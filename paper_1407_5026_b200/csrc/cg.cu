@@ -333,8 +333,11 @@ static_assert(CG_DEPTH <= 8 && CG_DEPTH < CG_SRING, "named barriers, slot ring")
 // state.  Otherwise CTA b evaluates labels [b per, (b+1) per) from scratch.
 // Warp 0 of every CTA does the exchange and all bookkeeping; the other worker warps only test their
 // proposals and update their part of the eps slab, and learn the outcome from a small descriptor.
+// Written as a device function of (parameters, CTA index, CTA count) so that one launch can also hold
+// several sims side by side (cg_pr_persistent_many): nothing in it looks at blockIdx or gridDim, and all
+// synchronisation between CTAs goes through the sim's own slots and publication words.
 template <int THREADS, int RP, bool CACHED>
-__global__ void __launch_bounds__(THREADS, 1) cg_pr_persistent(const CgParams p)
+__device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 b, const u32 nb)
 {
     constexpr int TW = THREADS - 64;      // worker threads; then the control warp and the service warp
     constexpr int NWK = TW / 32;          // worker warps = index of the control warp
@@ -360,7 +363,6 @@ __global__ void __launch_bounds__(THREADS, 1) cg_pr_persistent(const CgParams p)
 #endif
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const u32 b = blockIdx.x, nb = gridDim.x;
     const int L = p.L, lg = p.lgL;
     const u32 N = p.N, M = p.M;
     const u32 mask = ((u32)(L - 1) << (lg + 1)) | (u32)(L - 1);
@@ -811,6 +813,30 @@ __global__ void __launch_bounds__(THREADS, 1) cg_pr_persistent(const CgParams p)
         for (u32 w = tid; w < (N + 31) / 32; w += TW) p.nbits[w] = s_n[w];
 }
 
+template <int THREADS, int RP, bool CACHED>
+__global__ void __launch_bounds__(THREADS, 1) cg_pr_persistent(const CgParams p)
+{
+    pr_persistent_body<THREADS, RP, CACHED>(p, blockIdx.x, gridDim.x);
+}
+
+// Replica packing (the paper recommends averaging many samples): ONE launch,
+// CTAs [first[s], first[s+1]) run sim s with its own parameter block.  The sims share nothing.
+template <int THREADS, int RP, bool CACHED>
+__global__ void __launch_bounds__(THREADS, 1)
+cg_pr_persistent_many(const CgParams* __restrict__ ps, const u32* __restrict__ first, const u32 n_sims)
+{
+    __shared__ CgParams sp;
+    __shared__ u32 s_b, s_nb;
+    if (threadIdx.x == 0) {
+        u32 s = 0;
+        while (s + 1 < n_sims && first[s + 1] <= blockIdx.x) ++s;
+        s_b = blockIdx.x - first[s]; s_nb = first[s + 1] - first[s];
+        sp = ps[s];
+    }
+    __syncthreads();
+    pr_persistent_body<THREADS, RP, CACHED>(sp, s_b, s_nb);
+}
+
 // Step a6 alone: scripted hops, update in place (no readers), one launch.
 template <int THREADS, int RP>
 __global__ void __launch_bounds__(THREADS, 1)
@@ -959,6 +985,7 @@ struct cg_sim {
     u64* d_slots = nullptr; CgCtl* d_ctl = nullptr; u64* d_red = nullptr;
     void* d_log = nullptr; bool own_log = false; u64 log_cap = 0;
     u64* d_trace = nullptr; u32 trace_iters = 0;
+    void* d_many = nullptr; size_t many_cap = 0;      // parameter blocks of cg_run_many (owned by its first sim)
     // launch shape
     int num_sms = 0, n_ctas = 0, threads = 0, smem = 0, rp = 0, pl = 0;   // pl > 0: cached proposals
     std::string err;
@@ -974,6 +1001,7 @@ static int fail_cuda(cg_sim* s, cudaError_t e, const char* what)
     return CG_ECUDA;
 }
 #define CK(call) do { cudaError_t e__ = (call); if (e__ != cudaSuccess) return fail_cuda(s, e__, #call); } while (0)
+#define CK0(sim, call) do { cudaError_t e__ = (call); if (e__ != cudaSuccess) return fail_cuda(sim, e__, #call); } while (0)
 
 static size_t align256(size_t v) { return (v + 255) & ~(size_t)255; }
 
@@ -1135,6 +1163,24 @@ static persist_fn persistent_kernel(int threads, int rp, bool cached)
                    return cached ? persistent_kernel_t<1024, true>(rp) : persistent_kernel_t<1024, false>(rp);
     }
     return nullptr;
+}
+typedef void (*many_fn)(const CgParams*, const u32*, u32);
+template <bool CACHED>
+static many_fn many_kernel_t(int rp)
+{
+    switch (rp) {
+        case 0: return cg_pr_persistent_many<512, 0, CACHED>;
+        case 1: return cg_pr_persistent_many<512, 1, CACHED>;
+        case 2: return cg_pr_persistent_many<512, 2, CACHED>;
+        case 4: return cg_pr_persistent_many<512, 4, CACHED>;
+        case 8: return cg_pr_persistent_many<512, 8, CACHED>;
+    }
+    return nullptr;
+}
+static many_fn many_kernel(int threads, int rp, bool cached)
+{
+    if (threads != 512) return nullptr;
+    return cached ? many_kernel_t<true>(rp) : many_kernel_t<false>(rp);
 }
 static scripted_fn scripted_kernel(int rp)
 {
@@ -1304,6 +1350,7 @@ extern "C" void cg_free(cg_sim* s)
     if (!s) return;
     if (s->stream || s->ws) cudaStreamSynchronize(s->stream);
     if (s->own_log && s->d_log) cudaFree(s->d_log);
+    if (s->d_many) cudaFree(s->d_many);
     if (s->own_ws && s->ws) cudaFree(s->ws);
     delete s;
 }
@@ -1317,6 +1364,54 @@ extern "C" int cg_run(cg_sim* s, uint64_t n_hops)
     CgParams p = make_params(s, n_hops);
     void* args[] = {&p};
     CK(cudaLaunchCooperativeKernel((const void*)f, dim3(s->n_ctas), dim3(s->threads), args, (size_t)s->smem, s->stream));
+    return CG_OK;
+}
+
+extern "C" int cg_run_many(cg_sim* const* sims, int n_sims, uint64_t n_hops)
+{
+    if (!sims || n_sims < 1 || n_sims > CG_MAX_CTAS) return CG_EINVAL;
+    cg_sim* s0 = sims[0];
+    if (!s0) return CG_EINVAL;
+    if (n_hops == 0) return CG_OK;
+    std::vector<CgParams> ps((size_t)n_sims);
+    std::vector<u32> first((size_t)n_sims + 1, 0u);
+    int smem = 0;
+    for (int k = 0; k < n_sims; ++k) {
+        cg_sim* s = sims[k];
+        if (!s) return CG_EINVAL;
+        for (int m = 0; m < k; ++m) if (sims[m] == s) return CG_EINVAL;       // a sim may appear once
+        if (s->stream != s0->stream || s->threads != s0->threads || s->rp != s0->rp || (s->pl > 0) != (s0->pl > 0)) {
+            s0->err = "cg_run_many: the sims must share stream and launch shape (threads, register tiling, cached labels)";
+            return CG_EINVAL;
+        }
+        ps[(size_t)k] = make_params(s, n_hops);
+        first[(size_t)k + 1] = first[(size_t)k] + (u32)s->n_ctas;
+        smem = std::max(smem, s->smem);
+    }
+    many_fn f = many_kernel(s0->threads, s0->rp, s0->pl > 0);
+    if (!f) { s0->err = "cg_run_many: only 512-thread launch shapes"; return CG_EUNSUPPORTED; }
+    CK0(s0, cudaFuncSetAttribute((const void*)f, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+    int per_sm = 0;
+    CK0(s0, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, (const void*)f, s0->threads, smem));
+    const u32 total = first[(size_t)n_sims];
+    if (total > (u32)(per_sm * s0->num_sms)) {     // every CTA of every sim must be resident: they wait for each other
+        s0->err = "cg_run_many: the sims' CTAs do not fit on the device together";
+        return CG_EUNSUPPORTED;
+    }
+    const size_t need = ps.size() * sizeof(CgParams) + first.size() * sizeof(u32);
+    if (s0->many_cap < need) {
+        if (s0->d_many) { CK0(s0, cudaStreamSynchronize(s0->stream)); cudaFree(s0->d_many); s0->d_many = nullptr; s0->many_cap = 0; }
+        CK0(s0, cudaMalloc(&s0->d_many, need));
+        s0->many_cap = need;
+    }
+    CgParams* d_ps = (CgParams*)s0->d_many;
+    u32* d_first = (u32*)((char*)s0->d_many + ps.size() * sizeof(CgParams));
+    // pageable sources: the copies are staged before the calls return
+    CK0(s0, cudaMemcpyAsync(d_ps, ps.data(), ps.size() * sizeof(CgParams), cudaMemcpyHostToDevice, s0->stream));
+    CK0(s0, cudaMemcpyAsync(d_first, first.data(), first.size() * sizeof(u32), cudaMemcpyHostToDevice, s0->stream));
+    u32 n = (u32)n_sims;
+    void* args[] = {&d_ps, &d_first, &n};
+    CK0(s0, cudaLaunchCooperativeKernel((const void*)f, dim3(total), dim3(s0->threads), args, (size_t)smem, s0->stream));
     return CG_OK;
 }
 

@@ -12,7 +12,8 @@ W_R = time per hop - W_U (in the persistent kernel the two overlap, so W_R is wh
 explain), the update's algorithmic GB/s (16 N bytes per hop) and the drift of the incremental eps against a
 full-sum recomputation.
 
---replicas: independent sims on separate CUDA streams, persistent kernels side by side on one GPU.
+--replicas: independent sims side by side on one GPU: packed into ONE persistent launch (`cg_run_many`), and
+as separate persistent kernels on separate CUDA streams.
 
 Needs a CUDA device; nothing here computes on the host.
 """
@@ -111,6 +112,30 @@ def report_replicas(hops):
             name, len(sims), sims[0].launch()["n_ctas"], len(sims) * hops / ms * 1e3, hops / ms * 1e3))
         sys.stdout.flush()
 
+    def packed(name, idxs, copies, n_ctas=0):
+        """The same replica sets through cg_run_many: one launch, every sim on its own CTAs."""
+        sims = []
+        for r in range(copies):
+            for i in idxs:
+                kw = workloads.init_args(workloads.CONFIGS[name][i])
+                kw["seed"] += 100 * r
+                g = binding.CoulombGlass(**kw)
+                if n_ctas:
+                    g.set_launch(n_ctas, 512)
+                sims.append(g)
+        binding.run_many(sims, 1000)
+        torch.cuda.synchronize()
+        ms = _timed(lambda: binding.run_many(sims, hops))
+        print("%s x%d replicas packed into one launch (%d CTAs each): %.0f hops/s aggregate, %.0f per replica" % (
+            name, len(sims), sims[0].launch()["n_ctas"], len(sims) * hops / ms * 1e3, hops / ms * 1e3))
+        sys.stdout.flush()
+
+    sms = torch.cuda.get_device_properties(0).multi_processor_count
+    packed("cfg3_L128", [0, 1, 2, 3], 1)
+    packed("cfg3_L128", [0, 1, 2, 3], 2, n_ctas=sms // 8)
+    packed("cfg1_L16", [0], 32)
+    packed("cfg1_L16", [0], sms)
+    packed("cfg2_L64", [0], sms // 5)
     run("cfg3_L128", [0, 1, 2, 3], 1)     # the temperature sweep of config 3 as one replica set
     run("cfg3_L128", [0, 1, 2, 3], 2)
     run("cfg1_L16", [0], 1)

@@ -261,6 +261,52 @@ def test_replicas_on_separate_streams_run_concurrently_and_independently(cg, ora
         _compare(g, o, 5000)
 
 
+def test_replicas_packed_into_one_launch(cg, oracle_lib):
+    """cg_run_many: config 3's four temperatures, 19 CTAs each, side by side
+    in ONE persistent launch, in two calls (the chains continue); each is its own serial chain."""
+    sims = []
+    for cfg in workloads.CONFIGS["cfg3_L128"]:
+        kw = workloads.init_args(cfg)
+        sims.append((kw, cg.CoulombGlass(hop_log=5000, **kw)))
+    cg.run_many([g for _, g in sims], 3000)
+    cg.run_many([g for _, g in sims][::-1], 2000)      # order in the launch does not matter
+    for kw, g in sims:
+        o = oracle_lib.Oracle(**kw)
+        o.run(5000)
+        _compare(g, o, 5000)
+
+
+def test_many_one_cta_replicas_and_mixed_calls(cg, oracle_lib):
+    """One CTA per sim, one sim per SM, different seeds and temperatures; cg_run and cg_run_many mix freely."""
+    import torch
+    sms = torch.cuda.get_device_properties(0).multi_processor_count
+    kws = [dict(L=16, W=1.0, xi=1.0, T=0.05 + 0.001 * r, E=0.01, seed=900 + r, M=256) for r in range(sms)]
+    sims = [cg.CoulombGlass(hop_log=4000, **kw) for kw in kws]
+    sims[3].run(500)
+    cg.run_many(sims[:3] + sims[4:], 500)
+    cg.run_many(sims, 3500)
+    for r in (0, 3, 77, sms - 1):
+        o = oracle_lib.Oracle(**kws[r])
+        o.run(4000)
+        _compare(sims[r], o, 4000)
+    for g in sims:
+        assert g.counters()["hops"] == 4000 and g.recompute_eps() < 1e-9
+
+
+def test_run_many_refuses_what_it_cannot_run(cg):
+    kw = workloads.init_args(workloads.CONFIGS["cfg5_L512"][0])
+    a, b = cg.CoulombGlass(**kw), cg.CoulombGlass(**dict(kw, seed=99))
+    with pytest.raises(cg.CgError):          # 2 x 148 CTAs cannot be resident together
+        cg.run_many([a, b], 10)
+    with pytest.raises(cg.CgError):          # the same sim twice
+        cg.run_many([a, a], 10)
+    c = cg.CoulombGlass(16, T=0.1, seed=1, M=256)
+    with pytest.raises(cg.CgError):          # different launch shapes (register tiling)
+        cg.run_many([a, c], 10)
+    cg.run_many([a], 10)                     # a single sim is fine
+    assert a.counters()["hops"] == 10
+
+
 FULL = [("cfg1_L16", 0), ("cfg2_L64", 0), ("cfg3_L128", 0), ("cfg3_L128", 1), ("cfg3_L128", 2), ("cfg3_L128", 3),
         ("cfg4_L256", 2), ("cfg5_L512", 0)]
 
