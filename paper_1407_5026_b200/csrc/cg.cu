@@ -310,6 +310,21 @@ __device__ __forceinline__ bool metropolis(double dE, u32 uh, u32 ul, double T, 
 #else
 #define TRACE(ev, extra) do { } while (0)
 #endif
+#ifdef CG_TRACE_T
+// Time line: absolute SM clocks of 64 consecutive iterations (2000..2063 of a launch) of CTAs 0..31,
+// p.trace[((it - 2000) * 32 + b) * 32 + k]: k < 10 control warp (loop top, publication check done, early look
+// done, arrival at [A], CTA minimum, posted, scan done, before [B], arrived at [B], end), 10 scan position,
+// 11 attempts consumed; 16 + k worker warp 0 and 24 + k last worker warp (proposals known, tested, warp
+// minimum stored, [A] done, slab update done, [B] done, descriptor read, loop top).
+__device__ __forceinline__ u64 clk_now() { u64 t; asm volatile("mov.u64 %0, %%clock64;" : "=l"(t) :: "memory"); return t; }
+#define TS_CTL(k) do { if (lane == 0 && p.trace && b < 32u && it_local - 2000u < 64u) \
+    p.trace[((it_local - 2000u) * 32u + b) * 32u + (k)] = clk_now(); } while (0)
+#define TS_WRK(k) do { if (lane == 0 && (warp == 0 || warp == NWK - 1) && p.trace && b < 32u && itw - 2000u < 64u) \
+    p.trace[((itw - 2000u) * 32u + b) * 32u + 16u + (warp ? 8u : 0u) + (k)] = clk_now(); } while (0)
+#else
+#define TS_CTL(k) do { } while (0)
+#define TS_WRK(k) do { } while (0)
+#endif
 
 // What warp 0 tells the other warps of its CTA about an exchange (written before the second barrier).
 struct Desc {
@@ -478,6 +493,7 @@ __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 
         while (hl < p.n_hops) {
             const u32 e32 = e_start + it_local;
             const u32 kb = b >= c_first ? b - c_first : b + nb - c_first;    // my scan position
+            TS_CTL(0);
 #ifdef CG_TRACE
             if (lane == 0) { if (t_prev == 0) t_prev = clock64(); s_seg[CLS_ + 15] += 1; }
 #endif
@@ -505,6 +521,7 @@ __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 
                 fence_acquire_gpu();
             }
             TRACE(6, 0);
+            TS_CTL(1);
             // A CTA that does not hold the start of the window usually runs behind the one that does: the
             // winner of this exchange may already be posted.  One look at the first two scan positions
             // before the barrier takes that round trip off the path between the two barriers.
@@ -535,7 +552,9 @@ __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 
 #ifdef CG_TRACE_W
             cw[15] += 1; if (eq != CG_NONE) cw[14] += 1; if (kb == 0) cw[13] += 1;
 #endif
+            TS_CTL(2);
             barX_sync(TB);                // [A] the workers have tested their proposals
+            TS_CTL(3);
             TRACE(3, 0);
             // ---- step 3: lowest accepting label: CTA, then grid
             u32 gmin; u64 gpay;
@@ -552,12 +571,14 @@ __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 
             // order; the scan stops there: slots of later CTAs are never waited for (their proposals
             // cannot win), and the first CTA, when it accepts, waits for nobody.
             const bool own_low = gmin != CG_NONE && (!CACHED || kb != 0 || gmin < tail0);
+            TS_CTL(4);
             // A CTA can be up to DEPTH + 1 exchanges ahead of the slowest reader of its slot (bounded by the
             // publication check and by every fully rejected window, which needs all slots): ring of CG_SRING.
             if (nb > 1 && lane == 0)
                 slot_store(my_slot + ring, ((u64)e32 << 32) | gmin,
                            ((u64)(e32 & 0xFFFFu) << 48) | ((gpay >> 32) << 24) | (gpay & 0xFFFFFFu));
             u32 q = gmin; u64 wp = gpay;
+            TS_CTL(5);
             TRACE(10, 0);
             if (eq != CG_NONE) { q = eq; wp = ewp; }                   // answered before the barrier
             else if (!(own_low && kb == 0) && nb > 1) {
@@ -613,6 +634,7 @@ __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 
             }
 #endif
             TRACE(4, 0);
+            TS_CTL(6);
             // ---- what the workers need: attempts consumed (m = (p-1)M + q per executed hop, PAPER.md:39,
             // 78), the hop (step 3a), occupations, pending list
             const u32 used = q == CG_NONE ? M : q + 1;
@@ -631,7 +653,14 @@ __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 
                 }
             }
             TRACE(5, 0);
+            TS_CTL(7);
             barB_arrive(TB);              // [B] the workers may read the descriptor; this warp goes on
+            TS_CTL(8);
+#ifdef CG_TRACE_T
+            if (lane == 0 && p.trace && b < 32u && it_local - 2000u < 64u) {
+                p.trace[((it_local - 2000u) * 32u + b) * 32u + 10] = kb; p.trace[((it_local - 2000u) * 32u + b) * 32u + 11] = used;
+            }
+#endif
             // ---- the rest of the bookkeeping, while the workers run
             if (CACHED) {
                 if (t0r + used < per) t0r += used;
@@ -657,6 +686,7 @@ __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 
                 // and awaited before that
                 need_pub = hl >= CG_DEPTH ? pub_base + hl - CG_DEPTH + 1 : 0;
             }
+            TS_CTL(9);
             TRACE(0, 0);
         }
 #ifdef CG_TRACE
@@ -697,7 +727,11 @@ __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 
 #endif
     u64 a0 = a_start;                     // first attempt of the window (used when labels are not cached)
     uint4 d4 = make_uint4(0u, 0u, 0u, 0u);       // used, hop, ci, cj of the previous exchange
+#ifdef CG_TRACE_T
+    u32 itw = 0;
+#endif
     for (;;) {
+        TS_WRK(7);
         if (CACHED) {
             if (has_label && d4.x) {
                 if (lab >= d4.x) lab -= d4.x;
@@ -717,6 +751,7 @@ __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 
             upd = true;
         }
         if (hl >= p.n_hops) break;
+        TS_WRK(0);
 #ifdef CG_TRACE_W
         const long long w0 = clock64();
 #endif
@@ -769,6 +804,7 @@ __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 
                 if (metropolis(dE, w2 & 0x1FFFFFu, w3, p.T, p.inv_T)) { best = l; bi = i; bj = j; break; }
             }
         }
+        TS_WRK(1);
 #ifdef CG_TRACE_W
         const long long w1 = clock64();
 #endif
@@ -778,10 +814,12 @@ __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 
             const int src = __ffs(__ballot_sync(CG_FULL, best == wmin)) - 1;
             if (lane == src) { s_wlab[warp] = wmin; s_wpay[warp] = ((u64)bi << 32) | (u64)bj; }
         }
+        TS_WRK(2);
 #ifdef CG_TRACE_W
         const long long w2 = clock64();
 #endif
         barX_sync(TB);                    // [A]
+        TS_WRK(3);
 #ifdef CG_TRACE_W
         const long long w3 = clock64();
 #endif
@@ -790,10 +828,12 @@ __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 
         // CTA holds the start of the window, the decode one attempt ahead
         if (upd) { slab.issue(tf, mask, pr0, pr1, hci, hcj); finish_update(); }
         if (has_label && !nxt_valid && ahead) { nxt = decode_attempt(tb, p, a_cur + P); nxt_valid = true; }
+        TS_WRK(4);
 #ifdef CG_TRACE_W
         const long long w4 = clock64();
 #endif
         barB_sync(TB);                    // [B] the control warp has written the descriptor
+        TS_WRK(5);
 #ifdef CG_TRACE_W
         {
             const long long w5 = clock64();
@@ -804,6 +844,10 @@ __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 
 #endif
         d4 = *reinterpret_cast<const uint4*>(&s_desc);      // used, hop, ci, cj
         ahead = s_desc.ahead != 0;
+        TS_WRK(6);
+#ifdef CG_TRACE_T
+        ++itw;
+#endif
     }
 #ifdef CG_TRACE_W
     if (p.trace && lane == 0) for (int k = 0; k < 7; ++k) p.trace[((size_t)b * 16 + warp) * 8 + k] = tw[k];
@@ -1632,7 +1676,7 @@ extern "C" int cg_set_trace(cg_sim* s, void* dev_buf, size_t bytes, uint32_t ite
     if (!s) return CG_EINVAL;
     CK(cudaStreamSynchronize(s->stream));
     if (!dev_buf || !iterations) { s->d_trace = nullptr; s->trace_iters = 0; return CG_OK; }
-#if !defined(CG_TRACE) && !defined(CG_TRACE_W)
+#if !defined(CG_TRACE) && !defined(CG_TRACE_W) && !defined(CG_TRACE_T)
     return CG_EUNSUPPORTED;                   // the library was built without -DCG_TRACE
 #endif
     if (((uintptr_t)dev_buf & 7) || bytes < (size_t)8 * 64 * CG_MAX_CTAS) return CG_EINVAL;
