@@ -335,8 +335,8 @@ struct Desc {
     u32 pad[3];
 };
 struct Pend {               // pending hops, for threads that start to follow a pair of sites
-    u32 npend, rbuf, head;  // entry k (oldest first) is c[(head + k) % CG_DEPTH]
-    u32 c[CG_DEPTH][2];     // coded sites (i, j)
+    u32 npend, rbuf, first, pad;   // buffer rbuf + the npend hops c[(first + k) % CG_DEPTH], k = 0.. (oldest first)
+    u32 c[CG_DEPTH][2];     // coded sites (i, j) of the last CG_DEPTH executed hops, hop number h at (h - 1) % CG_DEPTH
 };
 static_assert(CG_DEPTH <= 8 && CG_DEPTH < CG_SRING, "named barriers, slot ring");
 
@@ -369,7 +369,7 @@ __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 
     __shared__ u64 s_wpay[32];
     __shared__ u64 s_verified;            // newest publication sequence number seen from ALL CTAs (service warp)
     __shared__ __align__(16) Desc s_desc;
-    __shared__ __align__(8) Pend s_pend;
+    __shared__ __align__(16) Pend s_pend;
     const Tables tb = {s_cdfi, s_invr, s_fld, s_disp, s_guide};
 #ifdef CG_TRACE
     __shared__ u64 s_seg[64];
@@ -390,7 +390,7 @@ __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 
     for (u32 w = tid; w < (N + 31) / 32; w += THREADS) s_n[w] = p.nbits[w];
     if (tid == 0) {
         s_verified = p.ctl->pub_base;
-        s_pend.npend = 0; s_pend.rbuf = p.ctl->cur; s_pend.head = 0;
+        s_pend.npend = 0; s_pend.rbuf = p.ctl->cur; s_pend.first = 0;
     }
 
     const u64 a_start = p.ctl->attempts, pub_base = p.ctl->pub_base;
@@ -477,16 +477,18 @@ __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 
         long long dP = 0;
         u32 it_local = 0;                 // PR iterations of this launch
         // Pending hops.  eps lives in a ring of CG_RING buffers: hop h writes eps_h (each CTA its own
-        // slab) into the buffer after the one hop h-1 wrote.  Nobody reads the two newest buffers, which
-        // other CTAs may still be writing: a proposal that starts to follow a pair of sites reads
-        // eps_{h-2} (buffer rbuf, complete on every CTA: checked against pub_count) and adds the terms
-        // 1/r_lj - 1/r_li of the npend <= 2 newest hops itself, in hop order - the same single rounded
-        // adds the update performs, so the values are bit-identical.  A CTA writes eps_{h+1} only when
-        // every CTA has published hop h-1, i.e. reads eps_{h-3} or newer: five buffers are never
-        // written while read.
-        u32 rbuf = wbuf, npend = 0, head = 0;     // as in s_pend
+        // slab) into the buffer after the one hop h-1 wrote.  Nobody reads buffers that other CTAs may
+        // still be writing: a proposal that starts to follow a pair of sites reads eps_v, v = the newest
+        // hop every CTA has published (buffer rbuf; v >= h - DEPTH by the publication check), and adds
+        // the terms 1/r_lj - 1/r_li of the hops v+1 .. h itself, in hop order - the same single rounded
+        // adds the update performs, so the values are bit-identical whatever v is.  A CTA writes
+        // eps_{h'} only when every CTA has published hop h' - DEPTH; a reader at hop h has published
+        // at most h, so h' <= h + DEPTH while it reads v >= h - DEPTH: with 2 DEPTH + 1 buffers a
+        // buffer is never written while read.
+        const u32 cur0 = wbuf;            // buffer that holds eps at the start of this launch
         // CTA c has published hop number h of this launch once its pub word is >= pub_base + h
-        u64 need_pub = 0;                 // ... for the hop whose buffer becomes rbuf at the next executed hop
+        u64 need_pub = 0;                 // hop hl - DEPTH + 1: readers never reach back further than DEPTH hops
+        u64 ver = pub_base;               // newest publication seen from ALL CTAs
 #ifdef CG_TRACE_W
         u64 cw[16] = {}; long long cprev = clock64();
 #endif
@@ -497,10 +499,11 @@ __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 
 #ifdef CG_TRACE
             if (lane == 0) { if (t_prev == 0) t_prev = clock64(); s_seg[CLS_ + 15] += 1; }
 #endif
-            // The buffer that becomes rbuf at the next executed hop must be complete on every CTA before the
-            // workers of this CTA are let into the next iteration: one publication word per CTA, each in its
+            // Hop hl - DEPTH + 1 must be complete on every CTA before the workers of this CTA are let into the
+            // next iteration (readers reach back at most DEPTH hops): one publication word per CTA, each in its
             // own L2 slice.  This warp is idle while the workers test their proposals, so the check is free.
-            if (nb > 1 && *(volatile u64*)&s_verified < need_pub) {     // rarely: the service warp has usually seen it
+            if (nb > 1) ver = max(ver, *(volatile u64*)&s_verified);
+            if (nb > 1 && ver < need_pub) {                             // rarely: the service warp has usually seen it
                 for (;;) {
                     bool ok = true;
                     for (u32 c0 = lane; c0 < nb; c0 += 32 * 8) {        // eight independent loads in flight
@@ -519,6 +522,7 @@ __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 
                     if (__all_sync(CG_FULL, ok)) break;
                 }
                 fence_acquire_gpu();
+                ver = need_pub;
             }
             TRACE(6, 0);
             TS_CTL(1);
@@ -641,15 +645,26 @@ __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 
             const u32 hi_ = (u32)(wp >> 32), hj_ = (u32)wp;
             const u32 ci = site_code(hi_, L), cj = site_code(hj_, L);
             if (lane == 0) *reinterpret_cast<uint4*>(&s_desc) = make_uint4(used, q != CG_NONE, ci, cj);
-            if (q != CG_NONE) {
-                const u32 pos = npend < CG_DEPTH ? (head + npend) % CG_DEPTH : head;
-                if (npend < CG_DEPTH) ++npend;
-                else { head = (head + 1) % CG_DEPTH; rbuf = rbuf == CG_RING - 1 ? 0u : rbuf + 1u; }
+            // Readers start from a buffer that is complete on every CTA (hop v; this CTA's own slab of hop hl is
+            // finished in the gap that ends at [B]) and add the hops v+1 .. themselves, in hop order.
+            {
+                const u32 hn_ = (u32)hl + (q != CG_NONE ? 1u : 0u);                 // hops executed so far
+#ifdef CG_VNEW
+                const u32 v = nb > 1 ? (u32)(ver - pub_base) : (u32)hl;
+#else
+                // one CTA: its own slab is always complete.  Several: DEPTH hops back is what the publication
+                // check guarantees; starting from the newest buffer seen complete (ver) saves pending terms but
+                // measured slower at 19 CTAs (-5 %) and equal at 148.
+                const u32 v = nb > 1 ? (hn_ > CG_DEPTH ? hn_ - CG_DEPTH : 0u) : (u32)hl;
+#endif
+                const u32 np_ = hn_ - v;                                            // <= DEPTH
                 if (lane == 0) {              // the workers are between the two barriers: nobody reads these
-                    atomicAnd(&s_n[hi_ >> 5], ~(1u << (hi_ & 31)));     // no return value: fire and forget
-                    atomicOr(&s_n[hj_ >> 5], 1u << (hj_ & 31));
-                    s_pend.c[pos][0] = ci; s_pend.c[pos][1] = cj;
-                    s_pend.npend = npend; s_pend.rbuf = rbuf; s_pend.head = head;
+                    if (q != CG_NONE) {
+                        atomicAnd(&s_n[hi_ >> 5], ~(1u << (hi_ & 31)));     // no return value: fire and forget
+                        atomicOr(&s_n[hj_ >> 5], 1u << (hj_ & 31));
+                        *reinterpret_cast<uint2*>(&s_pend.c[(u32)hl % CG_DEPTH][0]) = make_uint2(ci, cj);
+                    }
+                    *reinterpret_cast<uint4*>(&s_pend) = make_uint4(np_, (cur0 + v) % CG_RING, v % CG_DEPTH, 0u);
                 }
             }
             TRACE(5, 0);
@@ -682,8 +697,8 @@ __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 
                     p.log_a[h] = a_start + used_sum - 1; p.log_i[h] = hi_; p.log_j[h] = hj_;
                 }
                 ++hl;
-                // all slabs of hop hl - DEPTH + 1: they are read (as rbuf) once the NEXT hop is executed,
-                // and awaited before that
+                // all slabs of hop hl - DEPTH + 1: the oldest buffer a reader may start from once the NEXT
+                // hop is executed, awaited before that
                 need_pub = hl >= CG_DEPTH ? pub_base + hl - CG_DEPTH + 1 : 0;
             }
             TS_CTL(9);
@@ -700,7 +715,7 @@ __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 
             CgCtl* c = p.ctl;
             c->attempts = a_start + used_sum; c->hops = hops_start + hl;
             c->iterations += it_local; c->proposals += (u64)M * it_local;
-            c->dP += dP; c->cur = rbuf + npend >= CG_RING ? rbuf + npend - CG_RING : rbuf + npend; c->epoch += it_local;
+            c->dP += dP; c->cur = (u32)((cur0 + hl) % CG_RING); c->epoch += it_local;
             c->pub_base = pub_base + hl;
             c->cyc_total += (u64)(clock64() - t_begin);
         }
@@ -735,10 +750,13 @@ __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 
         if (CACHED) {
             if (has_label && d4.x) {
                 if (lab >= d4.x) lab -= d4.x;
-                else {                              // my attempt was consumed: take the next one
-                    lab += P - d4.x;
-                    if (!nxt_valid) nxt = decode_attempt(tb, p, a_cur + P);
-                    take(nxt); a_cur += P; nxt_valid = false;
+                else {                              // my attempt was consumed: the next one, P attempts later
+                    lab += P - d4.x; a_cur += P;
+                    // (deferring this decode to the gap between the barriers, for attempts that re-enter far
+                    // outside the window, measured slower: here it hides behind the warps that start to follow
+                    // new pairs)
+                    if (!nxt_valid) nxt = decode_attempt(tb, p, a_cur);
+                    take(nxt); nxt_valid = false;
                 }
             }
         } else a0 += d4.x;
@@ -765,7 +783,7 @@ __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 
                     const double* __restrict__ erd = p.eps[s_pend.rbuf];
                     ei = ld_cg(erd + ci_); ej = ld_cg(erd + cj_);
                     for (u32 k = 0; k < np; ++k) {
-                        const u32 e_ = (s_pend.head + k) % CG_DEPTH;
+                        const u32 e_ = (s_pend.first + k) % CG_DEPTH;
                         const u32 ki = s_pend.c[e_][0], kj = s_pend.c[e_][1];
                         ei = __dadd_rn(ei, hop_term(tf, mask, sci, ki, kj));
                         ej = __dadd_rn(ej, hop_term(tf, mask, scj, ki, kj));
@@ -795,7 +813,7 @@ __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 
                 double vi = ld_cg(erd + i), vj = ld_cg(erd + j);
                 const u32 si = site_code(i, L) | (u32)L, sj = site_code(j, L) | (u32)L;
                 for (u32 t = 0; t < np; ++t) {
-                    const u32 e_ = (s_pend.head + t) % CG_DEPTH;
+                    const u32 e_ = (s_pend.first + t) % CG_DEPTH;
                     const u32 ki = s_pend.c[e_][0], kj = s_pend.c[e_][1];
                     vi = __dadd_rn(vi, hop_term(tf, mask, si, ki, kj));
                     vj = __dadd_rn(vj, hop_term(tf, mask, sj, ki, kj));
