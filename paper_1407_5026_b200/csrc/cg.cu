@@ -365,8 +365,8 @@ __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 
     int* s_disp = reinterpret_cast<int*>(s_fld + KL);
     u32* s_guide = reinterpret_cast<u32*>(s_disp + KL);
     u32* s_n = s_guide + CG_GUIDE;
-    __shared__ u32 s_wlab[32];
-    __shared__ u64 s_wpay[32];
+    __shared__ u32 s_key;                 // lowest accepting (label << 5 | warp) of the CTA in this iteration
+    __shared__ u64 s_wpay[32];            // (i, j) of each warp's lowest accepting label
     __shared__ u64 s_verified;            // newest publication sequence number seen from ALL CTAs (service warp)
     __shared__ __align__(16) Desc s_desc;
     __shared__ __align__(16) Pend s_pend;
@@ -389,6 +389,7 @@ __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 
     for (int k = tid; k < CG_GUIDE; k += THREADS) s_guide[k] = p.guide[k];
     for (u32 w = tid; w < (N + 31) / 32; w += THREADS) s_n[w] = p.nbits[w];
     if (tid == 0) {
+        s_key = CG_NONE;
         s_verified = p.ctl->pub_base;
         s_pend.npend = 0; s_pend.rbuf = p.ctl->cur; s_pend.first = 0;
     }
@@ -561,14 +562,12 @@ __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 
             TS_CTL(3);
             TRACE(3, 0);
             // ---- step 3: lowest accepting label: CTA, then grid
-            u32 gmin; u64 gpay;
-            {
-                const u32 l_ = lane < NWK ? s_wlab[lane] : CG_NONE;
-                const u64 pay = lane < NWK ? s_wpay[lane] : 0ull;
-                gmin = __reduce_min_sync(CG_FULL, l_);
-                const int src = __ffs(__ballot_sync(CG_FULL, l_ == gmin)) - 1;
-                gpay = __shfl_sync(CG_FULL, pay, src);
-            }
+            // (every worker warp has put its lowest accepting label into one shared-memory minimum)
+            const u32 key = *(volatile u32*)&s_key;
+            const u32 gmin = key == CG_NONE ? CG_NONE : key >> 5;
+            const u64 gpay = key == CG_NONE ? 0ull : s_wpay[key & 31u];     // (0: the slot's fields must not overflow)
+            __syncwarp();
+            if (lane == 0) *(volatile u32*)&s_key = CG_NONE;          // for the next iteration (ordered by [B])
             // In scan order (CTA order starting at the CTA that holds attempt a0) every CTA holds lower
             // labels than the next one, except that CACHED the first CTA also holds the end of the window
             // in its threads below a0's ("tail" labels).  The winner is the first non-tail accept in scan
@@ -829,8 +828,10 @@ __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 
         // ---- step 3: lowest accepting label: warp, then the control warp
         {
             const u32 wmin = __reduce_min_sync(CG_FULL, best);
-            const int src = __ffs(__ballot_sync(CG_FULL, best == wmin)) - 1;
-            if (lane == src) { s_wlab[warp] = wmin; s_wpay[warp] = ((u64)bi << 32) | (u64)bj; }
+            if (wmin != CG_NONE && best == wmin) {     // labels are distinct: one lane
+                s_wpay[warp] = ((u64)bi << 32) | (u64)bj;
+                atomicMin(&s_key, (wmin << 5) | (u32)warp);
+            }
         }
         TS_WRK(2);
 #ifdef CG_TRACE_W
