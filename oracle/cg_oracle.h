@@ -93,6 +93,20 @@ uint64_t cgo_near_ties(const cgo_sim* s);   /* O10 certificate counter */
 uint64_t cgo_exp_evaluations(const cgo_sim* s);
 double   cgo_update_seconds(const cgo_sim* s); /* wall time spent in the O(N) update (W_U) */
 
+
+/* Observables.
+ * O11 stochastic time: per executed hop h (0-based count since cgo_init),
+ *     dt = m/Gamma + (sqrt(m)/Gamma) * z_h  (PAPER.md:78 step 3c), z_h standard
+ *     normal by Box-Muller from Philox domain 3 (reading G19), summed in hop order.
+ * O12 density of states as bin counts.
+ * O13 polarisation series (t_h, P_h) over the hop log.
+ * O14 sigma0 = dP/(N E t). */
+double cgo_normal_of_hop(const cgo_sim* s, uint64_t h);
+int  cgo_get_time_stochastic(const cgo_sim* s, double* t_tau0);
+int  cgo_dos(const cgo_sim* s, double lo, double width, uint32_t nbins, uint64_t* hist, uint64_t* outside);
+int  cgo_get_series(const cgo_sim* s, uint64_t first, uint64_t count, double* t, int64_t* P);
+int  cgo_sigma0(const cgo_sim* s, double* sigma0);
+
 #ifdef __cplusplus
 }
 #endif

@@ -61,6 +61,11 @@ def lib():
             "cgo_near_ties": (u64, [vp]),
             "cgo_exp_evaluations": (u64, [vp]),
             "cgo_update_seconds": (dbl, [vp]),
+            "cgo_normal_of_hop": (dbl, [vp, u64]),
+            "cgo_get_time_stochastic": (C.c_int, [vp, P(dbl)]),
+            "cgo_dos": (C.c_int, [vp, dbl, dbl, u32, vp, P(u64)]),
+            "cgo_get_series": (C.c_int, [vp, u64, u64, vp, vp]),
+            "cgo_sigma0": (C.c_int, [vp, P(dbl)]),
         }
         for name, (res, args) in sig.items():
             f = getattr(L, name)
@@ -199,3 +204,31 @@ class Oracle:
 
     def update_seconds(self):
         return lib().cgo_update_seconds(self._h)
+
+    # ---- observables (O11-O14 in cg_oracle.h)
+    def normal_of_hop(self, h):
+        return lib().cgo_normal_of_hop(self._h, int(h))
+
+    def time_stochastic(self):
+        t = C.c_double()
+        self._check(lib().cgo_get_time_stochastic(self._h, C.byref(t)))
+        return t.value
+
+    def dos(self, lo, width, nbins):
+        hist = np.zeros(nbins, np.uint64)
+        out = C.c_uint64()
+        self._check(lib().cgo_dos(self._h, float(lo), float(width), int(nbins), _ptr(hist), C.byref(out)))
+        return hist, out.value
+
+    def series(self, first=0, count=None):
+        if count is None:
+            count = self.counters()["hops"] - first
+        t = np.empty(count, np.float64)
+        P = np.empty(count, np.int64)
+        self._check(lib().cgo_get_series(self._h, int(first), int(count), _ptr(t), _ptr(P)))
+        return t, P
+
+    def sigma0(self):
+        v = C.c_double()
+        self._check(lib().cgo_sigma0(self._h, C.byref(v)))
+        return v.value
