@@ -107,6 +107,32 @@ int cg_enable_hop_log(cg_sim* s, uint64_t capacity, void* dev_buf, size_t bytes)
 int cg_get_hops(cg_sim* s, uint64_t first, uint64_t count,
                 uint64_t* attempt, uint32_t* i, uint32_t* j);
 
+/* ---- Observables: read-only device passes, outside the hot loop; each
+ * synchronises the sim's stream.  All output pointers are HOST pointers owned by the caller.
+ *
+ * cg_get_time_stochastic: elapsed time with the random increment of step 3c:
+ *   per executed hop h, dt_h = m_h/Gamma + (sqrt(m_h)/Gamma) z_h, m_h = attempts consumed
+ *   since the previous executed hop, z_h a standard normal deviate (Box-Muller of the Philox
+ *   block counter = (h lo, h hi, 3, 0), h = 0-based count of executed hops; G19).
+ *   m_h comes from the hop log, so the log must be enabled and must hold EVERY hop executed by
+ *   cg_run since it was enabled (CG_EINVAL otherwise); time before the enabling point enters
+ *   with the deterministic increment.  Summed in a fixed tree order (bit-reproducible).
+ * cg_get_normals: z[k] = z_{first_hop + k}, k < count (parity hook for the above).
+ * cg_get_dos: density of states as bin counts of eps: hist[b] = #{k : lo + b*width
+ *   <= eps_k < lo + (b+1)*width}, b < nbins <= 2^24, width > 0; *outside (may be NULL) = sites in
+ *   no bin.  g(eps) = hist / (N * width).
+ * cg_get_series: polarisation against time (Fig.3 inset) over logged hops
+ *   [first, first+count): t[k] = (a_h + 1)/Gamma (deterministic increment) and
+ *   P[k] = sum of dx over logged hops 0..h, h = first + k; t or P may be NULL.
+ *   Needs the complete hop log like cg_get_time_stochastic.
+ * cg_get_sigma0: sigma0 = dP/(N E t), t deterministic (Eq.(3));
+ *   CG_EINVAL for E = 0 or t = 0. */
+int cg_get_time_stochastic(cg_sim* s, double* t_tau0);
+int cg_get_normals(cg_sim* s, uint64_t first_hop, uint64_t count, double* z);
+int cg_get_dos(cg_sim* s, double lo, double width, uint32_t nbins, uint64_t* hist, uint64_t* outside);
+int cg_get_series(cg_sim* s, uint64_t first, uint64_t count, double* t, int64_t* P);
+int cg_get_sigma0(cg_sim* s, double* sigma0);
+
 /* Recompute eps from its definition eps_i = phi_i + sum_{j!=i}(n_j - 1/2)/r_ij
  * on the device and return max_i |eps_i - eps_i^incremental|. */
 int cg_recompute_eps(cg_sim* s, double* max_abs_dev);

@@ -17,6 +17,7 @@ CG_OK, CG_EINVAL, CG_ENOMEM, CG_ECUDA, CG_EUNSUPPORTED = 0, -1, -2, -3, -4
 
 EXPORTS = [
     "cg_init", "cg_workspace_bytes", "cg_init_ws", "cg_run", "cg_run_many", "cg_get_state", "cg_set_state",
+    "cg_get_time_stochastic", "cg_get_normals", "cg_get_dos", "cg_get_series", "cg_get_sigma0",
     "cg_get_counters", "cg_enable_hop_log", "cg_get_hops", "cg_recompute_eps", "cg_apply_hops",
     "cg_get_table_sizes", "cg_get_tables", "cg_get_phi", "cg_set_launch", "cg_get_launch",
     "cg_get_phase_cycles", "cg_set_trace", "cg_bench_l2_rmw", "cg_free", "cg_strerror", "cg_last_error",
@@ -53,6 +54,11 @@ def lib():
         "cg_enable_hop_log": (ci, [vp, u64, vp, sz]),
         "cg_get_hops": (ci, [vp, u64, u64, vp, vp, vp]),
         "cg_recompute_eps": (ci, [vp, P(dbl)]),
+        "cg_get_time_stochastic": (ci, [vp, P(dbl)]),
+        "cg_get_normals": (ci, [vp, u64, u64, vp]),
+        "cg_get_dos": (ci, [vp, dbl, dbl, u32, vp, P(u64)]),
+        "cg_get_series": (ci, [vp, u64, u64, vp, vp]),
+        "cg_get_sigma0": (ci, [vp, P(dbl)]),
         "cg_apply_hops": (ci, [vp, u64, vp, vp, P(C.c_float)]),
         "cg_get_table_sizes": (ci, [vp, P(i64), P(i64)]),
         "cg_get_tables": (ci, [vp, vp, vp, vp, vp, P(dbl), P(dbl)]),
@@ -202,6 +208,41 @@ class CoulombGlass:
         if self._log is None:
             return 0
         return min(self.counters()["hops"] - self._log_base, self._log_cap)
+
+    # ---- observables (include/cg.h "Observables"): argument marshalling only
+    def time_stochastic(self):
+        t = C.c_double()
+        with self._torch.cuda.device(self.device):
+            self._check(self._lib.cg_get_time_stochastic(self._h, C.byref(t)))
+        return t.value
+
+    def normals(self, first_hop, count):
+        z = np.empty(int(count), np.float64)
+        with self._torch.cuda.device(self.device):
+            self._check(self._lib.cg_get_normals(self._h, int(first_hop), int(count), _ptr(z)))
+        return z
+
+    def dos(self, lo, width, nbins):
+        hist = np.zeros(int(nbins), np.uint64)
+        outside = C.c_uint64()
+        with self._torch.cuda.device(self.device):
+            self._check(self._lib.cg_get_dos(self._h, float(lo), float(width), int(nbins), _ptr(hist),
+                                             C.byref(outside)))
+        return hist, outside.value
+
+    def series(self, first=0, count=None):
+        if count is None:
+            count = self.logged_hops() - first
+        t = np.empty(int(count), np.float64)
+        P = np.empty(int(count), np.int64)
+        with self._torch.cuda.device(self.device):
+            self._check(self._lib.cg_get_series(self._h, int(first), int(count), _ptr(t), _ptr(P)))
+        return t, P
+
+    def sigma0(self):
+        v = C.c_double()
+        self._check(self._lib.cg_get_sigma0(self._h, C.byref(v)))
+        return v.value
 
     def recompute_eps(self):
         dev = C.c_double()

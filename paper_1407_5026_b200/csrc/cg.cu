@@ -65,7 +65,8 @@ struct CgCtl {              // device-resident control block (one per sim)
     u64 pub_base;           // publication sequence number of the last hop of the previous launch: CTA c
                             // stores pub_base + h into its pub word once its slab of hop h of a launch is
                             // written (never reset, so stale words of other launch shapes are always smaller)
-    u64 pub_pad[3];
+    u64 log_a0;             // attempts consumed when the hop log was enabled (observables: m of the first logged hop)
+    u64 pub_pad[2];
 };
 
 struct CgParams {           // kernel parameter block
@@ -1520,7 +1521,7 @@ extern "C" int cg_set_state(cg_sim* s, const int8_t* n, const double* eps, uint6
     int rc = read_ctl(s, &c);
     if (rc != CG_OK) return rc;
     c.attempts = attempts; c.hops = hops; c.dP = dP; c.iterations = 0; c.proposals = 0; c.cur = 0;
-    c.log_base = hops;
+    c.log_base = hops; c.log_a0 = attempts;
     CK(cudaMemcpyAsync(s->d_eps[0], eps, 8 * (size_t)s->N, cudaMemcpyHostToDevice, s->stream));
     CK(cudaMemcpyAsync(s->d_nbits, bits.data(), 4 * bits.size(), cudaMemcpyHostToDevice, s->stream));
     CK(cudaMemcpyAsync(s->d_ctl, &c, sizeof c, cudaMemcpyHostToDevice, s->stream));
@@ -1560,7 +1561,7 @@ extern "C" int cg_enable_hop_log(cg_sim* s, uint64_t capacity, void* dev_buf, si
         }
         s->log_cap = capacity;
     }
-    c.log_base = c.hops;
+    c.log_base = c.hops; c.log_a0 = c.attempts;
     CK(cudaMemcpyAsync(s->d_ctl, &c, sizeof c, cudaMemcpyHostToDevice, s->stream));
     CK(cudaStreamSynchronize(s->stream));
     return CG_OK;
@@ -1767,3 +1768,297 @@ extern "C" const char* cg_strerror(int code)
 }
 
 extern "C" const char* cg_last_error(cg_sim* s) { return s ? s->err.c_str() : ""; }
+
+// ------------------------------------------------ observables --
+// Read-only passes over device state, outside the hot loop: the Gaussian time increment of step 3c
+// (PAPER.md:78), the density of states, the polarisation series and sigma0.
+
+// Standard normal deviate of executed hop h (reading G19): Box-Muller of the Philox block
+// counter = (h lo, h hi, 3, 0); u1 in (0,1], u2 in [0,1), 53 bits each.
+__device__ __forceinline__ double normal_of_hop(u64 h, u32 seed_lo, u32 seed_hi)
+{
+    u32 w0, w1, w2, w3;
+    philox4x32_10((u32)h, (u32)(h >> 32), 3u, 0u, seed_lo, seed_hi, w0, w1, w2, w3);
+    const u64 a = (((u64)w0 << 32) | w1) >> 11, b = (((u64)w2 << 32) | w3) >> 11;
+    const double u1 = (double)(a + 1) * 0x1p-53, u2 = (double)b * 0x1p-53;
+    const double rad = sqrt(__dmul_rn(-2.0, log(u1)));
+    const double ang = __dmul_rn(6.283185307179586476925286766559, u2);
+    return __dmul_rn(rad, cos(ang));
+}
+
+__global__ void cg_normals(double* __restrict__ z, u64 first, u64 count, u32 seed_lo, u32 seed_hi)
+{
+    for (u64 k = blockIdx.x * (u64)blockDim.x + threadIdx.x; k < count; k += (u64)gridDim.x * blockDim.x)
+        z[k] = normal_of_hop(first + k, seed_lo, seed_hi);
+}
+
+// Fixed-shape tree sum of a CTA's values (256 threads): the result depends on the launch shape only.
+__device__ __forceinline__ double cta_sum_256(double v, double* sh)
+{
+#pragma unroll
+    for (int o = 16; o; o >>= 1) v = __dadd_rn(v, __shfl_down_sync(CG_FULL, v, o));
+    if ((threadIdx.x & 31) == 0) sh[threadIdx.x >> 5] = v;
+    __syncthreads();
+    double r = 0.0;
+    if (threadIdx.x < 32) {
+        r = threadIdx.x < 8 ? sh[threadIdx.x] : 0.0;
+#pragma unroll
+        for (int o = 4; o; o >>= 1) r = __dadd_rn(r, __shfl_down_sync(CG_FULL, r, o));
+    }
+    __syncthreads();
+    return r;                               // valid in thread 0
+}
+
+// dt_h = m_h/Gamma + (sqrt(m_h)/Gamma) z_h, m_h from consecutive logged attempt indices;
+// CTA c sums logged hops [c*chunk, (c+1)*chunk) in a fixed order.
+__global__ void __launch_bounds__(256) cg_stoch_time_partial(const u64* __restrict__ log_a, u64 count, u64 a0,
+                                                             u64 hop0, double Gamma, u32 seed_lo, u32 seed_hi,
+                                                             u64 chunk, double* __restrict__ partial)
+{
+    __shared__ double sh[8];
+    const u64 lo = blockIdx.x * chunk, hi = min(lo + chunk, count);
+    double acc = 0.0;
+    for (u64 h = lo + threadIdx.x; h < hi; h += 256) {
+        const u64 prev = h ? log_a[h - 1] + 1 : a0;
+        const double m = (double)(log_a[h] + 1 - prev);
+        const double mean = __ddiv_rn(m, Gamma), sd = __ddiv_rn(sqrt(m), Gamma);
+        acc = __dadd_rn(acc, __dadd_rn(mean, __dmul_rn(sd, normal_of_hop(hop0 + h, seed_lo, seed_hi))));
+    }
+    const double r = cta_sum_256(acc, sh);
+    if (threadIdx.x == 0) partial[blockIdx.x] = r;
+}
+
+__global__ void __launch_bounds__(256) cg_sum_partials(const double* __restrict__ partial, u32 n, double* out)
+{
+    __shared__ double sh[8];
+    double acc = 0.0;
+    for (u32 k = threadIdx.x; k < n; k += 256) acc = __dadd_rn(acc, partial[k]);
+    const double r = cta_sum_256(acc, sh);
+    if (threadIdx.x == 0) *out = r;
+}
+
+// Density of states as bin counts: bin b = [lo + b*width, lo + (b+1)*width).
+// CTA-private bins in shared memory when they fit (nsh = nbins), else global atomics (nsh = 0).
+__global__ void __launch_bounds__(256) cg_dos(const double* __restrict__ eps, u32 N, double lo, double width,
+                                              u32 nbins, u32 nsh, unsigned long long* __restrict__ hist /* nbins + 1 */)
+{
+    extern __shared__ u32 sh_bins[];
+    for (u32 b = threadIdx.x; b < nsh; b += 256) sh_bins[b] = 0;
+    __syncthreads();
+    u32 outside = 0;
+    for (u32 k = blockIdx.x * 256 + threadIdx.x; k < N; k += gridDim.x * 256) {
+        const double x = floor(__ddiv_rn(__dsub_rn(eps[k], lo), width));
+        if (x >= 0.0 && x < (double)nbins) {
+            if (nsh) atomicAdd(&sh_bins[(u32)x], 1u);
+            else atomicAdd(&hist[(u32)x], 1ull);
+        } else ++outside;
+    }
+    outside = __reduce_add_sync(CG_FULL, outside);
+    if ((threadIdx.x & 31) == 0 && outside) atomicAdd(&hist[nbins], (unsigned long long)outside);
+    __syncthreads();
+    for (u32 b = threadIdx.x; b < nsh; b += 256)
+        if (sh_bins[b]) atomicAdd(&hist[b], (unsigned long long)sh_bins[b]);
+}
+
+// Polarisation series: P_h = sum of dx over logged hops 0..h, t_h = (a_h + 1)/Gamma.
+#define CG_SCAN_ITEMS 8
+#define CG_SCAN_CHUNK (256 * CG_SCAN_ITEMS)
+__device__ __forceinline__ int hop_dx(u32 i, u32 j, int L)
+{
+    int d = ((int)(j & (u32)(L - 1)) - (int)(i & (u32)(L - 1))) & (L - 1);
+    return d > L / 2 ? d - L : d;           // minimum image, tie -> +L/2 (G3)
+}
+
+__global__ void __launch_bounds__(256) cg_series_chunk_sums(const u32* __restrict__ li, const u32* __restrict__ lj,
+                                                            u64 count, int L, long long* __restrict__ sums)
+{
+    __shared__ long long sh[8];
+    const u64 base = blockIdx.x * (u64)CG_SCAN_CHUNK;
+    long long acc = 0;
+    for (int k = 0; k < CG_SCAN_ITEMS; ++k) {
+        const u64 h = base + (u64)k * 256 + threadIdx.x;
+        if (h < count) acc += hop_dx(li[h], lj[h], L);
+    }
+#pragma unroll
+    for (int o = 16; o; o >>= 1) acc += __shfl_down_sync(CG_FULL, acc, o);
+    if ((threadIdx.x & 31) == 0) sh[threadIdx.x >> 5] = acc;
+    __syncthreads();
+    if (threadIdx.x == 0) { long long t = 0; for (int w = 0; w < 8; ++w) t += sh[w]; sums[blockIdx.x] = t; }
+}
+
+__global__ void cg_series_scan_sums(long long* sums, u32 n)       // exclusive scan, one CTA of 256 threads
+{
+    __shared__ long long sh[256];
+    __shared__ long long carry;
+    if (threadIdx.x == 0) carry = 0;
+    __syncthreads();
+    for (u32 base = 0; base < n; base += 256) {
+        const u32 k = base + threadIdx.x;
+        const long long v = k < n ? sums[k] : 0;
+        sh[threadIdx.x] = v;
+        __syncthreads();
+        for (int o = 1; o < 256; o <<= 1) {
+            const long long t = threadIdx.x >= (u32)o ? sh[threadIdx.x - o] : 0;
+            __syncthreads();
+            sh[threadIdx.x] += t;
+            __syncthreads();
+        }
+        if (k < n) sums[k] = carry + sh[threadIdx.x] - v;
+        __syncthreads();
+        if (threadIdx.x == 0) carry += sh[255];
+        __syncthreads();
+    }
+}
+
+__global__ void __launch_bounds__(256) cg_series_write(const u64* __restrict__ la, const u32* __restrict__ li,
+                                                       const u32* __restrict__ lj, u64 first, u64 end, int L,
+                                                       double Gamma, const long long* __restrict__ sums,
+                                                       double* __restrict__ t, long long* __restrict__ P)
+{
+    __shared__ long long sh[8];
+    const u64 h0 = blockIdx.x * (u64)CG_SCAN_CHUNK + (u64)threadIdx.x * CG_SCAN_ITEMS;   // 8 consecutive hops per thread
+    long long v[CG_SCAN_ITEMS], run = 0;
+#pragma unroll
+    for (int k = 0; k < CG_SCAN_ITEMS; ++k) {
+        const u64 h = h0 + k;
+        run += h < end ? hop_dx(li[h], lj[h], L) : 0;
+        v[k] = run;
+    }
+    long long inc = run;                                         // inclusive scan of the thread totals
+    const u32 lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) { const long long y = __shfl_up_sync(CG_FULL, inc, o); if (lane >= (u32)o) inc += y; }
+    if (lane == 31) sh[w] = inc;
+    __syncthreads();
+    long long off = sums[blockIdx.x] + inc - run;
+    for (u32 k = 0; k < w; ++k) off += sh[k];
+#pragma unroll
+    for (int k = 0; k < CG_SCAN_ITEMS; ++k) {
+        const u64 h = h0 + k;
+        if (h >= first && h < end) {
+            if (P) P[h - first] = off + v[k];
+            if (t) t[h - first] = __ddiv_rn((double)(la[h] + 1), Gamma);
+        }
+    }
+}
+
+// Logged hops since the log was enabled; CG_EINVAL when the log is off or has overflowed (the observables
+// over the log need every hop since the enabling point).
+static int logged_hops(cg_sim* s, const CgCtl& c, u64* have)
+{
+    if (!s->d_log || !s->log_cap) return CG_EINVAL;
+    const u64 n = c.hops - c.log_base;
+    if (n > s->log_cap) return CG_EINVAL;
+    *have = n;
+    return CG_OK;
+}
+
+struct DevTmp {             // scratch of one observable call, released on every return path
+    void* p = nullptr;
+    ~DevTmp() { if (p) cudaFree(p); }
+};
+
+extern "C" int cg_get_normals(cg_sim* s, uint64_t first_hop, uint64_t count, double* z)
+{
+    if (!s || (count && !z)) return CG_EINVAL;
+    if (!count) return CG_OK;
+    DevTmp tmp;
+    CK(cudaMalloc(&tmp.p, 8 * count));
+    const unsigned grid = (unsigned)std::min<u64>((count + 255) / 256, 148 * 8);
+    cg_normals<<<grid, 256, 0, s->stream>>>((double*)tmp.p, first_hop, count, (u32)s->seed, (u32)(s->seed >> 32));
+    CK(cudaGetLastError());
+    CK(cudaMemcpyAsync(z, tmp.p, 8 * count, cudaMemcpyDeviceToHost, s->stream));
+    CK(cudaStreamSynchronize(s->stream));
+    return CG_OK;
+}
+
+extern "C" int cg_get_time_stochastic(cg_sim* s, double* t_tau0)
+{
+    if (!s || !t_tau0) return CG_EINVAL;
+    CgCtl c;
+    int rc = read_ctl(s, &c);
+    if (rc != CG_OK) return rc;
+    u64 have = 0;
+    if ((rc = logged_hops(s, c, &have)) != CG_OK) return rc;
+    const double t0 = (double)c.log_a0 / s->Gamma;           // before the log: deterministic increment
+    if (!have) { *t_tau0 = t0; return CG_OK; }
+    const u64 chunk = 4096;
+    const u32 nchunks = (u32)((have + chunk - 1) / chunk);
+    DevTmp tmp;
+    CK(cudaMalloc(&tmp.p, 8 * ((size_t)nchunks + 1)));
+    double* partial = (double*)tmp.p;
+    cg_stoch_time_partial<<<nchunks, 256, 0, s->stream>>>((const u64*)s->d_log, have, c.log_a0, c.log_base, s->Gamma,
+                                                         (u32)s->seed, (u32)(s->seed >> 32), chunk, partial);
+    cg_sum_partials<<<1, 256, 0, s->stream>>>(partial, nchunks, partial + nchunks);
+    CK(cudaGetLastError());
+    double sum = 0.0;
+    CK(cudaMemcpyAsync(&sum, partial + nchunks, 8, cudaMemcpyDeviceToHost, s->stream));
+    CK(cudaStreamSynchronize(s->stream));
+    *t_tau0 = t0 + sum;
+    return CG_OK;
+}
+
+extern "C" int cg_get_dos(cg_sim* s, double lo, double width, uint32_t nbins, uint64_t* hist, uint64_t* outside)
+{
+    if (!s || !hist || !(width > 0.0) || nbins == 0 || nbins > (1u << 24)) return CG_EINVAL;
+    CgCtl c;
+    int rc = read_ctl(s, &c);
+    if (rc != CG_OK) return rc;
+    DevTmp tmp;
+    CK(cudaMalloc(&tmp.p, 8 * ((size_t)nbins + 1)));
+    CK(cudaMemsetAsync(tmp.p, 0, 8 * ((size_t)nbins + 1), s->stream));
+    const u32 nsh = nbins <= 8192 ? nbins : 0;               // 32 KB of CTA-private bins
+    const unsigned grid = std::max(1u, std::min((s->N + 2047) / 2048, 148u * 4));
+    cg_dos<<<grid, 256, 4 * (size_t)nsh, s->stream>>>(s->d_eps[c.cur % CG_RING], s->N, lo, width, nbins, nsh,
+                                                      (unsigned long long*)tmp.p);
+    CK(cudaGetLastError());
+    std::vector<uint64_t> h((size_t)nbins + 1);
+    CK(cudaMemcpyAsync(h.data(), tmp.p, 8 * h.size(), cudaMemcpyDeviceToHost, s->stream));
+    CK(cudaStreamSynchronize(s->stream));
+    memcpy(hist, h.data(), 8 * (size_t)nbins);
+    if (outside) *outside = h[nbins];
+    return CG_OK;
+}
+
+extern "C" int cg_get_series(cg_sim* s, uint64_t first, uint64_t count, double* t, int64_t* P)
+{
+    if (!s) return CG_EINVAL;
+    CgCtl c;
+    int rc = read_ctl(s, &c);
+    if (rc != CG_OK) return rc;
+    u64 have = 0;
+    if ((rc = logged_hops(s, c, &have)) != CG_OK) return rc;
+    if (first + count > have) return CG_EINVAL;
+    if (!count || (!t && !P)) return CG_OK;
+    const u64 end = first + count;
+    const u32 nchunks = (u32)((end + CG_SCAN_CHUNK - 1) / CG_SCAN_CHUNK);
+    DevTmp tmp;
+    const size_t off_t = align256(8 * (size_t)nchunks), off_P = off_t + align256(8 * count);
+    CK(cudaMalloc(&tmp.p, off_P + 8 * count));
+    long long* sums = (long long*)tmp.p;
+    double* d_t = (double*)((char*)tmp.p + off_t);
+    long long* d_P = (long long*)((char*)tmp.p + off_P);
+    const u64* la = (const u64*)s->d_log;
+    const u32* li = (const u32*)((const char*)s->d_log + 8 * s->log_cap);
+    const u32* lj = (const u32*)((const char*)s->d_log + 12 * s->log_cap);
+    cg_series_chunk_sums<<<nchunks, 256, 0, s->stream>>>(li, lj, end, s->L, sums);
+    cg_series_scan_sums<<<1, 256, 0, s->stream>>>(sums, nchunks);
+    cg_series_write<<<nchunks, 256, 0, s->stream>>>(la, li, lj, first, end, s->L, s->Gamma, sums, d_t, d_P);
+    CK(cudaGetLastError());
+    if (t) CK(cudaMemcpyAsync(t, d_t, 8 * count, cudaMemcpyDeviceToHost, s->stream));
+    if (P) CK(cudaMemcpyAsync(P, d_P, 8 * count, cudaMemcpyDeviceToHost, s->stream));
+    CK(cudaStreamSynchronize(s->stream));
+    return CG_OK;
+}
+
+extern "C" int cg_get_sigma0(cg_sim* s, double* sigma0)
+{
+    if (!s || !sigma0) return CG_EINVAL;
+    CgCtl c;
+    int rc = read_ctl(s, &c);
+    if (rc != CG_OK) return rc;
+    if (s->E == 0.0 || c.attempts == 0) return CG_EINVAL;
+    const double t = (double)c.attempts / s->Gamma;
+    *sigma0 = (double)c.dP / (((double)s->N * s->E) * t);    // sigma0 = P/(N E t)
+    return CG_OK;
+}
