@@ -149,6 +149,7 @@ __device__ __forceinline__ void fence_acquire_gpu() { asm volatile("fence.acquir
 __device__ __forceinline__ void barN_arrive(u32 k, int n) { CG_BARN("bar.arrive") }   // k < CG_DEPTH <= 8
 __device__ __forceinline__ void barN_sync(u32 k, int n) { CG_BARN("bar.sync") }
 __device__ __forceinline__ void barX_sync(int n) { asm volatile("bar.sync 0, %0;" ::"r"(n) : "memory"); }
+__device__ __forceinline__ void barX_arrive(int n) { asm volatile("bar.arrive 0, %0;" ::"r"(n) : "memory"); }
 // barrier 5: second CTA barrier of an iteration; the control warp only arrives
 __device__ __forceinline__ void barB_sync(int n) { asm volatile("bar.sync 5, %0;" ::"r"(n) : "memory"); }
 __device__ __forceinline__ void barB_arrive(int n) { asm volatile("bar.arrive 5, %0;" ::"r"(n) : "memory"); }
@@ -838,7 +839,7 @@ __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 
 #ifdef CG_TRACE_W
         const long long w2 = clock64();
 #endif
-        barX_sync(TB);                    // [A]
+        barX_arrive(TB);                  // [A] only the control warp waits here: the workers go on to their slabs
         TS_WRK(3);
 #ifdef CG_TRACE_W
         const long long w3 = clock64();
