@@ -748,6 +748,14 @@ __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 
 #endif
     for (;;) {
         TS_WRK(7);
+        newhop = d4.y != 0;
+        // the term of the hop executed last iteration for the pair I follow: the four gathers start before the
+        // label bookkeeping (discarded if my attempt was consumed or theta_ij turns out to have changed)
+        double a_i = 0, b_i = 0, a_j = 0, b_j = 0;
+        if (CACHED && tracked && newhop) {
+            a_i = __ldg(tf + ((sci - d4.w) & mask)); b_i = __ldg(tf + ((sci - d4.z) & mask));
+            a_j = __ldg(tf + ((scj - d4.w) & mask)); b_j = __ldg(tf + ((scj - d4.z) & mask));
+        }
         if (CACHED) {
             if (has_label && d4.x) {
                 if (lab >= d4.x) lab -= d4.x;
@@ -761,7 +769,6 @@ __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 
                 }
             }
         } else a0 += d4.x;
-        newhop = d4.y != 0;
         if (newhop) {
             // step 3b: local energies of my slab, into the next buffer of the ring
             ++hl;
@@ -790,9 +797,7 @@ __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 
                         ej = __dadd_rn(ej, hop_term(tf, mask, scj, ki, kj));
                     }
                     tracked = true;
-                } else if (newhop) {       // the term of the hop executed last iteration
-                    const double a_i = __ldg(tf + ((sci - hcj) & mask)), b_i = __ldg(tf + ((sci - hci) & mask));
-                    const double a_j = __ldg(tf + ((scj - hcj) & mask)), b_j = __ldg(tf + ((scj - hci) & mask));
+                } else if (newhop) {       // the term of the hop executed last iteration (gathered above)
                     ei = __dadd_rn(ei, __dsub_rn(a_i, b_i)); ej = __dadd_rn(ej, __dsub_rn(a_j, b_j));
                 }
                 // dH_ij = eps_j - eps_i - 1/r_ij - E dx_ij
