@@ -852,8 +852,9 @@ __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 
         // while the control warp does the exchange: the slab of the previous hop (its table gathers,
         // issued when that hop was executed, have had the whole propose phase to arrive) and, if another
         // CTA holds the start of the window, the decode one attempt ahead
-        if (upd) { slab.issue(tf, mask, pr0, pr1, hci, hcj); finish_update(); }
-        if (has_label && !nxt_valid && ahead) { nxt = decode_attempt(tb, p, a_cur + P); nxt_valid = true; }
+        if (upd) slab.issue(tf, mask, pr0, pr1, hci, hcj);
+        if (has_label && !nxt_valid) { nxt = decode_attempt(tb, p, a_cur + P); nxt_valid = true; }   // behind the gathers
+        if (upd) finish_update();
         TS_WRK(4);
 #ifdef CG_TRACE_W
         const long long w4 = clock64();
