@@ -254,10 +254,11 @@ def run_ours(args):
     out["roofline"] = {
         "bound": "l2", "kernel": "cg_pr_persistent (the whole hop: propose, select, apply, update; one launch per step)",
         "achieved": achieved, "peak": l2_peak, "unit": "GB/s", "frac": achieved / l2_peak,
-        # ncu --set full (profiles/r1j_ncu_pr_persistent.txt): 0.71 KB of DRAM traffic and 6.5 MB of L2 sectors
-        # (4.4 read + 2.1 written) per hop - the state is L2-resident, so DRAM bytes are not the bound
-        "traffic": 710.0 * c["hops"] / K, "traffic_source": "ncu dram__bytes per hop x hops per launch",
-        "l2_bytes_per_hop_ncu": 6.54e6,
+        # ncu --set full (profiles/r1l_ncu_pr_persistent.txt, 20 000 hops): 4.37 MB of DRAM traffic per launch =
+        # 0.22 KB per hop and 6.95 MB of L2 sectors (4.84 read + 2.11 written) per hop - the state is L2-resident,
+        # so DRAM bytes are not the bound
+        "traffic": 219.0 * c["hops"] / K, "traffic_source": "ncu dram__bytes per hop x hops per launch",
+        "l2_bytes_per_hop_ncu": 6.95e6,
         "peak_source": "measured live: cg_bench_l2_rmw, 16-byte ld.cg/st.cg RMW over a resident %d-byte "
                        "buffer, 2000 passes per launch, best of 10 (MEASURED_PEAKS.json has no L2 figure)" % (16 * N),
         "algorithmic_bytes_per_hop": 16 * N,
