@@ -2,6 +2,7 @@
 
     python -m paper_1407_5026_b200.report --configs [--hops 200000] [--warm 2000]
     python -m paper_1407_5026_b200.report --replicas [--hops 100000]
+    python -m paper_1407_5026_b200.report --observables [--hops 200000]
 
 --configs: every workload of BASELINE.json (workloads.CONFIGS), a bounded prefix of its chain, one line each:
 accepted hops/s, window proposals evaluated/s (M per PR iteration), attempts consumed/s
@@ -14,6 +15,12 @@ full-sum recomputation.
 
 --replicas: independent sims side by side on one GPU: packed into ONE persistent launch (`cg_run_many`), and
 as separate persistent kernels on separate CUDA streams.
+
+--observables: the read-only device passes of include/cg.h "Observables" on a chain with its hop log: the
+deterministic clock t = attempts/Gamma next to the stochastic one of step 3c ("does not produce any
+appreciable difference"), sigma0 = dP/(N E t), the density of states around the
+Coulomb gap, the length of the P(t) series, and what each call costs (wall time of the whole call,
+device-to-host copy included).
 
 Needs a CUDA device; nothing here computes on the host.
 """
@@ -144,10 +151,43 @@ def report_replicas(hops):
     run("cfg2_L64", [0], 29)
 
 
+def report_observables(hops):
+    import time
+    print("# %s; %d hops from the random start, hop log on" % (torch.cuda.get_device_name(0), hops))
+
+    def wall(fn):
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        r = fn()
+        return r, 1e3 * (time.perf_counter() - t0)
+
+    for name, idx in (("cfg3_L128", 1), ("cfg5_L512", 0)):
+        cfg = workloads.CONFIGS[name][idx]
+        kw = workloads.init_args(cfg)
+        g = binding.CoulombGlass(hop_log=hops, **kw)
+        g.run(hops)
+        t_det = g.state()[2]
+        g.time_stochastic()                                  # first call: context warm-up
+        t_st, ms_t = wall(g.time_stochastic)
+        (hist, outside), ms_d = wall(lambda: g.dos(-4.0, 2.0**-4, 128))
+        (t, P), ms_s = wall(g.series)
+        sig, _ = wall(g.sigma0)
+        gdos = hist / (g.N * 2.0**-4)
+        mid = 64                                             # bin [0, 1/16)
+        print("%s T=%-5g: t_det %.6e  t_stoch %.6e (rel. diff %+.2e)  sigma0 %.4e  dP %d" % (
+            name, kw["T"], t_det, t_st, t_st / t_det - 1, sig, P[-1]))
+        print("    g(eps) at eps = -2, -1, -0.5, -0.25, 0, 0.25, 0.5, 1, 2: %s  (outside [-4,4): %d)" % (
+            " ".join("%.3f" % gdos[mid + int(e * 16)] for e in (-2, -1, -0.5, -0.25, 0, 0.25, 0.5, 1, 2)), outside))
+        print("    cost: time_stochastic %.2f ms (%d logged hops), dos %.2f ms (N = %d), series %.2f ms (%d points)" % (
+            ms_t, hops, ms_d, g.N, ms_s, t.size))
+        sys.stdout.flush()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--configs", action="store_true")
     ap.add_argument("--replicas", action="store_true")
+    ap.add_argument("--observables", action="store_true")
     ap.add_argument("--hops", type=int, default=0)
     ap.add_argument("--warm", type=int, default=2000)
     a = ap.parse_args()
@@ -157,6 +197,8 @@ def main():
         report_configs(a.hops or 200_000, a.warm)
     if a.replicas:
         report_replicas(a.hops or 100_000)
+    if a.observables:
+        report_observables(a.hops or 200_000)
 
 
 if __name__ == "__main__":
