@@ -115,7 +115,8 @@ int cg_get_hops(cg_sim* s, uint64_t first, uint64_t count,
  *   since the previous executed hop, z_h a standard normal deviate (Box-Muller of the Philox
  *   block counter = (h lo, h hi, 3, 0), h = 0-based count of executed hops; G19).
  *   m_h comes from the hop log, so the log must be enabled and must hold EVERY hop executed by
- *   cg_run since it was enabled (CG_EINVAL otherwise); time before the enabling point enters
+ *   cg_run since it was enabled (CG_EINVAL otherwise, also after scripted hops of cg_apply_hops, which
+ *   are not logged, until the log is enabled again or cg_set_state is called); time before the enabling point enters
  *   with the deterministic increment.  Summed in a fixed tree order (bit-reproducible).
  * cg_get_normals: z[k] = z_{first_hop + k}, k < count (parity hook for the above).
  * cg_get_dos: density of states as bin counts of eps: hist[b] = #{k : lo + b*width

@@ -1055,6 +1055,7 @@ struct cg_sim {
     u32* d_guide = nullptr;
     u64* d_slots = nullptr; CgCtl* d_ctl = nullptr; u64* d_red = nullptr;
     void* d_log = nullptr; bool own_log = false; u64 log_cap = 0;
+    bool log_gap = false;                 // scripted hops (cg_apply_hops) were executed while the log was on: it no longer holds every hop
     u64* d_trace = nullptr; u32 trace_iters = 0;
     void* d_many = nullptr; size_t many_cap = 0;      // parameter blocks of cg_run_many (owned by its first sim)
     // launch shape
@@ -1528,7 +1529,7 @@ extern "C" int cg_set_state(cg_sim* s, const int8_t* n, const double* eps, uint6
     int rc = read_ctl(s, &c);
     if (rc != CG_OK) return rc;
     c.attempts = attempts; c.hops = hops; c.dP = dP; c.iterations = 0; c.proposals = 0; c.cur = 0;
-    c.log_base = hops; c.log_a0 = attempts;
+    c.log_base = hops; c.log_a0 = attempts; s->log_gap = false;
     CK(cudaMemcpyAsync(s->d_eps[0], eps, 8 * (size_t)s->N, cudaMemcpyHostToDevice, s->stream));
     CK(cudaMemcpyAsync(s->d_nbits, bits.data(), 4 * bits.size(), cudaMemcpyHostToDevice, s->stream));
     CK(cudaMemcpyAsync(s->d_ctl, &c, sizeof c, cudaMemcpyHostToDevice, s->stream));
@@ -1557,7 +1558,7 @@ extern "C" int cg_enable_hop_log(cg_sim* s, uint64_t capacity, void* dev_buf, si
     int rc = read_ctl(s, &c);
     if (rc != CG_OK) return rc;
     if (s->own_log && s->d_log) { cudaFree(s->d_log); }
-    s->d_log = nullptr; s->own_log = false; s->log_cap = 0;
+    s->d_log = nullptr; s->own_log = false; s->log_cap = 0; s->log_gap = false;
     if (capacity) {
         if (dev_buf) {
             if (bytes < 16 * capacity || ((uintptr_t)dev_buf & 7)) return CG_EINVAL;
@@ -1619,6 +1620,7 @@ extern "C" int cg_apply_hops(cg_sim* s, uint64_t count, const uint32_t* i, const
     for (u64 h = 0; h < count; ++h)
         if (i[h] >= s->N || j[h] >= s->N || i[h] == j[h]) return CG_EINVAL;
     u32* d_ij = nullptr;
+    if (s->d_log) s->log_gap = true;
     CK(cudaMalloc(&d_ij, 8 * count));
     struct Free { void* p; ~Free() { cudaFree(p); } } fr{d_ij};
     CK(cudaMemcpyAsync(d_ij, i, 4 * count, cudaMemcpyHostToDevice, s->stream));
@@ -1953,7 +1955,7 @@ __global__ void __launch_bounds__(256) cg_series_write(const u64* __restrict__ l
 // over the log need every hop since the enabling point).
 static int logged_hops(cg_sim* s, const CgCtl& c, u64* have)
 {
-    if (!s->d_log || !s->log_cap) return CG_EINVAL;
+    if (!s->d_log || !s->log_cap || s->log_gap) return CG_EINVAL;
     const u64 n = c.hops - c.log_base;
     if (n > s->log_cap) return CG_EINVAL;
     *have = n;

@@ -109,6 +109,16 @@ def test_observables_need_a_complete_log(cg):
     g.run(1)                                              # the log has overflowed: m of later hops is lost
     with pytest.raises(cg.binding.CgError):
         g.time_stochastic()
+    # scripted hops are not logged: the log-based observables refuse until the log is enabled again
+    g.enable_hop_log(100)
+    g.run(5)
+    _, hi, hj = g.hops(4, 1)
+    g.apply_hops(hj, hi)                                  # a valid scripted hop: the last executed one, reversed
+    with pytest.raises(cg.binding.CgError):
+        g.series(0, 1)
+    g.enable_hop_log(100)
+    g.run(3)
+    assert g.series()[0].size == 3
     # the density of states needs no log; bad arguments are refused
     h, out = g.dos(-4.0, 0.5, 16)
     assert int(h.sum()) + out == g.N
