@@ -73,3 +73,15 @@ def test_diagnostic_entry_points_validate_arguments(cg):
     assert lib.cg_get_counters(None, None, None, None, None) == cg.binding.CG_EINVAL
     out = C.c_double()
     assert lib.cg_bench_l2_rmw(100, 1, 1, C.byref(out)) == cg.binding.CG_EINVAL      # too small a buffer
+
+
+def test_observable_entry_points_validate_arguments(cg):
+    """include/cg.h "Observables": a null sim or result pointer is CG_EINVAL, never a crash."""
+    lib = cg.lib()
+    E = cg.binding.CG_EINVAL
+    d, u = C.c_double(), C.c_uint64()
+    assert lib.cg_get_time_stochastic(None, C.byref(d)) == E
+    assert lib.cg_get_normals(None, 0, 1, None) == E
+    assert lib.cg_get_dos(None, 0.0, 1.0, 4, None, C.byref(u)) == E
+    assert lib.cg_get_series(None, 0, 0, None, None) == E
+    assert lib.cg_get_sigma0(None, C.byref(d)) == E
