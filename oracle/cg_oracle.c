@@ -4,6 +4,11 @@
  * Plain, slow, serial C in fp64, written from /root/reference/PAPER.md
  * (arXiv 1407.5026).  Every function cites the passage it follows; step
  * numbers O1..O10 are the bit-level readings listed in DESIGN.md.
+ * The same code runs the 2D lattice of the paper and its
+ * cubic 3D extension (reading G22 in DESIGN.md): a 2D lattice
+ * is the case Lz = 1 of an Lz x L x L torus, site s = (z L + y) L + x, so every
+ * loop below runs over (z, y, x) and visits the sites of a 2D lattice in the
+ * order s = y L + x.
  * Build: gcc -O2 -ffp-contract=off (no fast-math).  OpenMP is used ONLY for
  * the one-time O(N^2) full-sum of eps over the outer site index s; the sum
  * over t stays sequential (O6), and the Monte Carlo loop is single-threaded.
@@ -17,8 +22,9 @@
 
 struct cgo_sim {
     /* parameters */
-    int      L;
-    uint32_t N;
+    int      L;        /* lattice side                                          */
+    int      Lz;       /* 1: the paper's 2D L x L lattice; L: cubic 3D */
+    uint32_t N;        /* Lz * L * L sites, s = (z L + y) L + x                 */
     double   W, xi, T, E;
     uint64_t seed;
     uint32_t M;
@@ -27,8 +33,9 @@ struct cgo_sim {
     int8_t*  n;        /* N   occupations                    */
     double*  eps;      /* N   single-particle energies       */
     /* translation-invariant tables */
-    double*  invr;     /* L*L 1/r for offset ((dy mod L),(dx mod L))       */
+    double*  invr;     /* Lz*L*L 1/r for offset ((dz mod Lz),(dy mod L),(dx mod L)) */
     int64_t  K;        /* number of allowed displacements                  */
+    int32_t* ddz;      /* K   (all 0 in 2D)                                */
     int32_t* ddy;      /* K                                                */
     int32_t* ddx;      /* K                                                */
     double*  invr_k;   /* K   1/r of displacement k                        */
@@ -113,25 +120,37 @@ static int wrap(int v, int L)
     return v;
 }
 
+/* Coordinates of site a = (z L + y) L + x (z = 0 in 2D). */
+static inline void site_zyx(const cgo_sim* s, uint32_t a, int* z, int* y, int* x)
+{
+    uint32_t L = (uint32_t)s->L;
+    *x = (int)(a % L);
+    *y = (int)((a / L) % L);
+    *z = (int)(a / (L * L));
+}
+
 /* 1/r_ab under minimum image for sites a, b; 0 on the diagonal (O4). */
 static inline double invr_sites(const cgo_sim* s, uint32_t a, uint32_t b)
 {
-    int L = s->L;
-    int ya = (int)(a / (uint32_t)L), xa = (int)(a % (uint32_t)L);
-    int yb = (int)(b / (uint32_t)L), xb = (int)(b % (uint32_t)L);
-    return s->invr[(size_t)wrap(ya - yb, L) * (size_t)L + (size_t)wrap(xa - xb, L)];
+    int L = s->L, Lz = s->Lz;
+    int za, ya, xa, zb, yb, xb;
+    site_zyx(s, a, &za, &ya, &xa);
+    site_zyx(s, b, &zb, &yb, &xb);
+    return s->invr[((size_t)wrap(za - zb, Lz) * (size_t)L + (size_t)wrap(ya - yb, L)) * (size_t)L
+                   + (size_t)wrap(xa - xb, L)];
 }
 
 double cgo_invr_sites(const cgo_sim* s, uint32_t a, uint32_t b) { return invr_sites(s, a, b); }
 
 /* ---------------------------------------------------------------- O4/O5 - */
-struct disp { int64_t r2; int32_t dy, dx; };
+struct disp { int64_t r2; int32_t dz, dy, dx; };
 
 static int disp_cmp(const void* pa, const void* pb)
 {
     const struct disp* a = (const struct disp*)pa;
     const struct disp* b = (const struct disp*)pb;
     if (a->r2 != b->r2) return a->r2 < b->r2 ? -1 : 1;
+    if (a->dz != b->dz) return a->dz < b->dz ? -1 : 1;
     if (a->dy != b->dy) return a->dy < b->dy ? -1 : 1;
     if (a->dx != b->dx) return a->dx < b->dx ? -1 : 1;
     return 0;
@@ -139,42 +158,47 @@ static int disp_cmp(const void* pa, const void* pb)
 
 static int build_tables(cgo_sim* s)
 {
-    int L = s->L, h = L / 2;
+    int L = s->L, Lz = s->Lz, h = L / 2;
     /* 1/r for every offset of the torus, r = minimum-image Euclidean distance
      * in lattice units; no image sums. */
-    s->invr = (double*)malloc(sizeof(double) * (size_t)L * (size_t)L);
+    s->invr = (double*)malloc(sizeof(double) * (size_t)Lz * (size_t)L * (size_t)L);
     if (!s->invr) return CGO_ENOMEM;
-    for (int a = 0; a < L; ++a)
-        for (int b = 0; b < L; ++b) {
-            int da = min_image(a, L), db = min_image(b, L);
-            int64_t r2 = (int64_t)da * da + (int64_t)db * db;
-            s->invr[(size_t)a * L + b] = (r2 == 0) ? 0.0 : 1.0 / sqrt((double)r2);
-        }
+    for (int c = 0; c < Lz; ++c)
+        for (int a = 0; a < L; ++a)
+            for (int b = 0; b < L; ++b) {
+                int dc = min_image(c, Lz), da = min_image(a, L), db = min_image(b, L);
+                int64_t r2 = (int64_t)dc * dc + (int64_t)da * da + (int64_t)db * db;
+                s->invr[((size_t)c * L + a) * L + b] = (r2 == 0) ? 0.0 : 1.0 / sqrt((double)r2);
+            }
     /* Allowed hops: 0 < r <= L/2 ("We do not allow hops larger than L/2",
-     * PAPER.md:90), each ordered pair once: components in (-L/2, L/2]. */
-    size_t cap = (size_t)L * (size_t)L;
+     * PAPER.md:90), each ordered pair once: components in (-L/2, L/2]
+     * (dz = 0 only, in 2D). */
+    int zlo = (Lz == 1) ? 0 : -h + 1, zhi = (Lz == 1) ? 0 : h;
+    size_t cap = (size_t)Lz * (size_t)L * (size_t)L;
     struct disp* d = (struct disp*)malloc(sizeof(struct disp) * cap);
     if (!d) return CGO_ENOMEM;
     int64_t K = 0;
-    for (int dy = -h + 1; dy <= h; ++dy)
-        for (int dx = -h + 1; dx <= h; ++dx) {
-            int64_t r2 = (int64_t)dy * dy + (int64_t)dx * dx;
-            if (r2 > 0 && r2 <= (int64_t)h * h) {
-                d[K].r2 = r2; d[K].dy = dy; d[K].dx = dx; ++K;
+    for (int dz = zlo; dz <= zhi; ++dz)
+        for (int dy = -h + 1; dy <= h; ++dy)
+            for (int dx = -h + 1; dx <= h; ++dx) {
+                int64_t r2 = (int64_t)dz * dz + (int64_t)dy * dy + (int64_t)dx * dx;
+                if (r2 > 0 && r2 <= (int64_t)h * h) {
+                    d[K].r2 = r2; d[K].dz = dz; d[K].dy = dy; d[K].dx = dx; ++K;
+                }
             }
-        }
-    qsort(d, (size_t)K, sizeof(struct disp), disp_cmp);     /* order (r2, dy, dx): G12 */
+    qsort(d, (size_t)K, sizeof(struct disp), disp_cmp);     /* order (r2, dz, dy, dx): G12, G22 */
     s->K = K;
+    s->ddz = (int32_t*)malloc(sizeof(int32_t) * (size_t)K);
     s->ddy = (int32_t*)malloc(sizeof(int32_t) * (size_t)K);
     s->ddx = (int32_t*)malloc(sizeof(int32_t) * (size_t)K);
     s->invr_k = (double*)malloc(sizeof(double) * (size_t)K);
     s->cdf = (double*)malloc(sizeof(double) * (size_t)K);
-    if (!s->ddy || !s->ddx || !s->invr_k || !s->cdf) { free(d); return CGO_ENOMEM; }
+    if (!s->ddz || !s->ddy || !s->ddx || !s->invr_k || !s->cdf) { free(d); return CGO_ENOMEM; }
     /* Tower of Gamma^T_ij = exp(-2 r_ij / xi): running sum in
      * list order, normalised by the total. */
     double run = 0.0;
     for (int64_t k = 0; k < K; ++k) {
-        s->ddy[k] = d[k].dy; s->ddx[k] = d[k].dx;
+        s->ddz[k] = d[k].dz; s->ddy[k] = d[k].dy; s->ddx[k] = d[k].dx;
         double r = sqrt((double)d[k].r2);
         s->invr_k[k] = 1.0 / r;
         double t = -2.0 * r;
@@ -197,20 +221,23 @@ static int build_tables(cgo_sim* s)
  * summed in index order j = 0..N-1. */
 static void full_sum_eps(const cgo_sim* s, double* out)
 {
-    int L = s->L;
+    int L = s->L, Lz = s->Lz;
     int64_t N = (int64_t)s->N;
 #pragma omp parallel for schedule(static)
     for (int64_t a = 0; a < N; ++a) {
-        int ya = (int)(a / L), xa = (int)(a % L);
+        int za, ya, xa;
+        site_zyx(s, (uint32_t)a, &za, &ya, &xa);
         double e = s->phi[a];
-        for (int yb = 0; yb < L; ++yb) {                 /* b = yb*L + xb ascending */
-            const double* row = s->invr + (size_t)wrap(ya - yb, L) * (size_t)L;
-            const int8_t* nb = s->n + (size_t)yb * (size_t)L;
-            for (int xb = 0; xb < L; ++xb) {
-                if (yb == ya && xb == xa) continue;
-                e += ((double)nb[xb] - 0.5) * row[wrap(xa - xb, L)];
+        for (int zb = 0; zb < Lz; ++zb)
+            for (int yb = 0; yb < L; ++yb) {             /* b = (zb*L + yb)*L + xb ascending */
+                const double* row = s->invr + ((size_t)wrap(za - zb, Lz) * (size_t)L
+                                               + (size_t)wrap(ya - yb, L)) * (size_t)L;
+                const int8_t* nb = s->n + ((size_t)zb * (size_t)L + (size_t)yb) * (size_t)L;
+                for (int xb = 0; xb < L; ++xb) {
+                    if (zb == za && yb == ya && xb == xa) continue;
+                    e += ((double)nb[xb] - 0.5) * row[wrap(xa - xb, L)];
+                }
             }
-        }
         out[a] = e;
     }
 }
@@ -256,16 +283,17 @@ static int build_disorder_and_occupations(cgo_sim* s)
 }
 
 /* ------------------------------------------------------------------------ */
-int cgo_init(cgo_sim** out, int L, double W, double xi, double T, double E,
-             uint64_t seed, uint32_t M)
+static int init_lattice(cgo_sim** out, int dim, int L, double W, double xi, double T, double E,
+                        uint64_t seed, uint32_t M)
 {
     if (!out) return CGO_EINVAL;
     *out = NULL;
-    if (L < 2 || (L % 2) != 0 || L > 4096) return CGO_EINVAL;
+    if (L < 2 || (L % 2) != 0 || L > (dim == 3 ? 256 : 4096)) return CGO_EINVAL;
     if (!(xi > 0.0) || !(T > 0.0) || !(W >= 0.0) || M < 1 || !isfinite(E)) return CGO_EINVAL;
     cgo_sim* s = (cgo_sim*)calloc(1, sizeof(cgo_sim));
     if (!s) return CGO_ENOMEM;
-    s->L = L; s->N = (uint32_t)L * (uint32_t)L;
+    s->L = L; s->Lz = (dim == 3) ? L : 1;
+    s->N = (uint32_t)s->Lz * (uint32_t)L * (uint32_t)L;
     s->W = W; s->xi = xi; s->T = T; s->E = E; s->seed = seed; s->M = M;
     s->fixed_A = -1.0;
     s->phi = (double*)malloc(sizeof(double) * s->N);
@@ -280,11 +308,27 @@ int cgo_init(cgo_sim** out, int L, double W, double xi, double T, double E,
     return CGO_OK;
 }
 
+int cgo_init(cgo_sim** out, int L, double W, double xi, double T, double E,
+             uint64_t seed, uint32_t M)
+{
+    return init_lattice(out, 2, L, W, xi, T, E, seed, M);
+}
+
+/* The cubic lattice the paper names as the natural extension (PAPER.md:118
+ * "significantly more advantageous in 3D than in 2D", "easily
+ * extended to higher dimensions"): N = L^3, same Hamiltonian, rates and
+ * algorithm, field along x (reading G22). */
+int cgo_init3(cgo_sim** out, int L, double W, double xi, double T, double E,
+              uint64_t seed, uint32_t M)
+{
+    return init_lattice(out, 3, L, W, xi, T, E, seed, M);
+}
+
 void cgo_free(cgo_sim* s)
 {
     if (!s) return;
     free(s->phi); free(s->eps); free(s->n); free(s->invr);
-    free(s->ddy); free(s->ddx); free(s->invr_k); free(s->cdf);
+    free(s->ddz); free(s->ddy); free(s->ddx); free(s->invr_k); free(s->cdf);
     free(s->log_a); free(s->log_i); free(s->log_j);
     free(s);
 }
@@ -307,10 +351,11 @@ static void decode_attempt(const cgo_sim* s, uint64_t a, uint32_t* i, uint32_t* 
     int64_t kk = 0;
     while (!(*u_d < s->cdf[kk])) ++kk;          /* tower sampling [7]: smallest k with u < cdf_k */
     *k = kk;
-    int L = s->L;
-    int yi = (int)(*i / (uint32_t)L), xi_ = (int)(*i % (uint32_t)L);
-    int yj = wrap(yi + s->ddy[kk], L), xj = wrap(xi_ + s->ddx[kk], L);
-    *j = (uint32_t)yj * (uint32_t)L + (uint32_t)xj;
+    int L = s->L, Lz = s->Lz;
+    int zi, yi, xi_;
+    site_zyx(s, *i, &zi, &yi, &xi_);
+    int zj = wrap(zi + s->ddz[kk], Lz), yj = wrap(yi + s->ddy[kk], L), xj = wrap(xi_ + s->ddx[kk], L);
+    *j = ((uint32_t)zj * (uint32_t)L + (uint32_t)yj) * (uint32_t)L + (uint32_t)xj;
 }
 
 int cgo_decode_attempt(const cgo_sim* s, uint64_t a, uint32_t* i, uint32_t* j, int64_t* k,
@@ -362,22 +407,24 @@ static double now_seconds(void)
  * +1/r_ij at l=i and -1/r_ij at l=j as the paper lists (reading G1). */
 static void execute_hop(cgo_sim* s, uint32_t i, uint32_t j)
 {
-    int L = s->L;
+    int L = s->L, Lz = s->Lz;
     s->n[i] = 0;
     s->n[j] = 1;
-    int yi = (int)(i / (uint32_t)L), xi_ = (int)(i % (uint32_t)L);
-    int yj = (int)(j / (uint32_t)L), xj = (int)(j % (uint32_t)L);
+    int zi, yi, xi_, zj, yj, xj;
+    site_zyx(s, i, &zi, &yi, &xi_);
+    site_zyx(s, j, &zj, &yj, &xj);
     s->dP += (int64_t)min_image(xj - xi_, L);
     double t0 = now_seconds();
-    for (int y = 0; y < L; ++y) {
-        const double* row_j = s->invr + (size_t)wrap(y - yj, L) * (size_t)L;
-        const double* row_i = s->invr + (size_t)wrap(y - yi, L) * (size_t)L;
-        double* e = s->eps + (size_t)y * (size_t)L;
-        for (int x = 0; x < L; ++x) {
-            double d = row_j[wrap(x - xj, L)] - row_i[wrap(x - xi_, L)];
-            e[x] = e[x] + d;
+    for (int z = 0; z < Lz; ++z)
+        for (int y = 0; y < L; ++y) {
+            const double* row_j = s->invr + ((size_t)wrap(z - zj, Lz) * (size_t)L + (size_t)wrap(y - yj, L)) * (size_t)L;
+            const double* row_i = s->invr + ((size_t)wrap(z - zi, Lz) * (size_t)L + (size_t)wrap(y - yi, L)) * (size_t)L;
+            double* e = s->eps + ((size_t)z * (size_t)L + (size_t)y) * (size_t)L;
+            for (int x = 0; x < L; ++x) {
+                double d = row_j[wrap(x - xj, L)] - row_i[wrap(x - xi_, L)];
+                e[x] = e[x] + d;
+            }
         }
-    }
     s->update_seconds += now_seconds() - t0;
 }
 
@@ -557,6 +604,15 @@ int cgo_get_tables(const cgo_sim* s, int32_t* dy, int32_t* dx, double* cdf, doub
     if (Gamma) *Gamma = s->Gamma;
     return CGO_OK;
 }
+
+int cgo_get_dz(const cgo_sim* s, int32_t* dz)
+{
+    if (!s || !dz) return CGO_EINVAL;
+    memcpy(dz, s->ddz, sizeof(int32_t) * (size_t)s->K);
+    return CGO_OK;
+}
+
+int cgo_dimension(const cgo_sim* s) { return s ? (s->Lz == 1 ? 2 : 3) : 0; }
 
 int cgo_get_phi(const cgo_sim* s, double* phi)
 {

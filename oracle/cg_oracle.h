@@ -50,6 +50,11 @@ void cgo_pr_split(uint64_t m, uint32_t M, uint64_t* p, uint32_t* q);
  * Philox seed, logical PR width M (only enters the iteration bookkeeping). */
 int  cgo_init(cgo_sim** out, int L, double W, double xi, double T, double E,
               uint64_t seed, uint32_t M);
+/* Cubic 3D lattice, N = L^3, site s = (z L + y) L + x, field along x — the
+ * extension the paper names; everything else as cgo_init.
+ * Every other call works on either kind of sim (N is then L^3). */
+int  cgo_init3(cgo_sim** out, int L, double W, double xi, double T, double E,
+               uint64_t seed, uint32_t M);
 void cgo_free(cgo_sim* s);
 
 /* Advance exactly n_hops executed hops of the serial mixed algorithm. */
@@ -74,6 +79,8 @@ int  cgo_recompute_eps(const cgo_sim* s, double* eps_out /*N or NULL*/, double* 
 int64_t cgo_num_displacements(const cgo_sim* s);
 int  cgo_get_tables(const cgo_sim* s, int32_t* dy, int32_t* dx, double* cdf, double* invr_k,
                     double* S, double* Gamma);
+int  cgo_get_dz(const cgo_sim* s, int32_t* dz /* K; all 0 in 2D; list order is (r2, dz, dy, dx) */);
+int  cgo_dimension(const cgo_sim* s);   /* 2 or 3 */
 /* 1/r under minimum image between sites a and b (0 for a==b). */
 double cgo_invr_sites(const cgo_sim* s, uint32_t a, uint32_t b);
 

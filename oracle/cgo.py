@@ -42,6 +42,9 @@ def lib():
             "cgo_philox4x32_10": (None, [P(u32), P(u32), P(u32)]),
             "cgo_pr_split": (None, [u64, u32, P(u64), P(u32)]),
             "cgo_init": (C.c_int, [P(vp), C.c_int, dbl, dbl, dbl, dbl, u64, u32]),
+            "cgo_init3": (C.c_int, [P(vp), C.c_int, dbl, dbl, dbl, dbl, u64, u32]),
+            "cgo_get_dz": (C.c_int, [vp, vp]),
+            "cgo_dimension": (C.c_int, [vp]),
             "cgo_free": (None, [vp]),
             "cgo_run": (C.c_int, [vp, u64]),
             "cgo_get_state": (C.c_int, [vp, vp, vp, P(dbl), P(i64)]),
@@ -95,13 +98,14 @@ def _ptr(a):
 class Oracle:
     """cgo_init / cgo_run / cgo_get_state with the same shape as the CUDA binding."""
 
-    def __init__(self, L, W=1.0, xi=1.0, T=0.05, E=0.0, seed=1, M=1, hop_log=True):
+    def __init__(self, L, W=1.0, xi=1.0, T=0.05, E=0.0, seed=1, M=1, hop_log=True, dim=2):
         self._h = C.c_void_p()
-        rc = lib().cgo_init(C.byref(self._h), int(L), float(W), float(xi), float(T), float(E),
-                            int(seed), int(M))
+        assert dim in (2, 3)
+        init = lib().cgo_init if dim == 2 else lib().cgo_init3
+        rc = init(C.byref(self._h), int(L), float(W), float(xi), float(T), float(E), int(seed), int(M))
         if rc != 0:
-            raise ValueError("cgo_init failed with code %d" % rc)
-        self.L, self.N, self.M = int(L), int(L) * int(L), int(M)
+            raise ValueError("cgo_init%s failed with code %d" % ("" if dim == 2 else "3", rc))
+        self.L, self.N, self.M, self.dim = int(L), int(L) ** dim, int(M), dim
         if hop_log:
             lib().cgo_enable_hop_log(self._h, 1)
 
@@ -153,6 +157,7 @@ class Oracle:
 
     def tables(self):
         K = lib().cgo_num_displacements(self._h)
+        dz = np.empty(K, np.int32)
         dy = np.empty(K, np.int32)
         dx = np.empty(K, np.int32)
         cdf = np.empty(K, np.float64)
@@ -160,7 +165,9 @@ class Oracle:
         S, G = C.c_double(), C.c_double()
         self._check(lib().cgo_get_tables(self._h, _ptr(dy), _ptr(dx), _ptr(cdf), _ptr(invr),
                                          C.byref(S), C.byref(G)))
-        return {"K": K, "dy": dy, "dx": dx, "cdf": cdf, "invr_k": invr, "S": S.value, "Gamma": G.value}
+        self._check(lib().cgo_get_dz(self._h, _ptr(dz)))
+        return {"K": K, "dz": dz, "dy": dy, "dx": dx, "cdf": cdf, "invr_k": invr, "S": S.value,
+                "Gamma": G.value}
 
     def invr_sites(self, a, b):
         return lib().cgo_invr_sites(self._h, int(a), int(b))

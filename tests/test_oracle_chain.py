@@ -177,3 +177,65 @@ def test_apply_hops_reproduces_run(oracle_lib):
     s = oracle_lib.Oracle(16, T=0.1, seed=1, M=8); s.apply_hops(i, j)
     assert np.array_equal(o.state()[0], s.state()[0]) and np.array_equal(o.state()[1], s.state()[1])
     assert o.state()[3] == s.state()[3]
+
+
+def test_near_tie_certificate_fires_inside_its_band_only(oracle_lib):
+    """O10 / reading G10: an attempt that reaches the Metropolis factor with |u_a - exp(-dH/T)| <=
+    2^-50 exp(-dH/T) must be counted, one a few times further away must not (a certificate with a
+    wrong scale would be a silent no-op).  dH of a fixed uphill attempt on the 4x4 lattice comes from
+    Eq.(1) by brute force; T is then tuned, ulp by ulp, so that exp(-dH/T) lands next to that
+    attempt's own u_a (T only enters through this one division)."""
+    L = 4
+    base = oracle_lib.Oracle(L, T=0.5, E=0.0, seed=4242, M=4)
+    n0, eps0, _, _ = base.state()
+    phi = base.phi()
+    inv = base.tables()["invr_k"]
+    H0 = hamiltonian(n0, phi, L)
+    found = None
+    for a in range(200000):                      # an attempt with theta_ij = 1, dH > 0 and a mid-range u_a
+        i, j, k, ud, ua = base.decode_attempt(a)
+        if n0[i] != 1 or n0[j] != 0 or not 0.05 < ua < 0.6:
+            continue
+        m = n0.copy(); m[i] = 0; m[j] = 1
+        if hamiltonian(m, phi, L) - H0 > 0.2:
+            found = (a, i, j, k, ua)
+            break
+    assert found
+    a, i, j, k, ua = found
+    dE = (eps0[j] - eps0[i]) - inv[k]            # the oracle's operands (O7), E = 0; pinned against Eq.(1) below
+    assert dE == pytest.approx(hamiltonian(m, phi, L) - H0, abs=1e-12)
+
+    def p_of(T):
+        return math.exp((-dE) / T)
+
+    T = -dE / math.log(ua)                       # exp(-dE/T) = u_a up to rounding; walk T to the nearest ulp
+    while p_of(T) < ua:
+        T = np.nextafter(T, np.inf)
+    while p_of(T) > ua:
+        T = np.nextafter(T, -np.inf)
+    cand = [np.nextafter(T, -np.inf), T, np.nextafter(T, np.inf), np.nextafter(np.nextafter(T, np.inf), np.inf)]
+    T_in = min(cand, key=lambda t: abs(p_of(t) - ua))
+    assert abs(p_of(T_in) - ua) <= 2.0 ** -52 * ua          # well inside the 2^-50 band
+    T_out = T_in
+    while abs(p_of(T_out) - ua) <= 2.0 ** -48 * ua:         # walk out of the band, but stay close
+        T_out = np.nextafter(T_out, np.inf)
+    assert 2.0 ** -48 * ua < abs(p_of(T_out) - ua) < 2.0 ** -44 * ua
+
+    def ties_at(T):
+        o = oracle_lib.Oracle(L, T=float(T), E=0.0, seed=4242, M=4)
+        o.set_state(n0, a)                       # the next attempt evaluated is a
+        o.run(1)
+        first = int(o.hops(0, 1)[0][0])
+        # count only what attempt a itself contributed: replay from a + 1 and subtract
+        rest = 0
+        if first != a:
+            o2 = oracle_lib.Oracle(L, T=float(T), E=0.0, seed=4242, M=4)
+            o2.set_state(n0, a + 1)
+            o2.run(1)
+            rest = o2.near_ties()
+        return o.near_ties() - rest, o.exp_evaluations()
+
+    inside, evals = ties_at(T_in)
+    assert evals >= 1 and inside == 1
+    outside, evals = ties_at(T_out)
+    assert evals >= 1 and outside == 0
