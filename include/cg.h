@@ -4,7 +4,8 @@
  * (arXiv 1407.5026; citations are lines of /root/reference/PAPER.md).
  *
  * What the library computes: the "mixed PR algorithm" of PAPER.md:71-78 on an
- * L x L periodic lattice at half filling —
+ * L x L periodic lattice at half filling (cg_init), or on the L x L x L cubic
+ * lattice the paper names as its natural extension (cg_init3) —
  *   1. M labelled proposals per iteration, each (i, j) drawn with probability
  *      Gamma^T_ij / Gamma, Gamma^T_ij = exp(-2 r_ij / xi)
  *   2. each accepted with probability theta_ij min[1, exp(-dH_ij/T)],
@@ -18,8 +19,8 @@
  * ("mathematically equivalent") and does not depend on M or on the
  * launch shape.  DESIGN.md lists every reading of the paper this relies on.
  *
- * Conventions: site s = y*L + x (row-major, x = field direction), sites, labels
- * and attempt indices 0-based.  All pointers are HOST pointers unless the name
+ * Conventions: site s = y*L + x (row-major, x = field direction; 3D: s = (z*L + y)*L + x),
+ * sites, labels and attempt indices 0-based.  All pointers are HOST pointers unless the name
  * starts with dev_.  All functions return CG_OK (0) or a negative CG_E* code;
  * none throws, aborts or prints.  A sim is not thread-safe; distinct sims are
  * independent.  There is no CPU fallback: without a CUDA device every compute
@@ -42,8 +43,16 @@ typedef struct cg_sim cg_sim; /* opaque; owned by the library, released by cg_fr
 #define CG_ENOMEM       (-2)  /* host or device allocation failed / workspace too small */
 #define CG_ECUDA        (-3)  /* a CUDA call failed; text kept for cg_last_error       */
 #define CG_EUNSUPPORTED (-4)  /* valid problem the sm_100a path does not cover:
-                                 L not a power of two, L > 1024, or a tower too
-                                 long for shared memory (very large xi)            */
+                                 L not a power of two, L > 1024 (3D: L > 64),
+                                 M > 2^27, or a live tower longer than 65535
+                                 displacements (very large xi)                     */
+#define CG_EDEVICE      (-5)  /* the device-side watchdog abandoned a launch: some
+                                 wait inside the persistent kernel took longer than
+                                 10 s (CG_WATCHDOG_MS in the environment of cg_init
+                                 overrides; 0 = never).  Reported by the next call
+                                 that synchronises; the state is undefined until
+                                 cg_set_state.  Never seen in a correct build: it
+                                 turns a would-be hang into an error              */
 
 /* Problem statement.  L: lattice side, N = L*L sites, a power
  * of two in [4, 1024]; W: full width of the uniform disorder, phi_i in [-W/2, W/2);
@@ -56,6 +65,14 @@ typedef struct cg_sim cg_sim; /* opaque; owned by the library, released by cg_fr
 int cg_init(cg_sim** out, int L, double W, double xi, double T, double E,
             uint64_t seed, uint32_t M);
 
+/* The same on the cubic lattice, N = L^3 sites, L a power of two in [4, 64]
+ * ("significantly more advantageous in 3D than in 2D", PAPER.md:122
+ * "easily extended to higher dimensions"): displacements (dz, dy, dx) with
+ * 0 < r <= L/2 in the order (r^2, dz, dy, dx), field along x.  Every other call
+ * takes either kind of sim. */
+int cg_init3(cg_sim** out, int L, double W, double xi, double T, double E,
+             uint64_t seed, uint32_t M);
+
 /* Same, for callers that own device memory (e.g. a torch uint8 tensor) and a
  * stream: dev_workspace must hold cg_workspace_bytes(L, M) bytes, be 256-byte
  * aligned and outlive the sim; cuda_stream is a cudaStream_t (NULL = default). */
@@ -63,9 +80,13 @@ size_t cg_workspace_bytes(int L, uint32_t M);
 int cg_init_ws(cg_sim** out, int L, double W, double xi, double T, double E,
                uint64_t seed, uint32_t M,
                void* dev_workspace, size_t bytes, void* cuda_stream);
+size_t cg_workspace_bytes3(int L, uint32_t M);
+int cg_init3_ws(cg_sim** out, int L, double W, double xi, double T, double E,
+                uint64_t seed, uint32_t M,
+                void* dev_workspace, size_t bytes, void* cuda_stream);
 
 /* Advance exactly n_accepted_hops executed hops (not iterations) of the chain.
- * One persistent cooperative kernel; asynchronous on the sim's stream.
+ * One persistent cooperative kernel per 2^30 hops; asynchronous on the sim's stream.
  * cg_run(a); cg_run(b) is the same chain as cg_run(a+b). */
 int cg_run(cg_sim* s, uint64_t n_accepted_hops);
 
@@ -74,8 +95,8 @@ int cg_run(cg_sim* s, uint64_t n_accepted_hops);
  * n_accepted_hops executed hops in ONE persistent launch, every sim on its own
  * CTAs side by side; each chain is exactly the one cg_run would produce.
  * sims[] is a host array of distinct sims that share device, stream and launch
- * shape (512 threads, same register tiling and label caching: true for sims of
- * equal L whose M fits their CTAs; see cg_get_launch / cg_set_launch); the sum of
+ * shape (544 threads, no clusters, same register tiling and label caching: true for
+ * sims of equal L whose M fits their CTAs; see cg_get_launch / cg_set_launch); the sum of
  * their CTA counts must fit on the device at once, else CG_EUNSUPPORTED.
  * Asynchronous on that stream; the array is not referenced after the call. */
 int cg_run_many(cg_sim* const* sims, int n_sims, uint64_t n_accepted_hops);
@@ -102,7 +123,9 @@ int cg_get_counters(cg_sim* s, uint64_t* attempts, uint64_t* proposals_evaluated
 /* Hop log: (attempt index, i, j) of executed hops.  cg_enable_hop_log reserves
  * room for `capacity` hops counted from the current hop; dev_buf (may be NULL:
  * the library allocates) must hold 16*capacity bytes.  cg_get_hops copies hops
- * [first, first+count) of the log (indices relative to the enabling point). */
+ * [first, first+count) of the log (indices relative to the enabling point);
+ * CG_EINVAL outside the logged range, and after cg_apply_hops (scripted hops are
+ * not logged) until the log is enabled again. */
 int cg_enable_hop_log(cg_sim* s, uint64_t capacity, void* dev_buf, size_t bytes);
 int cg_get_hops(cg_sim* s, uint64_t first, uint64_t count,
                 uint64_t* attempt, uint32_t* i, uint32_t* j);
@@ -141,8 +164,10 @@ int cg_recompute_eps(cg_sim* s, double* max_abs_dev);
 /* Step a6 alone: execute `count` scripted hops i[h] -> j[h] (occupations,
  * dP and the O(N) update of PAPER.md:77; no acceptance test, no time) in one
  * launch of the update kernel.  Used for parity of the update against the
- * oracle and for its bandwidth measurement.  ms (may be NULL) receives the
- * device time of the launch measured with CUDA events on the sim's stream. */
+ * oracle and for its bandwidth measurement.  Every hop must satisfy theta_ij
+ * (n_i = 1, n_j = 0) at its turn: otherwise CG_EINVAL and nothing is changed.
+ * ms (may be NULL) receives the device time of the launch measured with CUDA
+ * events on the sim's stream. */
 int cg_apply_hops(cg_sim* s, uint64_t count, const uint32_t* i, const uint32_t* j, float* ms);
 
 /* Diagnostics of the one-time set-up (step a0): translation-invariant tables
@@ -152,46 +177,43 @@ int cg_apply_hops(cg_sim* s, uint64_t count, const uint32_t* i, const uint32_t* 
 int cg_get_table_sizes(cg_sim* s, int64_t* K, int64_t* K_live);
 int cg_get_tables(cg_sim* s, int32_t* dy, int32_t* dx, double* cdf, double* invr_k, /* K_live each */
                   double* S, double* Gamma);
+int cg_get_table_dz(cg_sim* s, int32_t* dz /* K_live; all 0 on the 2D lattice */);
 int cg_get_phi(cg_sim* s, double* phi /* N */);
 
-/* Launch shape of the persistent kernel: n_ctas in [1, co-resident maximum],
- * threads in {256, 512, 1024}; 0 keeps the heuristic.  Results never depend on
- * it.  cg_get_launch reports the shape in use. */
+/* Launch shape of the persistent kernel: n_ctas in [1, co-resident maximum] (a multiple
+ * of the cluster size), threads in {256, 544, 608, 1024} = 32 x (5, 14, 16 or 29 worker
+ * warps + 3 service warps); 0 keeps the heuristic.  Results never depend on it.
+ * cg_get_launch reports the shape in use. */
 int cg_set_launch(cg_sim* s, int n_ctas, int threads);
 int cg_get_launch(cg_sim* s, int* n_ctas, int* threads, int* smem_bytes);
 
-/* SM clock cycles CTA 0 spent inside the persistent kernel, accumulated over cg_run calls
- * (*total).  The propose and update phases of a hop overlap, so there is no meaningful split
- * into the paper's W_R and W_U inside this kernel: *wait, *update and *propose
- * are returned as 0; use cg_apply_hops for the update alone and cg_set_trace for a breakdown.
- * reset != 0 zeroes the counter. */
+/* Tuning that never changes results.  snapshot_interval H in {1, 2, 4, 8} (default 4): the
+ * eps slabs, kept current in registers after every hop, are written through to memory
+ * every H hops (deferred update; PAPER.md:77, 106 W_U); cluster_size in {1, 2, 4, 8, 16}
+ * (default 1): CTAs per thread-block cluster, whose members post their results into each
+ * other's shared memory instead of through L2.  0 leaves a value as it is.  A new cluster
+ * size re-derives the launch shape (CG_EUNSUPPORTED if the device cannot co-schedule it). */
+int cg_set_tuning(cg_sim* s, int snapshot_interval, int cluster_size);
+int cg_get_tuning(cg_sim* s, int* snapshot_interval, int* cluster_size);
+
+/* The paper's split of the time per hop into rejection and update time (PAPER.md:106:
+ * "the sum of two main contributions: the rejection time W_R ... and the update time W_U"),
+ * measured inside the persistent kernel that runs, in SM clock cycles, accumulated over
+ * cg_run calls: *total = cycles CTA 0 spent in the kernel; the other three are SUMS over
+ * the *warps worker warps of CTA 0 of the cycles a warp spent (propose) consuming the
+ * previous outcome, testing its proposals and handing in its lowest accept, (update)
+ * updating its part of the eps slab, (wait) waiting for the outcome of the iteration.
+ * Per warp, propose + update + wait = total up to start-up; W_U per hop = update / warps /
+ * hops, W_R per hop = (propose + wait) / warps / hops.  reset != 0 zeroes the counters. */
 int cg_get_phase_cycles(cg_sim* s, uint64_t* total, uint64_t* wait, uint64_t* update,
-                        uint64_t* propose, int reset);
+                        uint64_t* propose, uint64_t* warps, int reset);
 
-/* Optional segment timers of the persistent kernel (diagnostic; needs a library built with
- * -DCG_TRACE, else CG_EUNSUPPORTED; NULL / 0 switches it off).  Every following cg_run adds, for
- * CTA b, to dev_buf[b*64 + c*16 + k] the SM cycles the CTA's control warp spent in segment k of
- * the iterations in which the CTA was at scan position 0 (c = 0: it holds the start of the window),
- * position 1 (c = 2), the last position (c = 3) or elsewhere (c = 1): 6 publication check,
- * 3 waiting for its workers, 10 CTA minimum and posting it, 4 scanning other CTAs' slots,
- * 5 what the workers wait for of the bookkeeping, 0 the rest of it; k = 15 counts iterations,
- * 8 passes of the publication check, 9 scans, 11-14, 1, 2 a histogram of the scan time
- * (< 500, 1000, 2000, 4000, 8000 cycles, more).
- * A library built with -DCG_TRACE_W instead keeps cheap clock64 sums in registers (no measurable
- * slow-down): dev_buf[(b*16 + w)*8 + k] for worker warp w of CTA b, k = 0 test phase, 1 warp minimum,
- * 2 first barrier, 3 slab update, 4 second barrier, 5 descriptor and labels, 6 iterations; and
- * dev_buf[32768 + b*16 + k] for the control warp, k = 6 publication check, 7 early look, 3 first
- * barrier, 10 CTA minimum and post, 4 scan, 5 before and 0 after the second barrier, 15 iterations,
- * 14 early looks that found the winner, 13 iterations at scan position 0.  (A barrier's wait shows
- * up in the segment AFTER it: the clock is read when the barrier instruction issues.)
- * dev_buf: zeroed device memory, 8-byte aligned, 8*64*1024 bytes; `iterations` must be non-zero. */
-int cg_set_trace(cg_sim* s, void* dev_buf, size_t bytes, uint32_t iterations);
-
-/* L2 roofline denominator: one kernel, all SMs,
- * 16-byte L1-bypassing read-modify-write over a resident buffer of `bytes`
- * repeated `reps` times inside the launch.  Returns GB/s counting
- * 2*bytes*reps (read + write) over the best of `trials` launches. */
-int cg_bench_l2_rmw(size_t bytes, int reps, int trials, double* gbps);
+/* L2 roofline probe: one kernel, `ctas_per_sm` CTAs of `threads`
+ * threads per SM, L1-bypassing accesses of vec_bytes (16 or 32) over a resident buffer of
+ * `bytes`, `reps` passes inside the launch; mode 0 read-modify-write, 1 read only, 2 write
+ * only.  Returns GB/s (mode 0 counts read + written bytes) of the best of `trials` launches. */
+int cg_bench_l2(size_t bytes, int reps, int trials, int mode, int ctas_per_sm, int threads,
+                int vec_bytes, double* gbps);
 
 void cg_free(cg_sim* s);
 const char* cg_strerror(int code);

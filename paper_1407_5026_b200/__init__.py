@@ -3,4 +3,4 @@
 The product is libcg.so (C ABI in include/cg.h, CUDA in csrc/cg.cu); this package is its thin
 ctypes binding.  See DESIGN.md.
 """
-from .binding import CgError, CoulombGlass, bench_l2_rmw, run_many, lib, EXPORTS  # noqa: F401
+from .binding import CgError, CoulombGlass, bench_l2, run_many, lib, EXPORTS  # noqa: F401

@@ -13,14 +13,16 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB_PATH = os.path.join(_HERE, "libcg.so")
 _lib = None
 
-CG_OK, CG_EINVAL, CG_ENOMEM, CG_ECUDA, CG_EUNSUPPORTED = 0, -1, -2, -3, -4
+CG_OK, CG_EINVAL, CG_ENOMEM, CG_ECUDA, CG_EUNSUPPORTED, CG_EDEVICE = 0, -1, -2, -3, -4, -5
 
 EXPORTS = [
-    "cg_init", "cg_workspace_bytes", "cg_init_ws", "cg_run", "cg_run_many", "cg_get_state", "cg_set_state",
+    "cg_init", "cg_workspace_bytes", "cg_init_ws", "cg_init3", "cg_workspace_bytes3", "cg_init3_ws",
+    "cg_run", "cg_run_many", "cg_get_state", "cg_set_state",
     "cg_get_time_stochastic", "cg_get_normals", "cg_get_dos", "cg_get_series", "cg_get_sigma0",
     "cg_get_counters", "cg_enable_hop_log", "cg_get_hops", "cg_recompute_eps", "cg_apply_hops",
-    "cg_get_table_sizes", "cg_get_tables", "cg_get_phi", "cg_set_launch", "cg_get_launch",
-    "cg_get_phase_cycles", "cg_set_trace", "cg_bench_l2_rmw", "cg_free", "cg_strerror", "cg_last_error",
+    "cg_get_table_sizes", "cg_get_tables", "cg_get_table_dz", "cg_get_phi", "cg_set_launch", "cg_get_launch",
+    "cg_set_tuning", "cg_get_tuning", "cg_get_phase_cycles", "cg_bench_l2", "cg_free", "cg_strerror",
+    "cg_last_error",
 ]
 
 
@@ -46,6 +48,9 @@ def lib():
         "cg_init": (ci, [P(vp), ci, dbl, dbl, dbl, dbl, u64, u32]),
         "cg_workspace_bytes": (sz, [ci, u32]),
         "cg_init_ws": (ci, [P(vp), ci, dbl, dbl, dbl, dbl, u64, u32, vp, sz, vp]),
+        "cg_init3": (ci, [P(vp), ci, dbl, dbl, dbl, dbl, u64, u32]),
+        "cg_workspace_bytes3": (sz, [ci, u32]),
+        "cg_init3_ws": (ci, [P(vp), ci, dbl, dbl, dbl, dbl, u64, u32, vp, sz, vp]),
         "cg_run": (ci, [vp, u64]),
         "cg_run_many": (ci, [P(vp), ci, u64]),
         "cg_get_state": (ci, [vp, vp, vp, P(dbl), P(i64)]),
@@ -62,12 +67,14 @@ def lib():
         "cg_apply_hops": (ci, [vp, u64, vp, vp, P(C.c_float)]),
         "cg_get_table_sizes": (ci, [vp, P(i64), P(i64)]),
         "cg_get_tables": (ci, [vp, vp, vp, vp, vp, P(dbl), P(dbl)]),
+        "cg_get_table_dz": (ci, [vp, vp]),
         "cg_get_phi": (ci, [vp, vp]),
         "cg_set_launch": (ci, [vp, ci, ci]),
         "cg_get_launch": (ci, [vp, P(ci), P(ci), P(ci)]),
-        "cg_get_phase_cycles": (ci, [vp, P(u64), P(u64), P(u64), P(u64), ci]),
-        "cg_set_trace": (ci, [vp, vp, sz, u32]),
-        "cg_bench_l2_rmw": (ci, [sz, ci, ci, P(dbl)]),
+        "cg_set_tuning": (ci, [vp, ci, ci]),
+        "cg_get_tuning": (ci, [vp, P(ci), P(ci)]),
+        "cg_get_phase_cycles": (ci, [vp, P(u64), P(u64), P(u64), P(u64), P(u64), ci]),
+        "cg_bench_l2": (ci, [sz, ci, ci, ci, ci, ci, ci, P(dbl)]),
         "cg_free": (None, [vp]),
         "cg_strerror": (C.c_char_p, [ci]),
         "cg_last_error": (C.c_char_p, [vp]),
@@ -83,10 +90,14 @@ def _ptr(a):
     return a.ctypes.data_as(C.c_void_p)
 
 
-def bench_l2_rmw(nbytes, reps=1000, trials=10):
-    """cg_bench_l2_rmw: GB/s of an L1-bypassing 16-byte read-modify-write over a resident buffer."""
+L2_MODES = {"rmw": 0, "read": 1, "write": 2}
+
+
+def bench_l2(nbytes, reps=1000, trials=10, mode="rmw", ctas_per_sm=2, threads=512, vec_bytes=16):
+    """cg_bench_l2: GB/s of L1-bypassing accesses over a resident buffer (read-modify-write counts both ways)."""
     out = C.c_double()
-    rc = lib().cg_bench_l2_rmw(int(nbytes), int(reps), int(trials), C.byref(out))
+    rc = lib().cg_bench_l2(int(nbytes), int(reps), int(trials), L2_MODES[mode], int(ctas_per_sm), int(threads),
+                           int(vec_bytes), C.byref(out))
     if rc != 0:
         raise CgError(rc, lib().cg_strerror(rc).decode())
     return out.value
@@ -107,24 +118,27 @@ class CoulombGlass:
     """cg_init / cg_run / cg_get_state on cuda:`device`."""
 
     def __init__(self, L, W=1.0, xi=1.0, T=0.05, E=0.0, seed=1, M=1024, hop_log=0, device=0,
-                 stream=None):
+                 stream=None, dim=2):
         import torch  # device memory and streams only
         if not torch.cuda.is_available():
             raise RuntimeError("paper_1407_5026_b200 needs a CUDA device (no CPU fallback)")
         self._lib = lib()
         self._torch = torch
         self.device = torch.device("cuda", device)
-        self.L, self.N, self.M = int(L), int(L) * int(L), int(M)
+        if dim not in (2, 3):
+            raise ValueError("dim must be 2 (cg_init) or 3 (cg_init3)")
+        self.L, self.N, self.M, self.dim = int(L), int(L) ** dim, int(M), dim
         self._h = C.c_void_p()
+        ws_bytes = self._lib.cg_workspace_bytes if dim == 2 else self._lib.cg_workspace_bytes3
+        init_ws = self._lib.cg_init_ws if dim == 2 else self._lib.cg_init3_ws
         with torch.cuda.device(self.device):
-            nbytes = self._lib.cg_workspace_bytes(self.L, self.M)
+            nbytes = ws_bytes(self.L, self.M)
             self._stream = stream if stream is not None else torch.cuda.current_stream(self.device)
             # +256 so the base can be rounded up to the 256-byte alignment cg_init_ws asks for
             self._ws = torch.empty(max(nbytes, 1) + 256, dtype=torch.uint8, device=self.device)
             base = (self._ws.data_ptr() + 255) & ~255
-            rc = self._lib.cg_init_ws(C.byref(self._h), self.L, float(W), float(xi), float(T), float(E),
-                                      int(seed), self.M, C.c_void_p(base), nbytes,
-                                      C.c_void_p(self._stream.cuda_stream))
+            rc = init_ws(C.byref(self._h), self.L, float(W), float(xi), float(T), float(E),
+                         int(seed), self.M, C.c_void_p(base), nbytes, C.c_void_p(self._stream.cuda_stream))
         if rc != 0:
             self._h = C.c_void_p()
             raise CgError(rc, self._lib.cg_strerror(rc).decode())
@@ -149,7 +163,7 @@ class CoulombGlass:
     def _check(self, rc):
         if rc != 0:
             text = self._lib.cg_strerror(rc).decode()
-            if rc == CG_ECUDA:
+            if rc in (CG_ECUDA, CG_EDEVICE):
                 text += ": " + self._lib.cg_last_error(self._h).decode()
             raise CgError(rc, text)
 
@@ -191,7 +205,8 @@ class CoulombGlass:
         capacity = int(capacity)
         self._log = torch.empty(16 * capacity + 8, dtype=torch.uint8, device=self.device) if capacity else None
         ptr = (self._log.data_ptr() + 7) & ~7 if capacity else 0
-        self._check(self._lib.cg_enable_hop_log(self._h, capacity, C.c_void_p(ptr), 16 * capacity))
+        with torch.cuda.device(self.device):
+            self._check(self._lib.cg_enable_hop_log(self._h, capacity, C.c_void_p(ptr), 16 * capacity))
         self._log_cap, self._log_base = capacity, self.counters()["hops"]
 
     def hops(self, first=0, count=None):
@@ -246,7 +261,8 @@ class CoulombGlass:
 
     def recompute_eps(self):
         dev = C.c_double()
-        self._check(self._lib.cg_recompute_eps(self._h, C.byref(dev)))
+        with self._torch.cuda.device(self.device):
+            self._check(self._lib.cg_recompute_eps(self._h, C.byref(dev)))
         return dev.value
 
     def apply_hops(self, i, j):
@@ -268,7 +284,9 @@ class CoulombGlass:
         S, G = C.c_double(), C.c_double()
         self._check(self._lib.cg_get_tables(self._h, _ptr(dy), _ptr(dx), _ptr(cdf), _ptr(invr),
                                             C.byref(S), C.byref(G)))
-        return {"K": K.value, "K_live": n, "dy": dy, "dx": dx, "cdf": cdf, "invr_k": invr,
+        dz = np.empty(n, np.int32)
+        self._check(self._lib.cg_get_table_dz(self._h, _ptr(dz)))
+        return {"K": K.value, "K_live": n, "dz": dz, "dy": dy, "dx": dx, "cdf": cdf, "invr_k": invr,
                 "S": S.value, "Gamma": G.value}
 
     def phi(self):
@@ -285,25 +303,19 @@ class CoulombGlass:
         self._check(self._lib.cg_get_launch(self._h, C.byref(a), C.byref(b), C.byref(c)))
         return {"n_ctas": a.value, "threads": b.value, "smem_bytes": c.value}
 
-    def set_trace(self, on=True):
-        """Segment timers of the persistent kernel (library built with -DCG_TRACE); see cg_set_trace."""
-        torch = self._torch
-        if not on:
-            self._check(self._lib.cg_set_trace(self._h, None, 0, 0))
-            self._trace = None
-            return
-        self._trace = torch.zeros(64 * 1024, dtype=torch.int64, device=self.device)
-        self._check(self._lib.cg_set_trace(self._h, C.c_void_p(self._trace.data_ptr()),
-                                           self._trace.numel() * 8, 1))
+    def set_tuning(self, snapshot_interval=0, cluster_size=0):
+        """cg_set_tuning: eps write-through every H hops, CTAs per thread-block cluster (0: unchanged)."""
+        with self._torch.cuda.device(self.device):
+            self._check(self._lib.cg_set_tuning(self._h, int(snapshot_interval), int(cluster_size)))
 
-    def trace(self):
-        """-> int64 array [n_ctas, 4, 16] of SM cycles (see cg_set_trace in include/cg.h)."""
-        self._torch.cuda.synchronize(self.device)
-        n = self.launch()["n_ctas"]
-        return self._trace.view(1024, 4, 16)[:n].cpu().numpy()
+    def tuning(self):
+        a, b = C.c_int(), C.c_int()
+        self._check(self._lib.cg_get_tuning(self._h, C.byref(a), C.byref(b)))
+        return {"snapshot_interval": a.value, "cluster_size": b.value}
 
     def phase_cycles(self, reset=False):
-        t, w, u, p = C.c_uint64(), C.c_uint64(), C.c_uint64(), C.c_uint64()
+        """cg_get_phase_cycles: W_R / W_U of PAPER.md:106 from the persistent kernel itself (SM cycles)."""
+        t, w, u, p, n = C.c_uint64(), C.c_uint64(), C.c_uint64(), C.c_uint64(), C.c_uint64()
         self._check(self._lib.cg_get_phase_cycles(self._h, C.byref(t), C.byref(w), C.byref(u), C.byref(p),
-                                                  1 if reset else 0))
-        return {"total": t.value, "wait": w.value, "update": u.value, "propose": p.value}
+                                                  C.byref(n), 1 if reset else 0))
+        return {"total": t.value, "wait": w.value, "update": u.value, "propose": p.value, "warps": n.value}

@@ -30,8 +30,7 @@ def build(force=False, verbose=False):
                                             os.path.getmtime(__file__)))
     if force or stale:
         tmp = LIB + ".tmp.%d" % os.getpid()
-        extra = os.environ.get("CG_NVCC_EXTRA", "").split()      # experiments only (-D switches)
-        cmd = [nvcc(), *NVCC_FLAGS, *extra, "-I", os.path.join(ROOT, "include"), "-o", tmp, SRC]
+        cmd = [nvcc(), *NVCC_FLAGS, "-I", os.path.join(ROOT, "include"), "-o", tmp, SRC]
         if verbose:
             cmd.insert(1, "-Xptxas=-v")
             print(" ".join(cmd))

@@ -1,25 +1,32 @@
-// cg.cu — libcg.so: parallel-rejection kinetic Monte Carlo of the 2D Coulomb glass
+// cg.cu — libcg.so: parallel-rejection kinetic Monte Carlo of the Coulomb glass
 // (Ferrero, Kolton, Palassini, arXiv 1407.5026) for NVIDIA B200 (sm_100a).
 //
 // The ABI is declared and documented in include/cg.h.  DESIGN.md explains the
 // kernel design; the short version:
 //   * one persistent cooperative kernel runs the whole propose -> select ->
-//     apply -> update loop, one CTA per SM; in each CTA 14 worker
-//     warps test proposals and update eps, a control warp does the exchange and the
-//     bookkeeping, a service warp publishes finished slab updates;
-//   * the grid exchange is one-way most of the time: slots are scanned in label
-//     order and the scan stops at the first accepting CTA, so the CTA that holds
-//     the start of the window never waits for the others;
+//     apply -> update loop, one CTA per SM, as a DATAFLOW between
+//     warps instead of CTA-wide barriers: worker warps test proposals and update
+//     their eps slab, a collector warp reduces the workers' results in label order
+//     (stopping at the first accept), an exchange warp decides the iteration from
+//     the CTAs' posts and publishes its outcome in a small ring of descriptors
+//     (mbarrier full/empty pairs), a service warp publishes finished eps snapshots;
+//     a worker may lag the exchange warp by up to CG_XR - 1 iterations, so only the
+//     warps that hold the lowest labels sit on the critical path;
+//   * the grid exchange is one-way most of the time: posts are scanned in label
+//     order and the scan stops at the first accepting CTA; CTAs of one thread-block
+//     cluster post into each other's shared memory (DSMEM), the others through L2;
 //   * every thread owns the attempts a = g (mod P), keeps its proposal decoded and,
 //     while theta_ij = 1, follows the two local energies it needs in registers by
 //     adding every executed hop's term itself (the same rounded adds as the update);
 //   * each CTA keeps its eps slab in registers and writes it through to a ring of
-//     buffers; readers only touch a buffer that every CTA has published and add the
-//     terms of the (at most CG_DEPTH) newer hops in hop order, so no reader ever
-//     waits for a writer and every value is bit-identical to the serial algorithm;
-//   * occupations live as a bitmap in every CTA's shared memory, next to the live
-//     part of the tower and its guide table; 1/r comes from an
-//     unfolded table in L2 indexed with one subtraction and one mask.
+//     snapshot buffers every H hops (deferred update); readers only
+//     touch a snapshot that every CTA has published and add the terms of the newer
+//     hops in hop order, so no reader ever waits for a writer and every value is
+//     bit-identical to the serial algorithm;
+//   * occupations live as a bitmap in every CTA's shared memory (updated lazily,
+//     readers replay the newest hops), next to the head of the tower (PAPER.md:71,
+//     80) and its guide table; 1/r comes from an unfolded table in L2 indexed with
+//     one subtraction and one mask (2D and 3D lattices share the code).
 // Nothing in this file is shared with oracle/ (the CPU reference).
 #include "cg.h"
 
@@ -28,6 +35,7 @@
 #include <algorithm>
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <string>
@@ -42,14 +50,23 @@ typedef unsigned int u32;
 
 // ------------------------------------------------------------------ device --
 
-#ifndef CG_DEPTH
-#define CG_DEPTH 4          // pending hops: proposals read eps_{h-DEPTH} and add the newer hops' terms themselves
+#ifndef CG_XR
+#define CG_XR 4             // descriptor ring: the exchange warp may be this many iterations ahead of the slowest consumer
 #endif
-#define CG_RING (2 * CG_DEPTH + 1)   // eps buffers: eps_{h+1-2 DEPTH} .. eps_{h+1} can be live at the same time
-#define CG_SRING 16         // exchange slots per CTA: a CTA posts up to DEPTH exchanges ahead of the slowest reader
-#define CG_PUB_U64 32       // offset of a CTA's publication word in its slot block (u64 units)
-#define CG_SLOT_U64 64      // one block per CTA, 512-byte stride: the slot ring in the first half, the pub word after it
+#define CG_PB 8             // publication barriers (snapshots a CTA's workers may be ahead of its service warp)
+#define CG_HR 32            // hop ring: coded sites of the last CG_HR executed hops, for readers that catch up
+#define CG_RING 12          // eps snapshot buffers (see "snapshots" in pr_persistent_body)
+#define CG_SRING 32         // exchange slots per CTA (a CTA's posts may be this many iterations ahead of their slowest reader)
+#define CG_SLOT_U64 128     // one 1 KiB block per CTA: the slot ring in the first half, the publication word after it
+#define CG_PUB_U64 64
 #define CG_GUIDE 352        // tower guide: (43 + 1) binades x 8 sub-buckets of t = 2^43 - m
+#define CG_KS 2048          // head of the tower kept in shared memory (the rest, hardly ever drawn, stays in L2)
+#define CG_MAX_CLUSTER 16
+#define CG_MAX_SNAP 8       // largest snapshot interval H
+
+#define CG_F_HOP 1u         // descriptor flags: the iteration executed a hop
+#define CG_F_LAST 2u        //   ... and it was the last one of this launch
+#define CG_F_ABORT 4u       //   watchdog: give up
 
 struct CgCtl {              // device-resident control block (one per sim)
     u64 attempts;           // attempts consumed = next unused attempt index
@@ -61,36 +78,42 @@ struct CgCtl {              // device-resident control block (one per sim)
     u32 bad_hops;           // scripted hops that violated theta_ij
     u64 epoch;              // next exchange epoch; never reset, so stale slots can never match
     u64 log_base;           // hop count at which the hop log was enabled
-    u64 cyc_total, cyc_wait, cyc_update, cyc_propose;
-    u64 pub_base;           // publication sequence number of the last hop of the previous launch: CTA c
-                            // stores pub_base + h into its pub word once its slab of hop h of a launch is
+    u64 cyc_total, cyc_wait, cyc_update, cyc_propose;   // phase timers of CTA 0 (cg_get_phase_cycles)
+    u64 pub_base;           // publication sequence number at the start of the next launch: CTA c stores
+                            // pub_base + s into its pub word once its slab of snapshot s of a launch is
                             // written (never reset, so stale words of other launch shapes are always smaller)
     u64 log_a0;             // attempts consumed when the hop log was enabled (observables: m of the first logged hop)
-    u64 pub_pad[2];
+    u32 abort;              // != 0: the watchdog of the persistent kernel fired (which wait: see cg.h)
+    u32 pad;
+    u64 cyc_warps;          // worker warps that contributed to cyc_wait/update/propose
 };
 
 struct CgParams {           // kernel parameter block
-    double* eps[CG_RING];   // ring of local-energy buffers, N each (see "pending hops" below)
-    const double* tf;       // unfolded table 1/r, L rows of pitch 2L (see site_code)
-    const double* tq;       // quarter table 1/r, (L/2+1) x (L/2+1), indexed by the folded offsets
+    double* eps[CG_RING];   // ring of local-energy snapshot buffers, N each
+    double* work;           // RP == 0 only: the CTAs' private working copy of eps
+    const double* tf;       // unfolded table 1/r (see site_code)
+    const double* tq;       // folded table 1/r, (Lz/2+1) x (L/2+1) x (L/2+1)
     u32* nbits;             // occupations, bit s of word s/32
     const u64* cdfi;        // live tower as integer thresholds: u_d < cdf_k  <=>  m < cdfi_k
     const double* invr_k;   // 1/r of displacement k (live part)
     const double* fld_k;    // E * dx of displacement k
-    const int* disp;        // (dy << 16) | (dx & 0xffff)
+    const u32* disp;        // coded displacement: site_code of ((dz mod L), (dy mod L), (dx mod L))
     const u32* guide;       // tower guide: klo | khi << 16 per bucket
     u64* slots;             // exchange slots, CG_SLOT_U64 per CTA
     CgCtl* ctl;
     u64* log_a; u32* log_i; u32* log_j; u64 log_cap;
-    int L, lgL, pitch, Klive;
+    int L, lgL, Klive, Ksm; // Ksm = min(Klive, CG_KS) tower entries in shared memory
+    u32 hi1, hi2, spare, mask;   // site coding (site_code)
     u32 N, M;
     u32 PL;                 // CACHED: threads per CTA that own attempts
     u32 seed_lo, seed_hi;
     double T, E;
     float inv_T;            // (float)(1/T), pre-test of the Metropolis factor only
-    u64 n_hops;
-    u64* trace;             // optional segment timers (cg_set_trace), 64 words per CTA
-    u32 trace_iters;
+    u32 n_hops;             // hops of this launch (cg_run splits longer runs)
+    u32 snap_shift;         // snapshots every H = 1 << snap_shift hops
+    u32 gate;               // G: hop h waits until every CTA has published the snapshot that covers hop h - G
+    u32 cluster;            // CTAs per thread-block cluster (1: none)
+    u64 watchdog_ns;        // a wait longer than this aborts the launch (0: never)
 };
 
 // Philox4x32-10 (Salmon et al., SC'11): counter (c0..c3), key (k0,k1).
@@ -110,6 +133,7 @@ __device__ __forceinline__ void philox4x32_10(u32 c0, u32 c1, u32 c2, u32 c3, u3
 
 __device__ __forceinline__ double ld_cg(const double* p) { return __ldcg(p); }
 
+// ---- global memory: exchange slots and publication words ------------------------------
 __device__ __forceinline__ void slot_store(u64* p, u64 a, u64 b)
 {
     asm volatile("st.relaxed.gpu.global.v2.u64 [%0], {%1, %2};" ::"l"(p), "l"(a), "l"(b) : "memory");
@@ -124,6 +148,12 @@ __device__ __forceinline__ u64 ld_relaxed_u64(const u64* p)
     asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
     return v;
 }
+__device__ __forceinline__ u32 ld_relaxed_u32(const u32* p)
+{
+    u32 v;
+    asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
 __device__ __forceinline__ void st_release_u64(u64* p, u64 v)
 {
     asm volatile("st.release.gpu.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
@@ -135,35 +165,110 @@ __device__ __forceinline__ u64 global_ns()
     return t;
 }
 __device__ __forceinline__ void fence_acquire_gpu() { asm volatile("fence.acquire.gpu;" ::: "memory"); }
-// named barriers 1 .. CG_DEPTH (cyclic in the hop number): the warps that wrote eps arrive, the
-// service warp waits for them; barrier 0 with an explicit count synchronises the worker warps only
-#define CG_BARN(OP) switch (k) { \
-        case 0: asm volatile(OP " 1, %0;" ::"r"(n) : "memory"); break; \
-        case 1: asm volatile(OP " 2, %0;" ::"r"(n) : "memory"); break; \
-        case 2: asm volatile(OP " 3, %0;" ::"r"(n) : "memory"); break; \
-        case 3: asm volatile(OP " 4, %0;" ::"r"(n) : "memory"); break; \
-        case 4: asm volatile(OP " 6, %0;" ::"r"(n) : "memory"); break; \
-        case 5: asm volatile(OP " 7, %0;" ::"r"(n) : "memory"); break; \
-        case 6: asm volatile(OP " 8, %0;" ::"r"(n) : "memory"); break; \
-        default: asm volatile(OP " 9, %0;" ::"r"(n) : "memory"); break; }
-__device__ __forceinline__ void barN_arrive(u32 k, int n) { CG_BARN("bar.arrive") }   // k < CG_DEPTH <= 8
-__device__ __forceinline__ void barN_sync(u32 k, int n) { CG_BARN("bar.sync") }
-__device__ __forceinline__ void barX_sync(int n) { asm volatile("bar.sync 0, %0;" ::"r"(n) : "memory"); }
-__device__ __forceinline__ void barX_arrive(int n) { asm volatile("bar.arrive 0, %0;" ::"r"(n) : "memory"); }
-// barrier 5: second CTA barrier of an iteration; the control warp only arrives
-__device__ __forceinline__ void barB_sync(int n) { asm volatile("bar.sync 5, %0;" ::"r"(n) : "memory"); }
-__device__ __forceinline__ void barB_arrive(int n) { asm volatile("bar.arrive 5, %0;" ::"r"(n) : "memory"); }
 
-// ---- the unfolded 1/r table ------------------------------------------------------------
-// tf[dy * 2L + dx] = 1/r of the offset (dy, dx) under minimum image, dy in [0, L),
-// dx in [0, L] (dx = L repeats dx = 0, so the pair (dx, dx+1) never wraps); 0 at the origin.
-// A site s = y L + x is coded as c(s) = y 2L + x; with bit L (the spare bit between the fields) set
-// in the minuend, ONE subtraction and ONE mask give both periodic differences:
-//   ((c(s) | L) - c(t)) & mask  =  ((y_s - y_t) mod L) 2L + ((x_s - x_t) mod L).
-__device__ __forceinline__ u32 site_code(u32 s, int L) { return s + (s & ~(u32)(L - 1)); }
+// ---- shared memory: 16-byte records, mbarriers, cluster (DSMEM) -----------------------
+__device__ __forceinline__ u32 smem_u32(const void* p) { return (u32)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void lds128(const void* p, u64& a, u64& b)
+{
+    asm volatile("ld.volatile.shared.v2.u64 {%0, %1}, [%2];" : "=l"(a), "=l"(b) : "r"(smem_u32(p)) : "memory");
+}
+__device__ __forceinline__ void sts128(void* p, u64 a, u64 b)
+{
+    asm volatile("st.volatile.shared.v2.u64 [%0], {%1, %2};" ::"r"(smem_u32(p)), "l"(a), "l"(b) : "memory");
+}
+__device__ __forceinline__ uint4 lds128u(const void* p)
+{
+    uint4 v;
+    asm volatile("ld.volatile.shared.v4.u32 {%0, %1, %2, %3}, [%4];"
+                 : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(smem_u32(p)) : "memory");
+    return v;
+}
+__device__ __forceinline__ void sts128u(void* p, u32 x, u32 y, u32 z, u32 w)
+{
+    asm volatile("st.volatile.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(smem_u32(p)), "r"(x), "r"(y), "r"(z), "r"(w) : "memory");
+}
+__device__ __forceinline__ void sts64u(void* p, u32 x, u32 y)
+{
+    asm volatile("st.volatile.shared.v2.u32 [%0], {%1, %2};" ::"r"(smem_u32(p)), "r"(x), "r"(y) : "memory");
+}
+__device__ __forceinline__ uint2 lds64u(const void* p)
+{
+    uint2 v;
+    asm volatile("ld.volatile.shared.v2.u32 {%0, %1}, [%2];" : "=r"(v.x), "=r"(v.y) : "r"(smem_u32(p)) : "memory");
+    return v;
+}
+__device__ __forceinline__ u32 ld_acquire_cta(const u32* p)
+{
+    u32 v;
+    asm volatile("ld.acquire.cta.shared.u32 %0, [%1];" : "=r"(v) : "r"(smem_u32(p)) : "memory");
+    return v;
+}
+__device__ __forceinline__ void max_release_cta(u32* p, u32 v)
+{
+    asm volatile("red.release.cta.shared.max.u32 [%0], %1;" ::"r"(smem_u32(p)), "r"(v) : "memory");
+}
+__device__ __forceinline__ void mbar_init(u64* b, u32 count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(b)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(u64* b)
+{
+    asm volatile("mbarrier.arrive.release.cta.shared::cta.b64 _, [%0];" ::"r"(smem_u32(b)) : "memory");
+}
+__device__ __forceinline__ bool mbar_try(u64* b, u32 parity, u32 hint_ns)
+{
+    u32 ok;
+    asm volatile("{\n\t.reg .pred p;\n\t"
+                 "mbarrier.try_wait.parity.acquire.cta.shared::cta.b64 p, [%1], %2, %3;\n\t"
+                 "selp.b32 %0, 1, 0, p;\n\t}"
+                 : "=r"(ok) : "r"(smem_u32(b)), "r"(parity), "r"(hint_ns) : "memory");
+    return ok != 0;
+}
+__device__ __forceinline__ u32 cluster_ctarank()
+{
+    u32 r;
+    asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
+    return r;
+}
+__device__ __forceinline__ u32 mapa_cluster(u32 smem_addr, u32 rank)
+{
+    u32 r;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(smem_addr), "r"(rank));
+    return r;
+}
+__device__ __forceinline__ void st_cluster128(u32 cluster_addr, u64 a, u64 b)
+{
+    asm volatile("st.shared::cluster.v2.u64 [%0], {%1, %2};" ::"r"(cluster_addr), "l"(a), "l"(b) : "memory");
+}
+__device__ __forceinline__ void cluster_sync_all()
+{
+    asm volatile("barrier.cluster.arrive.release;\n\tbarrier.cluster.wait.acquire;" ::: "memory");
+}
+
+// ---- site coding and the unfolded 1/r table ---------------------------------------------
+// A site s = (z L + y) L + x (z = 0 in 2D) is coded as c(s) = (z 2L + y) 2L + x: one spare bit above
+// the x and the y field.  With the spare bits set in the minuend, ONE subtraction and ONE mask give
+// all periodic coordinate differences:
+//   ((c(s) | spare) - c(t)) & mask = (((z_s - z_t) mod L) 2L + ((y_s - y_t) mod L)) 2L + ((x_s - x_t) mod L),
+// which indexes tf[] = 1/r of that offset under minimum image, 0 at the origin; likewise
+// (c(s) + c(d)) & mask is the code of the site s displaced by d.
+struct Geo {
+    u32 hi1, hi2, spare, mask, Lm1; int lg;
+    __device__ __forceinline__ u32 code(u32 s) const { return s + (s & hi1) + ((s & hi2) << 1); }
+    __device__ __forceinline__ u32 site(u32 c) const
+    {
+        return (c & Lm1) | ((c >> 1) & (Lm1 << lg)) | ((c >> 2) & (Lm1 << (2 * lg)));
+    }
+    __device__ __forceinline__ int dx(u32 si, u32 sj) const     // minimum image along the field, tie -> +L/2 (G3)
+    {
+        const int L = (int)Lm1 + 1;
+        int d = ((int)(sj & Lm1) - (int)(si & Lm1)) & (int)Lm1;
+        return d > L / 2 ? d - L : d;
+    }
+};
 
 // Step 3b of the mixed PR algorithm: what hop i->j adds to eps at the site coded sc
-// (spare bit set): 1/r_lj - 1/r_li (difference first, then ONE add by the caller).
+// (spare bits set): 1/r_lj - 1/r_li (difference first, then ONE add by the caller).
 __device__ __forceinline__ double hop_term(const double* __restrict__ tf, u32 mask, u32 sc, u32 ci, u32 cj)
 {
     return __dsub_rn(__ldg(tf + ((sc - cj) & mask)), __ldg(tf + ((sc - ci) & mask)));
@@ -171,17 +276,17 @@ __device__ __forceinline__ double hop_term(const double* __restrict__ tf, u32 ma
 
 // eps slab of one CTA: sites [2 pr0, 2 pr1).  With RP > 0 warp w keeps the blocks of 64 consecutive
 // sites number w, w + TW/32, ... (RP of them) in registers across hops - lane l holds sites l and
-// 32 + l of a block, so that every load and store of the warp covers 256 contiguous bytes (the L1
-// wavefront rate, not L2 bandwidth, bounds this kernel) - and writes every new value through to global
-// memory for the other CTAs' gathers; with RP == 0 the slab streams src -> dst.
-// issue() starts the table gathers of a hop, finish() adds and stores: the caller puts independent
+// 32 + l of a block, so that every load and store of the warp covers 256 contiguous bytes - and writes
+// the values through to a snapshot buffer when asked to; with RP == 0 the slab lives in the CTA's part
+// of a private working buffer in global memory (L2).
+// issue() starts the table gathers of a hop, finish() adds (and stores): the caller puts independent
 // work between the two.
 template <int TW, int RP>
 struct Slab {
     static constexpr int R = RP > 0 ? RP : 1;
     double ea[R], eb[R];
     double ja[R], ia[R], jb[R], ib[R];
-    u32 sca[R], scb[R];                  // coded sites (spare bit set); 0 marks a site outside the slab
+    u32 sca[R], scb[R];                  // coded sites (spare bits set); 0 marks a site outside the slab
     u32 hci, hcj;
     u32 tix;                             // index of this thread among the TW threads that hold the slab
 
@@ -190,20 +295,24 @@ struct Slab {
         return 2u * (pr0 + (u32)k * TW + (tix & ~31u)) + (tix & 31u);
     }
 
-    __device__ __forceinline__ void load(const double* src, u32 pr0, u32 pr1, int L, u32 t)
+    __device__ __forceinline__ void load(const double* src, double* work, u32 pr0, u32 pr1, const Geo& g, u32 t)
     {
         tix = t;
+        if (RP > 0) {
 #pragma unroll
-        for (int k = 0; k < RP; ++k) {
-            const u32 sa = site_a(pr0, k), sb = sa + 32u;
-            sca[k] = sa < 2u * pr1 ? site_code(sa, L) | (u32)L : 0u;
-            scb[k] = sb < 2u * pr1 ? site_code(sb, L) | (u32)L : 0u;
-            if (sca[k]) ea[k] = __ldcg(src + sa);
-            if (scb[k]) eb[k] = __ldcg(src + sb);
+            for (int k = 0; k < RP; ++k) {
+                const u32 sa = site_a(pr0, k), sb = sa + 32u;
+                sca[k] = sa < 2u * pr1 ? g.code(sa) | g.spare : 0u;
+                scb[k] = sb < 2u * pr1 ? g.code(sb) | g.spare : 0u;
+                if (sca[k]) ea[k] = __ldcg(src + sa);
+                if (scb[k]) eb[k] = __ldcg(src + sb);
+            }
+        } else if (work != src) {
+            for (u32 s = 2u * pr0 + tix; s < 2u * pr1; s += TW) __stcg(work + s, __ldcg(src + s));
         }
     }
 
-    __device__ __forceinline__ void issue(const double* __restrict__ tf, u32 mask, u32 pr0, u32 pr1, u32 ci, u32 cj)
+    __device__ __forceinline__ void issue(const double* __restrict__ tf, u32 mask, u32 ci, u32 cj)
     {
         hci = ci; hcj = cj;
 #pragma unroll
@@ -213,35 +322,57 @@ struct Slab {
         }
     }
 
-    // dst = eps + (1/r_lj - 1/r_li) for every site l of the slab
-    __device__ __forceinline__ void finish(const double* __restrict__ tf, u32 mask, int L, const double* src,
-                                           double* dst, u32 pr0, u32 pr1)
+    // eps += 1/r_lj - 1/r_li for every site l of the slab; snap != nullptr: also stored there
+    __device__ __forceinline__ void finish(const double* __restrict__ tf, u32 mask, const Geo& g, double* work,
+                                           double* snap, u32 pr0, u32 pr1)
     {
         if (RP > 0) {
 #pragma unroll
             for (int k = 0; k < RP; ++k) {
                 const u32 sa = site_a(pr0, k);
-                if (sca[k]) { ea[k] = __dadd_rn(ea[k], __dsub_rn(ja[k], ia[k])); __stcg(dst + sa, ea[k]); }
-                if (scb[k]) { eb[k] = __dadd_rn(eb[k], __dsub_rn(jb[k], ib[k])); __stcg(dst + sa + 32u, eb[k]); }
+                if (sca[k]) { ea[k] = __dadd_rn(ea[k], __dsub_rn(ja[k], ia[k])); if (snap) __stcg(snap + sa, ea[k]); }
+                if (scb[k]) { eb[k] = __dadd_rn(eb[k], __dsub_rn(jb[k], ib[k])); if (snap) __stcg(snap + sa + 32u, eb[k]); }
             }
         } else {
             for (u32 s = 2u * pr0 + tix; s < 2u * pr1; s += TW) {
-                const u32 c = site_code(s, L) | (u32)L;
-                const double v = __ldcg(src + s);
+                const u32 c = g.code(s) | g.spare;
                 const double tj = __ldg(tf + ((c - hcj) & mask)), ti = __ldg(tf + ((c - hci) & mask));
-                __stcg(dst + s, __dadd_rn(v, __dsub_rn(tj, ti)));
+                const double v = __dadd_rn(__ldcg(work + s), __dsub_rn(tj, ti));
+                __stcg(work + s, v);
+                if (snap) __stcg(snap + s, v);
             }
+        }
+    }
+
+    // the slab as it stands, into a snapshot buffer (end of a launch)
+    __device__ __forceinline__ void flush(const double* work, double* snap, u32 pr0, u32 pr1) const
+    {
+        if (RP > 0) {
+#pragma unroll
+            for (int k = 0; k < RP; ++k) {
+                const u32 sa = site_a(pr0, k);
+                if (sca[k]) __stcg(snap + sa, ea[k]);
+                if (scb[k]) __stcg(snap + sa + 32u, eb[k]);
+            }
+        } else {
+            for (u32 s = 2u * pr0 + tix; s < 2u * pr1; s += TW) __stcg(snap + s, __ldcg(work + s));
         }
     }
 };
 
 struct Prop {               // one decoded attempt (a pure function of seed and attempt index)
-    u32 i, j, k;            // sites and tower index
+    u32 ci, cj, k;          // coded sites (no spare bits) and tower index
     u32 uh, ul;             // the 53 acceptance bits: u_a = (uh 2^32 + ul) 2^-53, uh < 2^21
 };
 
-struct Tables {             // shared-memory views
-    const u64* cdfi; const double* invr; const double* fld; const int* disp; const u32* guide;
+struct Tables {             // the tower: head in shared memory, the rest in global memory
+    const u64* cdfi; const double* invr; const double* fld; const u32* disp; const u32* guide;
+    const u64* g_cdfi; const double* g_invr; const double* g_fld; const u32* g_disp;
+    u32 ks;
+    __device__ __forceinline__ u64 cdf(u32 k) const { return k < ks ? cdfi[k] : __ldg(g_cdfi + k); }
+    __device__ __forceinline__ double inv(u32 k) const { return k < ks ? invr[k] : __ldg(g_invr + k); }
+    __device__ __forceinline__ double field(u32 k) const { return k < ks ? fld[k] : __ldg(g_fld + k); }
+    __device__ __forceinline__ u32 dcode(u32 k) const { return k < ks ? disp[k] : __ldg(g_disp + k); }
 };
 
 // Tower sampling: smallest k with u_d < cdf_k, u_d = m 2^-43, as the equivalent integer
@@ -256,29 +387,21 @@ __device__ __forceinline__ u32 tower_search(const Tables& t, u64 m)
     u32 lo = g & 0xFFFFu, hi = g >> 16;
     while (lo < hi) {
         const u32 mid = (lo + hi) >> 1;
-        if (m < t.cdfi[mid]) hi = mid; else lo = mid + 1;
+        if (m < t.cdf(mid)) hi = mid; else lo = mid + 1;
     }
     return lo;
 }
 
-__device__ __forceinline__ u32 hop_target(const Tables& t, u32 i, u32 k, int L, int lg)
-{
-    const int d = t.disp[k];
-    const int dy = d >> 16, dx = (int)(short)(d & 0xFFFF);
-    const int yj = ((int)(i >> lg) + dy) & (L - 1), xj = ((int)(i & (L - 1)) + dx) & (L - 1);
-    return ((u32)yj << lg) | (u32)xj;
-}
-
 // Attempt a -> proposal (reading G9): one Philox block, i = (w0 N) >> 32,
 // displacement from 43 bits, acceptance uniform from the remaining 53.
-__device__ __forceinline__ Prop decode_attempt(const Tables& t, const CgParams& p, u64 a)
+__device__ __forceinline__ Prop decode_attempt(const Tables& t, const CgParams& p, const Geo& g, u64 a)
 {
     u32 w0, w1, w2, w3;
     philox4x32_10((u32)a, (u32)(a >> 32), 0u, 0u, p.seed_lo, p.seed_hi, w0, w1, w2, w3);
     Prop r;
-    r.i = __umulhi(w0, p.N);
+    r.ci = g.code(__umulhi(w0, p.N));
     r.k = tower_search(t, ((u64)w1 << 11) | (u64)(w2 >> 21));
-    r.j = hop_target(t, r.i, r.k, p.L, p.lgL);
+    r.cj = (r.ci + t.dcode(r.k)) & g.mask;
     r.uh = w2 & 0x1FFFFFu; r.ul = w3;
     return r;
 }
@@ -301,108 +424,148 @@ __device__ __forceinline__ bool metropolis(double dE, u32 uh, u32 ul, double T, 
 
 #define BIT(sn, s) (((sn)[(s) >> 5] >> ((s) & 31)) & 1u)
 
-#ifdef CG_TRACE
-// segment timers of thread 0 (SM cycles), summed over the launch, separately for iterations in which
-// this CTA held the start of the window (class 0) or not (class 1): p.trace[b*32 + class*16 + segment]
-#define CLS_ (kb == 0 ? 0 : kb == 1 ? 32 : kb == nb - 1 ? 48 : 16)
-#define TRACE(ev, extra) do { if (lane == 0) { const long long now_ = clock64(); \
-    s_seg[CLS_ + (ev)] += (u64)(now_ - t_prev); t_prev = now_; } } while (0)
-#elif defined(CG_TRACE_W)
-#define TRACE(ev, extra) do { const long long now_ = clock64(); cw[ev] += (u64)(now_ - cprev); cprev = now_; } while (0)
-#else
-#define TRACE(ev, extra) do { } while (0)
-#endif
-#ifdef CG_TRACE_T
-// Time line: absolute SM clocks of 64 consecutive iterations (2000..2063 of a launch) of CTAs 0..31,
-// p.trace[((it - 2000) * 32 + b) * 32 + k]: k < 10 control warp (loop top, publication check done, early look
-// done, arrival at [A], CTA minimum, posted, scan done, before [B], arrived at [B], end), 10 scan position,
-// 11 attempts consumed; 16 + k worker warp 0 and 24 + k last worker warp (proposals known, tested, warp
-// minimum stored, [A] done, slab update done, [B] done, descriptor read, loop top).
-__device__ __forceinline__ u64 clk_now() { u64 t; asm volatile("mov.u64 %0, %%clock64;" : "=l"(t) :: "memory"); return t; }
-#define TS_CTL(k) do { if (lane == 0 && p.trace && b < 32u && it_local - 2000u < 64u) \
-    p.trace[((it_local - 2000u) * 32u + b) * 32u + (k)] = clk_now(); } while (0)
-#define TS_WRK(k) do { if (lane == 0 && (warp == 0 || warp == NWK - 1) && p.trace && b < 32u && itw - 2000u < 64u) \
-    p.trace[((itw - 2000u) * 32u + b) * 32u + 16u + (warp ? 8u : 0u) + (k)] = clk_now(); } while (0)
-#else
-#define TS_CTL(k) do { } while (0)
-#define TS_WRK(k) do { } while (0)
-#endif
-
-// What warp 0 tells the other warps of its CTA about an exchange (written before the second barrier).
-struct Desc {
+// What the exchange warp publishes about iteration e, in slot e % CG_XR of the descriptor ring.
+struct __align__(16) Desc {
     u32 used;               // attempts consumed: q + 1, or M when the whole window was rejected
-    u32 hop;                // 1: a hop was executed
-    u32 ci, cj;             // its coded sites (site_code)
-    u32 ahead;              // 1: another CTA holds the start of the next window (time to decode ahead)
-    u32 pad[3];
+    u32 flags;              // CG_F_*
+    u32 ci, cj;             // coded sites of the executed hop
+    u32 c_first, t0r;       // CTA at scan position 0 of the NEXT iteration and the offset of its first label
+    u32 hopno, pad;         // hops executed in this launch including this one
 };
-struct Pend {               // pending hops, for threads that start to follow a pair of sites
-    u32 npend, rbuf, first, pad;   // buffer rbuf + the npend hops c[(first + k) % CG_DEPTH], k = 0.. (oldest first)
-    u32 c[CG_DEPTH][2];     // coded sites (i, j) of the last CG_DEPTH executed hops, hop number h at (h - 1) % CG_DEPTH
+
+// The whole per-CTA communication area (static shared memory).
+struct __align__(16) Comm {
+    u64 full[CG_XR];        // mbarrier: descriptor e published (count 1)
+    u64 empty[CG_XR];       // mbarrier: descriptor e consumed by every worker warp and the collector
+    u64 pubbar[CG_PB];      // mbarrier: snapshot s stored by every worker warp
+    Desc desc[CG_XR];
+    u64 res[2 * CG_XR][32][2];  // results of the worker warps: (epoch << 32 | lowest accepting label, i << 32 | j);
+                            // a worker is at most CG_XR iterations ahead of the collector, hence twice the ring
+    u64 own[CG_XR][2];      // the CTA's result (collector -> exchange warp), same format
+    u64 peer[CG_MAX_CLUSTER][CG_SRING][2];   // posts of the other CTAs of the cluster (DSMEM), slot format
+    u32 hops[CG_HR][2];     // coded sites (i, j) of executed hop h at h % CG_HR
+    u32 ver;                // newest snapshot that every CTA has published (count within this launch)
+    u32 nlow;               // hops up to this one are in the occupation bitmap
+    u32 abort;              // the launch is being abandoned
+    u32 xe;                 // iterations decided so far
 };
-static_assert(CG_DEPTH <= 8 && CG_DEPTH < CG_SRING, "named barriers, slot ring");
+
+struct Waiter {             // watchdog state of one waiting warp
+    u64 t0; u32 spins;
+    __device__ __forceinline__ void reset() { t0 = 0; spins = 0; }
+};
+
+// One step of a wait loop; true: give up (the launch is being abandoned or the watchdog fired).
+__device__ __forceinline__ bool wait_poll(Waiter& w, const CgParams& p, Comm* cm, u32 code)
+{
+    if (((++w.spins) & 63u) != 0u) return false;
+    if (*(volatile u32*)&cm->abort) return true;
+    if ((w.spins & 1023u) != 0u) return false;
+    if (ld_relaxed_u32(&p.ctl->abort)) { *(volatile u32*)&cm->abort = 1u; return true; }
+    if (!p.watchdog_ns) return false;
+    const u64 now = global_ns();
+    if (!w.t0) { w.t0 = now; return false; }
+    if (now - w.t0 > p.watchdog_ns) {
+        atomicCAS(&p.ctl->abort, 0u, code);
+        *(volatile u32*)&cm->abort = 1u;
+        return true;
+    }
+    return false;
+}
+
+// wait for the phase with this parity of an mbarrier; false: gave up
+__device__ __forceinline__ bool mbar_wait(u64* b, u32 parity, const CgParams& p, Comm* cm, u32 code)
+{
+    if (mbar_try(b, parity, 2000u)) return true;
+    Waiter w; w.reset();
+    u32 n = 0;
+    for (;;) {
+        if (mbar_try(b, parity, 20000u)) return true;
+        if (*(volatile u32*)&cm->abort) return false;
+        if (((++n) & 15u) == 0u) { w.spins = 1023u; if (wait_poll(w, p, cm, code)) return false; }
+    }
+}
 
 // The persistent kernel: steps 1, 2, 3a-3c of the mixed PR algorithm.
-// CACHED: thread g of the grid owns the attempts a = g (mod P), P = gridDim.x * PL >= M, keeps its
-// current and its next proposal decoded in registers (a proposal is a pure function of the seed and
-// the attempt index) and, while theta_ij = 1, also the two local energies it needs, to which it adds
-// the term of every executed hop itself; an iteration then only re-tests the proposal on the current
-// state.  Otherwise CTA b evaluates labels [b per, (b+1) per) from scratch.
-// Warp 0 of every CTA does the exchange and all bookkeeping; the other worker warps only test their
-// proposals and update their part of the eps slab, and learn the outcome from a small descriptor.
+//
+// CACHED: thread g of the grid owns the attempts a = g (mod P), P = nb * PL >= M, keeps its current and
+// its next proposal decoded in registers (a proposal is a pure function of the seed and the attempt
+// index) and, while theta_ij = 1, also the two local energies it needs, to which it adds the term of
+// every executed hop itself; an iteration then only re-tests the proposal on the current state.
+// Otherwise (M > P) CTA b evaluates labels [b per, (b+1) per) from scratch in every iteration, with the
+// warps of the CTA in lock step (the occupation bitmap is then always current).
+//
+// Roles: warps 0 .. NW-1 workers; warp NW the collector (C); NW+1 the exchange warp (X); NW+2 the
+// service warp (S).  Iteration e ("exchange"), state S_e before it, outcome O_e:
+//   worker:  test own label on S_e -> res[e][warp]; slab update of the hop of O_{e-1}; wait for O_e (mbarrier
+//            full[e]); consume it (labels, occupations of the followed pair, followed energies); arrive empty[e]
+//   C:       reduce res[e][*] in label order, stopping at the first accept -> own[e], the CTA's slot in L2
+//            and the shared memory of its cluster peers; consume O_e
+//   X:       gate on published snapshots; find the first accepting CTA in scan order (own[e], cluster
+//            peers in shared memory, the others' slots in L2), stopping there; publish O_e; counters, log
+//   S:       per snapshot: wait until every worker warp has stored its part (mbarrier pubbar), publish the
+//            CTA's sequence number (st.release.gpu), find the newest snapshot published by ALL CTAs
+//
+// Snapshots (deferred update).  Snapshot s = eps after hop s H of this launch, in buffer
+// (cur0 + s) % CG_RING; workers keep their slab current in registers after every hop but store it only
+// then.  A proposal that starts to follow a pair of sites at hop h reads snapshot v = cm->ver (complete
+// on every CTA) and adds the terms of hops v H + 1 .. h itself, in hop order - the same single rounded
+// adds the update performs, so the values are bit-identical whatever v is.  X lets hop h through only
+// when every CTA has published snapshot floor((h - G)/H): all workers of the grid are then within
+// G + H - 1 hops of each other, a reader has at most that many terms to add (the hop ring holds them),
+// and with CG_RING H > 2 G + 2 H - 2 no buffer is overwritten while it can still be read.
+// Occupations: the bitmap lags (X applies the hop of O_{e - CG_XR} when it recycles that descriptor,
+// i.e. when every warp has consumed it), so it is never ahead of a reader; a reader replays the hops
+// after cm->nlow (set/clear in hop order is idempotent).
+//
 // Written as a device function of (parameters, CTA index, CTA count) so that one launch can also hold
-// several sims side by side (cg_pr_persistent_many): nothing in it looks at blockIdx or gridDim, and all
-// synchronisation between CTAs goes through the sim's own slots and publication words.
-template <int THREADS, int RP, bool CACHED>
+// several sims side by side (cg_pr_persistent_many): nothing in it looks at blockIdx or gridDim.
+template <int NW, int RP, bool CACHED>
 __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 b, const u32 nb)
 {
-    constexpr int TW = THREADS - 64;      // worker threads; then the control warp and the service warp
-    constexpr int NWK = TW / 32;          // worker warps = index of the control warp
-    constexpr int TB = TW + 32;           // threads at the CTA barriers of an iteration (workers + control)
+    constexpr int TW = NW * 32;           // worker threads
+    constexpr int THREADS = TW + 96;
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    const int KL = p.Klive;
+    const int KS = p.Ksm;
     u64* s_cdfi = reinterpret_cast<u64*>(smem_raw);
-    double* s_invr = reinterpret_cast<double*>(s_cdfi + KL);
-    double* s_fld = s_invr + KL;
-    int* s_disp = reinterpret_cast<int*>(s_fld + KL);
-    u32* s_guide = reinterpret_cast<u32*>(s_disp + KL);
+    double* s_invr = reinterpret_cast<double*>(s_cdfi + KS);
+    double* s_fld = s_invr + KS;
+    u32* s_disp = reinterpret_cast<u32*>(s_fld + KS);
+    u32* s_guide = s_disp + KS;
     u32* s_n = s_guide + CG_GUIDE;
-    __shared__ u32 s_key;                 // lowest accepting (label << 5 | warp) of the CTA in this iteration
-    __shared__ u64 s_wpay[32];            // (i, j) of each warp's lowest accepting label
-    __shared__ u64 s_verified;            // newest publication sequence number seen from ALL CTAs (service warp)
-    __shared__ __align__(16) Desc s_desc;
-    __shared__ __align__(16) Pend s_pend;
-    const Tables tb = {s_cdfi, s_invr, s_fld, s_disp, s_guide};
-#ifdef CG_TRACE
-    __shared__ u64 s_seg[64];
-    if (threadIdx.x < 64) s_seg[threadIdx.x] = 0;
-    long long t_prev = 0;
-#endif
+    __shared__ Comm cmem;
+    Comm* const cm = &cmem;
+    const Tables tb = {s_cdfi, s_invr, s_fld, s_disp, s_guide, p.cdfi, p.invr_k, p.fld_k, p.disp, (u32)KS};
+    const Geo geo = {p.hi1, p.hi2, p.spare, p.mask, (u32)(p.L - 1), p.lgL};
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int L = p.L, lg = p.lgL;
-    const u32 N = p.N, M = p.M;
-    const u32 mask = ((u32)(L - 1) << (lg + 1)) | (u32)(L - 1);
+    const u32 N = p.N, M = p.M, mask = p.mask;
     const double* __restrict__ tf = p.tf;
+    const u32 Hs = p.snap_shift, Hm = (1u << Hs) - 1u;
 
-    for (int k = tid; k < KL; k += THREADS) {
+    for (int k = tid; k < KS; k += THREADS) {
         s_cdfi[k] = p.cdfi[k]; s_invr[k] = p.invr_k[k]; s_fld[k] = p.fld_k[k]; s_disp[k] = p.disp[k];
     }
     for (int k = tid; k < CG_GUIDE; k += THREADS) s_guide[k] = p.guide[k];
     for (u32 w = tid; w < (N + 31) / 32; w += THREADS) s_n[w] = p.nbits[w];
+    // no record may look like one of this launch: tag them with the epoch before its first
+    const u64 stale = (u64)((u32)p.ctl->epoch - 1u) << 32;
+    for (u32 k = tid; k < sizeof(cm->res) / 8; k += THREADS) (&cm->res[0][0][0])[k] = stale;
+    for (u32 k = tid; k < sizeof(cm->peer) / 8; k += THREADS) (&cm->peer[0][0][0])[k] = stale;
     if (tid == 0) {
-        s_key = CG_NONE;
-        s_verified = p.ctl->pub_base;
-        s_pend.npend = 0; s_pend.rbuf = p.ctl->cur; s_pend.first = 0;
+        for (int k = 0; k < CG_XR; ++k) {
+            mbar_init(&cm->full[k], 1); mbar_init(&cm->empty[k], NW + 1);
+            cm->own[k][0] = stale; cm->own[k][1] = 0;
+        }
+        for (int k = 0; k < CG_PB; ++k) mbar_init(&cm->pubbar[k], NW);
+        cm->ver = 0; cm->nlow = 0; cm->abort = 0; cm->xe = 0;
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
 
     const u64 a_start = p.ctl->attempts, pub_base = p.ctl->pub_base;
-    u64 hl = 0;                           // hops executed in this launch
-    u32 wbuf = p.ctl->cur;                // buffer of the ring that holds the newest eps
-    bool upd = false;                     // slab update issued, not yet finished
-    bool newhop = false;                  // the previous iteration executed a hop ...
-    u32 hci = 0, hcj = 0;                 // ... with these coded sites
-    bool ahead = false;                   // another CTA holds the start of the window
+    const u32 cur0 = p.ctl->cur;          // snapshot 0 of this launch: the complete state it starts from
+    const u32 e_start = (u32)p.ctl->epoch;
+    const u32 n_hops = p.n_hops;
     const long long t_begin = clock64();
 
     // labels: CTA-blocked (scan order = CTA order) or, CACHED, cyclic in the global thread index
@@ -411,489 +574,479 @@ __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 
     const u32 P = nb * per;               // CACHED: attempts a = g (mod P) belong to thread g
     u32 c_first = 0, t0r = 0;             // CACHED: CTA at scan position 0 and the offset of a0 in it
     if (CACHED) { const u32 g0 = (u32)(a_start % P); c_first = g0 / per; t0r = g0 - c_first * per; }
-    const bool has_label = CACHED && (u32)tid < per;
+    const u32 csz = p.cluster;            // posts inside a cluster go through shared memory
+    const u32 cl0 = csz > 1 ? b - cluster_ctarank() : b;        // first CTA of my cluster
     __syncthreads();
-    if (warp == NWK + 1) {
-        // service warp: once per executed hop, wait until every worker has stored its part of the
-        // slab (named barrier), fence those stores and bump the publication counter - off the
-        // workers' critical path.  Workers run at most CG_DEPTH hops ahead of it (the exchange of hop
-        // h+DEPTH waits for the publication of hop h by every CTA, this one included), hence as many
-        // barriers.
-        // After publishing it looks at every CTA's publication word once and leaves the newest hop that
-        // ALL of them have published in shared memory: the control warp, which must know that before it
-        // lets a hop through, then rarely has to look itself.
-        if (nb > 1)
-            for (u64 h = 0; h < p.n_hops; ++h) {
-                barN_sync((u32)(h % CG_DEPTH), TB);
-                if (lane == 0) st_release_u64(p.slots + (size_t)b * CG_SLOT_U64 + CG_PUB_U64, pub_base + h + 1);
-                u64 vmin = ~0ull;
-                for (u32 c0 = lane; c0 < nb; c0 += 32 * 8) {            // eight independent loads in flight
-                    u64 v[8];
-#pragma unroll
-                    for (int k = 0; k < 8; ++k) {
-                        const u32 c = c0 + 32 * k;
-                        v[k] = c < nb ? ld_relaxed_u64(p.slots + (size_t)c * CG_SLOT_U64 + CG_PUB_U64) : ~0ull;
-                    }
-#pragma unroll
-                    for (int k = 0; k < 8; ++k) vmin = min(vmin, v[k]);
-                }
-#pragma unroll
-                for (int o = 16; o > 0; o >>= 1) vmin = min(vmin, __shfl_xor_sync(CG_FULL, vmin, o));
-                fence_acquire_gpu();
-                if (lane == 0 && vmin > pub_base) *(volatile u64*)&s_verified = vmin;    // stale words are smaller
-            }
-        return;
-    }
-    // CACHED per-thread state: label of my attempt relative to the window start, the decoded proposal
-    // and what its test needs; the attempt after it, decoded ahead when there is idle time
-    u32 lab = CG_NONE;
-    u64 a_cur = 0;
-    u32 ci_ = 0, cj_ = 0, sci = 0, scj = 0, cuh = 0, cul = 0;
-    double c_invr = 0, c_fld = 0, ei = 0, ej = 0;
-    bool tracked = false;                 // ei, ej hold the current local energies of my two sites
-    Prop nxt = {0, 0, 0, 0, 0};
-    bool nxt_valid = false;
-    auto take = [&](const Prop& q) {
-        ci_ = q.i; cj_ = q.j; cuh = q.uh; cul = q.ul;
-        sci = site_code(q.i, L) | (u32)L; scj = site_code(q.j, L) | (u32)L;
-        c_invr = s_invr[q.k]; c_fld = s_fld[q.k];
-        tracked = false;
-    };
-    if (has_label) {
-        const u32 g = b * per + (u32)tid, g0 = c_first * per + t0r;
-        lab = g >= g0 ? g - g0 : g + P - g0;
-        a_cur = a_start + lab;
-        take(decode_attempt(tb, p, a_cur));
-    }
-    ahead = CACHED && c_first != b;
+    if (csz > 1) cluster_sync_all();      // the peers' mbarriers and post areas exist before anybody writes to them
 
     const u32 pairs = N / 2, pper = (pairs + nb - 1) / nb;
     const u32 pr0 = min(pairs, b * pper), pr1 = min(pairs, pr0 + pper);
     u64* const my_slot = p.slots + (size_t)b * CG_SLOT_U64;
+    const u32 n_snaps = n_hops >> Hs;     // regular snapshots of this launch
 
-    if (warp == NWK) {
-        // ------------------------------------------------------------------ control warp ----
-        // Exchange and bookkeeping of the CTA; it holds no labels and no eps.
+    if (warp == NW + 2) {
+        // ------------------------------------------------------------------ service warp ----
+        for (u32 s = 1; s <= n_snaps; ++s) {
+            if (!mbar_wait(&cm->pubbar[(s - 1) % CG_PB], ((s - 1) / CG_PB) & 1u, p, cm, 1u)) break;
+            if (nb == 1) { if (lane == 0) max_release_cta(&cm->ver, s); continue; }
+            if (lane == 0) st_release_u64(my_slot + CG_PUB_U64, pub_base + s);
+            u64 vmin = ~0ull;
+            for (u32 c0 = lane; c0 < nb; c0 += 32 * 8) {                // eight independent loads in flight
+                u64 v[8];
+#pragma unroll
+                for (int k = 0; k < 8; ++k) {
+                    const u32 c = c0 + 32 * k;
+                    v[k] = c < nb ? ld_relaxed_u64(p.slots + (size_t)c * CG_SLOT_U64 + CG_PUB_U64) : ~0ull;
+                }
+#pragma unroll
+                for (int k = 0; k < 8; ++k) vmin = min(vmin, v[k]);
+            }
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) vmin = min(vmin, __shfl_xor_sync(CG_FULL, vmin, o));
+            fence_acquire_gpu();
+            if (lane == 0 && vmin > pub_base) max_release_cta(&cm->ver, (u32)(vmin - pub_base));    // stale words are smaller
+        }
+    } else if (warp == NW) {
+        // ---------------------------------------------------------------- collector warp ----
+        // The CTA's lowest accepting label of every iteration (step 3), found in label order:
+        // lane r looks at the r-th warp in that order.  In scan order every worker warp holds lower labels
+        // than the next one, except that (CACHED) at scan position 0 the threads below the first label of
+        // the window hold its END ("tail" labels >= tail0): those rank after every other label.
+        u32 cf = c_first, tr = t0r;
+        Waiter wd;
+        for (u32 e = 0;; ++e) {
+            const u32 xs = e % CG_XR, e32 = e_start + e;
+            const u32 kb = b >= cf ? b - cf : b + nb - cf;
+            const u32 tail0 = (CACHED && kb == 0) ? per - tr : CG_NONE;
+            const u32 w0 = (CACHED && kb == 0) ? tr >> 5 : 0u;
+            u32 wr = w0 + (u32)lane; if (wr >= (u32)NW) wr -= NW;
+            const bool mine = lane < NW;
+            bool ready = !mine; u32 l = CG_NONE, tl = CG_NONE; u64 pay = 0;
+            u32 gmin = CG_NONE; u64 gpay = 0;
+            wd.reset();
+            bool quit = false;
+            for (;;) {
+                if (!ready) {
+                    u64 q0, q1;
+                    lds128(&cm->res[e % (2 * CG_XR)][wr][0], q0, q1);
+                    if ((u32)(q0 >> 32) == e32) {
+                        ready = true; pay = q1;
+                        const u32 v = (u32)q0;
+                        if (v != CG_NONE && v >= tail0) tl = v; else l = v;
+                    }
+                }
+                const u32 racc = __ballot_sync(CG_FULL, ready && l != CG_NONE);
+                const u32 rnot = __ballot_sync(CG_FULL, !ready);
+                const int fa = racc ? __ffs(racc) - 1 : 32, fn = rnot ? __ffs(rnot) - 1 : 32;
+                if (CACHED && fa < fn) {                        // first accept in label order, everything before it rejected
+                    gmin = __shfl_sync(CG_FULL, l, fa); gpay = __shfl_sync(CG_FULL, pay, fa);
+                    break;
+                }
+                if (!rnot) {                                    // every warp is in (lock step, not CACHED: always waited for)
+                    const u32 hm = __reduce_min_sync(CG_FULL, l);
+                    const u32 tm = hm != CG_NONE ? hm : __reduce_min_sync(CG_FULL, tl);    // no head accept: lowest tail accept
+                    if (tm != CG_NONE) {
+                        const int src = __ffs(__ballot_sync(CG_FULL, (hm != CG_NONE ? l : tl) == tm)) - 1;
+                        gmin = tm; gpay = __shfl_sync(CG_FULL, pay, src);
+                    }
+                    break;
+                }
+                if (wait_poll(wd, p, cm, 2u)) { quit = true; break; }
+            }
+            if (quit) break;
+            // post: own[] for the exchange warp, the slot in L2 for the other CTAs, the peers' shared memory
+            const u64 s0 = ((u64)e32 << 32) | gmin;
+            if (lane == 0) sts128(&cm->own[xs][0], s0, gpay);
+            if (nb > 1) {
+                const u32 ring = e32 & (CG_SRING - 1u);
+                const u64 s1 = ((u64)(e32 & 0xFFFFu) << 48) | ((gpay >> 32) << 24) | (gpay & 0xFFFFFFu);
+                if (csz > 1 && (u32)lane < csz && cl0 + (u32)lane != b) {
+                    const u32 ra = mapa_cluster(smem_u32(&cm->peer[b - cl0][ring][0]), (u32)lane);
+                    st_cluster128(ra, s0, s1);
+                }
+                if (lane == 0) slot_store(my_slot + 2u * ring, s0, s1);
+            }
+            // consume O_e
+            if (!mbar_wait(&cm->full[xs], (e / CG_XR) & 1u, p, cm, 3u)) break;
+            const uint4 d0 = lds128u(&cm->desc[xs]);
+            const uint4 d1 = lds128u(&cm->desc[xs].c_first);
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&cm->empty[xs]);
+            if (d0.y & (CG_F_LAST | CG_F_ABORT)) break;
+            cf = d1.x; tr = d1.y;
+        }
+    } else if (warp == NW + 1) {
+        // ----------------------------------------------------------------- exchange warp ----
         const u64 log_base = p.ctl->log_base, hops_start = p.ctl->hops;
-        const u32 e_start = (u32)p.ctl->epoch;
         u64 used_sum = 0;                 // attempts consumed in this launch
         long long dP = 0;
-        u32 it_local = 0;                 // PR iterations of this launch
-        // Pending hops.  eps lives in a ring of CG_RING buffers: hop h writes eps_h (each CTA its own
-        // slab) into the buffer after the one hop h-1 wrote.  Nobody reads buffers that other CTAs may
-        // still be writing: a proposal that starts to follow a pair of sites reads eps_v, v = the newest
-        // hop every CTA has published (buffer rbuf; v >= h - DEPTH by the publication check), and adds
-        // the terms 1/r_lj - 1/r_li of the hops v+1 .. h itself, in hop order - the same single rounded
-        // adds the update performs, so the values are bit-identical whatever v is.  A CTA writes
-        // eps_{h'} only when every CTA has published hop h' - DEPTH; a reader at hop h has published
-        // at most h, so h' <= h + DEPTH while it reads v >= h - DEPTH: with 2 DEPTH + 1 buffers a
-        // buffer is never written while read.
-        const u32 cur0 = wbuf;            // buffer that holds eps at the start of this launch
-        // CTA c has published hop number h of this launch once its pub word is >= pub_base + h
-        u64 need_pub = 0;                 // hop hl - DEPTH + 1: readers never reach back further than DEPTH hops
-        u64 ver = pub_base;               // newest publication seen from ALL CTAs
-#ifdef CG_TRACE_W
-        u64 cw[16] = {}; long long cprev = clock64();
-#endif
-        while (hl < p.n_hops) {
-            const u32 e32 = e_start + it_local;
-            const u32 kb = b >= c_first ? b - c_first : b + nb - c_first;    // my scan position
-            TS_CTL(0);
-#ifdef CG_TRACE
-            if (lane == 0) { if (t_prev == 0) t_prev = clock64(); s_seg[CLS_ + 15] += 1; }
-#endif
-            // Hop hl - DEPTH + 1 must be complete on every CTA before the workers of this CTA are let into the
-            // next iteration (readers reach back at most DEPTH hops): one publication word per CTA, each in its
-            // own L2 slice.  This warp is idle while the workers test their proposals, so the check is free.
-            if (nb > 1) ver = max(ver, *(volatile u64*)&s_verified);
-            if (nb > 1 && ver < need_pub) {                             // rarely: the service warp has usually seen it
-                for (;;) {
-                    bool ok = true;
-                    for (u32 c0 = lane; c0 < nb; c0 += 32 * 8) {        // eight independent loads in flight
-                        u64 v[8];
-#pragma unroll
-                        for (int k = 0; k < 8; ++k) {
-                            const u32 c = c0 + 32 * k;
-                            v[k] = c < nb ? ld_relaxed_u64(p.slots + (size_t)c * CG_SLOT_U64 + CG_PUB_U64) : ~0ull;
-                        }
-#pragma unroll
-                        for (int k = 0; k < 8; ++k) ok = ok && v[k] >= need_pub;
-                    }
-#ifdef CG_TRACE
-                    if (lane == 0) s_seg[CLS_ + 8] += 1;      // passes of the publication check
-#endif
-                    if (__all_sync(CG_FULL, ok)) break;
-                }
-                fence_acquire_gpu();
-                ver = need_pub;
+        u32 e = 0, hc = 0;                // iterations and hops decided in this launch
+        u32 e_app = 0;                    // descriptors below this one are in the occupation bitmap
+        u32 ver = 0;                      // newest snapshot known to be published by every CTA
+        Waiter wd;
+        bool quit = false;
+        // the hop of descriptor ea goes into the bitmap (every warp has consumed it)
+        auto apply = [&](u32 ea) {
+            const uint4 d0 = lds128u(&cm->desc[ea % CG_XR]);
+            if (lane == 0 && (d0.y & CG_F_HOP)) {
+                const u32 si = geo.site(d0.z), sj = geo.site(d0.w);
+                atomicAnd(&s_n[si >> 5], ~(1u << (si & 31)));
+                atomicOr(&s_n[sj >> 5], 1u << (sj & 31));
+                __threadfence_block();
+                *(volatile u32*)&cm->nlow = cm->desc[ea % CG_XR].hopno;
             }
-            TRACE(6, 0);
-            TS_CTL(1);
-            // A CTA that does not hold the start of the window usually runs behind the one that does: the
-            // winner of this exchange may already be posted.  One look at the first two scan positions
-            // before the barrier takes that round trip off the path between the two barriers.
-            const u32 tail0 = CACHED ? per - t0r : CG_NONE;            // position 0: labels >= tail0 are tail labels
-            const u32 ring = (e32 & (CG_SRING - 1u)) * 2u;
-            const u32 e16 = e32 & 0xFFFFu;
-            u32 eq = CG_NONE; u64 ewp = 0;
-            if (nb > 1 && kb != 0) {
-                const bool mine = lane < 2 && (u32)lane < kb;
-                u32 c = c_first + lane; if (c >= nb) c -= nb;
-                u32 l = CG_NONE; u64 q0 = 0, q1 = 0; bool ready = false;
-                if (mine) {
-                    slot_load(p.slots + (size_t)c * CG_SLOT_U64 + ring, q0, q1);
-                    ready = (u32)(q0 >> 32) == e32 && (u32)(q1 >> 48) == e16;
-                    l = ready ? (u32)q0 : CG_NONE;
-                    if (CACHED && lane == 0 && l != CG_NONE && l >= tail0) l = CG_NONE;    // tail labels never win early
-                }
-                const u32 racc = __ballot_sync(CG_FULL, mine && ready && l != CG_NONE);
-                const u32 rnot = __ballot_sync(CG_FULL, mine && !ready);
-                const int fa = racc ? __ffs(racc) - 1 : 32, fn = rnot ? __ffs(rnot) - 1 : 32;
-                if (fa < fn) {
-                    eq = __shfl_sync(CG_FULL, l, fa);
-                    ewp = __shfl_sync(CG_FULL, q1, fa);
-                    ewp = ((ewp >> 24) & 0xFFFFFFull) << 32 | (ewp & 0xFFFFFFull);
-                }
+        };
+        while (hc < n_hops) {
+            const u32 xs = e % CG_XR, e32 = e_start + e;
+            // (1) recycle the descriptor slot: every consumer is past iteration e - CG_XR
+            if (CACHED && e >= CG_XR) {
+                if (!mbar_wait(&cm->empty[xs], ((e - CG_XR) / CG_XR) & 1u, p, cm, 4u)) { quit = true; break; }
+                apply(e_app); ++e_app;
             }
-            TRACE(7, 0);
-#ifdef CG_TRACE_W
-            cw[15] += 1; if (eq != CG_NONE) cw[14] += 1; if (kb == 0) cw[13] += 1;
-#endif
-            TS_CTL(2);
-            barX_sync(TB);                // [A] the workers have tested their proposals
-            TS_CTL(3);
-            TRACE(3, 0);
-            // ---- step 3: lowest accepting label: CTA, then grid
-            // (every worker warp has put its lowest accepting label into one shared-memory minimum)
-            const u32 key = *(volatile u32*)&s_key;
-            const u32 gmin = key == CG_NONE ? CG_NONE : key >> 5;
-            const u64 gpay = key == CG_NONE ? 0ull : s_wpay[key & 31u];     // (0: the slot's fields must not overflow)
-            __syncwarp();
-            if (lane == 0) *(volatile u32*)&s_key = CG_NONE;          // for the next iteration (ordered by [B])
-            // In scan order (CTA order starting at the CTA that holds attempt a0) every CTA holds lower
-            // labels than the next one, except that CACHED the first CTA also holds the end of the window
-            // in its threads below a0's ("tail" labels).  The winner is the first non-tail accept in scan
-            // order; the scan stops there: slots of later CTAs are never waited for (their proposals
-            // cannot win), and the first CTA, when it accepts, waits for nobody.
-            const bool own_low = gmin != CG_NONE && (!CACHED || kb != 0 || gmin < tail0);
-            TS_CTL(4);
-            // A CTA can be up to DEPTH + 1 exchanges ahead of the slowest reader of its slot (bounded by the
-            // publication check and by every fully rejected window, which needs all slots): ring of CG_SRING.
-            if (nb > 1 && lane == 0)
-                slot_store(my_slot + ring, ((u64)e32 << 32) | gmin,
-                           ((u64)(e32 & 0xFFFFu) << 48) | ((gpay >> 32) << 24) | (gpay & 0xFFFFFFu));
-            u32 q = gmin; u64 wp = gpay;
-            TS_CTL(5);
-            TRACE(10, 0);
-            if (eq != CG_NONE) { q = eq; wp = ewp; }                   // answered before the barrier
-            else if (!(own_low && kb == 0) && nb > 1) {
-#ifdef CG_TRACE
-                if (lane == 0) s_seg[CLS_ + 9] += 1;      // scans
-#endif
-                u32 tlab = CG_NONE; u64 tpay = 0;                      // tail accept of position 0
-                const u32 k_end = own_low ? kb : nb;    // an accept of my own: only earlier CTAs can beat it
-                u32 k0 = 0;                             // 32 scan positions at a time (measured best)
-                bool found = false;
-                while (!found && k0 < k_end) {
-                    const u32 k = k0 + lane;
-                    const bool mine = k < k_end && k != kb;
-                    u32 c = c_first + k; if (c >= nb) c -= nb;
-                    const u64* sl = p.slots + (size_t)(mine ? c : b) * CG_SLOT_U64 + ring;
-                    bool ready = !mine; u32 l = CG_NONE; u64 q1 = 0;
+            // (2) gate: every CTA has published the snapshot that covers hop hc + 1 - G
+            if (nb > 1 && hc + 1u > p.gate) {
+                const u32 need = (hc + 1u - p.gate) >> Hs;
+                if (ver < need) ver = max(ver, *(volatile u32*)&cm->ver);
+                if (ver < need) {
+                    const u64 want = pub_base + need;
+                    wd.reset();
                     for (;;) {
-                        if (!ready) {
-                            u64 q0;
-                            slot_load(sl, q0, q1);
+                        bool ok = true;
+                        for (u32 c0 = lane; c0 < nb; c0 += 32 * 8) {
+                            u64 v[8];
+#pragma unroll
+                            for (int k = 0; k < 8; ++k) {
+                                const u32 c = c0 + 32 * k;
+                                v[k] = c < nb ? ld_relaxed_u64(p.slots + (size_t)c * CG_SLOT_U64 + CG_PUB_U64) : ~0ull;
+                            }
+#pragma unroll
+                            for (int k = 0; k < 8; ++k) ok = ok && v[k] >= want;
+                        }
+                        if (__all_sync(CG_FULL, ok)) break;
+                        wd.spins |= 63u;
+                        if (wait_poll(wd, p, cm, 5u)) { quit = true; break; }
+                    }
+                    if (quit) break;
+                    fence_acquire_gpu();
+                    ver = need;
+                    if (lane == 0) max_release_cta(&cm->ver, need);
+                }
+            }
+            // (3) the first accepting CTA in scan order (step 3).  Position 0 holds the start of
+            // the window; a window of scan positions is polled at a time, starting narrow (the winner is nearly
+            // always at the first positions), and polling stops at the first accept: posts of later CTAs are
+            // never waited for, and the CTA at position 0, when it accepts, waits for nobody.
+            const u32 kb = b >= c_first ? b - c_first : b + nb - c_first;
+            const u32 tail0 = CACHED ? per - t0r : CG_NONE;
+            const u32 ring = e32 & (CG_SRING - 1u), e16 = e32 & 0xFFFFu;
+            u32 q = CG_NONE; u64 wp = 0;
+            u32 tlab = CG_NONE; u64 tpay = 0;                          // tail accept of position 0
+            u32 lo = 0, hi = kb == 0 ? 1u : min(nb, 4u);
+            wd.reset();
+            while (lo < nb) {
+                const u32 k = lo + (u32)lane;
+                const bool mine = k < hi;
+                u32 c = c_first + k; if (c >= nb) c -= nb;
+                const bool local = mine && k != kb && csz > 1 && c - cl0 < csz;
+                bool ready = !mine; u32 l = CG_NONE; u64 pay = 0;
+                bool found = false;
+                for (;;) {
+                    if (!ready) {
+                        u64 q0, q1;
+                        if (k == kb) {
+                            lds128(&cm->own[xs][0], q0, q1);
+                            if ((u32)(q0 >> 32) == e32) { ready = true; l = (u32)q0; pay = q1; }
+                        } else {
+                            if (local) lds128(&cm->peer[c - cl0][ring][0], q0, q1);
+                            else slot_load(p.slots + (size_t)c * CG_SLOT_U64 + 2u * ring, q0, q1);
                             if ((u32)(q0 >> 32) == e32 && (u32)(q1 >> 48) == e16) {
                                 ready = true; l = (u32)q0;
-                                if (CACHED && k == 0 && l != CG_NONE && l >= tail0) { tlab = l; tpay = q1; l = CG_NONE; }
+                                pay = ((q1 >> 24) & 0xFFFFFFull) << 32 | (q1 & 0xFFFFFFull);
                             }
                         }
-                        const u32 racc = __ballot_sync(CG_FULL, ready && l != CG_NONE);
-                        const u32 rnot = __ballot_sync(CG_FULL, !ready);
-                        const int fa = racc ? __ffs(racc) - 1 : 32;
-                        const int fn = rnot ? __ffs(rnot) - 1 : 32;
-                        if (fa < fn) {                  // first accepting slot, everything before it rejected
-                            q = __shfl_sync(CG_FULL, l, fa);
-                            wp = __shfl_sync(CG_FULL, q1, fa);
-                            wp = ((wp >> 24) & 0xFFFFFFull) << 32 | (wp & 0xFFFFFFull);
-                            found = true;
-                            break;
-                        }
-                        if (!rnot) break;               // whole chunk rejected: next chunk
+                        if (ready && k == 0 && l != CG_NONE && l >= tail0) { tlab = l; tpay = pay; l = CG_NONE; }
                     }
-                    if (k0 == 0) {                      // position 0 sits in lane 0 of the first chunk
-                        tlab = __shfl_sync(CG_FULL, tlab, 0); tpay = __shfl_sync(CG_FULL, tpay, 0);
+                    const u32 racc = __ballot_sync(CG_FULL, ready && l != CG_NONE);
+                    const u32 rnot = __ballot_sync(CG_FULL, !ready);
+                    const int fa = racc ? __ffs(racc) - 1 : 32, fn = rnot ? __ffs(rnot) - 1 : 32;
+                    if (fa < fn) {                      // first accepting position, everything before it rejected
+                        q = __shfl_sync(CG_FULL, l, fa); wp = __shfl_sync(CG_FULL, pay, fa);
+                        found = true;
+                        break;
                     }
-                    k0 += 32;
+                    if (!rnot) break;                   // whole window rejected: widen
+                    if (kb != 0 || lo != 0) wd.spins |= 63u;      // polls through L2 are slow: look at the clock more often
+                    if (wait_poll(wd, p, cm, 6u)) { quit = true; break; }
                 }
-                if (!found && !own_low && kb != 0 && tlab != CG_NONE) {   // only the tail of the window accepted
-                    q = tlab; wp = ((tpay >> 24) & 0xFFFFFFull) << 32 | (tpay & 0xFFFFFFull);
+                if (quit || found) break;
+                if (lo == 0) { tlab = __shfl_sync(CG_FULL, tlab, 0); tpay = __shfl_sync(CG_FULL, tpay, 0); }
+                lo = hi; hi = min(nb, lo + 32u);
+            }
+            if (quit) break;
+            if (q == CG_NONE && tlab != CG_NONE) { q = tlab; wp = tpay; }   // only the tail of the window accepted
+            // lock step (not CACHED): every warp of this CTA has finished its tests of this iteration before the
+            // bitmap changes
+            if (!CACHED) {
+                wd.reset();
+                for (;;) {
+                    u64 q0, q1;
+                    lds128(&cm->own[xs][0], q0, q1);
+                    if ((u32)(q0 >> 32) == e32) break;
+                    if (wait_poll(wd, p, cm, 7u)) { quit = true; break; }
                 }
+                if (quit) break;
+                if (e >= CG_XR && !mbar_wait(&cm->empty[xs], ((e - CG_XR) / CG_XR) & 1u, p, cm, 4u)) { quit = true; break; }
             }
-#ifdef CG_TRACE
-            if (lane == 0 && !(own_low && kb == 0) && nb > 1) {       // histogram of the scan time
-                const long long dt = clock64() - t_prev;
-                const int bin = dt < 500 ? 11 : dt < 1000 ? 12 : dt < 2000 ? 13 : dt < 4000 ? 14 : dt < 8000 ? 1 : 2;
-                s_seg[CLS_ + bin] += 1;
-            }
-#endif
-            TRACE(4, 0);
-            TS_CTL(6);
-            // ---- what the workers need: attempts consumed (m = (p-1)M + q per executed hop, PAPER.md:39,
-            // 78), the hop (step 3a), occupations, pending list
+            // (4) publish O_e: attempts consumed (m = (p-1)M + q per executed hop), the hop
+            // (step 3a)
             const u32 used = q == CG_NONE ? M : q + 1;
             const u32 hi_ = (u32)(wp >> 32), hj_ = (u32)wp;
-            const u32 ci = site_code(hi_, L), cj = site_code(hj_, L);
-            if (lane == 0) *reinterpret_cast<uint4*>(&s_desc) = make_uint4(used, q != CG_NONE, ci, cj);
-            // Readers start from a buffer that is complete on every CTA (hop v; this CTA's own slab of hop hl is
-            // finished in the gap that ends at [B]) and add the hops v+1 .. themselves, in hop order.
-            {
-                const u32 hn_ = (u32)hl + (q != CG_NONE ? 1u : 0u);                 // hops executed so far
-#ifdef CG_VNEW
-                const u32 v = nb > 1 ? (u32)(ver - pub_base) : (u32)hl;
-#else
-                // one CTA: its own slab is always complete.  Several: DEPTH hops back is what the publication
-                // check guarantees; starting from the newest buffer seen complete (ver) saves pending terms but
-                // measured slower at 19 CTAs (-5 %) and equal at 148.
-                const u32 v = nb > 1 ? (hn_ > CG_DEPTH ? hn_ - CG_DEPTH : 0u) : (u32)hl;
-#endif
-                const u32 np_ = hn_ - v;                                            // <= DEPTH
-                if (lane == 0) {              // the workers are between the two barriers: nobody reads these
-                    if (q != CG_NONE) {
-                        atomicAnd(&s_n[hi_ >> 5], ~(1u << (hi_ & 31)));     // no return value: fire and forget
-                        atomicOr(&s_n[hj_ >> 5], 1u << (hj_ & 31));
-                        *reinterpret_cast<uint2*>(&s_pend.c[(u32)hl % CG_DEPTH][0]) = make_uint2(ci, cj);
-                    }
-                    *reinterpret_cast<uint4*>(&s_pend) = make_uint4(np_, (cur0 + v) % CG_RING, v % CG_DEPTH, 0u);
-                }
-            }
-            TRACE(5, 0);
-            TS_CTL(7);
-            barB_arrive(TB);              // [B] the workers may read the descriptor; this warp goes on
-            TS_CTL(8);
-#ifdef CG_TRACE_T
-            if (lane == 0 && p.trace && b < 32u && it_local - 2000u < 64u) {
-                p.trace[((it_local - 2000u) * 32u + b) * 32u + 10] = kb; p.trace[((it_local - 2000u) * 32u + b) * 32u + 11] = used;
-            }
-#endif
-            // ---- the rest of the bookkeeping, while the workers run
+            const u32 ci = geo.code(hi_), cj = geo.code(hj_);
+            const bool hop = q != CG_NONE;
             if (CACHED) {
                 if (t0r + used < per) t0r += used;
                 else {
                     u32 g0 = c_first * per + t0r + used; if (g0 >= P) g0 -= P;      // used <= M <= P
                     c_first = g0 / per; t0r = g0 - c_first * per;
                 }
-                // a hint only (time to decode ahead): the workers may still see the previous value
-                if (lane == 0) s_desc.ahead = c_first != b;
             }
+            if (hop) ++hc;
+            const u32 flags = (hop ? CG_F_HOP : 0u) | (hc >= n_hops ? CG_F_LAST : 0u);
+            if (lane == 0) {
+                if (hop) sts64u(&cm->hops[hc % CG_HR][0], ci, cj);
+                Desc* d = &cm->desc[xs];
+                sts128u(&d->c_first, c_first, t0r, hc, 0u);
+                sts128u(&d->used, used, flags, ci, cj);
+                if (!CACHED && hop) {         // lock step: the bitmap is always current
+                    atomicAnd(&s_n[hi_ >> 5], ~(1u << (hi_ & 31)));
+                    atomicOr(&s_n[hj_ >> 5], 1u << (hj_ & 31));
+                    *(volatile u32*)&cm->nlow = hc;
+                }
+                mbar_arrive(&cm->full[xs]);   // release: the stores above are visible to whoever sees the phase complete
+                *(volatile u32*)&cm->xe = e + 1u;
+            }
+            // (5) the rest of the bookkeeping, off the critical path
             used_sum += used;
-            ++it_local;
-            if (q != CG_NONE) {
-                const int xi = hi_ & (L - 1), xj = hj_ & (L - 1);
-                int ddx = (xj - xi) & (L - 1); if (ddx > L / 2) ddx -= L;   // minimum image, tie -> +L/2
-                dP += ddx;                                                   // step 3b: dP = dx
-                if (lane == 0 && b == 0 && hops_start + hl - log_base < p.log_cap) {
-                    const u64 h = hops_start + hl - log_base;
+            ++e;
+            if (hop) {
+                dP += geo.dx(hi_, hj_);                                  // step 3b: dP = dx
+                const u64 h = hops_start + hc - 1u - log_base;
+                if (lane == 0 && b == 0 && h < p.log_cap) {
                     p.log_a[h] = a_start + used_sum - 1; p.log_i[h] = hi_; p.log_j[h] = hj_;
                 }
-                ++hl;
-                // all slabs of hop hl - DEPTH + 1: the oldest buffer a reader may start from once the NEXT
-                // hop is executed, awaited before that
-                need_pub = hl >= CG_DEPTH ? pub_base + hl - CG_DEPTH + 1 : 0;
             }
-            TS_CTL(9);
-            TRACE(0, 0);
         }
-#ifdef CG_TRACE
-        __syncwarp();
-        if (p.trace) { p.trace[(size_t)b * 64 + lane] += s_seg[lane]; p.trace[(size_t)b * 64 + 32 + lane] += s_seg[32 + lane]; }
-#endif
-#ifdef CG_TRACE_W
-        if (p.trace && lane == 0) for (int k = 0; k < 16; ++k) p.trace[32768 + (size_t)b * 16 + k] = cw[k];
-#endif
+        if (quit) {                       // let the consumers of this CTA go (they see the abort flag in their waits)
+            if (lane == 0) *(volatile u32*)&cm->abort = 1u;
+            return;
+        }
+        // end of the launch: the remaining hops go into the bitmap once every warp is done with it
+        asm volatile("bar.sync 1, %0;" ::"r"(THREADS) : "memory");
+        if (CACHED) for (; e_app < e; ++e_app) apply(e_app);
         if (b == 0 && lane == 0) {
             CgCtl* c = p.ctl;
-            c->attempts = a_start + used_sum; c->hops = hops_start + hl;
-            c->iterations += it_local; c->proposals += (u64)M * it_local;
-            c->dP += dP; c->cur = (u32)((cur0 + hl) % CG_RING); c->epoch += it_local;
-            c->pub_base = pub_base + hl;
+            const u32 ns = n_snaps + ((n_hops & Hm) ? 1u : 0u);
+            c->attempts = a_start + used_sum; c->hops = hops_start + hc;
+            c->iterations += e; c->proposals += (u64)M * e;
+            c->dP += dP; c->cur = (cur0 + ns) % CG_RING; c->epoch += e;
+            c->pub_base = pub_base + ns;
             c->cyc_total += (u64)(clock64() - t_begin);
         }
+        __syncwarp();
+        asm volatile("bar.sync 2, %0;" ::"r"(THREADS) : "memory");
+        if (b == 0) for (u32 w = lane; w < (N + 31) / 32; w += 32) p.nbits[w] = s_n[w];
+        if (csz > 1) cluster_sync_all();  // no CTA leaves while a peer may still post into its shared memory
         return;
-    }
-
-    Slab<TW, RP> slab;
-    slab.load(p.eps[wbuf], pr0, pr1, L, (u32)tid);
-
-    // finish the issued slab update and hand it to the service warp for publication
-    auto finish_update = [&]() {
-        const u32 src = wbuf == 0 ? CG_RING - 1u : wbuf - 1u;
-        slab.finish(tf, mask, L, p.eps[src], p.eps[wbuf], pr0, pr1);
-        if (nb > 1) barN_arrive((u32)((hl - 1) % CG_DEPTH), TB);   // hop hl (1-based) on barrier 1 + (hl - 1) % DEPTH
-        upd = false;
-    };
-
-    // ---------------------------------------------------------------------- worker warps ----
-    // One loop body = outcome of the previous exchange (descriptor) -> table gathers of its hop ->
-    // proposals -> slab update: gathers and update sit in the same body, so the gathers stay in flight
-    // during the whole propose phase.
-#ifdef CG_TRACE_W
-    u64 tw[7] = {}; long long wprev = 0;
-#endif
-    u64 a0 = a_start;                     // first attempt of the window (used when labels are not cached)
-    uint4 d4 = make_uint4(0u, 0u, 0u, 0u);       // used, hop, ci, cj of the previous exchange
-#ifdef CG_TRACE_T
-    u32 itw = 0;
-#endif
-    for (;;) {
-        TS_WRK(7);
-        newhop = d4.y != 0;
-        // the term of the hop executed last iteration for the pair I follow: the four gathers start before the
-        // label bookkeeping (discarded if my attempt was consumed or theta_ij turns out to have changed)
-        double a_i = 0, b_i = 0, a_j = 0, b_j = 0;
-        if (CACHED && tracked && newhop) {
-            a_i = __ldg(tf + ((sci - d4.w) & mask)); b_i = __ldg(tf + ((sci - d4.z) & mask));
-            a_j = __ldg(tf + ((scj - d4.w) & mask)); b_j = __ldg(tf + ((scj - d4.z) & mask));
+    } else {
+        // ------------------------------------------------------------------ worker warps ----
+        // CACHED per-thread state: label of my attempt relative to the window start, the decoded proposal and
+        // what its test needs; the attempt after it, decoded ahead when there is idle time
+        const bool has_label = CACHED && (u32)tid < per;
+        u32 lab = CG_NONE;
+        u64 a_cur = 0;
+        u32 sci = 0, scj = 0, cuh = 0, cul = 0;   // coded sites with the spare bits set
+        double c_invr = 0, c_fld = 0, ei = 0, ej = 0;
+        bool tracked = false;             // ei, ej hold the current local energies of my two sites
+        bool ni = false, nj = false;      // occupations of my two sites
+        Prop nxt = {0, 0, 0, 0, 0};
+        bool nxt_valid = false;
+        u32 hl = 0;                       // hops consumed in this launch
+        auto take = [&](const Prop& q) {
+            cuh = q.uh; cul = q.ul;
+            sci = q.ci | geo.spare; scj = q.cj | geo.spare;
+            c_invr = tb.inv(q.k); c_fld = tb.field(q.k);
+            tracked = false;
+        };
+        // occupations of a pair as of hop hl: the bitmap (complete up to hop nlow, never ahead of me) and the
+        // newer hops replayed in order
+        auto read_n = [&](u32 ci, u32 cj, bool& oi, bool& oj) {
+            const u32 vl = *(volatile u32*)&cm->nlow;
+            __threadfence_block();
+            const u32 si = geo.site(ci), sj = geo.site(cj);
+            bool a = BIT((volatile u32*)s_n, si) != 0u, c = BIT((volatile u32*)s_n, sj) != 0u;
+            for (u32 h = vl + 1u; h <= hl; ++h) {
+                const uint2 k = lds64u(&cm->hops[h % CG_HR][0]);
+                if (ci == k.x) a = false; if (ci == k.y) a = true;
+                if (cj == k.x) c = false; if (cj == k.y) c = true;
+            }
+            oi = a; oj = c;
+        };
+        // local energies of a pair as of hop hl: a snapshot that is complete on every CTA + the newer hops' terms
+        auto read_eps = [&](u32 sc_i, u32 sc_j, double& oi, double& oj) {
+            const u32 v = ld_acquire_cta(&cm->ver);
+            u32 buf = cur0 + v % CG_RING; if (buf >= CG_RING) buf -= CG_RING;
+            const double* __restrict__ erd = p.eps[buf];
+            double a = ld_cg(erd + geo.site(sc_i & mask)), c = ld_cg(erd + geo.site(sc_j & mask));
+            for (u32 h = (v << Hs) + 1u; h <= hl; ++h) {
+                const uint2 k = lds64u(&cm->hops[h % CG_HR][0]);
+                a = __dadd_rn(a, hop_term(tf, mask, sc_i, k.x, k.y));
+                c = __dadd_rn(c, hop_term(tf, mask, sc_j, k.x, k.y));
+            }
+            oi = a; oj = c;
+        };
+        if (has_label) {
+            const u32 g = b * per + (u32)tid, g0 = c_first * per + t0r;
+            lab = g >= g0 ? g - g0 : g + P - g0;
+            a_cur = a_start + lab;
+            take(decode_attempt(tb, p, geo, a_cur));
+            read_n(sci & mask, scj & mask, ni, nj);
         }
-        if (CACHED) {
-            if (has_label && d4.x) {
-                if (lab >= d4.x) lab -= d4.x;
-                else {                              // my attempt was consumed: the next one, P attempts later
-                    lab += P - d4.x; a_cur += P;
-                    // (deferring this decode to the gap between the barriers, for attempts that re-enter far
-                    // outside the window, measured slower: here it hides behind the warps that start to follow
-                    // new pairs)
-                    if (!nxt_valid) nxt = decode_attempt(tb, p, a_cur);
-                    take(nxt); nxt_valid = false;
+
+        Slab<TW, RP> slab;
+        {
+            const u32 c0 = cur0;
+            slab.load(p.eps[c0], p.work, pr0, pr1, geo, (u32)tid);
+        }
+        u64 a0 = a_start;                 // first attempt of the window (used when labels are not cached)
+        bool upd = false, last = false;
+        u32 hci = 0, hcj = 0;
+        double a_i = 0, b_i = 0, a_j = 0, b_j = 0;    // gathers in flight for the followed pair
+        bool addterm = false;
+        u64 t_test = 0, t_slab = 0, t_wait = 0;
+        long long tprev = clock64();
+        for (u32 e = 0;; ++e) {
+            const u32 xs = e % CG_XR, e32 = e_start + e;
+            // ---- steps 1-2: propose and test on S_e, state untouched
+            u32 best = CG_NONE, bi = 0, bj = 0;
+            if (CACHED) {
+                if (has_label) {
+                    const bool th = lab < M && ni && !nj;             // theta_ij, inside the window
+                    if (th) {
+                        if (!tracked) { read_eps(sci, scj, ei, ej); tracked = true; }
+                        else if (addterm) {       // the term of the hop consumed last (gathered below)
+                            ei = __dadd_rn(ei, __dsub_rn(a_i, b_i)); ej = __dadd_rn(ej, __dsub_rn(a_j, b_j));
+                        }
+                        // dH_ij = eps_j - eps_i - 1/r_ij - E dx_ij
+                        const double dE = __dsub_rn(__dsub_rn(__dsub_rn(ej, ei), c_invr), c_fld);
+                        if (metropolis(dE, cuh, cul, p.T, p.inv_T)) { best = lab; bi = sci; bj = scj; }
+                    } else tracked = false;
+                }
+            } else {
+                for (u32 l = lab0 + tid; l < lab1; l += TW) {
+                    const Prop q = decode_attempt(tb, p, geo, a0 + l);
+                    bool oi, oj;
+                    read_n(q.ci, q.cj, oi, oj);
+                    if (!oi || oj) continue;                                     // theta_ij
+                    double vi, vj;
+                    read_eps(q.ci | geo.spare, q.cj | geo.spare, vi, vj);
+                    const double dE = __dsub_rn(__dsub_rn(__dsub_rn(vj, vi), tb.inv(q.k)), tb.field(q.k));
+                    if (metropolis(dE, q.uh, q.ul, p.T, p.inv_T)) { best = l; bi = q.ci; bj = q.cj; break; }
                 }
             }
-        } else a0 += d4.x;
-        if (newhop) {
-            // step 3b: local energies of my slab, into the next buffer of the ring
-            ++hl;
-            hci = d4.z; hcj = d4.w;
-            wbuf = wbuf == CG_RING - 1 ? 0u : wbuf + 1u;
-            upd = true;
-        }
-        if (hl >= p.n_hops) break;
-        TS_WRK(0);
-#ifdef CG_TRACE_W
-        const long long w0 = clock64();
-#endif
-        // ---- steps 1-2: propose and test, state untouched
-        u32 best = CG_NONE, bi = 0, bj = 0;
-        if (CACHED) {
-            const bool th = lab < M && BIT(s_n, ci_) && !BIT(s_n, cj_);   // theta_ij, inside the window
-            if (th) {
-                if (!tracked) {            // start to follow (i, j): complete buffer + all pending hops
-                    const u32 np = s_pend.npend;
-                    const double* __restrict__ erd = p.eps[s_pend.rbuf];
-                    ei = ld_cg(erd + ci_); ej = ld_cg(erd + cj_);
-                    for (u32 k = 0; k < np; ++k) {
-                        const u32 e_ = (s_pend.first + k) % CG_DEPTH;
-                        const u32 ki = s_pend.c[e_][0], kj = s_pend.c[e_][1];
-                        ei = __dadd_rn(ei, hop_term(tf, mask, sci, ki, kj));
-                        ej = __dadd_rn(ej, hop_term(tf, mask, scj, ki, kj));
+            addterm = false;
+            // ---- step 3: lowest accepting label of the warp, for the collector
+            {
+                const u32 wmin = __reduce_min_sync(CG_FULL, best);
+                if (wmin == CG_NONE ? lane == 0 : best == wmin)     // labels are distinct: one lane
+                    sts128(&cm->res[e % (2 * CG_XR)][warp][0], ((u64)e32 << 32) | wmin,
+                           ((u64)geo.site(bi & mask) << 32) | (u64)geo.site(bj & mask));
+            }
+            const long long t1 = clock64();
+            t_test += (u64)(t1 - tprev);
+            // ---- step 3b for my part of the slab: the hop consumed last; behind its gathers the
+            // decode one attempt ahead
+            if (upd) slab.issue(tf, mask, hci, hcj);
+            if (has_label && !nxt_valid) { nxt = decode_attempt(tb, p, geo, a_cur + P); nxt_valid = true; }
+            if (upd) {
+                const bool snap = (hl & Hm) == 0u;
+                u32 buf = cur0 + (hl >> Hs) % CG_RING; if (buf >= CG_RING) buf -= CG_RING;
+                slab.finish(tf, mask, geo, p.work, snap ? p.eps[buf] : nullptr, pr0, pr1);
+                if (snap) {
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive(&cm->pubbar[((hl >> Hs) - 1u) % CG_PB]);
+                }
+                upd = false;
+            }
+            const long long t2 = clock64();
+            t_slab += (u64)(t2 - t1);
+            if (last) break;
+            // ---- O_e
+            if (!mbar_wait(&cm->full[xs], (e / CG_XR) & 1u, p, cm, 8u)) return;
+            const uint4 d = lds128u(&cm->desc[xs]);        // used, flags, ci, cj
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&cm->empty[xs]);
+            tprev = clock64();
+            t_wait += (u64)(tprev - t2);
+            if (d.y & CG_F_ABORT) return;
+            last = (d.y & CG_F_LAST) != 0u;
+            const bool newhop = (d.y & CG_F_HOP) != 0u;
+            if (CACHED) {
+                // the term of this hop for the pair I follow: the four gathers start before the label
+                // bookkeeping (discarded if my attempt was consumed or theta_ij turns out to have changed)
+                if (tracked && newhop) {
+                    a_i = __ldg(tf + ((sci - d.w) & mask)); b_i = __ldg(tf + ((sci - d.z) & mask));
+                    a_j = __ldg(tf + ((scj - d.w) & mask)); b_j = __ldg(tf + ((scj - d.z) & mask));
+                    addterm = true;
+                }
+                if (newhop) {
+                    ++hl; hci = d.z; hcj = d.w; upd = true;
+                    const u32 si = d.z | geo.spare, sj = d.w | geo.spare;
+                    if (sci == si) ni = false; if (sci == sj) ni = true;
+                    if (scj == si) nj = false; if (scj == sj) nj = true;
+                }
+                if (has_label && d.x) {
+                    if (lab >= d.x) lab -= d.x;
+                    else {                              // my attempt was consumed: the next one, P attempts later
+                        lab += P - d.x; a_cur += P;
+                        if (!nxt_valid) nxt = decode_attempt(tb, p, geo, a_cur);
+                        take(nxt); nxt_valid = false;
+                        addterm = false;
+                        read_n(sci & mask, scj & mask, ni, nj);
                     }
-                    tracked = true;
-                } else if (newhop) {       // the term of the hop executed last iteration (gathered above)
-                    ei = __dadd_rn(ei, __dsub_rn(a_i, b_i)); ej = __dadd_rn(ej, __dsub_rn(a_j, b_j));
                 }
-                // dH_ij = eps_j - eps_i - 1/r_ij - E dx_ij
-                const double dE = __dsub_rn(__dsub_rn(__dsub_rn(ej, ei), c_invr), c_fld);
-                if (metropolis(dE, cuh, cul, p.T, p.inv_T)) { best = lab; bi = ci_; bj = cj_; }
-            } else tracked = false;
-        } else {
-            const u32 np = s_pend.npend;
-            const double* __restrict__ erd = p.eps[s_pend.rbuf];
-            for (u32 l = lab0 + tid; l < lab1; l += TW) {
-                const u64 a = a0 + l;
-                u32 w0, w1, w2, w3;
-                philox4x32_10((u32)a, (u32)(a >> 32), 0u, 0u, p.seed_lo, p.seed_hi, w0, w1, w2, w3);
-                const u32 i = __umulhi(w0, N);                                   // uniform site
-                if (!BIT(s_n, i)) continue;                                      // n_i = 1 ?
-                const u32 k = tower_search(tb, ((u64)w1 << 11) | (u64)(w2 >> 21));
-                const u32 j = hop_target(tb, i, k, L, lg);
-                if (BIT(s_n, j)) continue;                                       // n_j = 0 ?
-                double vi = ld_cg(erd + i), vj = ld_cg(erd + j);
-                const u32 si = site_code(i, L) | (u32)L, sj = site_code(j, L) | (u32)L;
-                for (u32 t = 0; t < np; ++t) {
-                    const u32 e_ = (s_pend.first + t) % CG_DEPTH;
-                    const u32 ki = s_pend.c[e_][0], kj = s_pend.c[e_][1];
-                    vi = __dadd_rn(vi, hop_term(tf, mask, si, ki, kj));
-                    vj = __dadd_rn(vj, hop_term(tf, mask, sj, ki, kj));
-                }
-                const double dE = __dsub_rn(__dsub_rn(__dsub_rn(vj, vi), s_invr[k]), s_fld[k]);
-                if (metropolis(dE, w2 & 0x1FFFFFu, w3, p.T, p.inv_T)) { best = l; bi = i; bj = j; break; }
+            } else {
+                a0 += d.x;
+                if (newhop) { ++hl; hci = d.z; hcj = d.w; upd = true; }
             }
         }
-        TS_WRK(1);
-#ifdef CG_TRACE_W
-        const long long w1 = clock64();
-#endif
-        // ---- step 3: lowest accepting label: warp, then the control warp
-        {
-            const u32 wmin = __reduce_min_sync(CG_FULL, best);
-            if (wmin != CG_NONE && best == wmin) {     // labels are distinct: one lane
-                s_wpay[warp] = ((u64)bi << 32) | (u64)bj;
-                atomicMin(&s_key, (wmin << 5) | (u32)warp);
-            }
+        // the final state of my part of the slab, unless the last hop was a snapshot anyway
+        if (n_hops & Hm) {
+            u32 buf = cur0 + (n_snaps + 1u) % CG_RING; if (buf >= CG_RING) buf -= CG_RING;
+            slab.flush(p.work, p.eps[buf], pr0, pr1);
         }
-        TS_WRK(2);
-#ifdef CG_TRACE_W
-        const long long w2 = clock64();
-#endif
-        barX_arrive(TB);                  // [A] only the control warp waits here: the workers go on to their slabs
-        TS_WRK(3);
-#ifdef CG_TRACE_W
-        const long long w3 = clock64();
-#endif
-        // while the control warp does the exchange: the slab of the previous hop (its table gathers,
-        // issued when that hop was executed, have had the whole propose phase to arrive) and, if another
-        // CTA holds the start of the window, the decode one attempt ahead
-        if (upd) slab.issue(tf, mask, pr0, pr1, hci, hcj);
-        if (has_label && !nxt_valid) { nxt = decode_attempt(tb, p, a_cur + P); nxt_valid = true; }   // behind the gathers
-        if (upd) finish_update();
-        TS_WRK(4);
-#ifdef CG_TRACE_W
-        const long long w4 = clock64();
-#endif
-        barB_sync(TB);                    // [B] the control warp has written the descriptor
-        TS_WRK(5);
-#ifdef CG_TRACE_W
-        {
-            const long long w5 = clock64();
-            tw[0] += (u64)(w1 - w0); tw[1] += (u64)(w2 - w1); tw[2] += (u64)(w3 - w2); tw[3] += (u64)(w4 - w3); tw[4] += (u64)(w5 - w4);
-            if (wprev) tw[5] += (u64)(w0 - wprev);
-            wprev = w5; ++tw[6];
+        if (b == 0 && lane == 0) {
+            atomicAdd(&p.ctl->cyc_propose, t_test); atomicAdd(&p.ctl->cyc_update, t_slab);
+            atomicAdd(&p.ctl->cyc_wait, t_wait); atomicAdd(&p.ctl->cyc_warps, 1ull);
         }
-#endif
-        d4 = *reinterpret_cast<const uint4*>(&s_desc);      // used, hop, ci, cj
-        ahead = s_desc.ahead != 0;
-        TS_WRK(6);
-#ifdef CG_TRACE_T
-        ++itw;
-#endif
     }
-#ifdef CG_TRACE_W
-    if (p.trace && lane == 0) for (int k = 0; k < 7; ++k) p.trace[((size_t)b * 16 + warp) * 8 + k] = tw[k];
-#endif
-    if (upd) { slab.issue(tf, mask, pr0, pr1, hci, hcj); finish_update(); }
-    if (b == 0)
-        for (u32 w = tid; w < (N + 31) / 32; w += TW) p.nbits[w] = s_n[w];
+    // every warp but the exchange warp: the two barriers of the end of the launch (skipped when it was abandoned:
+    // the exchange warp is then not there)
+    if (*(volatile u32*)&cm->abort) return;
+    asm volatile("bar.sync 1, %0;" ::"r"(THREADS) : "memory");
+    asm volatile("bar.sync 2, %0;" ::"r"(THREADS) : "memory");
+    if (csz > 1) cluster_sync_all();
 }
 
-template <int THREADS, int RP, bool CACHED>
-__global__ void __launch_bounds__(THREADS, 1) cg_pr_persistent(const CgParams p)
+template <int NW, int RP, bool CACHED>
+__global__ void __launch_bounds__(NW * 32 + 96, 1) cg_pr_persistent(const CgParams p)
 {
-    pr_persistent_body<THREADS, RP, CACHED>(p, blockIdx.x, gridDim.x);
+    pr_persistent_body<NW, RP, CACHED>(p, blockIdx.x, gridDim.x);
 }
 
 // Replica packing (the paper recommends averaging many samples): ONE launch,
 // CTAs [first[s], first[s+1]) run sim s with its own parameter block.  The sims share nothing.
-template <int THREADS, int RP, bool CACHED>
-__global__ void __launch_bounds__(THREADS, 1)
+template <int NW, int RP, bool CACHED>
+__global__ void __launch_bounds__(NW * 32 + 96, 1)
 cg_pr_persistent_many(const CgParams* __restrict__ ps, const u32* __restrict__ first, const u32 n_sims)
 {
     __shared__ CgParams sp;
@@ -905,7 +1058,13 @@ cg_pr_persistent_many(const CgParams* __restrict__ ps, const u32* __restrict__ f
         sp = ps[s];
     }
     __syncthreads();
-    pr_persistent_body<THREADS, RP, CACHED>(sp, s_b, s_nb);
+    pr_persistent_body<NW, RP, CACHED>(sp, s_b, s_nb);
+}
+
+__device__ __forceinline__ Geo make_geo(const CgParams& p)
+{
+    const Geo g = {p.hi1, p.hi2, p.spare, p.mask, (u32)(p.L - 1), p.lgL};
+    return g;
 }
 
 // Step a6 alone: scripted hops, update in place (no readers), one launch.
@@ -914,16 +1073,15 @@ __global__ void __launch_bounds__(THREADS, 1)
 cg_update_scripted(const CgParams p, const u32* __restrict__ hop_i, const u32* __restrict__ hop_j, u64 count)
 {
     const u32 b = blockIdx.x, nb = gridDim.x;
-    const int L = p.L;
-    const u32 mask = ((u32)(L - 1) << (p.lgL + 1)) | (u32)(L - 1);
+    const Geo geo = make_geo(p);
     const u32 pairs = p.N / 2, pper = (pairs + nb - 1) / nb;
     const u32 pr0 = min(pairs, b * pper), pr1 = min(pairs, pr0 + pper);
     double* e = p.eps[p.ctl->cur];
     Slab<THREADS, RP> slab;
-    slab.load(e, pr0, pr1, L, threadIdx.x);
+    slab.load(e, e, pr0, pr1, geo, threadIdx.x);
     for (u64 h = 0; h < count; ++h) {
-        slab.issue(p.tf, mask, pr0, pr1, site_code(__ldg(hop_i + h), L), site_code(__ldg(hop_j + h), L));
-        slab.finish(p.tf, mask, L, e, e, pr0, pr1);
+        slab.issue(p.tf, p.mask, geo.code(__ldg(hop_i + h)), geo.code(__ldg(hop_j + h)));
+        slab.finish(p.tf, p.mask, geo, e, e, pr0, pr1);
     }
     if (b == 0 && threadIdx.x == 0) {       // occupations and dipole moment, in hop order
         long long dP = p.ctl->dP; u32 bad = 0;
@@ -933,25 +1091,27 @@ cg_update_scripted(const CgParams p, const u32* __restrict__ hop_i, const u32* _
             if (!((wi >> (i & 31)) & 1u) || ((wj >> (j & 31)) & 1u)) ++bad;
             p.nbits[i >> 5] &= ~(1u << (i & 31));
             p.nbits[j >> 5] |= (1u << (j & 31));
-            int ddx = ((int)(j & (L - 1)) - (int)(i & (L - 1))) & (L - 1); if (ddx > L / 2) ddx -= L;
-            dP += ddx;
+            dP += geo.dx(i, j);
         }
         p.ctl->dP = dP; p.ctl->hops += count; p.ctl->bad_hops += bad;
     }
 }
 
-// tf from the quarter table (one-time set-up)
-__global__ void cg_build_tf(const double* __restrict__ tq, double* __restrict__ tf, int L, int pitch)
+// ---- one-time set-up (step a0) --------------------------------------------------------------
+
+// tf from the folded table: entry (dz, dy, dx) of the unfolded index space (fields of width 2L)
+__global__ void cg_build_tf(const double* __restrict__ tq, double* __restrict__ tf, int L, int lg, int Lz, int pitch, u32 total)
 {
-    const int dy = blockIdx.x;
-    const int fy = min(dy, L - dy);
-    for (int dx = threadIdx.x; dx <= L; dx += blockDim.x) {
-        const int w = dx & (L - 1), fx = min(w, L - w);
-        tf[(size_t)dy * 2 * L + dx] = tq[fy * pitch + fx];
+    for (u32 idx = blockIdx.x * blockDim.x + threadIdx.x; idx < total; idx += gridDim.x * blockDim.x) {
+        const int dx = idx & (2 * L - 1), dy = (idx >> (lg + 1)) & (2 * L - 1), dz = idx >> (2 * lg + 2);
+        double v = 0.0;
+        if (dx < L && dy < L && dz < Lz) {
+            const int fx = min(dx, L - dx), fy = min(dy, L - dy), fz = min(dz, Lz - dz);
+            v = tq[((size_t)fz * pitch + fy) * pitch + fx];
+        }
+        tf[idx] = v;
     }
 }
-
-// ---- one-time set-up (step a0) --------------------------------------------------------------
 
 // phi_s = (u - 1/2) W with u from Philox domain 1; occupation key from domain 2.
 __global__ void cg_init_phi_keys(double* phi, u64* keys, u32 N, double W, u32 seed_lo, u32 seed_hi)
@@ -989,22 +1149,25 @@ __global__ void cg_init_occupations(const u64* __restrict__ keys, u32* nbits, u3
 // eps_s = phi_s + sum_{t != s} (n_t - 1/2)/r_st in index order t.
 __global__ void cg_full_sum_eps(const double* __restrict__ phi, const u32* __restrict__ nbits,
                                 const double* __restrict__ tq, double* __restrict__ out,
-                                int L, int lg, int pitch, u32 N)
+                                int L, int lg, int Lz, int pitch, u32 N)
 {
     const u32 s = blockIdx.x * blockDim.x + threadIdx.x;
     if (s >= N) return;
-    const int y = s >> lg, x = s & (L - 1);
+    const int z = s >> (2 * lg), y = (s >> lg) & (L - 1), x = s & (L - 1);
     double e = phi[s];
     u32 word = 0;
-    for (int yt = 0; yt < L; ++yt) {
-        int dy = (y - yt) & (L - 1); dy = min(dy, L - dy);
-        const double* row = tq + dy * pitch;
-        for (int xt = 0; xt < L; ++xt) {
-            const u32 t = ((u32)yt << lg) | (u32)xt;
-            if ((t & 31u) == 0u || xt == 0) word = __ldg(nbits + (t >> 5));
-            int dx = (x - xt) & (L - 1); dx = min(dx, L - dx);
-            const double half = __dmul_rn(0.5, __ldg(row + dx));  // exact; 0 on the diagonal
-            e = ((word >> (t & 31u)) & 1u) ? __dadd_rn(e, half) : __dsub_rn(e, half);
+    for (int zt = 0; zt < Lz; ++zt) {
+        int dz = (z - zt) & (Lz - 1); dz = min(dz, Lz - dz);
+        for (int yt = 0; yt < L; ++yt) {
+            int dy = (y - yt) & (L - 1); dy = min(dy, L - dy);
+            const double* row = tq + ((size_t)dz * pitch + dy) * pitch;
+            for (int xt = 0; xt < L; ++xt) {
+                const u32 t = ((((u32)zt << lg) | (u32)yt) << lg) | (u32)xt;
+                if ((t & 31u) == 0u || xt == 0) word = __ldg(nbits + (t >> 5));
+                int dx = (x - xt) & (L - 1); dx = min(dx, L - dx);
+                const double half = __dmul_rn(0.5, __ldg(row + dx));  // exact; 0 on the diagonal
+                e = ((word >> (t & 31u)) & 1u) ? __dadd_rn(e, half) : __dsub_rn(e, half);
+            }
         }
     }
     out[s] = e;
@@ -1019,47 +1182,70 @@ __global__ void cg_max_abs_diff(const double* a, const double* b, u32 N, u64* ou
     if ((threadIdx.x & 31) == 0) atomicMax(out_bits, (u64)__double_as_longlong(m)); // m >= 0
 }
 
-// L2 roofline probe: L1-bypassing 16-byte read-modify-write over a resident buffer.
-__global__ void __launch_bounds__(512) cg_l2_rmw(double2* buf, size_t n16, int reps)
+// L2 roofline probes: L1-bypassing accesses over a resident buffer, `reps` passes inside one launch.
+// mode 0: read-modify-write, 1: read only (the sum is kept alive through `sink`), 2: write only;
+// VEC = 16 or 32 bytes per access.
+template <int VEC>
+__global__ void cg_l2_probe(double* buf, size_t nvec, int reps, int mode, double* sink)
 {
     const size_t stride = (size_t)gridDim.x * blockDim.x;
+    double acc = 0.0;
     for (int r = 0; r < reps; ++r)
-        for (size_t k = (size_t)blockIdx.x * blockDim.x + threadIdx.x; k < n16; k += stride) {
-            double2 v = __ldcg(buf + k);
-            v.x += 1.0; v.y -= 1.0;
-            __stcg(buf + k, v);
+        for (size_t k = (size_t)blockIdx.x * blockDim.x + threadIdx.x; k < nvec; k += stride) {
+            if (VEC == 16) {
+                double2* q = reinterpret_cast<double2*>(buf) + k;
+                double2 v = make_double2((double)r, 1.0);
+                if (mode != 2) v = __ldcg(q);
+                if (mode == 1) acc += v.x + v.y;
+                else { v.x += 1.0; v.y -= 1.0; __stcg(q, v); }
+            } else {
+                double* q = buf + 4 * k;
+                double a = (double)r, b = 1.0, c = 2.0, d = 3.0;
+                if (mode != 2)
+                    asm volatile("ld.global.cg.v4.f64 {%0, %1, %2, %3}, [%4];" : "=d"(a), "=d"(b), "=d"(c), "=d"(d) : "l"(q) : "memory");
+                if (mode == 1) acc += (a + b) + (c + d);
+                else {
+                    a += 1.0; b -= 1.0; c += 1.0; d -= 1.0;
+                    asm volatile("st.global.cg.v4.f64 [%0], {%1, %2, %3, %4};" ::"l"(q), "d"(a), "d"(b), "d"(c), "d"(d) : "memory");
+                }
+            }
         }
+    if (mode == 1 && acc == 123.456) *sink = acc;
 }
 
 // -------------------------------------------------------------------- host --
 
 struct cg_sim {
-    int L = 0, lgL = 0, pitch = 0;
+    int dim = 2, L = 0, Lz = 1, lgL = 0, pitch = 0;
     u32 N = 0, M = 0;
     double W = 0, xi = 0, T = 0, E = 0;
     u64 seed = 0;
     // host tables (live part of the tower)
     int64_t K = 0, Klive = 0;
-    std::vector<int32_t> dy, dx;
+    std::vector<int32_t> dz, dy, dx;
     std::vector<double> cdf, invr_k, fld_k;
     std::vector<u64> cdfi;
     std::vector<u32> guide;
     double S = 0, Gamma = 0;
+    u32 hi1 = 0, hi2 = 0, spare = 0, mask = 0, tf_len = 0;
     // device
+    int device = 0;
     cudaStream_t stream = nullptr;
     void* ws = nullptr; bool own_ws = false;
     double* d_eps[CG_RING] = {};
-    double* d_scratch = nullptr; double* d_phi = nullptr;
+    double* d_work = nullptr; double* d_scratch = nullptr; double* d_phi = nullptr;
     u32* d_nbits = nullptr; double* d_tq = nullptr; double* d_tf = nullptr;
-    u64* d_cdfi = nullptr; double* d_invr_k = nullptr; double* d_fld_k = nullptr; int* d_disp = nullptr;
+    u64* d_cdfi = nullptr; double* d_invr_k = nullptr; double* d_fld_k = nullptr; u32* d_disp = nullptr;
     u32* d_guide = nullptr;
     u64* d_slots = nullptr; CgCtl* d_ctl = nullptr; u64* d_red = nullptr;
     void* d_log = nullptr; bool own_log = false; u64 log_cap = 0;
     bool log_gap = false;                 // scripted hops (cg_apply_hops) were executed while the log was on: it no longer holds every hop
-    u64* d_trace = nullptr; u32 trace_iters = 0;
     void* d_many = nullptr; size_t many_cap = 0;      // parameter blocks of cg_run_many (owned by its first sim)
-    // launch shape
+    // launch shape and tuning
     int num_sms = 0, n_ctas = 0, threads = 0, smem = 0, rp = 0, pl = 0;   // pl > 0: cached proposals
+    int snap_shift = 2;                   // snapshots every 4 hops
+    int cluster = 1;                      // CTAs per thread-block cluster
+    u64 watchdog_ns = 10ull * 1000 * 1000 * 1000;
     std::string err;
 };
 
@@ -1077,31 +1263,37 @@ static int fail_cuda(cg_sim* s, cudaError_t e, const char* what)
 
 static size_t align256(size_t v) { return (v + 255) & ~(size_t)255; }
 
-static bool valid_L(int L, int* lg)
+// supported lattices: L a power of two, 2D 4..1024, 3D 4..64 (N <= 2^20: the occupation bitmap of the whole
+// lattice lives in every CTA's shared memory)
+static bool valid_L(int dim, int L, int* lg)
 {
-    if (L < 4 || L > 1024 || (L & (L - 1))) return false;
+    if (L < 4 || L > (dim == 3 ? 64 : 1024) || (L & (L - 1))) return false;
     int k = 0; while ((1 << k) < L) ++k;
     if (lg) *lg = k;
     return true;
 }
 
-struct WsLayout { size_t eps0, scratch, phi, nbits, tq, tf, cdfi, invr_k, fld_k, disp, guide, slots, ctl, red, total; };
+struct WsLayout { size_t eps0, work, scratch, phi, nbits, tq, tf, cdfi, invr_k, fld_k, disp, guide, slots, ctl, red, total; };
 #define CG_SLOT_BYTES ((size_t)8 * CG_SLOT_U64 * CG_MAX_CTAS)
 
-static WsLayout ws_layout(int L)
+static WsLayout ws_layout(int dim, int L)
 {
-    const size_t N = (size_t)L * L, h = (size_t)L / 2 + 1;
+    const size_t N = dim == 3 ? (size_t)L * L * L : (size_t)L * L;
+    const size_t h = (size_t)L / 2 + 1, hz = dim == 3 ? h : 1;
+    const size_t tf_len = dim == 3 ? 4 * N : 2 * N;     // index space of the unfolded table (fields of width 2L)
+    const size_t kcap = std::min<size_t>(N, 65536);     // the live tower is capped at 65535 entries
     WsLayout w; size_t o = 0;
     w.eps0 = o; o += CG_RING * align256(8 * N);
+    w.work = o; o += align256(8 * N);
     w.scratch = o; o += align256(8 * N);
     w.phi = o; o += align256(8 * N);
     w.nbits = o; o += align256(N / 8 + 4);
-    w.tq = o; o += align256(8 * h * h);
-    w.tf = o; o += align256(16 * N);
-    w.cdfi = o; o += align256(8 * N);           // tower can never be longer than N entries
-    w.invr_k = o; o += align256(8 * N);
-    w.fld_k = o; o += align256(8 * N);
-    w.disp = o; o += align256(4 * N);
+    w.tq = o; o += align256(8 * hz * h * h);
+    w.tf = o; o += align256(8 * tf_len);
+    w.cdfi = o; o += align256(8 * kcap);
+    w.invr_k = o; o += align256(8 * kcap);
+    w.fld_k = o; o += align256(8 * kcap);
+    w.disp = o; o += align256(4 * kcap);
     w.guide = o; o += align256(4 * CG_GUIDE);
     w.slots = o; o += align256(CG_SLOT_BYTES);
     w.ctl = o; o += align256(sizeof(CgCtl));
@@ -1113,23 +1305,35 @@ static WsLayout ws_layout(int L)
 extern "C" size_t cg_workspace_bytes(int L, uint32_t M)
 {
     (void)M;
-    if (!valid_L(L, nullptr)) return 0;
-    return ws_layout(L).total;
+    if (!valid_L(2, L, nullptr)) return 0;
+    return ws_layout(2, L).total;
 }
+
+extern "C" size_t cg_workspace_bytes3(int L, uint32_t M)
+{
+    (void)M;
+    if (!valid_L(3, L, nullptr)) return 0;
+    return ws_layout(3, L).total;
+}
+
+static u32 host_code(const cg_sim* s, u32 site) { return site + (site & s->hi1) + ((site & s->hi2) << 1); }
 
 // Displacement list, tower and Gamma on the host.
 static void build_tables(cg_sim* s, std::vector<double>& tq)
 {
-    const int L = s->L, h = L / 2;
-    struct D { long long r2; int dy, dx; };
+    const int L = s->L, h = L / 2, Lz = s->Lz;
+    struct D { long long r2; int dz, dy, dx; };
     std::vector<D> d;
-    for (int dy = -h + 1; dy <= h; ++dy)
-        for (int dx = -h + 1; dx <= h; ++dx) {
-            const long long r2 = (long long)dy * dy + (long long)dx * dx;
-            if (r2 > 0 && r2 <= (long long)h * h) d.push_back({r2, dy, dx});
-        }
+    const int zlo = Lz == 1 ? 0 : -h + 1, zhi = Lz == 1 ? 0 : h;
+    for (int dz = zlo; dz <= zhi; ++dz)
+        for (int dy = -h + 1; dy <= h; ++dy)
+            for (int dx = -h + 1; dx <= h; ++dx) {
+                const long long r2 = (long long)dz * dz + (long long)dy * dy + (long long)dx * dx;
+                if (r2 > 0 && r2 <= (long long)h * h) d.push_back({r2, dz, dy, dx});
+            }
     std::sort(d.begin(), d.end(), [](const D& a, const D& b) {
         if (a.r2 != b.r2) return a.r2 < b.r2;
+        if (a.dz != b.dz) return a.dz < b.dz;
         if (a.dy != b.dy) return a.dy < b.dy;
         return a.dx < b.dx;
     });
@@ -1149,10 +1353,10 @@ static void build_tables(cg_sim* s, std::vector<double>& tq)
         if (c >= 1.0) { live = k + 1; break; }
     }
     s->Klive = (int64_t)live;
-    s->dy.resize(live); s->dx.resize(live); s->cdf.resize(live); s->invr_k.resize(live);
+    s->dz.resize(live); s->dy.resize(live); s->dx.resize(live); s->cdf.resize(live); s->invr_k.resize(live);
     s->fld_k.resize(live); s->cdfi.resize(live);
     for (size_t k = 0; k < live; ++k) {
-        s->dy[k] = d[k].dy; s->dx[k] = d[k].dx;
+        s->dz[k] = d[k].dz; s->dy[k] = d[k].dy; s->dx[k] = d[k].dx;
         s->cdf[k] = (k + 1 == K) ? 1.0 : run[k] / acc;
         s->invr_k[k] = 1.0 / std::sqrt((double)d[k].r2);
         s->fld_k[k] = s->E * (double)d[k].dx;              // the field term of dH
@@ -1162,8 +1366,10 @@ static void build_tables(cg_sim* s, std::vector<double>& tq)
     // of two and ceil are exact in double)
     for (size_t k = 0; k < live; ++k) s->cdfi[k] = (u64)std::ceil(std::ldexp(s->cdf[k], 43));
     // Guide over t = 2^43 - m: bucket = (binade of t, next 3 bits).  The tail of the tower is geometric
-    // in r, so every bucket brackets only a few k; both ends found by the plain search.
-    auto kstar = [&](u64 m) { size_t k = 0; while (!(m < s->cdfi[k])) ++k; return (u32)k; };
+    // in r, so every bucket brackets only a few k; both ends found by bisection.
+    auto kstar = [&](u64 m) {
+        return (u32)(std::upper_bound(s->cdfi.begin(), s->cdfi.end(), m) - s->cdfi.begin());   // smallest k with m < cdfi_k
+    };
     s->guide.assign(CG_GUIDE, 0u);
     for (int e = 0; e <= 43; ++e)
         for (int mant = 0; mant < 8; ++mant) {
@@ -1176,24 +1382,39 @@ static void build_tables(cg_sim* s, std::vector<double>& tq)
             const u32 klo = kstar(top - thi), khi = kstar(top - tlo);
             s->guide[(size_t)e * 8 + mant] = klo | (khi << 16);
         }
-    const int pitch = s->pitch;
-    tq.assign((size_t)pitch * pitch, 0.0);
-    for (int a = 0; a <= h; ++a)
-        for (int b = 0; b <= h; ++b) {
-            const long long r2 = (long long)a * a + (long long)b * b;
-            tq[(size_t)a * pitch + b] = r2 ? 1.0 / std::sqrt((double)r2) : 0.0;
-        }
+    const int pitch = s->pitch, hz = Lz == 1 ? 1 : pitch;
+    tq.assign((size_t)hz * pitch * pitch, 0.0);
+    for (int c = 0; c < hz; ++c)
+        for (int a = 0; a <= h; ++a)
+            for (int b = 0; b <= h; ++b) {
+                const long long r2 = (long long)c * c + (long long)a * a + (long long)b * b;
+                tq[((size_t)c * pitch + a) * pitch + b] = r2 ? 1.0 / std::sqrt((double)r2) : 0.0;
+            }
 }
 
 static size_t smem_bytes(const cg_sim* s)
 {
-    return (size_t)s->Klive * 28 + 4 * CG_GUIDE + 4 * (((size_t)s->N + 31) / 32) + 16;
+    const size_t ks = (size_t)std::min<int64_t>(s->Klive, CG_KS);
+    return ks * 28 + 4 * CG_GUIDE + 4 * (((size_t)s->N + 31) / 32) + 16;
 }
 
-static CgParams make_params(const cg_sim* s, u64 n_hops)
+// hops between snapshots -> gate distance G with CG_RING H > 2 G + 2 H - 2 (pr_persistent_body, "Snapshots")
+static u32 gate_for(int snap_shift)
+{
+    static const u32 g[4] = {5, 8, 8, 16};
+    return g[snap_shift];
+}
+static_assert(CG_RING * 1 > 2 * 5 + 2 * 1 - 2 && CG_RING * 2 > 2 * 8 + 2 * 2 - 2 && CG_RING * 4 > 2 * 8 + 2 * 4 - 2
+              && CG_RING * 8 > 2 * 16 + 2 * 8 - 2, "snapshot ring too short for the gate");
+static_assert(CG_HR > CG_XR + 16 + CG_MAX_SNAP - 1, "hop ring too short");
+static_assert(CG_SRING > 16 + CG_MAX_SNAP + CG_XR, "slot ring too short");
+static_assert(CG_PB > 16 / CG_MAX_SNAP + 1 && CG_PB > 5 + 1, "publication barriers");
+
+static CgParams make_params(const cg_sim* s, u32 n_hops)
 {
     CgParams p;
     for (int k = 0; k < CG_RING; ++k) p.eps[k] = s->d_eps[k];
+    p.work = s->d_work;
     p.tf = s->d_tf; p.tq = s->d_tq; p.nbits = s->d_nbits;
     p.cdfi = s->d_cdfi; p.invr_k = s->d_invr_k; p.fld_k = s->d_fld_k; p.disp = s->d_disp;
     p.guide = s->d_guide;
@@ -1202,37 +1423,45 @@ static CgParams make_params(const cg_sim* s, u64 n_hops)
     p.log_i = s->d_log ? (u32*)((char*)s->d_log + 8 * s->log_cap) : nullptr;
     p.log_j = s->d_log ? (u32*)((char*)s->d_log + 12 * s->log_cap) : nullptr;
     p.log_cap = s->d_log ? s->log_cap : 0;
-    p.L = s->L; p.lgL = s->lgL; p.pitch = s->pitch; p.Klive = (int)s->Klive;
+    p.L = s->L; p.lgL = s->lgL; p.Klive = (int)s->Klive; p.Ksm = (int)std::min<int64_t>(s->Klive, CG_KS);
+    p.hi1 = s->hi1; p.hi2 = s->hi2; p.spare = s->spare; p.mask = s->mask;
     p.N = s->N; p.M = s->M; p.PL = (u32)s->pl;
     p.seed_lo = (u32)s->seed; p.seed_hi = (u32)(s->seed >> 32);
     p.T = s->T; p.E = s->E; p.inv_T = (float)(1.0 / s->T); p.n_hops = n_hops;
-    p.trace = s->d_trace; p.trace_iters = s->trace_iters;
+    p.snap_shift = (u32)s->snap_shift; p.gate = gate_for(s->snap_shift);
+    p.cluster = (u32)s->cluster; p.watchdog_ns = s->watchdog_ns;
     return p;
 }
 
 typedef void (*persist_fn)(const CgParams);
 typedef void (*scripted_fn)(const CgParams, const u32*, const u32*, u64);
 
-// RP = eps pairs a thread keeps in registers (0: the slab streams through global memory)
-template <int THREADS, bool CACHED>
+// RP = eps pairs a thread keeps in registers (0: the slab lives in a working buffer in global memory)
+template <int NW, bool CACHED>
 static persist_fn persistent_kernel_t(int rp)
 {
     switch (rp) {
-        case 0: return cg_pr_persistent<THREADS, 0, CACHED>;
-        case 1: return cg_pr_persistent<THREADS, 1, CACHED>;
-        case 2: return cg_pr_persistent<THREADS, 2, CACHED>;
-        case 4: return cg_pr_persistent<THREADS, 4, CACHED>;
-        case 8: return cg_pr_persistent<THREADS, 8, CACHED>;
+        case 0: return cg_pr_persistent<NW, 0, CACHED>;
+        case 1: return cg_pr_persistent<NW, 1, CACHED>;
+        case 2: return cg_pr_persistent<NW, 2, CACHED>;
+        case 4: if (NW <= 16) return cg_pr_persistent<NW <= 16 ? NW : 5, 4, CACHED>; break;
+        case 8: if (NW <= 14) return cg_pr_persistent<NW <= 14 ? NW : 5, 8, CACHED>; break;
     }
     return nullptr;
 }
+// threads per CTA = 32 (worker warps + 3): 256 (5), 544 (14), 608 (16), 1024 (29)
+static int workers_of(int threads)
+{
+    switch (threads) { case 256: return 5; case 544: return 14; case 608: return 16; case 1024: return 29; }
+    return 0;
+}
 static persist_fn persistent_kernel(int threads, int rp, bool cached)
 {
-    switch (threads) {
-        case 256: return cached ? persistent_kernel_t<256, true>(rp) : persistent_kernel_t<256, false>(rp);
-        case 512: return cached ? persistent_kernel_t<512, true>(rp) : persistent_kernel_t<512, false>(rp);
-        case 1024: if (rp > 2) return nullptr;
-                   return cached ? persistent_kernel_t<1024, true>(rp) : persistent_kernel_t<1024, false>(rp);
+    switch (workers_of(threads)) {
+        case 5: return cached ? persistent_kernel_t<5, true>(rp) : persistent_kernel_t<5, false>(rp);
+        case 14: return cached ? persistent_kernel_t<14, true>(rp) : persistent_kernel_t<14, false>(rp);
+        case 16: return cached ? persistent_kernel_t<16, true>(rp) : persistent_kernel_t<16, false>(rp);
+        case 29: return cached ? persistent_kernel_t<29, true>(rp) : persistent_kernel_t<29, false>(rp);
     }
     return nullptr;
 }
@@ -1241,17 +1470,17 @@ template <bool CACHED>
 static many_fn many_kernel_t(int rp)
 {
     switch (rp) {
-        case 0: return cg_pr_persistent_many<512, 0, CACHED>;
-        case 1: return cg_pr_persistent_many<512, 1, CACHED>;
-        case 2: return cg_pr_persistent_many<512, 2, CACHED>;
-        case 4: return cg_pr_persistent_many<512, 4, CACHED>;
-        case 8: return cg_pr_persistent_many<512, 8, CACHED>;
+        case 0: return cg_pr_persistent_many<14, 0, CACHED>;
+        case 1: return cg_pr_persistent_many<14, 1, CACHED>;
+        case 2: return cg_pr_persistent_many<14, 2, CACHED>;
+        case 4: return cg_pr_persistent_many<14, 4, CACHED>;
+        case 8: return cg_pr_persistent_many<14, 8, CACHED>;
     }
     return nullptr;
 }
 static many_fn many_kernel(int threads, int rp, bool cached)
 {
-    if (threads != 512) return nullptr;
+    if (threads != 544) return nullptr;
     return cached ? many_kernel_t<true>(rp) : many_kernel_t<false>(rp);
 }
 static scripted_fn scripted_kernel(int rp)
@@ -1266,67 +1495,85 @@ static scripted_fn scripted_kernel(int rp)
     return nullptr;
 }
 
-// smallest supported register tiling that holds `pairs` pairs per CTA, else 0 (streaming)
-static int choose_rp(u64 pairs, int n_ctas, int threads)
+// smallest supported register tiling that holds `pairs` pairs per CTA on `workers` threads, else 0
+static int choose_rp(u64 pairs, int n_ctas, int workers, int cap)
 {
     const u64 per_cta = (pairs + n_ctas - 1) / n_ctas;
-    const u64 workers = (u64)threads - 64;               // the last two warps of a CTA hold no eps
     const u64 need = (per_cta + workers - 1) / workers;
-    const int cap = threads == 1024 ? 2 : 8;
     for (int rp = 1; rp <= cap; rp *= 2)
         if ((u64)rp >= need) return rp;
     return 0;
 }
+static int rp_cap(int threads) { return threads == 1024 ? 2 : threads == 608 ? 4 : 8; }
 
+// how many CTAs of this shape can be co-resident (in clusters of s->cluster)
 static int max_coresident(cg_sim* s, int threads, int rp, bool cached, int* out)
 {
     persist_fn f = persistent_kernel(threads, rp, cached);
     if (!f) return CG_EINVAL;
     CK(cudaFuncSetAttribute((const void*)f, cudaFuncAttributeMaxDynamicSharedMemorySize, s->smem));
+    if (s->cluster > 1) {
+        if (s->cluster > 8) CK(cudaFuncSetAttribute((const void*)f, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = dim3(s->cluster * s->num_sms); cfg.blockDim = dim3(threads); cfg.dynamicSmemBytes = (size_t)s->smem;
+        cudaLaunchAttribute at[1];
+        at[0].id = cudaLaunchAttributeClusterDimension;
+        at[0].val.clusterDim.x = (unsigned)s->cluster; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+        cfg.attrs = at; cfg.numAttrs = 1;
+        int nc = 0;
+        CK(cudaOccupancyMaxActiveClusters(&nc, (const void*)f, &cfg));
+        *out = std::min(nc * s->cluster, CG_MAX_CTAS);
+        return CG_OK;
+    }
     int per_sm = 0;
     CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, (const void*)f, threads, s->smem));
     *out = std::min(per_sm * s->num_sms, CG_MAX_CTAS);
     return CG_OK;
 }
 
-// threads per CTA that own attempts when the proposals can be cached (M <= n_ctas * pl), else 0
-static int choose_pl(u64 M, int n_ctas, int threads)
-{
-    return M <= (u64)n_ctas * (u64)(threads - 64) ? threads - 64 : 0;
-}
-
 static int choose_launch(cg_sim* s, int n_ctas, int threads)
 {
-    if (threads == 0) threads = 512;
-    if (threads != 256 && threads != 512 && threads != 1024) return CG_EINVAL;
+    const bool auto_threads = threads == 0;
+    if (auto_threads) threads = 544;
+    if (!workers_of(threads)) return CG_EINVAL;
     const bool heuristic = n_ctas == 0;
-    if (heuristic) {
-        const u64 work = std::max<u64>(s->M, s->N / 2);        // labels or pairs of sites, per worker thread
-        const u64 workers = (u64)threads - 64;
-        n_ctas = (int)std::min<u64>((work + workers - 1) / workers, (u64)s->num_sms);
-        n_ctas = std::max(1, n_ctas);
-    }
-    if (n_ctas < 1 || n_ctas > CG_MAX_CTAS) return CG_EINVAL;
-    int rp = choose_rp(s->N / 2, n_ctas, threads), pl = choose_pl(s->M, n_ctas, threads);
-    int cap = 0;
-    int rc = max_coresident(s, threads, rp, pl > 0, &cap);
-    if (rc != CG_OK) return rc;
-    if (cap < 1) { s->err = "persistent kernel does not fit on an SM"; return CG_EUNSUPPORTED; }
-    if (n_ctas > cap) {
-        if (!heuristic) return CG_EINVAL;
-        n_ctas = cap;
-        rp = choose_rp(s->N / 2, n_ctas, threads); pl = choose_pl(s->M, n_ctas, threads);
-        rc = max_coresident(s, threads, rp, pl > 0, &cap);
+    const int cs = s->cluster;
+    for (int attempt = 0; attempt < 2; ++attempt) {
+        const int workers = 32 * workers_of(threads);
+        int want = n_ctas;
+        if (heuristic) {
+            const u64 work = std::max<u64>(s->M, s->N / 2);        // labels or pairs of sites, per worker thread
+            want = (int)std::min<u64>((work + workers - 1) / workers, (u64)s->num_sms);
+            want = std::max(1, want);
+            want = (want + cs - 1) / cs * cs;
+        }
+        if (want < 1 || want > CG_MAX_CTAS || want % cs) return CG_EINVAL;
+        int rp = choose_rp(s->N / 2, want, workers, rp_cap(threads));
+        bool cached = s->M <= (u64)want * (u64)workers;
+        int cap = 0;
+        int rc = max_coresident(s, threads, rp, cached, &cap);
         if (rc != CG_OK) return rc;
-        if (n_ctas > cap) return CG_EUNSUPPORTED;
+        if (cap < cs) { s->err = "persistent kernel does not fit on the device in this cluster size"; return CG_EUNSUPPORTED; }
+        if (want > cap) {
+            if (!heuristic) return CG_EINVAL;
+            want = cap / cs * cs;
+            rp = choose_rp(s->N / 2, want, workers, rp_cap(threads));
+            cached = s->M <= (u64)want * (u64)workers;
+            rc = max_coresident(s, threads, rp, cached, &cap);
+            if (rc != CG_OK) return rc;
+            if (want > cap) return CG_EUNSUPPORTED;
+        }
+        // clusters strand SMs: if the labels no longer fit the threads, larger CTAs keep them cached
+        if (heuristic && auto_threads && !cached && threads == 544 && s->M <= (u64)want * 512u) { threads = 608; continue; }
+        if (want != s->n_ctas)    // slots of CTAs that no longer exist must not look published
+            CK(cudaMemsetAsync(s->d_slots, 0, CG_SLOT_BYTES, s->stream));
+        s->n_ctas = want; s->threads = threads; s->rp = rp; s->pl = cached ? workers : 0;
+        return CG_OK;
     }
-    if (n_ctas != s->n_ctas)   // slots of CTAs that no longer exist must not look published
-        CK(cudaMemsetAsync(s->d_slots, 0, CG_SLOT_BYTES, s->stream));
-    s->n_ctas = n_ctas; s->threads = threads; s->rp = rp; s->pl = pl;
-    return CG_OK;
+    return CG_EUNSUPPORTED;
 }
 
-static int init_impl(cg_sim** out, int L, double W, double xi, double T, double E, uint64_t seed,
+static int init_impl(cg_sim** out, int dim, int L, double W, double xi, double T, double E, uint64_t seed,
                      uint32_t M, void* dev_ws, size_t bytes, void* stream, bool own)
 {
     if (!out) return CG_EINVAL;
@@ -1335,18 +1582,26 @@ static int init_impl(cg_sim** out, int L, double W, double xi, double T, double 
     if (!(xi > 0.0) || !(T > 0.0) || !(W >= 0.0) || M < 1 || !std::isfinite(E) || !std::isfinite(W)
         || !std::isfinite(xi) || !std::isfinite(T)) return CG_EINVAL;
     int lg = 0;
-    if (!valid_L(L, &lg)) return CG_EUNSUPPORTED;
+    if (!valid_L(dim, L, &lg)) return CG_EUNSUPPORTED;
+    if (M > (1u << 27)) return CG_EUNSUPPORTED;            // labels travel in 32-bit records next to other fields
     cg_sim* s = new (std::nothrow) cg_sim();
     if (!s) return CG_ENOMEM;
     struct Guard { cg_sim* s; ~Guard() { if (s) cg_free(s); } } guard{s};
-    s->L = L; s->lgL = lg; s->pitch = L / 2 + 1; s->N = (u32)L * (u32)L; s->M = M;
+    s->dim = dim; s->L = L; s->Lz = dim == 3 ? L : 1; s->lgL = lg; s->pitch = L / 2 + 1;
+    s->N = dim == 3 ? (u32)L * (u32)L * (u32)L : (u32)L * (u32)L; s->M = M;
     s->W = W; s->xi = xi; s->T = T; s->E = E; s->seed = seed;
     s->stream = (cudaStream_t)stream;
+    // site coding: c(s) = (z 2L + y) 2L + x (csrc: struct Geo)
+    s->hi1 = ~(u32)(L - 1);
+    s->hi2 = dim == 3 ? ~(u32)(L * L - 1) : 0u;
+    s->spare = (u32)L | (dim == 3 ? (u32)(2 * L * L) : 0u);
+    s->mask = (u32)(L - 1) | ((u32)(L - 1) << (lg + 1)) | (dim == 3 ? (u32)(L - 1) << (2 * lg + 2) : 0u);
+    s->tf_len = dim == 3 ? 4u * s->N : 2u * s->N;
+    if (const char* w = getenv("CG_WATCHDOG_MS")) s->watchdog_ns = (u64)strtoull(w, nullptr, 10) * 1000000ull;
 
-    int dev = 0;
     cudaDeviceProp prop;
-    CK(cudaGetDevice(&dev));
-    CK(cudaGetDeviceProperties(&prop, dev));
+    CK(cudaGetDevice(&s->device));
+    CK(cudaGetDeviceProperties(&prop, s->device));
     s->num_sms = prop.multiProcessorCount;
     if (!prop.cooperativeLaunch) { s->err = "device lacks cooperative launch"; return CG_EUNSUPPORTED; }
 
@@ -1354,9 +1609,9 @@ static int init_impl(cg_sim** out, int L, double W, double xi, double T, double 
     try { build_tables(s, tq); } catch (const std::bad_alloc&) { return CG_ENOMEM; }
     if (s->Klive > 65535) return CG_EUNSUPPORTED;           // the guide packs k in 16 bits
     s->smem = (int)smem_bytes(s);
-    if ((size_t)s->smem > (size_t)prop.sharedMemPerBlockOptin - 1024) return CG_EUNSUPPORTED;
+    if ((size_t)s->smem + sizeof(Comm) + 1024 > (size_t)prop.sharedMemPerBlockOptin) return CG_EUNSUPPORTED;
 
-    const WsLayout w = ws_layout(L);
+    const WsLayout w = ws_layout(dim, L);
     if (own) {
         CK(cudaMalloc(&s->ws, w.total));
         s->own_ws = true;
@@ -1367,18 +1622,22 @@ static int init_impl(cg_sim** out, int L, double W, double xi, double T, double 
     }
     char* base = (char*)s->ws;
     for (int k = 0; k < CG_RING; ++k) s->d_eps[k] = (double*)(base + w.eps0 + (size_t)k * align256(8 * (size_t)s->N));
+    s->d_work = (double*)(base + w.work);
     s->d_scratch = (double*)(base + w.scratch); s->d_phi = (double*)(base + w.phi);
     s->d_nbits = (u32*)(base + w.nbits); s->d_tq = (double*)(base + w.tq); s->d_tf = (double*)(base + w.tf);
     s->d_cdfi = (u64*)(base + w.cdfi); s->d_invr_k = (double*)(base + w.invr_k);
     s->d_fld_k = (double*)(base + w.fld_k); s->d_guide = (u32*)(base + w.guide);
-    s->d_disp = (int*)(base + w.disp); s->d_slots = (u64*)(base + w.slots);
+    s->d_disp = (u32*)(base + w.disp); s->d_slots = (u64*)(base + w.slots);
     s->d_ctl = (CgCtl*)(base + w.ctl); s->d_red = (u64*)(base + w.red);
 
-    std::vector<int> disp((size_t)s->Klive);
-    for (int64_t k = 0; k < s->Klive; ++k) disp[k] = (s->dy[k] << 16) | (s->dx[k] & 0xFFFF);
+    std::vector<u32> disp((size_t)s->Klive);
+    for (int64_t k = 0; k < s->Klive; ++k) {
+        const u32 mz = (u32)(s->dz[k] & (s->Lz - 1)), my = (u32)(s->dy[k] & (L - 1)), mx = (u32)(s->dx[k] & (L - 1));
+        disp[k] = host_code(s, (((mz << lg) | my) << lg) | mx);
+    }
     cudaStream_t st = s->stream;
     CK(cudaMemcpyAsync(s->d_tq, tq.data(), 8 * tq.size(), cudaMemcpyHostToDevice, st));
-    cg_build_tf<<<L, 256, 0, st>>>(s->d_tq, s->d_tf, L, s->pitch);
+    cg_build_tf<<<std::min<u32>((s->tf_len + 255) / 256, 4096u), 256, 0, st>>>(s->d_tq, s->d_tf, L, lg, s->Lz, s->pitch, s->tf_len);
     CK(cudaMemcpyAsync(s->d_cdfi, s->cdfi.data(), 8 * (size_t)s->Klive, cudaMemcpyHostToDevice, st));
     CK(cudaMemcpyAsync(s->d_invr_k, s->invr_k.data(), 8 * (size_t)s->Klive, cudaMemcpyHostToDevice, st));
     CK(cudaMemcpyAsync(s->d_fld_k, s->fld_k.data(), 8 * (size_t)s->Klive, cudaMemcpyHostToDevice, st));
@@ -1393,9 +1652,9 @@ static int init_impl(cg_sim** out, int L, double W, double xi, double T, double 
     const int tb = (int)std::min<u32>(N, 256);
     u64* keys = (u64*)s->d_eps[1];
     cg_init_phi_keys<<<(N + tb - 1) / tb, tb, 0, st>>>(s->d_phi, keys, N, W, (u32)seed, (u32)(seed >> 32));
-    const int ob = (int)std::min<u32>(N, 1024);          // N = 4^k >= 16, so ob divides N and is a warp multiple
+    const int ob = (int)std::min<u32>(N, 1024);          // N = 2^k >= 16, so ob divides N and is a warp multiple
     cg_init_occupations<<<N / ob, ob, 0, st>>>(keys, s->d_nbits, N);
-    cg_full_sum_eps<<<(N + 127) / 128, 128, 0, st>>>(s->d_phi, s->d_nbits, s->d_tq, s->d_eps[0], L, lg, s->pitch, N);
+    cg_full_sum_eps<<<(N + 127) / 128, 128, 0, st>>>(s->d_phi, s->d_nbits, s->d_tq, s->d_eps[0], L, lg, s->Lz, s->pitch, N);
     CK(cudaGetLastError());
     CK(cudaStreamSynchronize(st));                        // host vectors above go out of scope
 
@@ -1408,13 +1667,24 @@ static int init_impl(cg_sim** out, int L, double W, double xi, double T, double 
 
 extern "C" int cg_init(cg_sim** out, int L, double W, double xi, double T, double E, uint64_t seed, uint32_t M)
 {
-    return init_impl(out, L, W, xi, T, E, seed, M, nullptr, 0, nullptr, true);
+    return init_impl(out, 2, L, W, xi, T, E, seed, M, nullptr, 0, nullptr, true);
 }
 
 extern "C" int cg_init_ws(cg_sim** out, int L, double W, double xi, double T, double E, uint64_t seed,
                           uint32_t M, void* dev_workspace, size_t bytes, void* cuda_stream)
 {
-    return init_impl(out, L, W, xi, T, E, seed, M, dev_workspace, bytes, cuda_stream, false);
+    return init_impl(out, 2, L, W, xi, T, E, seed, M, dev_workspace, bytes, cuda_stream, false);
+}
+
+extern "C" int cg_init3(cg_sim** out, int L, double W, double xi, double T, double E, uint64_t seed, uint32_t M)
+{
+    return init_impl(out, 3, L, W, xi, T, E, seed, M, nullptr, 0, nullptr, true);
+}
+
+extern "C" int cg_init3_ws(cg_sim** out, int L, double W, double xi, double T, double E, uint64_t seed,
+                           uint32_t M, void* dev_workspace, size_t bytes, void* cuda_stream)
+{
+    return init_impl(out, 3, L, W, xi, T, E, seed, M, dev_workspace, bytes, cuda_stream, false);
 }
 
 extern "C" void cg_free(cg_sim* s)
@@ -1427,15 +1697,36 @@ extern "C" void cg_free(cg_sim* s)
     delete s;
 }
 
+// one cooperative launch, in clusters when the sim asks for them
+static cudaError_t launch_coop(const void* f, int grid, int threads, int smem, cudaStream_t st, int cluster, void** args)
+{
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(grid); cfg.blockDim = dim3(threads); cfg.dynamicSmemBytes = (size_t)smem; cfg.stream = st;
+    cudaLaunchAttribute at[2];
+    at[0].id = cudaLaunchAttributeCooperative; at[0].val.cooperative = 1;
+    cfg.attrs = at; cfg.numAttrs = 1;
+    if (cluster > 1) {
+        at[1].id = cudaLaunchAttributeClusterDimension;
+        at[1].val.clusterDim.x = (unsigned)cluster; at[1].val.clusterDim.y = 1; at[1].val.clusterDim.z = 1;
+        cfg.numAttrs = 2;
+    }
+    return cudaLaunchKernelExC(&cfg, f, args);
+}
+
+#define CG_MAX_LAUNCH_HOPS (1u << 30)     // the kernel counts hops and iterations of one launch in 32 bits
+
 extern "C" int cg_run(cg_sim* s, uint64_t n_hops)
 {
     if (!s) return CG_EINVAL;
-    if (n_hops == 0) return CG_OK;
     persist_fn f = persistent_kernel(s->threads, s->rp, s->pl > 0);
     if (!f) return CG_EINVAL;
-    CgParams p = make_params(s, n_hops);
-    void* args[] = {&p};
-    CK(cudaLaunchCooperativeKernel((const void*)f, dim3(s->n_ctas), dim3(s->threads), args, (size_t)s->smem, s->stream));
+    while (n_hops) {
+        const u32 chunk = (u32)std::min<uint64_t>(n_hops, CG_MAX_LAUNCH_HOPS);
+        CgParams p = make_params(s, chunk);
+        void* args[] = {&p};
+        CK(launch_coop((const void*)f, s->n_ctas, s->threads, s->smem, s->stream, s->cluster, args));
+        n_hops -= chunk;
+    }
     return CG_OK;
 }
 
@@ -1452,16 +1743,17 @@ extern "C" int cg_run_many(cg_sim* const* sims, int n_sims, uint64_t n_hops)
         cg_sim* s = sims[k];
         if (!s) return CG_EINVAL;
         for (int m = 0; m < k; ++m) if (sims[m] == s) return CG_EINVAL;       // a sim may appear once
-        if (s->stream != s0->stream || s->threads != s0->threads || s->rp != s0->rp || (s->pl > 0) != (s0->pl > 0)) {
-            s0->err = "cg_run_many: the sims must share stream and launch shape (threads, register tiling, cached labels)";
+        if (s->device != s0->device || s->stream != s0->stream || s->threads != s0->threads || s->rp != s0->rp
+            || (s->pl > 0) != (s0->pl > 0) || s->cluster != 1) {
+            s0->err = "cg_run_many: the sims must share device, stream and launch shape (threads, register tiling, "
+                      "cached labels) and use no clusters";
             return CG_EINVAL;
         }
-        ps[(size_t)k] = make_params(s, n_hops);
         first[(size_t)k + 1] = first[(size_t)k] + (u32)s->n_ctas;
         smem = std::max(smem, s->smem);
     }
     many_fn f = many_kernel(s0->threads, s0->rp, s0->pl > 0);
-    if (!f) { s0->err = "cg_run_many: only 512-thread launch shapes"; return CG_EUNSUPPORTED; }
+    if (!f) { s0->err = "cg_run_many: only 544-thread launch shapes"; return CG_EUNSUPPORTED; }
     CK0(s0, cudaFuncSetAttribute((const void*)f, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
     int per_sm = 0;
     CK0(s0, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, (const void*)f, s0->threads, smem));
@@ -1478,19 +1770,32 @@ extern "C" int cg_run_many(cg_sim* const* sims, int n_sims, uint64_t n_hops)
     }
     CgParams* d_ps = (CgParams*)s0->d_many;
     u32* d_first = (u32*)((char*)s0->d_many + ps.size() * sizeof(CgParams));
-    // pageable sources: the copies are staged before the calls return
-    CK0(s0, cudaMemcpyAsync(d_ps, ps.data(), ps.size() * sizeof(CgParams), cudaMemcpyHostToDevice, s0->stream));
-    CK0(s0, cudaMemcpyAsync(d_first, first.data(), first.size() * sizeof(u32), cudaMemcpyHostToDevice, s0->stream));
-    u32 n = (u32)n_sims;
-    void* args[] = {&d_ps, &d_first, &n};
-    CK0(s0, cudaLaunchCooperativeKernel((const void*)f, dim3(total), dim3(s0->threads), args, (size_t)smem, s0->stream));
+    while (n_hops) {
+        const u32 chunk = (u32)std::min<uint64_t>(n_hops, CG_MAX_LAUNCH_HOPS);
+        for (int k = 0; k < n_sims; ++k) ps[(size_t)k] = make_params(sims[k], chunk);
+        // pageable sources: the copies are staged before the calls return
+        CK0(s0, cudaMemcpyAsync(d_ps, ps.data(), ps.size() * sizeof(CgParams), cudaMemcpyHostToDevice, s0->stream));
+        CK0(s0, cudaMemcpyAsync(d_first, first.data(), first.size() * sizeof(u32), cudaMemcpyHostToDevice, s0->stream));
+        u32 n = (u32)n_sims;
+        void* args[] = {&d_ps, &d_first, &n};
+        CK0(s0, launch_coop((const void*)f, (int)total, s0->threads, smem, s0->stream, 1, args));
+        n_hops -= chunk;
+    }
     return CG_OK;
 }
 
+// the control block, after everything queued on the stream; CG_EDEVICE when a launch was abandoned
 static int read_ctl(cg_sim* s, CgCtl* c)
 {
     CK(cudaMemcpyAsync(c, s->d_ctl, sizeof *c, cudaMemcpyDeviceToHost, s->stream));
     CK(cudaStreamSynchronize(s->stream));
+    if (c->abort) {
+        char buf[160];
+        snprintf(buf, sizeof buf, "the persistent kernel gave up waiting (watchdog, wait %u); the state is undefined until "
+                                  "cg_set_state", c->abort);
+        s->err = buf;
+        return CG_EDEVICE;
+    }
     return CG_OK;
 }
 
@@ -1527,8 +1832,8 @@ extern "C" int cg_set_state(cg_sim* s, const int8_t* n, const double* eps, uint6
     if (sum != s->N / 2) return CG_EINVAL;                   // sum_i n_i = nu N
     CgCtl c;
     int rc = read_ctl(s, &c);
-    if (rc != CG_OK) return rc;
-    c.attempts = attempts; c.hops = hops; c.dP = dP; c.iterations = 0; c.proposals = 0; c.cur = 0;
+    if (rc != CG_OK && rc != CG_EDEVICE) return rc;          // a new state is the way out of an abandoned launch
+    c.attempts = attempts; c.hops = hops; c.dP = dP; c.iterations = 0; c.proposals = 0; c.cur = 0; c.abort = 0;
     c.log_base = hops; c.log_a0 = attempts; s->log_gap = false;
     CK(cudaMemcpyAsync(s->d_eps[0], eps, 8 * (size_t)s->N, cudaMemcpyHostToDevice, s->stream));
     CK(cudaMemcpyAsync(s->d_nbits, bits.data(), 4 * bits.size(), cudaMemcpyHostToDevice, s->stream));
@@ -1561,7 +1866,7 @@ extern "C" int cg_enable_hop_log(cg_sim* s, uint64_t capacity, void* dev_buf, si
     s->d_log = nullptr; s->own_log = false; s->log_cap = 0; s->log_gap = false;
     if (capacity) {
         if (dev_buf) {
-            if (bytes < 16 * capacity || ((uintptr_t)dev_buf & 7)) return CG_EINVAL;
+            if (bytes / 16 < capacity || ((uintptr_t)dev_buf & 7)) return CG_EINVAL;
             s->d_log = dev_buf;
         } else {
             CK(cudaMalloc(&s->d_log, 16 * capacity));
@@ -1581,8 +1886,9 @@ extern "C" int cg_get_hops(cg_sim* s, uint64_t first, uint64_t count, uint64_t* 
     CgCtl c;
     int rc = read_ctl(s, &c);
     if (rc != CG_OK) return rc;
+    if (s->log_gap) return CG_EINVAL;                        // scripted hops are not logged: the indices would lie
     const u64 have = std::min<u64>(c.hops - c.log_base, s->log_cap);
-    if (first + count > have) return CG_EINVAL;
+    if (first > have || count > have - first) return CG_EINVAL;
     if (!count) return CG_OK;
     const char* base = (const char*)s->d_log;
     if (attempt) CK(cudaMemcpyAsync(attempt, base + 8 * first, 8 * count, cudaMemcpyDeviceToHost, s->stream));
@@ -1599,7 +1905,7 @@ extern "C" int cg_recompute_eps(cg_sim* s, double* max_abs_dev)
     int rc = read_ctl(s, &c);
     if (rc != CG_OK) return rc;
     cg_full_sum_eps<<<(s->N + 127) / 128, 128, 0, s->stream>>>(s->d_phi, s->d_nbits, s->d_tq, s->d_scratch,
-                                                               s->L, s->lgL, s->pitch, s->N);
+                                                               s->L, s->lgL, s->Lz, s->pitch, s->N);
     CK(cudaMemsetAsync(s->d_red, 0, 8, s->stream));
     cg_max_abs_diff<<<std::max(1u, std::min(s->N / 256, 1024u)), 256, 0, s->stream>>>(s->d_scratch, s->d_eps[c.cur % CG_RING],
                                                                                      s->N, s->d_red);
@@ -1612,41 +1918,57 @@ extern "C" int cg_recompute_eps(cg_sim* s, double* max_abs_dev)
     return CG_OK;
 }
 
+struct EventPair {          // released on every return path
+    cudaEvent_t a = nullptr, b = nullptr;
+    ~EventPair() { if (a) cudaEventDestroy(a); if (b) cudaEventDestroy(b); }
+};
+
 extern "C" int cg_apply_hops(cg_sim* s, uint64_t count, const uint32_t* i, const uint32_t* j, float* ms)
 {
     if (!s || (count && (!i || !j))) return CG_EINVAL;
     if (ms) *ms = 0.f;
     if (!count) return CG_OK;
-    for (u64 h = 0; h < count; ++h)
-        if (i[h] >= s->N || j[h] >= s->N || i[h] == j[h]) return CG_EINVAL;
+    CgCtl c;
+    int rc = read_ctl(s, &c);
+    if (rc != CG_OK) return rc;
+    // theta_ij of every scripted hop, in hop order, BEFORE anything is touched
+    {
+        std::vector<u32> bits((s->N + 31) / 32);
+        CK(cudaMemcpyAsync(bits.data(), s->d_nbits, 4 * bits.size(), cudaMemcpyDeviceToHost, s->stream));
+        CK(cudaStreamSynchronize(s->stream));
+        for (u64 h = 0; h < count; ++h) {
+            const u32 a = i[h], b = j[h];
+            if (a >= s->N || b >= s->N || a == b) return CG_EINVAL;
+            if (!((bits[a >> 5] >> (a & 31)) & 1u) || ((bits[b >> 5] >> (b & 31)) & 1u)) return CG_EINVAL;
+            bits[a >> 5] &= ~(1u << (a & 31)); bits[b >> 5] |= 1u << (b & 31);
+        }
+    }
     u32* d_ij = nullptr;
     if (s->d_log) s->log_gap = true;
     CK(cudaMalloc(&d_ij, 8 * count));
     struct Free { void* p; ~Free() { cudaFree(p); } } fr{d_ij};
     CK(cudaMemcpyAsync(d_ij, i, 4 * count, cudaMemcpyHostToDevice, s->stream));
     CK(cudaMemcpyAsync(d_ij + count, j, 4 * count, cudaMemcpyHostToDevice, s->stream));
-    cudaEvent_t e0, e1;
-    CK(cudaEventCreate(&e0)); CK(cudaEventCreate(&e1));
+    EventPair ev;
+    CK(cudaEventCreate(&ev.a)); CK(cudaEventCreate(&ev.b));
     CgParams p = make_params(s, 0);
     // many small CTAs per SM (one block of 64 sites per warp; 128 threads measured best) keep enough
     // requests in flight to make the stand-alone update throughput-bound; larger lattices fall back to
     // one CTA per SM
     const u64 g1 = (s->N / 2 + 127) / 128;
     const int grid = (int)std::max<u64>(1, std::min<u64>((s->N / 2 + 511) / 512, (u64)s->num_sms));
-    CK(cudaEventRecord(e0, s->stream));
+    CK(cudaEventRecord(ev.a, s->stream));
     if (g1 <= (u64)s->num_sms * 12) cg_update_scripted<128, 1><<<(int)g1, 128, 0, s->stream>>>(p, d_ij, d_ij + count, count);
-    else scripted_kernel(choose_rp(s->N / 2, grid, 512))<<<grid, 512, 0, s->stream>>>(p, d_ij, d_ij + count, count);
-    CK(cudaEventRecord(e1, s->stream));
+    else scripted_kernel(choose_rp(s->N / 2, grid, 512, 8))<<<grid, 512, 0, s->stream>>>(p, d_ij, d_ij + count, count);
+    CK(cudaEventRecord(ev.b, s->stream));
     CK(cudaGetLastError());
     CK(cudaStreamSynchronize(s->stream));
     float t = 0.f;
-    CK(cudaEventElapsedTime(&t, e0, e1));
-    cudaEventDestroy(e0); cudaEventDestroy(e1);
+    CK(cudaEventElapsedTime(&t, ev.a, ev.b));
     if (ms) *ms = t;
-    CgCtl c;
-    int rc = read_ctl(s, &c);
+    rc = read_ctl(s, &c);
     if (rc != CG_OK) return rc;
-    if (c.bad_hops) {
+    if (c.bad_hops) {                          // cannot happen after the check above; kept as a device-side assertion
         c.bad_hops = 0;
         CK(cudaMemcpyAsync(s->d_ctl, &c, sizeof c, cudaMemcpyHostToDevice, s->stream));
         CK(cudaStreamSynchronize(s->stream));
@@ -1676,6 +1998,13 @@ extern "C" int cg_get_tables(cg_sim* s, int32_t* dy, int32_t* dx, double* cdf, d
     return CG_OK;
 }
 
+extern "C" int cg_get_table_dz(cg_sim* s, int32_t* dz)
+{
+    if (!s || !dz) return CG_EINVAL;
+    memcpy(dz, s->dz.data(), 4 * (size_t)s->Klive);
+    return CG_OK;
+}
+
 extern "C" int cg_get_phi(cg_sim* s, double* phi)
 {
     if (!s || !phi) return CG_EINVAL;
@@ -1700,21 +2029,38 @@ extern "C" int cg_get_launch(cg_sim* s, int* n_ctas, int* threads, int* smem)
     return CG_OK;
 }
 
-extern "C" int cg_set_trace(cg_sim* s, void* dev_buf, size_t bytes, uint32_t iterations)
+extern "C" int cg_set_tuning(cg_sim* s, int snapshot_interval, int cluster_size)
 {
     if (!s) return CG_EINVAL;
+    int shift = s->snap_shift, cs = s->cluster;
+    if (snapshot_interval) {
+        if (snapshot_interval != 1 && snapshot_interval != 2 && snapshot_interval != 4 && snapshot_interval != 8) return CG_EINVAL;
+        shift = snapshot_interval == 1 ? 0 : snapshot_interval == 2 ? 1 : snapshot_interval == 4 ? 2 : 3;
+    }
+    if (cluster_size) {
+        if (cluster_size < 1 || cluster_size > CG_MAX_CLUSTER || (cluster_size & (cluster_size - 1))) return CG_EINVAL;
+        cs = cluster_size;
+    }
     CK(cudaStreamSynchronize(s->stream));
-    if (!dev_buf || !iterations) { s->d_trace = nullptr; s->trace_iters = 0; return CG_OK; }
-#if !defined(CG_TRACE) && !defined(CG_TRACE_W) && !defined(CG_TRACE_T)
-    return CG_EUNSUPPORTED;                   // the library was built without -DCG_TRACE
-#endif
-    if (((uintptr_t)dev_buf & 7) || bytes < (size_t)8 * 64 * CG_MAX_CTAS) return CG_EINVAL;
-    s->d_trace = (u64*)dev_buf; s->trace_iters = iterations;
+    const int old_shift = s->snap_shift, old_cs = s->cluster;
+    s->snap_shift = shift; s->cluster = cs;
+    if (cs != old_cs) {
+        const int rc = choose_launch(s, 0, 0);
+        if (rc != CG_OK) { s->snap_shift = old_shift; s->cluster = old_cs; choose_launch(s, 0, 0); return rc; }
+    }
+    return CG_OK;
+}
+
+extern "C" int cg_get_tuning(cg_sim* s, int* snapshot_interval, int* cluster_size)
+{
+    if (!s) return CG_EINVAL;
+    if (snapshot_interval) *snapshot_interval = 1 << s->snap_shift;
+    if (cluster_size) *cluster_size = s->cluster;
     return CG_OK;
 }
 
 extern "C" int cg_get_phase_cycles(cg_sim* s, uint64_t* total, uint64_t* wait, uint64_t* update,
-                                   uint64_t* propose, int reset)
+                                   uint64_t* propose, uint64_t* warps, int reset)
 {
     if (!s) return CG_EINVAL;
     CgCtl c;
@@ -1724,43 +2070,52 @@ extern "C" int cg_get_phase_cycles(cg_sim* s, uint64_t* total, uint64_t* wait, u
     if (wait) *wait = c.cyc_wait;
     if (update) *update = c.cyc_update;
     if (propose) *propose = c.cyc_propose;
+    if (warps) *warps = c.cyc_warps;
     if (reset) {
-        c.cyc_total = c.cyc_wait = c.cyc_update = c.cyc_propose = 0;
+        c.cyc_total = c.cyc_wait = c.cyc_update = c.cyc_propose = c.cyc_warps = 0;
         CK(cudaMemcpyAsync(s->d_ctl, &c, sizeof c, cudaMemcpyHostToDevice, s->stream));
         CK(cudaStreamSynchronize(s->stream));
     }
     return CG_OK;
 }
 
-extern "C" int cg_bench_l2_rmw(size_t bytes, int reps, int trials, double* gbps)
+extern "C" int cg_bench_l2(size_t bytes, int reps, int trials, int mode, int ctas_per_sm, int threads, int vec_bytes,
+                           double* gbps)
 {
     cg_sim* s = nullptr;
-    if (!gbps || bytes < 4096 || (bytes & 15) || reps < 1 || trials < 1) return CG_EINVAL;
+    if (!gbps || bytes < 4096 || (bytes & 31) || reps < 1 || trials < 1 || mode < 0 || mode > 2 || ctas_per_sm < 1
+        || ctas_per_sm > 16 || threads < 32 || threads > 1024 || (threads & 31) || (vec_bytes != 16 && vec_bytes != 32))
+        return CG_EINVAL;
     int dev = 0, sms = 0;
     CK(cudaGetDevice(&dev));
     CK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
-    double2* buf = nullptr;
-    CK(cudaMalloc(&buf, bytes));
+    double* buf = nullptr;
+    CK(cudaMalloc(&buf, bytes + 256));
     struct Free { void* p; ~Free() { cudaFree(p); } } fr{buf};
-    CK(cudaMemset(buf, 0, bytes));
-    cudaEvent_t e0, e1;
-    CK(cudaEventCreate(&e0)); CK(cudaEventCreate(&e1));
-    const size_t n16 = bytes / 16;
-    const int grid = (int)std::max<size_t>(1, std::min<size_t>((n16 + 511) / 512, (size_t)sms * 2));
-    cg_l2_rmw<<<grid, 512>>>(buf, n16, 2);                 // warm-up
+    CK(cudaMemset(buf, 0, bytes + 256));
+    EventPair ev;
+    CK(cudaEventCreate(&ev.a)); CK(cudaEventCreate(&ev.b));
+    const size_t nvec = bytes / (size_t)vec_bytes;
+    const int grid = (int)std::max<size_t>(1, std::min<size_t>((nvec + threads - 1) / threads, (size_t)sms * ctas_per_sm));
+    double* sink = buf + bytes / 8;
+    auto launch = [&](int r) {
+        if (vec_bytes == 16) cg_l2_probe<16><<<grid, threads>>>(buf, nvec, r, mode, sink);
+        else cg_l2_probe<32><<<grid, threads>>>(buf, nvec, r, mode, sink);
+    };
+    launch(2);                                             // warm-up
     float best = 1e30f;
     for (int t = 0; t < trials; ++t) {
-        CK(cudaEventRecord(e0));
-        cg_l2_rmw<<<grid, 512>>>(buf, n16, reps);
-        CK(cudaEventRecord(e1));
-        CK(cudaEventSynchronize(e1));
+        CK(cudaEventRecord(ev.a));
+        launch(reps);
+        CK(cudaEventRecord(ev.b));
+        CK(cudaEventSynchronize(ev.b));
         float ms = 0.f;
-        CK(cudaEventElapsedTime(&ms, e0, e1));
+        CK(cudaEventElapsedTime(&ms, ev.a, ev.b));
         best = std::min(best, ms);
     }
     CK(cudaGetLastError());
-    cudaEventDestroy(e0); cudaEventDestroy(e1);
-    *gbps = 2.0 * (double)bytes * (double)reps / ((double)best * 1e-3) / 1e9;
+    const double moved = (mode == 0 ? 2.0 : 1.0) * (double)bytes * (double)reps;
+    *gbps = moved / ((double)best * 1e-3) / 1e9;
     return CG_OK;
 }
 
@@ -1772,6 +2127,7 @@ extern "C" const char* cg_strerror(int code)
         case CG_ENOMEM: return "out of memory or workspace too small";
         case CG_ECUDA: return "CUDA error (see cg_last_error)";
         case CG_EUNSUPPORTED: return "problem not supported by the sm_100a path";
+        case CG_EDEVICE: return "the persistent kernel abandoned a launch (see cg_last_error)";
     }
     return "unknown error";
 }
@@ -2037,7 +2393,7 @@ extern "C" int cg_get_series(cg_sim* s, uint64_t first, uint64_t count, double* 
     if (rc != CG_OK) return rc;
     u64 have = 0;
     if ((rc = logged_hops(s, c, &have)) != CG_OK) return rc;
-    if (first + count > have) return CG_EINVAL;
+    if (first > have || count > have - first) return CG_EINVAL;
     if (!count || (!t && !P)) return CG_OK;
     const u64 end = first + count;
     const u32 nchunks = (u32)((end + CG_SCAN_CHUNK - 1) / CG_SCAN_CHUNK);

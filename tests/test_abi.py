@@ -42,6 +42,10 @@ def test_argument_validation_and_loud_failure_without_gpu(cg):
     assert lib.cg_init(C.byref(h), 16, 1.0, 1.0, 0.1, 0.0, 1, 0) == cg.binding.CG_EINVAL
     assert lib.cg_init(C.byref(h), 24, 1.0, 1.0, 0.1, 0.0, 1, 4) == cg.binding.CG_EUNSUPPORTED
     assert lib.cg_init(C.byref(h), 2048, 1.0, 1.0, 0.1, 0.0, 1, 4) == cg.binding.CG_EUNSUPPORTED
+    assert lib.cg_init(C.byref(h), 16, 1.0, 1.0, 0.1, 0.0, 1, (1 << 27) + 1) == cg.binding.CG_EUNSUPPORTED
+    assert lib.cg_init3(C.byref(h), 128, 1.0, 1.0, 0.1, 0.0, 1, 4) == cg.binding.CG_EUNSUPPORTED and not h.value
+    assert lib.cg_init3(C.byref(h), 7, 1.0, 1.0, 0.1, 0.0, 1, 4) == cg.binding.CG_EINVAL
+    assert lib.cg_workspace_bytes3(64, 65536) >= 12 * 8 * 64 ** 3 and lib.cg_workspace_bytes3(128, 4) == 0
     assert lib.cg_init(None, 16, 1.0, 1.0, 0.1, 0.0, 1, 4) == cg.binding.CG_EINVAL
     assert lib.cg_run(None, 1) == cg.binding.CG_EINVAL
     assert lib.cg_workspace_bytes(512, 65536) >= 4 * 8 * 512 * 512
@@ -68,11 +72,16 @@ def test_product_path_never_touches_the_oracle():
 
 def test_diagnostic_entry_points_validate_arguments(cg):
     lib = cg.lib()
-    assert lib.cg_set_trace(None, None, 0, 0) == cg.binding.CG_EINVAL
+    assert lib.cg_set_tuning(None, 0, 0) == cg.binding.CG_EINVAL
+    assert lib.cg_get_tuning(None, None, None) == cg.binding.CG_EINVAL
+    assert lib.cg_get_phase_cycles(None, None, None, None, None, None, 0) == cg.binding.CG_EINVAL
     assert lib.cg_set_launch(None, 0, 0) == cg.binding.CG_EINVAL
     assert lib.cg_get_counters(None, None, None, None, None) == cg.binding.CG_EINVAL
     out = C.c_double()
-    assert lib.cg_bench_l2_rmw(100, 1, 1, C.byref(out)) == cg.binding.CG_EINVAL      # too small a buffer
+    assert lib.cg_bench_l2(100, 1, 1, 0, 2, 512, 16, C.byref(out)) == cg.binding.CG_EINVAL       # too small a buffer
+    assert lib.cg_bench_l2(1 << 20, 1, 1, 3, 2, 512, 16, C.byref(out)) == cg.binding.CG_EINVAL   # no such mode
+    assert lib.cg_bench_l2(1 << 20, 1, 1, 0, 2, 512, 24, C.byref(out)) == cg.binding.CG_EINVAL   # 16 or 32 bytes
+    assert lib.cg_strerror(cg.binding.CG_EDEVICE).decode().startswith("the persistent kernel abandoned")
 
 
 def test_observable_entry_points_validate_arguments(cg):

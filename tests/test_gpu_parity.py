@@ -87,7 +87,7 @@ def test_split_runs_continue_the_same_chain(cg, oracle_lib):
     _compare(g, o, 5000)
 
 
-@pytest.mark.parametrize("n_ctas,threads", [(1, 256), (3, 256), (8, 512), (37, 1024), (148, 512), (131, 1024)])
+@pytest.mark.parametrize("n_ctas,threads", [(1, 256), (3, 256), (8, 544), (37, 1024), (148, 544), (131, 1024), (100, 608)])
 def test_result_is_independent_of_launch_shape(cg, oracle_lib, n_ctas, threads):
     kw = dict(L=64, T=0.05, E=0.02, seed=77, M=1000)     # M not a multiple of anything: ragged label tail
     g = cg.CoulombGlass(hop_log=4000, **kw)
@@ -192,7 +192,7 @@ def test_launch_shape_may_change_between_runs(cg, oracle_lib):
     next: the chain must not notice (stale words of other shapes are never mistaken for arrivals)."""
     kw = dict(L=128, T=0.1, E=0.01, seed=21, M=4096)
     g = cg.CoulombGlass(hop_log=6000, **kw)
-    for n_ctas, threads, hops in ((0, 0, 1500), (37, 256, 1000), (148, 1024, 1500), (5, 512, 500), (0, 0, 1500)):
+    for n_ctas, threads, hops in ((0, 0, 1500), (37, 256, 1000), (148, 1024, 1500), (5, 544, 500), (0, 0, 1500)):
         g.set_launch(n_ctas, threads)
         g.run(hops)
     o = oracle_lib.Oracle(**kw)
@@ -201,7 +201,7 @@ def test_launch_shape_may_change_between_runs(cg, oracle_lib):
     assert g.recompute_eps() < 1e-9
 
 
-@pytest.mark.parametrize("n_ctas,threads,M", [(148, 512, 303104), (148, 256, 65536), (20, 1024, 65536), (148, 1024, 65536)])
+@pytest.mark.parametrize("n_ctas,threads,M", [(148, 544, 303104), (148, 256, 65536), (20, 1024, 65536), (148, 1024, 65536)])
 def test_labels_recomputed_or_cached(cg, oracle_lib, n_ctas, threads, M):
     """M larger than the label-owning threads of the grid takes the path that decodes every label in
     every iteration; otherwise proposals are cached.  Both must give the serial chain."""
@@ -307,24 +307,155 @@ def test_run_many_refuses_what_it_cannot_run(cg):
     assert a.counters()["hops"] == 10
 
 
+def test_tuning_never_changes_results(cg, oracle_lib):
+    """cg_set_tuning: snapshot interval H (deferred eps write-through) and thread-block clusters
+    (posts through distributed shared memory) are performance knobs only: the chain is the oracle's for every
+    setting, also when they change between runs of one chain, with several CTAs per cluster and ragged shapes."""
+    kw = dict(L=128, T=0.1, E=0.01, seed=21, M=4096)
+    o = oracle_lib.Oracle(**kw)
+    o.run(6000)
+    for H, cs in ((1, 1), (2, 2), (8, 1), (4, 4), (4, 8), (1, 16)):
+        g = cg.CoulombGlass(hop_log=6000, **kw)
+        g.set_tuning(H, cs)
+        assert g.tuning() == {"snapshot_interval": H, "cluster_size": cs}
+        assert g.launch()["n_ctas"] % cs == 0
+        for hops in (1, 2, 3, 1994, 7, 3993):      # launches that end between snapshots
+            g.run(hops)
+        _compare(g, o, 6000)
+        assert g.recompute_eps() < 1e-9
+    g = cg.CoulombGlass(hop_log=6000, **kw)
+    for H, cs, n_ctas, hops in ((4, 1, 0, 1000), (8, 2, 6, 1000), (1, 4, 16, 1000), (2, 8, 8, 1500), (4, 16, 32, 1500)):
+        g.set_tuning(H, cs)
+        g.set_launch(n_ctas, 544)
+        g.run(hops)
+    _compare(g, o, 6000)
+
+
+def test_headline_config_in_clusters(cg, oracle_lib):
+    """Config 5 (L=512, M=65536) launched in thread-block clusters: fewer, larger CTAs (the GPCs strand SMs)."""
+    kw = workloads.init_args(workloads.CONFIGS["cfg5_L512"][0])
+    o = oracle_lib.Oracle(**kw)
+    o.run(3000)
+    for cs in (2, 8, 16):
+        g = cg.CoulombGlass(hop_log=3000, **kw)
+        g.set_tuning(0, cs)
+        g.run(3000)
+        _compare(g, o, 3000)
+
+
+@pytest.mark.parametrize("L,M,hops", [(4, 16, 5000), (8, 64, 5000), (16, 1024, 6000), (32, 8192, 3000)])
+def test_cubic_lattice_matches_oracle(cg, oracle_lib, L, M, hops):
+    """the L^3 lattice.  Tables, disorder, occupations and the full-sum eps
+    bit-identical, then the chain."""
+    kw = dict(L=L, W=1.0, xi=1.0, T=0.1, E=0.02, seed=300 + L, M=M)
+    g = cg.CoulombGlass(hop_log=hops, dim=3, **kw)
+    o = oracle_lib.Oracle(dim=3, **kw)
+    tg, to = g.tables(), o.tables()
+    kl = tg["K_live"]
+    assert tg["K"] == to["K"] and tg["S"] == to["S"] and tg["Gamma"] == to["Gamma"]
+    for key in ("dz", "dy", "dx", "cdf", "invr_k"):
+        assert np.array_equal(tg[key], to[key][:kl]), key
+    assert np.all(to["cdf"][kl - 1:] == 1.0)
+    assert np.array_equal(g.phi(), o.phi())
+    assert np.array_equal(g.state()[0], o.state()[0]) and np.array_equal(g.state()[1], o.state()[1])
+    assert g.recompute_eps() == 0.0
+    g.run(hops)
+    o.run(hops)
+    _compare(g, o, hops)
+    assert g.recompute_eps() < 1e-9
+
+
+def test_cubic_lattice_at_the_headline_footprint(cg, oracle_lib):
+    """L = 64 cubed: N = 262144, the footprint of config 5, all SMs; the live tower (about 48 000 displacements)
+    no longer fits shared memory, its tail is read from L2.  Launch shapes and tuning as in 2D."""
+    kw = dict(L=64, W=1.0, xi=1.0, T=0.05, E=0.01, seed=64, M=65536)
+    o = oracle_lib.Oracle(dim=3, **kw)
+    g = cg.CoulombGlass(hop_log=2500, dim=3, **kw)
+    assert g.tables()["K_live"] > 2048
+    assert np.array_equal(g.state()[1], o.state()[1])
+    g.run(1500)
+    g.set_tuning(2, 4)
+    g.run(1000)
+    o.run(2500)
+    _compare(g, o, 2500)
+    assert g.recompute_eps() < 1e-9
+    # the update alone on the oracle's hops
+    u = cg.CoulombGlass(dim=3, **kw)
+    _, i, j = o.hops()
+    assert u.apply_hops(i, j) > 0
+    assert np.array_equal(u.state()[1], o.state()[1]) and u.state()[3] == o.state()[3]
+
+
+def test_scripted_hops_are_validated_before_anything_changes(cg):
+    g = cg.CoulombGlass(16, T=0.1, seed=3, M=64, hop_log=10)
+    n, eps, _, dP = g.state()
+    occ, emp = np.flatnonzero(n == 1), np.flatnonzero(n == 0)
+    with pytest.raises(cg.CgError):           # the third hop starts from a site the first one emptied
+        g.apply_hops([occ[0], occ[1], occ[0]], [emp[0], emp[1], emp[2]])
+    n2, eps2, _, dP2 = g.state()
+    assert np.array_equal(n, n2) and np.array_equal(eps, eps2) and dP == dP2 and g.counters()["hops"] == 0
+    g.apply_hops([occ[0], emp[0]], [emp[0], occ[0]])       # there and back: legal in this order
+    assert np.array_equal(g.state()[0], n) and np.allclose(g.state()[1], eps, atol=1e-13)
+    with pytest.raises(cg.CgError):           # scripted hops are not in the log
+        g.hops(0, 1)
+    with pytest.raises(cg.CgError):           # first + count must not wrap
+        g._check(g._lib.cg_get_hops(g._h, 2**64 - 1, 2, None, None, None))
+
+
 FULL = [("cfg1_L16", 0), ("cfg2_L64", 0), ("cfg3_L128", 0), ("cfg3_L128", 1), ("cfg3_L128", 2), ("cfg3_L128", 3),
-        ("cfg4_L256", 2), ("cfg5_L512", 0)]
+        ("cfg4_L256", 2), ("cfg4_L256", 3), ("cfg5_L512", 0)]
+
+
+@pytest.fixture(scope="module")
+def full_oracles(oracle_lib):
+    """The oracle's runs of BASELINE.json's configs at their FULL hop counts, all started at once on host
+    threads (the C library runs without the interpreter lock; each run is single-threaded): about five
+    minutes of wall time on the GPU box instead of ten.  Config 4's trajectory does not depend on M
+    (reading G8), so its two M values share one run."""
+    import threading
+    runs = {}
+
+    def start(name, idx):
+        cfg = workloads.CONFIGS[name][idx]
+        o = oracle_lib.Oracle(**workloads.init_args(cfg))
+        th = threading.Thread(target=o.run, args=(cfg["hops"],))
+        th.start()
+        runs[(name, idx)] = (o, th)
+
+    for name, idx in FULL:
+        if (name, idx) != ("cfg4_L256", 3):
+            start(name, idx)
+    runs[("cfg4_L256", 3)] = runs[("cfg4_L256", 2)]
+    return runs
 
 
 @pytest.mark.slow
 @pytest.mark.parametrize("name,idx", FULL)
-def test_full_length_configs(cg, oracle_lib, name, idx):
-    """BASELINE.json's configs at their FULL hop counts (1e5 / 1e6 hops), hop log element by element.
-    About ten minutes of single-core oracle time: runs only with CG_FULL_PARITY=1."""
+def test_full_length_configs(cg, full_oracles, name, idx):
+    """BASELINE.json's configs at their FULL hop counts (1e5 / 1e6 hops), hop log, occupations, eps, clock,
+    dP and counters element by element.  CG_SKIP_FULL_PARITY=1 skips (several minutes of oracle time)."""
     import os
-    if os.environ.get("CG_FULL_PARITY") != "1":
-        pytest.skip("set CG_FULL_PARITY=1 to run the full-length parity check")
+    import torch
+    if os.environ.get("CG_SKIP_FULL_PARITY") == "1":
+        pytest.skip("CG_SKIP_FULL_PARITY=1")
     cfg = workloads.CONFIGS[name][idx]
-    kw = workloads.init_args(cfg)
+    sms = torch.cuda.get_device_properties(0).multi_processor_count
+    kw = workloads.init_args(cfg, sms * 2048)
     hops = cfg["hops"]
     g = cg.CoulombGlass(hop_log=hops, **kw)
     g.run(hops)
-    o = oracle_lib.Oracle(**kw)
-    o.run(hops)
-    _compare(g, o, hops)
     assert g.recompute_eps() < 1e-9
+    o, th = full_oracles[(name, idx)]
+    th.join()
+    if kw["M"] == o.M:
+        _compare(g, o, hops)
+    else:       # config 4 at M = resident threads: the oracle ran with M = 65536; iterations follow from its log
+        for x, y in zip(g.hops(0, hops), o.hops(0, hops)):
+            assert np.array_equal(x, y)
+        assert np.array_equal(g.state()[0], o.state()[0]) and np.array_equal(g.state()[1], o.state()[1])
+        assert g.state()[2:] == o.state()[2:] and o.near_ties() == 0
+        ends = o.hops(0, hops)[0].astype(np.int64) + 1
+        m = np.diff(np.concatenate([[0], ends]))
+        its = int(sum(oracle_lib.pr_split(int(v), kw["M"])[0] for v in m))     # p = ceil(m / M) per hop (PAPER.md:39)
+        c = g.counters()
+        assert c["attempts"] == ends[-1] and c["iterations"] == its and c["proposals_evaluated"] == its * kw["M"]
