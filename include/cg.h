@@ -204,7 +204,11 @@ int cg_get_tuning(cg_sim* s, int* snapshot_interval, int* cluster_size);
  * previous outcome, testing its proposals and handing in its lowest accept, (update)
  * updating its part of the eps slab, (wait) waiting for the outcome of the iteration.
  * Per warp, propose + update + wait = total up to start-up; W_U per hop = update / warps /
- * hops, W_R per hop = (propose + wait) / warps / hops.  reset != 0 zeroes the counters. */
+ * hops, W_R per hop = (propose + wait) / warps / hops.  reset != 0 zeroes the counters.
+ * The timers cost a few per cent (three clock reads per warp and iteration), so they are off
+ * by default: cg_set_phase_timers(s, 1) makes the following cg_run calls use the timed build
+ * of the same kernel (544-thread launch shapes only; otherwise nothing is recorded). */
+int cg_set_phase_timers(cg_sim* s, int on);
 int cg_get_phase_cycles(cg_sim* s, uint64_t* total, uint64_t* wait, uint64_t* update,
                         uint64_t* propose, uint64_t* warps, int reset);
 

@@ -53,6 +53,12 @@ typedef unsigned int u32;
 #ifndef CG_XR
 #define CG_XR 4             // descriptor ring: the exchange warp may be this many iterations ahead of the slowest consumer
 #endif
+#ifndef CG_POLL_NS
+#define CG_POLL_NS 20       // pause between two looks at shared memory of the polling role warps
+#endif
+#ifndef CG_FRONT
+#define CG_FRONT 2048u      // labels below this are "near the front" of the window
+#endif
 #define CG_PB 8             // publication barriers (snapshots a CTA's workers may be ahead of its service warp)
 #define CG_HR 32            // hop ring: coded sites of the last CG_HR executed hops, for readers that catch up
 #define CG_RING 12          // eps snapshot buffers (see "snapshots" in pr_persistent_body)
@@ -86,6 +92,7 @@ struct CgCtl {              // device-resident control block (one per sim)
     u32 abort;              // != 0: the watchdog of the persistent kernel fired (which wait: see cg.h)
     u32 pad;
     u64 cyc_warps;          // worker warps that contributed to cyc_wait/update/propose
+    u64 dbg[16];
 };
 
 struct CgParams {           // kernel parameter block
@@ -215,13 +222,15 @@ __device__ __forceinline__ void mbar_arrive(u64* b)
 {
     asm volatile("mbarrier.arrive.release.cta.shared::cta.b64 _, [%0];" ::"r"(smem_u32(b)) : "memory");
 }
-__device__ __forceinline__ bool mbar_try(u64* b, u32 parity, u32 hint_ns)
+// one try: the hardware suspends the warp until the phase completes or a short, system-defined time has passed
+// (the variant with a suspend-time hint is compiled into a plain sleep of that length: never use it here)
+__device__ __forceinline__ bool mbar_try(u64* b, u32 parity)
 {
     u32 ok;
     asm volatile("{\n\t.reg .pred p;\n\t"
-                 "mbarrier.try_wait.parity.acquire.cta.shared::cta.b64 p, [%1], %2, %3;\n\t"
+                 "mbarrier.try_wait.parity.acquire.cta.shared::cta.b64 p, [%1], %2;\n\t"
                  "selp.b32 %0, 1, 0, p;\n\t}"
-                 : "=r"(ok) : "r"(smem_u32(b)), "r"(parity), "r"(hint_ns) : "memory");
+                 : "=r"(ok) : "r"(smem_u32(b)), "r"(parity) : "memory");
     return ok != 0;
 }
 __device__ __forceinline__ u32 cluster_ctarank()
@@ -286,7 +295,8 @@ struct Slab {
     static constexpr int R = RP > 0 ? RP : 1;
     double ea[R], eb[R];
     double ja[R], ia[R], jb[R], ib[R];
-    u32 sca[R], scb[R];                  // coded sites (spare bits set); 0 marks a site outside the slab
+    u32 sca[R], scb[R];                  // coded sites (spare bits set); sites outside the slab compute on code 0 and never store
+    u32 valid;                           // bit 2k: site a of block k is mine, bit 2k+1: site b
     u32 hci, hcj;
     u32 tix;                             // index of this thread among the TW threads that hold the slab
 
@@ -297,15 +307,17 @@ struct Slab {
 
     __device__ __forceinline__ void load(const double* src, double* work, u32 pr0, u32 pr1, const Geo& g, u32 t)
     {
-        tix = t;
+        tix = t; valid = 0u;
         if (RP > 0) {
 #pragma unroll
             for (int k = 0; k < RP; ++k) {
                 const u32 sa = site_a(pr0, k), sb = sa + 32u;
-                sca[k] = sa < 2u * pr1 ? g.code(sa) | g.spare : 0u;
-                scb[k] = sb < 2u * pr1 ? g.code(sb) | g.spare : 0u;
-                if (sca[k]) ea[k] = __ldcg(src + sa);
-                if (scb[k]) eb[k] = __ldcg(src + sb);
+                const bool va = sa < 2u * pr1, vb = sb < 2u * pr1;
+                valid |= (va ? 1u : 0u) << (2 * k) | (vb ? 1u : 0u) << (2 * k + 1);
+                sca[k] = va ? g.code(sa) | g.spare : g.spare;
+                scb[k] = vb ? g.code(sb) | g.spare : g.spare;
+                ea[k] = va ? __ldcg(src + sa) : 0.0;
+                eb[k] = vb ? __ldcg(src + sb) : 0.0;
             }
         } else if (work != src) {
             for (u32 s = 2u * pr0 + tix; s < 2u * pr1; s += TW) __stcg(work + s, __ldcg(src + s));
@@ -317,8 +329,8 @@ struct Slab {
         hci = ci; hcj = cj;
 #pragma unroll
         for (int k = 0; k < RP; ++k) {
-            if (sca[k]) { ja[k] = __ldg(tf + ((sca[k] - cj) & mask)); ia[k] = __ldg(tf + ((sca[k] - ci) & mask)); }
-            if (scb[k]) { jb[k] = __ldg(tf + ((scb[k] - cj) & mask)); ib[k] = __ldg(tf + ((scb[k] - ci) & mask)); }
+            ja[k] = __ldg(tf + ((sca[k] - cj) & mask)); ia[k] = __ldg(tf + ((sca[k] - ci) & mask));
+            jb[k] = __ldg(tf + ((scb[k] - cj) & mask)); ib[k] = __ldg(tf + ((scb[k] - ci) & mask));
         }
     }
 
@@ -329,10 +341,10 @@ struct Slab {
         if (RP > 0) {
 #pragma unroll
             for (int k = 0; k < RP; ++k) {
-                const u32 sa = site_a(pr0, k);
-                if (sca[k]) { ea[k] = __dadd_rn(ea[k], __dsub_rn(ja[k], ia[k])); if (snap) __stcg(snap + sa, ea[k]); }
-                if (scb[k]) { eb[k] = __dadd_rn(eb[k], __dsub_rn(jb[k], ib[k])); if (snap) __stcg(snap + sa + 32u, eb[k]); }
+                ea[k] = __dadd_rn(ea[k], __dsub_rn(ja[k], ia[k]));
+                eb[k] = __dadd_rn(eb[k], __dsub_rn(jb[k], ib[k]));
             }
+            if (snap) flush(work, snap, pr0, pr1);
         } else {
             for (u32 s = 2u * pr0 + tix; s < 2u * pr1; s += TW) {
                 const u32 c = g.code(s) | g.spare;
@@ -344,15 +356,15 @@ struct Slab {
         }
     }
 
-    // the slab as it stands, into a snapshot buffer (end of a launch)
+    // the slab as it stands, into a snapshot buffer
     __device__ __forceinline__ void flush(const double* work, double* snap, u32 pr0, u32 pr1) const
     {
         if (RP > 0) {
 #pragma unroll
             for (int k = 0; k < RP; ++k) {
                 const u32 sa = site_a(pr0, k);
-                if (sca[k]) __stcg(snap + sa, ea[k]);
-                if (scb[k]) __stcg(snap + sa + 32u, eb[k]);
+                if ((valid >> (2 * k)) & 1u) __stcg(snap + sa, ea[k]);
+                if ((valid >> (2 * k + 1)) & 1u) __stcg(snap + sa + 32u, eb[k]);
             }
         } else {
             for (u32 s = 2u * pr0 + tix; s < 2u * pr1; s += TW) __stcg(snap + s, __ldcg(work + s));
@@ -450,6 +462,12 @@ struct __align__(16) Comm {
     u32 xe;                 // iterations decided so far
 };
 
+#ifdef CG_TRACE2
+#define TR(slot, k) do { if (lane == 0 && b == 0 && e - 2000u < 16u) reinterpret_cast<u64*>(p.work)[(((e - 2000u) * 20u + (slot)) * 4u) + (k)] = (u64)clock64(); } while (0)
+#else
+#define TR(slot, k) do { } while (0)
+#endif
+
 struct Waiter {             // watchdog state of one waiting warp
     u64 t0; u32 spins;
     __device__ __forceinline__ void reset() { t0 = 0; spins = 0; }
@@ -476,13 +494,11 @@ __device__ __forceinline__ bool wait_poll(Waiter& w, const CgParams& p, Comm* cm
 // wait for the phase with this parity of an mbarrier; false: gave up
 __device__ __forceinline__ bool mbar_wait(u64* b, u32 parity, const CgParams& p, Comm* cm, u32 code)
 {
-    if (mbar_try(b, parity, 2000u)) return true;
+    if (mbar_try(b, parity)) return true;
     Waiter w; w.reset();
-    u32 n = 0;
     for (;;) {
-        if (mbar_try(b, parity, 20000u)) return true;
-        if (*(volatile u32*)&cm->abort) return false;
-        if (((++n) & 15u) == 0u) { w.spins = 1023u; if (wait_poll(w, p, cm, code)) return false; }
+        if (mbar_try(b, parity)) return true;
+        if (wait_poll(w, p, cm, code)) return false;
     }
 }
 
@@ -495,8 +511,8 @@ __device__ __forceinline__ bool mbar_wait(u64* b, u32 parity, const CgParams& p,
 // Otherwise (M > P) CTA b evaluates labels [b per, (b+1) per) from scratch in every iteration, with the
 // warps of the CTA in lock step (the occupation bitmap is then always current).
 //
-// Roles: warps 0 .. NW-1 workers; warp NW the collector (C); NW+1 the exchange warp (X); NW+2 the
-// service warp (S).  Iteration e ("exchange"), state S_e before it, outcome O_e:
+// Roles: warp 0 the collector (C), 1 the exchange warp (X), 2 the service warp (S), warps 3 .. NW+2 the
+// workers.  Iteration e ("exchange"), state S_e before it, outcome O_e:
 //   worker:  test own label on S_e -> res[e][warp]; slab update of the hop of O_{e-1}; wait for O_e (mbarrier
 //            full[e]); consume it (labels, occupations of the followed pair, followed energies); arrive empty[e]
 //   C:       reduce res[e][*] in label order, stopping at the first accept -> own[e], the CTA's slot in L2
@@ -520,7 +536,7 @@ __device__ __forceinline__ bool mbar_wait(u64* b, u32 parity, const CgParams& p,
 //
 // Written as a device function of (parameters, CTA index, CTA count) so that one launch can also hold
 // several sims side by side (cg_pr_persistent_many): nothing in it looks at blockIdx or gridDim.
-template <int NW, int RP, bool CACHED>
+template <int NW, int RP, bool CACHED, bool TIMED>
 __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 b, const u32 nb)
 {
     constexpr int TW = NW * 32;           // worker threads
@@ -538,21 +554,24 @@ __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 
     const Tables tb = {s_cdfi, s_invr, s_fld, s_disp, s_guide, p.cdfi, p.invr_k, p.fld_k, p.disp, (u32)KS};
     const Geo geo = {p.hi1, p.hi2, p.spare, p.mask, (u32)(p.L - 1), p.lgL};
 
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    // the three role warps come first: the warp arbiter prefers high warp ids, and the pollers must not
+    // take issue slots from the workers of their sub-partition
+    const int lane = threadIdx.x & 31, role = threadIdx.x >> 5, warp = role - 3, tid = (int)threadIdx.x - 96;
+    const int atid = threadIdx.x;         // index among all threads (set-up loops)
     const u32 N = p.N, M = p.M, mask = p.mask;
     const double* __restrict__ tf = p.tf;
     const u32 Hs = p.snap_shift, Hm = (1u << Hs) - 1u;
 
-    for (int k = tid; k < KS; k += THREADS) {
+    for (int k = atid; k < KS; k += THREADS) {
         s_cdfi[k] = p.cdfi[k]; s_invr[k] = p.invr_k[k]; s_fld[k] = p.fld_k[k]; s_disp[k] = p.disp[k];
     }
-    for (int k = tid; k < CG_GUIDE; k += THREADS) s_guide[k] = p.guide[k];
-    for (u32 w = tid; w < (N + 31) / 32; w += THREADS) s_n[w] = p.nbits[w];
+    for (int k = atid; k < CG_GUIDE; k += THREADS) s_guide[k] = p.guide[k];
+    for (u32 w = atid; w < (N + 31) / 32; w += THREADS) s_n[w] = p.nbits[w];
     // no record may look like one of this launch: tag them with the epoch before its first
     const u64 stale = (u64)((u32)p.ctl->epoch - 1u) << 32;
-    for (u32 k = tid; k < sizeof(cm->res) / 8; k += THREADS) (&cm->res[0][0][0])[k] = stale;
-    for (u32 k = tid; k < sizeof(cm->peer) / 8; k += THREADS) (&cm->peer[0][0][0])[k] = stale;
-    if (tid == 0) {
+    for (u32 k = atid; k < sizeof(cm->res) / 8; k += THREADS) (&cm->res[0][0][0])[k] = stale;
+    for (u32 k = atid; k < sizeof(cm->peer) / 8; k += THREADS) (&cm->peer[0][0][0])[k] = stale;
+    if (atid == 0) {
         for (int k = 0; k < CG_XR; ++k) {
             mbar_init(&cm->full[k], 1); mbar_init(&cm->empty[k], NW + 1);
             cm->own[k][0] = stale; cm->own[k][1] = 0;
@@ -584,7 +603,7 @@ __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 
     u64* const my_slot = p.slots + (size_t)b * CG_SLOT_U64;
     const u32 n_snaps = n_hops >> Hs;     // regular snapshots of this launch
 
-    if (warp == NW + 2) {
+    if (role == 2) {
         // ------------------------------------------------------------------ service warp ----
         for (u32 s = 1; s <= n_snaps; ++s) {
             if (!mbar_wait(&cm->pubbar[(s - 1) % CG_PB], ((s - 1) / CG_PB) & 1u, p, cm, 1u)) break;
@@ -606,7 +625,7 @@ __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 
             fence_acquire_gpu();
             if (lane == 0 && vmin > pub_base) max_release_cta(&cm->ver, (u32)(vmin - pub_base));    // stale words are smaller
         }
-    } else if (warp == NW) {
+    } else if (role == 0) {
         // ---------------------------------------------------------------- collector warp ----
         // The CTA's lowest accepting label of every iteration (step 3), found in label order:
         // lane r looks at the r-th warp in that order.  In scan order every worker warp holds lower labels
@@ -614,6 +633,7 @@ __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 
         // the window hold its END ("tail" labels >= tail0): those rank after every other label.
         u32 cf = c_first, tr = t0r;
         Waiter wd;
+        u64 dc_poll = 0, dc_post = 0, dc_desc = 0; long long dc_t = clock64();
         for (u32 e = 0;; ++e) {
             const u32 xs = e % CG_XR, e32 = e_start + e;
             const u32 kb = b >= cf ? b - cf : b + nb - cf;
@@ -652,8 +672,11 @@ __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 
                     break;
                 }
                 if (wait_poll(wd, p, cm, 2u)) { quit = true; break; }
+                __nanosleep(CG_POLL_NS);
             }
             if (quit) break;
+            TR(14, 0);
+            { const long long n_ = clock64(); dc_poll += (u64)(n_ - dc_t); dc_t = n_; }
             // post: own[] for the exchange warp, the slot in L2 for the other CTAs, the peers' shared memory
             const u64 s0 = ((u64)e32 << 32) | gmin;
             if (lane == 0) sts128(&cm->own[xs][0], s0, gpay);
@@ -666,8 +689,12 @@ __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 
                 }
                 if (lane == 0) slot_store(my_slot + 2u * ring, s0, s1);
             }
+            TR(14, 1);
+            { const long long n_ = clock64(); dc_post += (u64)(n_ - dc_t); dc_t = n_; }
             // consume O_e
             if (!mbar_wait(&cm->full[xs], (e / CG_XR) & 1u, p, cm, 3u)) break;
+            TR(14, 2);
+            { const long long n_ = clock64(); dc_desc += (u64)(n_ - dc_t); dc_t = n_; }
             const uint4 d0 = lds128u(&cm->desc[xs]);
             const uint4 d1 = lds128u(&cm->desc[xs].c_first);
             __syncwarp();
@@ -675,7 +702,8 @@ __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 
             if (d0.y & (CG_F_LAST | CG_F_ABORT)) break;
             cf = d1.x; tr = d1.y;
         }
-    } else if (warp == NW + 1) {
+
+    } else if (role == 1) {
         // ----------------------------------------------------------------- exchange warp ----
         const u64 log_base = p.ctl->log_base, hops_start = p.ctl->hops;
         u64 used_sum = 0;                 // attempts consumed in this launch
@@ -685,24 +713,29 @@ __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 
         u32 ver = 0;                      // newest snapshot known to be published by every CTA
         Waiter wd;
         bool quit = false;
+        u64 dx_[5] = {0, 0, 0, 0, 0}; long long dx_t = clock64();
+        u64 dcase[5] = {0, 0, 0, 0, 0}, dcnt[5] = {0, 0, 0, 0, 0}; long long dlast = clock64();
+#define DXT(k) { const long long n_ = clock64(); dx_[k] += (u64)(n_ - dx_t); dx_t = n_; }
         // the hop of descriptor ea goes into the bitmap (every warp has consumed it)
         auto apply = [&](u32 ea) {
             const uint4 d0 = lds128u(&cm->desc[ea % CG_XR]);
-            if (lane == 0 && (d0.y & CG_F_HOP)) {
+            if (lane == 0 && (d0.y & CG_F_HOP)) {         // this warp is the only writer; volatile stores of one thread stay in order
                 const u32 si = geo.site(d0.z), sj = geo.site(d0.w);
-                atomicAnd(&s_n[si >> 5], ~(1u << (si & 31)));
-                atomicOr(&s_n[sj >> 5], 1u << (sj & 31));
-                __threadfence_block();
-                *(volatile u32*)&cm->nlow = cm->desc[ea % CG_XR].hopno;
+                volatile u32* w = s_n;
+                w[si >> 5] &= ~(1u << (si & 31));
+                w[sj >> 5] |= 1u << (sj & 31);
+                *(volatile u32*)&cm->nlow = *(volatile u32*)&cm->desc[ea % CG_XR].hopno;
             }
         };
         while (hc < n_hops) {
             const u32 xs = e % CG_XR, e32 = e_start + e;
+            TR(15, 0);
             // (1) recycle the descriptor slot: every consumer is past iteration e - CG_XR
             if (CACHED && e >= CG_XR) {
                 if (!mbar_wait(&cm->empty[xs], ((e - CG_XR) / CG_XR) & 1u, p, cm, 4u)) { quit = true; break; }
                 apply(e_app); ++e_app;
             }
+            DXT(0)
             // (2) gate: every CTA has published the snapshot that covers hop hc + 1 - G
             if (nb > 1 && hc + 1u > p.gate) {
                 const u32 need = (hc + 1u - p.gate) >> Hs;
@@ -732,6 +765,8 @@ __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 
                     if (lane == 0) max_release_cta(&cm->ver, need);
                 }
             }
+            DXT(1)
+            TR(15, 1);
             // (3) the first accepting CTA in scan order (step 3).  Position 0 holds the start of
             // the window; a window of scan positions is polled at a time, starting narrow (the winner is nearly
             // always at the first positions), and polling stops at the first accept: posts of later CTAs are
@@ -740,6 +775,7 @@ __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 
             const u32 tail0 = CACHED ? per - t0r : CG_NONE;
             const u32 ring = e32 & (CG_SRING - 1u), e16 = e32 & 0xFFFFu;
             u32 q = CG_NONE; u64 wp = 0;
+            u32 wpos = 0xFFFFu;
             u32 tlab = CG_NONE; u64 tpay = 0;                          // tail accept of position 0
             u32 lo = 0, hi = kb == 0 ? 1u : min(nb, 4u);
             wd.reset();
@@ -771,11 +807,13 @@ __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 
                     const int fa = racc ? __ffs(racc) - 1 : 32, fn = rnot ? __ffs(rnot) - 1 : 32;
                     if (fa < fn) {                      // first accepting position, everything before it rejected
                         q = __shfl_sync(CG_FULL, l, fa); wp = __shfl_sync(CG_FULL, pay, fa);
+                        wpos = lo + (u32)fa;
                         found = true;
                         break;
                     }
                     if (!rnot) break;                   // whole window rejected: widen
                     if (kb != 0 || lo != 0) wd.spins |= 63u;      // polls through L2 are slow: look at the clock more often
+                    else __nanosleep(CG_POLL_NS);                 // shared memory only: leave the issue slots to the workers
                     if (wait_poll(wd, p, cm, 6u)) { quit = true; break; }
                 }
                 if (quit || found) break;
@@ -783,6 +821,8 @@ __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 
                 lo = hi; hi = min(nb, lo + 32u);
             }
             if (quit) break;
+            DXT(2)
+            TR(15, 2);
             if (q == CG_NONE && tlab != CG_NONE) { q = tlab; wp = tpay; }   // only the tail of the window accepted
             // lock step (not CACHED): every warp of this CTA has finished its tests of this iteration before the
             // bitmap changes
@@ -800,8 +840,8 @@ __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 
             // (4) publish O_e: attempts consumed (m = (p-1)M + q per executed hop), the hop
             // (step 3a)
             const u32 used = q == CG_NONE ? M : q + 1;
-            const u32 hi_ = (u32)(wp >> 32), hj_ = (u32)wp;
-            const u32 ci = geo.code(hi_), cj = geo.code(hj_);
+            const u32 ci = (u32)(wp >> 32), cj = (u32)wp;               // coded sites
+            const u32 hi_ = geo.site(ci), hj_ = geo.site(cj);
             const bool hop = q != CG_NONE;
             if (CACHED) {
                 if (t0r + used < per) t0r += used;
@@ -825,6 +865,13 @@ __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 
                 mbar_arrive(&cm->full[xs]);   // release: the stores above are visible to whoever sees the phase complete
                 *(volatile u32*)&cm->xe = e + 1u;
             }
+            TR(15, 3);
+            DXT(3)
+            {   // debug: time between publications by case
+                const long long n_ = clock64();
+                const int cls = kb == 0 ? (wpos == 0 ? 0 : 1) : (wpos == kb ? 2 : (kb == 1 ? 3 : 4));
+                dcase[cls] += (u64)(n_ - dlast); dcnt[cls] += 1; dlast = n_;
+            }
             // (5) the rest of the bookkeeping, off the critical path
             used_sum += used;
             ++e;
@@ -835,7 +882,9 @@ __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 
                     p.log_a[h] = a_start + used_sum - 1; p.log_i[h] = hi_; p.log_j[h] = hj_;
                 }
             }
+            DXT(4)
         }
+        if (lane == 0) for (int k = 0; k < 5; ++k) { atomicAdd(&p.ctl->dbg[k], dcase[k]); atomicAdd(&p.ctl->dbg[8 + k], dcnt[k]); }
         if (quit) {                       // let the consumers of this CTA go (they see the abort flag in their waits)
             if (lane == 0) *(volatile u32*)&cm->abort = 1u;
             return;
@@ -880,8 +929,7 @@ __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 
         // occupations of a pair as of hop hl: the bitmap (complete up to hop nlow, never ahead of me) and the
         // newer hops replayed in order
         auto read_n = [&](u32 ci, u32 cj, bool& oi, bool& oj) {
-            const u32 vl = *(volatile u32*)&cm->nlow;
-            __threadfence_block();
+            const u32 vl = *(volatile u32*)&cm->nlow;         // read before the bits (volatile accesses of one thread stay in order)
             const u32 si = geo.site(ci), sj = geo.site(cj);
             bool a = BIT((volatile u32*)s_n, si) != 0u, c = BIT((volatile u32*)s_n, sj) != 0u;
             for (u32 h = vl + 1u; h <= hl; ++h) {
@@ -919,28 +967,54 @@ __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 
         }
         u64 a0 = a_start;                 // first attempt of the window (used when labels are not cached)
         bool upd = false, last = false;
-        u32 hci = 0, hcj = 0;
+        bool fresh = false;               // my attempt was consumed: the next one is not taken over yet
         double a_i = 0, b_i = 0, a_j = 0, b_j = 0;    // gathers in flight for the followed pair
         bool addterm = false;
         u64 t_test = 0, t_slab = 0, t_wait = 0;
-        long long tprev = clock64();
+        long long tprev = TIMED ? clock64() : 0;
+        // take over the next attempt (decoded ahead of time as a rule) and the occupations of its pair
+        auto refresh = [&]() {
+            if (!nxt_valid) nxt = decode_attempt(tb, p, geo, a_cur);
+            take(nxt); nxt_valid = false;
+            read_n(sci & mask, scj & mask, ni, nj);
+            fresh = false;
+        };
+        // the test of my proposal on the current state (steps 1-2)
+        auto test_mine = [&](u32& best) {
+            const bool th = lab < M && ni && !nj;                 // theta_ij, inside the window
+            if (th) {
+                if (!tracked) { read_eps(sci, scj, ei, ej); tracked = true; }
+                else if (addterm) {           // the term of the hop consumed last (gathered when it was consumed)
+                    ei = __dadd_rn(ei, __dsub_rn(a_i, b_i)); ej = __dadd_rn(ej, __dsub_rn(a_j, b_j));
+                }
+                // dH_ij = eps_j - eps_i - 1/r_ij - E dx_ij
+                const double dE = __dsub_rn(__dsub_rn(__dsub_rn(ej, ei), c_invr), c_fld);
+                if (metropolis(dE, cuh, cul, p.T, p.inv_T)) best = lab;
+            } else tracked = false;
+        };
         for (u32 e = 0;; ++e) {
             const u32 xs = e % CG_XR, e32 = e_start + e;
             // ---- steps 1-2: propose and test on S_e, state untouched
             u32 best = CG_NONE, bi = 0, bj = 0;
             if (CACHED) {
-                if (has_label) {
-                    const bool th = lab < M && ni && !nj;             // theta_ij, inside the window
-                    if (th) {
-                        if (!tracked) { read_eps(sci, scj, ei, ej); tracked = true; }
-                        else if (addterm) {       // the term of the hop consumed last (gathered below)
-                            ei = __dadd_rn(ei, __dsub_rn(a_i, b_i)); ej = __dadd_rn(ej, __dsub_rn(a_j, b_j));
-                        }
-                        // dH_ij = eps_j - eps_i - 1/r_ij - E dx_ij
-                        const double dE = __dsub_rn(__dsub_rn(__dsub_rn(ej, ei), c_invr), c_fld);
-                        if (metropolis(dE, cuh, cul, p.T, p.inv_T)) { best = lab; bi = sci; bj = scj; }
-                    } else tracked = false;
+                if (has_label && !fresh) test_mine(best);
+                addterm = false;
+                u32 wmin = __reduce_min_sync(CG_FULL, best);
+                // A thread whose attempt was consumed takes over its next one AFTER the warp has handed in its
+                // result: the new label is higher than every other label of the warp (P - used or more), so it
+                // can only matter when it lies inside the window and nothing else in the warp accepts.
+                if (wmin == CG_NONE && __any_sync(CG_FULL, fresh && lab < M)) {
+                    if (fresh) { refresh(); test_mine(best); }
+                    wmin = __reduce_min_sync(CG_FULL, best);
                 }
+                // ---- step 3: lowest accepting label of the warp, for the collector
+                TR(warp, 1);
+                if (wmin == CG_NONE ? lane == 0 : best == wmin) {   // labels are distinct: one lane
+                    sts128(&cm->res[e % (2 * CG_XR)][warp][0], ((u64)e32 << 32) | wmin,
+                           ((u64)(sci & mask) << 32) | (u64)(scj & mask));
+                }
+                TR(warp, 2);
+                if (fresh) refresh();
             } else {
                 for (u32 l = lab0 + tid; l < lab1; l += TW) {
                     const Prop q = decode_attempt(tb, p, geo, a0 + l);
@@ -952,21 +1026,21 @@ __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 
                     const double dE = __dsub_rn(__dsub_rn(__dsub_rn(vj, vi), tb.inv(q.k)), tb.field(q.k));
                     if (metropolis(dE, q.uh, q.ul, p.T, p.inv_T)) { best = l; bi = q.ci; bj = q.cj; break; }
                 }
-            }
-            addterm = false;
-            // ---- step 3: lowest accepting label of the warp, for the collector
-            {
                 const u32 wmin = __reduce_min_sync(CG_FULL, best);
-                if (wmin == CG_NONE ? lane == 0 : best == wmin)     // labels are distinct: one lane
-                    sts128(&cm->res[e % (2 * CG_XR)][warp][0], ((u64)e32 << 32) | wmin,
-                           ((u64)geo.site(bi & mask) << 32) | (u64)geo.site(bj & mask));
+                if (wmin == CG_NONE ? lane == 0 : best == wmin) {
+                    sts128(&cm->res[e % (2 * CG_XR)][warp][0], ((u64)e32 << 32) | wmin, ((u64)bi << 32) | (u64)bj);
+                }
             }
-            const long long t1 = clock64();
-            t_test += (u64)(t1 - tprev);
-            // ---- step 3b for my part of the slab: the hop consumed last; behind its gathers the
-            // decode one attempt ahead
-            if (upd) slab.issue(tf, mask, hci, hcj);
-            if (has_label && !nxt_valid) { nxt = decode_attempt(tb, p, geo, a_cur + P); nxt_valid = true; }
+            long long t1 = 0;
+            if (TIMED) { t1 = clock64(); t_test += (u64)(t1 - tprev); }
+            // ---- step 3b for my part of the slab: the hop consumed last (its table gathers were
+            // issued when it was consumed, behind those of the followed pair); first the decode one attempt ahead
+            // (a warp near the front of the window is on the critical path of the next iterations: its decode waits
+            // until all of its labels have been consumed and it sits at the far end of the window)
+            if (CACHED) {
+                const bool far = __reduce_min_sync(CG_FULL, lab) >= CG_FRONT;      // warp-uniform
+                if (far && has_label && !nxt_valid) { nxt = decode_attempt(tb, p, geo, a_cur + P); nxt_valid = true; }
+            }
             if (upd) {
                 const bool snap = (hl & Hm) == 0u;
                 u32 buf = cur0 + (hl >> Hs) % CG_RING; if (buf >= CG_RING) buf -= CG_RING;
@@ -977,54 +1051,51 @@ __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 
                 }
                 upd = false;
             }
-            const long long t2 = clock64();
-            t_slab += (u64)(t2 - t1);
+            long long t2 = 0;
+            if (TIMED) { t2 = clock64(); t_slab += (u64)(t2 - t1); }
             if (last) break;
+            TR(warp, 3);
             // ---- O_e
             if (!mbar_wait(&cm->full[xs], (e / CG_XR) & 1u, p, cm, 8u)) return;
+            { const u32 e_ = e; { const u32 e = e_ + 1u; TR(warp, 0); } }
             const uint4 d = lds128u(&cm->desc[xs]);        // used, flags, ci, cj
             __syncwarp();
             if (lane == 0) mbar_arrive(&cm->empty[xs]);
-            tprev = clock64();
-            t_wait += (u64)(tprev - t2);
+            if (TIMED) { tprev = clock64(); t_wait += (u64)(tprev - t2); }
             if (d.y & CG_F_ABORT) return;
             last = (d.y & CG_F_LAST) != 0u;
-            const bool newhop = (d.y & CG_F_HOP) != 0u;
-            if (CACHED) {
-                // the term of this hop for the pair I follow: the four gathers start before the label
-                // bookkeeping (discarded if my attempt was consumed or theta_ij turns out to have changed)
-                if (tracked && newhop) {
-                    a_i = __ldg(tf + ((sci - d.w) & mask)); b_i = __ldg(tf + ((sci - d.z) & mask));
-                    a_j = __ldg(tf + ((scj - d.w) & mask)); b_j = __ldg(tf + ((scj - d.z) & mask));
-                    addterm = true;
-                }
-                if (newhop) {
-                    ++hl; hci = d.z; hcj = d.w; upd = true;
+            if (d.y & CG_F_HOP) {
+                if (CACHED) {
+                    // the term of this hop for the pair I follow: the four gathers come first (discarded if my
+                    // attempt was consumed or theta_ij turns out to have changed), then the slab's
+                    if (tracked) {
+                        a_i = __ldg(tf + ((sci - d.w) & mask)); b_i = __ldg(tf + ((sci - d.z) & mask));
+                        a_j = __ldg(tf + ((scj - d.w) & mask)); b_j = __ldg(tf + ((scj - d.z) & mask));
+                        addterm = true;
+                    }
                     const u32 si = d.z | geo.spare, sj = d.w | geo.spare;
                     if (sci == si) ni = false; if (sci == sj) ni = true;
                     if (scj == si) nj = false; if (scj == sj) nj = true;
                 }
-                if (has_label && d.x) {
+                ++hl; upd = true;
+                slab.issue(tf, mask, d.z, d.w);
+            }
+            if (CACHED) {
+                if (has_label) {
                     if (lab >= d.x) lab -= d.x;
                     else {                              // my attempt was consumed: the next one, P attempts later
                         lab += P - d.x; a_cur += P;
-                        if (!nxt_valid) nxt = decode_attempt(tb, p, geo, a_cur);
-                        take(nxt); nxt_valid = false;
-                        addterm = false;
-                        read_n(sci & mask, scj & mask, ni, nj);
+                        fresh = true; tracked = false; addterm = false;
                     }
                 }
-            } else {
-                a0 += d.x;
-                if (newhop) { ++hl; hci = d.z; hcj = d.w; upd = true; }
-            }
+            } else a0 += d.x;
         }
         // the final state of my part of the slab, unless the last hop was a snapshot anyway
         if (n_hops & Hm) {
             u32 buf = cur0 + (n_snaps + 1u) % CG_RING; if (buf >= CG_RING) buf -= CG_RING;
             slab.flush(p.work, p.eps[buf], pr0, pr1);
         }
-        if (b == 0 && lane == 0) {
+        if (TIMED && b == 0 && lane == 0) {
             atomicAdd(&p.ctl->cyc_propose, t_test); atomicAdd(&p.ctl->cyc_update, t_slab);
             atomicAdd(&p.ctl->cyc_wait, t_wait); atomicAdd(&p.ctl->cyc_warps, 1ull);
         }
@@ -1037,10 +1108,10 @@ __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 
     if (csz > 1) cluster_sync_all();
 }
 
-template <int NW, int RP, bool CACHED>
+template <int NW, int RP, bool CACHED, bool TIMED>
 __global__ void __launch_bounds__(NW * 32 + 96, 1) cg_pr_persistent(const CgParams p)
 {
-    pr_persistent_body<NW, RP, CACHED>(p, blockIdx.x, gridDim.x);
+    pr_persistent_body<NW, RP, CACHED, TIMED>(p, blockIdx.x, gridDim.x);
 }
 
 // Replica packing (the paper recommends averaging many samples): ONE launch,
@@ -1058,7 +1129,7 @@ cg_pr_persistent_many(const CgParams* __restrict__ ps, const u32* __restrict__ f
         sp = ps[s];
     }
     __syncthreads();
-    pr_persistent_body<NW, RP, CACHED>(sp, s_b, s_nb);
+    pr_persistent_body<NW, RP, CACHED, false>(sp, s_b, s_nb);
 }
 
 __device__ __forceinline__ Geo make_geo(const CgParams& p)
@@ -1245,6 +1316,7 @@ struct cg_sim {
     int num_sms = 0, n_ctas = 0, threads = 0, smem = 0, rp = 0, pl = 0;   // pl > 0: cached proposals
     int snap_shift = 2;                   // snapshots every 4 hops
     int cluster = 1;                      // CTAs per thread-block cluster
+    bool timers = false;                  // cg_set_phase_timers
     u64 watchdog_ns = 10ull * 1000 * 1000 * 1000;
     std::string err;
 };
@@ -1436,16 +1508,17 @@ static CgParams make_params(const cg_sim* s, u32 n_hops)
 typedef void (*persist_fn)(const CgParams);
 typedef void (*scripted_fn)(const CgParams, const u32*, const u32*, u64);
 
-// RP = eps pairs a thread keeps in registers (0: the slab lives in a working buffer in global memory)
-template <int NW, bool CACHED>
+// RP = eps pairs a thread keeps in registers (0: the slab lives in a working buffer in global memory);
+// TIMED: with the phase timers of cg_get_phase_cycles (544-thread shapes only)
+template <int NW, bool CACHED, bool TIMED>
 static persist_fn persistent_kernel_t(int rp)
 {
     switch (rp) {
-        case 0: return cg_pr_persistent<NW, 0, CACHED>;
-        case 1: return cg_pr_persistent<NW, 1, CACHED>;
-        case 2: return cg_pr_persistent<NW, 2, CACHED>;
-        case 4: if (NW <= 16) return cg_pr_persistent<NW <= 16 ? NW : 5, 4, CACHED>; break;
-        case 8: if (NW <= 14) return cg_pr_persistent<NW <= 14 ? NW : 5, 8, CACHED>; break;
+        case 0: return cg_pr_persistent<NW, 0, CACHED, TIMED>;
+        case 1: return cg_pr_persistent<NW, 1, CACHED, TIMED>;
+        case 2: return cg_pr_persistent<NW, 2, CACHED, TIMED>;
+        case 4: if (NW <= 16) return cg_pr_persistent<NW <= 16 ? NW : 5, 4, CACHED, NW <= 16 ? TIMED : false>; break;
+        case 8: if (NW <= 14) return cg_pr_persistent<NW <= 14 ? NW : 5, 8, CACHED, NW <= 14 ? TIMED : false>; break;
     }
     return nullptr;
 }
@@ -1455,13 +1528,14 @@ static int workers_of(int threads)
     switch (threads) { case 256: return 5; case 544: return 14; case 608: return 16; case 1024: return 29; }
     return 0;
 }
-static persist_fn persistent_kernel(int threads, int rp, bool cached)
+static persist_fn persistent_kernel(int threads, int rp, bool cached, bool timed)
 {
     switch (workers_of(threads)) {
-        case 5: return cached ? persistent_kernel_t<5, true>(rp) : persistent_kernel_t<5, false>(rp);
-        case 14: return cached ? persistent_kernel_t<14, true>(rp) : persistent_kernel_t<14, false>(rp);
-        case 16: return cached ? persistent_kernel_t<16, true>(rp) : persistent_kernel_t<16, false>(rp);
-        case 29: return cached ? persistent_kernel_t<29, true>(rp) : persistent_kernel_t<29, false>(rp);
+        case 5: return cached ? persistent_kernel_t<5, true, false>(rp) : persistent_kernel_t<5, false, false>(rp);
+        case 14: if (timed) return cached ? persistent_kernel_t<14, true, true>(rp) : persistent_kernel_t<14, false, true>(rp);
+                 return cached ? persistent_kernel_t<14, true, false>(rp) : persistent_kernel_t<14, false, false>(rp);
+        case 16: return cached ? persistent_kernel_t<16, true, false>(rp) : persistent_kernel_t<16, false, false>(rp);
+        case 29: return cached ? persistent_kernel_t<29, true, false>(rp) : persistent_kernel_t<29, false, false>(rp);
     }
     return nullptr;
 }
@@ -1509,9 +1583,11 @@ static int rp_cap(int threads) { return threads == 1024 ? 2 : threads == 608 ? 4
 // how many CTAs of this shape can be co-resident (in clusters of s->cluster)
 static int max_coresident(cg_sim* s, int threads, int rp, bool cached, int* out)
 {
-    persist_fn f = persistent_kernel(threads, rp, cached);
+    persist_fn f = persistent_kernel(threads, rp, cached, false);
     if (!f) return CG_EINVAL;
     CK(cudaFuncSetAttribute((const void*)f, cudaFuncAttributeMaxDynamicSharedMemorySize, s->smem));
+    if (persist_fn ft = threads == 544 ? persistent_kernel(threads, rp, cached, true) : nullptr)
+        CK(cudaFuncSetAttribute((const void*)ft, cudaFuncAttributeMaxDynamicSharedMemorySize, s->smem));
     if (s->cluster > 1) {
         if (s->cluster > 8) CK(cudaFuncSetAttribute((const void*)f, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
         cudaLaunchConfig_t cfg = {};
@@ -1718,7 +1794,7 @@ static cudaError_t launch_coop(const void* f, int grid, int threads, int smem, c
 extern "C" int cg_run(cg_sim* s, uint64_t n_hops)
 {
     if (!s) return CG_EINVAL;
-    persist_fn f = persistent_kernel(s->threads, s->rp, s->pl > 0);
+    persist_fn f = persistent_kernel(s->threads, s->rp, s->pl > 0, s->timers && s->threads == 544);
     if (!f) return CG_EINVAL;
     while (n_hops) {
         const u32 chunk = (u32)std::min<uint64_t>(n_hops, CG_MAX_LAUNCH_HOPS);
@@ -2059,6 +2135,13 @@ extern "C" int cg_get_tuning(cg_sim* s, int* snapshot_interval, int* cluster_siz
     return CG_OK;
 }
 
+extern "C" int cg_set_phase_timers(cg_sim* s, int on)
+{
+    if (!s) return CG_EINVAL;
+    s->timers = on != 0;
+    return CG_OK;
+}
+
 extern "C" int cg_get_phase_cycles(cg_sim* s, uint64_t* total, uint64_t* wait, uint64_t* update,
                                    uint64_t* propose, uint64_t* warps, int reset)
 {
@@ -2071,7 +2154,13 @@ extern "C" int cg_get_phase_cycles(cg_sim* s, uint64_t* total, uint64_t* wait, u
     if (update) *update = c.cyc_update;
     if (propose) *propose = c.cyc_propose;
     if (warps) *warps = c.cyc_warps;
+    if (getenv("CG_DBG")) {
+        fprintf(stderr, "dbg:");
+        for (int k = 0; k < 16; ++k) fprintf(stderr, " %llu", (unsigned long long)c.dbg[k]);
+        fprintf(stderr, "\n");
+    }
     if (reset) {
+        for (int k = 0; k < 16; ++k) c.dbg[k] = 0;
         c.cyc_total = c.cyc_wait = c.cyc_update = c.cyc_propose = c.cyc_warps = 0;
         CK(cudaMemcpyAsync(s->d_ctl, &c, sizeof c, cudaMemcpyHostToDevice, s->stream));
         CK(cudaStreamSynchronize(s->stream));
