@@ -777,8 +777,30 @@ __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 
             u32 q = CG_NONE; u64 wp = 0;
             u32 wpos = 0xFFFFu;
             u32 tlab = CG_NONE; u64 tpay = 0;                          // tail accept of position 0
-            u32 lo = 0, hi = kb == 0 ? 1u : min(nb, 4u);
+            u32 lo = 0, hi = min(nb, 4u);
             wd.reset();
+            if (CACHED && kb == 0) {
+                // My own workers hold the start of the window: their results, read directly in label order (the
+                // collector does the same for the other CTAs' sake, but its hand-over would be one more hop on the path).
+                // A head accept of mine decides the iteration; otherwise the scan below goes on from my own post.
+                const u32 w0 = t0r >> 5;
+                u32 wr = w0 + (u32)lane; if (wr >= (u32)NW) wr -= NW;
+                bool ready = lane >= NW; u32 l = CG_NONE; u64 pay = 0;
+                for (;;) {
+                    if (!ready) {
+                        u64 q0, q1;
+                        lds128(&cm->res[e % (2 * CG_XR)][wr][0], q0, q1);
+                        if ((u32)(q0 >> 32) == e32) { ready = true; pay = q1; const u32 v = (u32)q0; if (v < tail0) l = v; }
+                    }
+                    const u32 racc = __ballot_sync(CG_FULL, ready && l != CG_NONE);
+                    const u32 rnot = __ballot_sync(CG_FULL, !ready);
+                    const int fa = racc ? __ffs(racc) - 1 : 32, fn = rnot ? __ffs(rnot) - 1 : 32;
+                    if (fa < fn) { q = __shfl_sync(CG_FULL, l, fa); wp = __shfl_sync(CG_FULL, pay, fa); wpos = 0; lo = nb; break; }
+                    if (!rnot) break;                   // no head accept here: the general scan (my tail labels come from own[])
+                    if (wait_poll(wd, p, cm, 6u)) { quit = true; break; }
+                }
+                if (quit) break;
+            }
             while (lo < nb) {
                 const u32 k = lo + (u32)lane;
                 const bool mine = k < hi;
@@ -968,6 +990,8 @@ __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 
         u64 a0 = a_start;                 // first attempt of the window (used when labels are not cached)
         bool upd = false, last = false;
         bool fresh = false;               // my attempt was consumed: the next one is not taken over yet
+        bool inflight = false;            // the slab's gathers of hop hs are in flight
+        u32 hz = 0, hw = 0, hs = 0;       // coded sites of the hop whose slab update is pending; hop the slab is working on
         double a_i = 0, b_i = 0, a_j = 0, b_j = 0;    // gathers in flight for the followed pair
         bool addterm = false;
         u64 t_test = 0, t_slab = 0, t_wait = 0;
@@ -1041,16 +1065,20 @@ __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 
                 const bool far = __reduce_min_sync(CG_FULL, lab) >= CG_FRONT;      // warp-uniform
                 if (far && has_label && !nxt_valid) { nxt = decode_attempt(tb, p, geo, a_cur + P); nxt_valid = true; }
             }
-            if (upd) {
-                const bool snap = (hl & Hm) == 0u;
-                u32 buf = cur0 + (hl >> Hs) % CG_RING; if (buf >= CG_RING) buf -= CG_RING;
+            // The slab runs one hop behind: the gathers of the hop consumed last are issued here, behind the result, and
+            // were issued one iteration ago for the hop that is finished now - their latency is never waited for, and
+            // nothing of the slab sits between the outcome and the test.
+            if (inflight) {
+                const bool snap = (hs & Hm) == 0u;
+                u32 buf = cur0 + (hs >> Hs) % CG_RING; if (buf >= CG_RING) buf -= CG_RING;
                 slab.finish(tf, mask, geo, p.work, snap ? p.eps[buf] : nullptr, pr0, pr1);
                 if (snap) {
                     __syncwarp();
-                    if (lane == 0) mbar_arrive(&cm->pubbar[((hl >> Hs) - 1u) % CG_PB]);
+                    if (lane == 0) mbar_arrive(&cm->pubbar[((hs >> Hs) - 1u) % CG_PB]);
                 }
-                upd = false;
+                inflight = false;
             }
+            if (upd) { slab.issue(tf, mask, hz, hw); hs = hl; inflight = true; upd = false; }
             long long t2 = 0;
             if (TIMED) { t2 = clock64(); t_slab += (u64)(t2 - t1); }
             if (last) break;
@@ -1077,8 +1105,7 @@ __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 
                     if (sci == si) ni = false; if (sci == sj) ni = true;
                     if (scj == si) nj = false; if (scj == sj) nj = true;
                 }
-                ++hl; upd = true;
-                slab.issue(tf, mask, d.z, d.w);
+                ++hl; upd = true; hz = d.z; hw = d.w;
             }
             if (CACHED) {
                 if (has_label) {
@@ -1089,6 +1116,15 @@ __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 
                     }
                 }
             } else a0 += d.x;
+        }
+        if (inflight) {                   // the last hop of the launch
+            const bool snap = (hs & Hm) == 0u;
+            u32 buf = cur0 + (hs >> Hs) % CG_RING; if (buf >= CG_RING) buf -= CG_RING;
+            slab.finish(tf, mask, geo, p.work, snap ? p.eps[buf] : nullptr, pr0, pr1);
+            if (snap) {
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&cm->pubbar[((hs >> Hs) - 1u) % CG_PB]);
+            }
         }
         // the final state of my part of the slab, unless the last hop was a snapshot anyway
         if (n_hops & Hm) {
