@@ -92,7 +92,6 @@ struct CgCtl {              // device-resident control block (one per sim)
     u32 abort;              // != 0: the watchdog of the persistent kernel fired (which wait: see cg.h)
     u32 pad;
     u64 cyc_warps;          // worker warps that contributed to cyc_wait/update/propose
-    u64 dbg[16];
 };
 
 struct CgParams {           // kernel parameter block
@@ -229,6 +228,15 @@ __device__ __forceinline__ bool mbar_try(u64* b, u32 parity)
     u32 ok;
     asm volatile("{\n\t.reg .pred p;\n\t"
                  "mbarrier.try_wait.parity.acquire.cta.shared::cta.b64 p, [%1], %2;\n\t"
+                 "selp.b32 %0, 1, 0, p;\n\t}"
+                 : "=r"(ok) : "r"(smem_u32(b)), "r"(parity) : "memory");
+    return ok != 0;
+}
+__device__ __forceinline__ bool mbar_test(u64* b, u32 parity)    // never suspends
+{
+    u32 ok;
+    asm volatile("{\n\t.reg .pred p;\n\t"
+                 "mbarrier.test_wait.parity.acquire.cta.shared::cta.b64 p, [%1], %2;\n\t"
                  "selp.b32 %0, 1, 0, p;\n\t}"
                  : "=r"(ok) : "r"(smem_u32(b)), "r"(parity) : "memory");
     return ok != 0;
@@ -455,15 +463,15 @@ struct __align__(16) Comm {
                             // a worker is at most CG_XR iterations ahead of the collector, hence twice the ring
     u64 own[CG_XR][2];      // the CTA's result (collector -> exchange warp), same format
     u64 peer[CG_MAX_CLUSTER][CG_SRING][2];   // posts of the other CTAs of the cluster (DSMEM), slot format
+    u32 hist[2 * CG_XR][4]; // the collector's copy of the last descriptors (flags, ci, cj, hopno), for the lazy bitmap
     u32 hops[CG_HR][2];     // coded sites (i, j) of executed hop h at h % CG_HR
     u32 ver;                // newest snapshot that every CTA has published (count within this launch)
     u32 nlow;               // hops up to this one are in the occupation bitmap
     u32 abort;              // the launch is being abandoned
-    u32 xe;                 // iterations decided so far
 };
 
 #ifdef CG_TRACE2
-#define TR(slot, k) do { if (lane == 0 && b == 0 && e - 2000u < 16u) reinterpret_cast<u64*>(p.work)[(((e - 2000u) * 20u + (slot)) * 4u) + (k)] = (u64)clock64(); } while (0)
+#define TR(slot, k) do { if (lane == 0 && trl && e - 2000u < 16u) reinterpret_cast<u64*>(p.work)[(((e - 2000u) * 20u + (slot)) * 4u) + (k)] = (u64)clock64(); } while (0)
 #else
 #define TR(slot, k) do { } while (0)
 #endif
@@ -577,7 +585,7 @@ __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 
             cm->own[k][0] = stale; cm->own[k][1] = 0;
         }
         for (int k = 0; k < CG_PB; ++k) mbar_init(&cm->pubbar[k], NW);
-        cm->ver = 0; cm->nlow = 0; cm->abort = 0; cm->xe = 0;
+        cm->ver = 0; cm->nlow = 0; cm->abort = 0;
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
 
@@ -633,10 +641,26 @@ __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 
         // the window hold its END ("tail" labels >= tail0): those rank after every other label.
         u32 cf = c_first, tr = t0r;
         Waiter wd;
-        u64 dc_poll = 0, dc_post = 0, dc_desc = 0; long long dc_t = clock64();
+        u32 c_app = 0;                    // descriptors below this one are in the occupation bitmap
+        // the hop of descriptor x goes into the bitmap (every warp has consumed it; this warp is the only writer of the
+        // bitmap, and volatile stores of one thread stay in order)
+        auto apply = [&](u32 x) {
+            const uint4 hx = lds128u(&cm->hist[x % (2 * CG_XR)][0]);
+            if (lane == 0 && (hx.x & CG_F_HOP)) {
+                const u32 si = geo.site(hx.y), sj = geo.site(hx.z);
+                volatile u32* w = s_n;
+                w[si >> 5] &= ~(1u << (si & 31));
+                w[sj >> 5] |= 1u << (sj & 31);
+                *(volatile u32*)&cm->nlow = hx.w;
+            }
+        };
+        u32 e_end = 0;
         for (u32 e = 0;; ++e) {
             const u32 xs = e % CG_XR, e32 = e_start + e;
             const u32 kb = b >= cf ? b - cf : b + nb - cf;
+#ifdef CG_TRACE2
+            const bool trl = kb == 0;
+#endif
             const u32 tail0 = (CACHED && kb == 0) ? per - tr : CG_NONE;
             const u32 w0 = (CACHED && kb == 0) ? tr >> 5 : 0u;
             u32 wr = w0 + (u32)lane; if (wr >= (u32)NW) wr -= NW;
@@ -676,7 +700,6 @@ __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 
             }
             if (quit) break;
             TR(14, 0);
-            { const long long n_ = clock64(); dc_poll += (u64)(n_ - dc_t); dc_t = n_; }
             // post: own[] for the exchange warp, the slot in L2 for the other CTAs, the peers' shared memory
             const u64 s0 = ((u64)e32 << 32) | gmin;
             if (lane == 0) sts128(&cm->own[xs][0], s0, gpay);
@@ -690,18 +713,33 @@ __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 
                 if (lane == 0) slot_store(my_slot + 2u * ring, s0, s1);
             }
             TR(14, 1);
-            { const long long n_ = clock64(); dc_post += (u64)(n_ - dc_t); dc_t = n_; }
             // consume O_e
             if (!mbar_wait(&cm->full[xs], (e / CG_XR) & 1u, p, cm, 3u)) break;
             TR(14, 2);
-            { const long long n_ = clock64(); dc_desc += (u64)(n_ - dc_t); dc_t = n_; }
             const uint4 d0 = lds128u(&cm->desc[xs]);
             const uint4 d1 = lds128u(&cm->desc[xs].c_first);
+            if (CACHED) {
+                // the lazy occupation bitmap: descriptors that every warp has consumed (their empty phase is complete;
+                // never more than one phase ahead of this test, because this warp is one of the consumers)
+                if (lane == 0) sts128u(&cm->hist[e % (2 * CG_XR)][0], d0.y, d0.z, d0.w, d1.z);
+                __syncwarp();
+                while (c_app < e && mbar_test(&cm->empty[c_app % CG_XR], (c_app / CG_XR) & 1u)) { apply(c_app); ++c_app; }
+            }
             __syncwarp();
             if (lane == 0) mbar_arrive(&cm->empty[xs]);
+            e_end = e + 1u;
             if (d0.y & (CG_F_LAST | CG_F_ABORT)) break;
             cf = d1.x; tr = d1.y;
         }
+        if (!*(volatile u32*)&cm->abort) {
+            // end of the launch: the remaining hops go into the bitmap once every warp is done with it
+            asm volatile("bar.sync 1, %0;" ::"r"(THREADS) : "memory");
+            if (CACHED) for (; c_app < e_end; ++c_app) apply(c_app);
+            __syncwarp();
+            asm volatile("bar.sync 2, %0;" ::"r"(THREADS) : "memory");
+            if (csz > 1) cluster_sync_all();
+        }
+        return;
 
     } else if (role == 1) {
         // ----------------------------------------------------------------- exchange warp ----
@@ -709,33 +747,17 @@ __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 
         u64 used_sum = 0;                 // attempts consumed in this launch
         long long dP = 0;
         u32 e = 0, hc = 0;                // iterations and hops decided in this launch
-        u32 e_app = 0;                    // descriptors below this one are in the occupation bitmap
         u32 ver = 0;                      // newest snapshot known to be published by every CTA
         Waiter wd;
         bool quit = false;
-        u64 dx_[5] = {0, 0, 0, 0, 0}; long long dx_t = clock64();
-        u64 dcase[5] = {0, 0, 0, 0, 0}, dcnt[5] = {0, 0, 0, 0, 0}; long long dlast = clock64();
-#define DXT(k) { const long long n_ = clock64(); dx_[k] += (u64)(n_ - dx_t); dx_t = n_; }
-        // the hop of descriptor ea goes into the bitmap (every warp has consumed it)
-        auto apply = [&](u32 ea) {
-            const uint4 d0 = lds128u(&cm->desc[ea % CG_XR]);
-            if (lane == 0 && (d0.y & CG_F_HOP)) {         // this warp is the only writer; volatile stores of one thread stay in order
-                const u32 si = geo.site(d0.z), sj = geo.site(d0.w);
-                volatile u32* w = s_n;
-                w[si >> 5] &= ~(1u << (si & 31));
-                w[sj >> 5] |= 1u << (sj & 31);
-                *(volatile u32*)&cm->nlow = *(volatile u32*)&cm->desc[ea % CG_XR].hopno;
-            }
-        };
         while (hc < n_hops) {
             const u32 xs = e % CG_XR, e32 = e_start + e;
+#ifdef CG_TRACE2
+            const bool trl = b == c_first;
+#endif
             TR(15, 0);
             // (1) recycle the descriptor slot: every consumer is past iteration e - CG_XR
-            if (CACHED && e >= CG_XR) {
-                if (!mbar_wait(&cm->empty[xs], ((e - CG_XR) / CG_XR) & 1u, p, cm, 4u)) { quit = true; break; }
-                apply(e_app); ++e_app;
-            }
-            DXT(0)
+            if (CACHED && e >= CG_XR && !mbar_wait(&cm->empty[xs], ((e - CG_XR) / CG_XR) & 1u, p, cm, 4u)) { quit = true; break; }
             // (2) gate: every CTA has published the snapshot that covers hop hc + 1 - G
             if (nb > 1 && hc + 1u > p.gate) {
                 const u32 need = (hc + 1u - p.gate) >> Hs;
@@ -765,7 +787,6 @@ __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 
                     if (lane == 0) max_release_cta(&cm->ver, need);
                 }
             }
-            DXT(1)
             TR(15, 1);
             // (3) the first accepting CTA in scan order (step 3).  Position 0 holds the start of
             // the window; a window of scan positions is polled at a time, starting narrow (the winner is nearly
@@ -775,7 +796,6 @@ __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 
             const u32 tail0 = CACHED ? per - t0r : CG_NONE;
             const u32 ring = e32 & (CG_SRING - 1u), e16 = e32 & 0xFFFFu;
             u32 q = CG_NONE; u64 wp = 0;
-            u32 wpos = 0xFFFFu;
             u32 tlab = CG_NONE; u64 tpay = 0;                          // tail accept of position 0
             u32 lo = 0, hi = min(nb, 4u);
             wd.reset();
@@ -795,7 +815,7 @@ __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 
                     const u32 racc = __ballot_sync(CG_FULL, ready && l != CG_NONE);
                     const u32 rnot = __ballot_sync(CG_FULL, !ready);
                     const int fa = racc ? __ffs(racc) - 1 : 32, fn = rnot ? __ffs(rnot) - 1 : 32;
-                    if (fa < fn) { q = __shfl_sync(CG_FULL, l, fa); wp = __shfl_sync(CG_FULL, pay, fa); wpos = 0; lo = nb; break; }
+                    if (fa < fn) { q = __shfl_sync(CG_FULL, l, fa); wp = __shfl_sync(CG_FULL, pay, fa); lo = nb; break; }
                     if (!rnot) break;                   // no head accept here: the general scan (my tail labels come from own[])
                     if (wait_poll(wd, p, cm, 6u)) { quit = true; break; }
                 }
@@ -829,7 +849,6 @@ __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 
                     const int fa = racc ? __ffs(racc) - 1 : 32, fn = rnot ? __ffs(rnot) - 1 : 32;
                     if (fa < fn) {                      // first accepting position, everything before it rejected
                         q = __shfl_sync(CG_FULL, l, fa); wp = __shfl_sync(CG_FULL, pay, fa);
-                        wpos = lo + (u32)fa;
                         found = true;
                         break;
                     }
@@ -843,7 +862,6 @@ __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 
                 lo = hi; hi = min(nb, lo + 32u);
             }
             if (quit) break;
-            DXT(2)
             TR(15, 2);
             if (q == CG_NONE && tlab != CG_NONE) { q = tlab; wp = tpay; }   // only the tail of the window accepted
             // lock step (not CACHED): every warp of this CTA has finished its tests of this iteration before the
@@ -863,7 +881,6 @@ __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 
             // (step 3a)
             const u32 used = q == CG_NONE ? M : q + 1;
             const u32 ci = (u32)(wp >> 32), cj = (u32)wp;               // coded sites
-            const u32 hi_ = geo.site(ci), hj_ = geo.site(cj);
             const bool hop = q != CG_NONE;
             if (CACHED) {
                 if (t0r + used < per) t0r += used;
@@ -880,40 +897,32 @@ __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 
                 sts128u(&d->c_first, c_first, t0r, hc, 0u);
                 sts128u(&d->used, used, flags, ci, cj);
                 if (!CACHED && hop) {         // lock step: the bitmap is always current
-                    atomicAnd(&s_n[hi_ >> 5], ~(1u << (hi_ & 31)));
-                    atomicOr(&s_n[hj_ >> 5], 1u << (hj_ & 31));
+                    const u32 si = geo.site(ci), sj = geo.site(cj);
+                    volatile u32* w = s_n;
+                    w[si >> 5] &= ~(1u << (si & 31));
+                    w[sj >> 5] |= 1u << (sj & 31);
                     *(volatile u32*)&cm->nlow = hc;
                 }
                 mbar_arrive(&cm->full[xs]);   // release: the stores above are visible to whoever sees the phase complete
-                *(volatile u32*)&cm->xe = e + 1u;
             }
             TR(15, 3);
-            DXT(3)
-            {   // debug: time between publications by case
-                const long long n_ = clock64();
-                const int cls = kb == 0 ? (wpos == 0 ? 0 : 1) : (wpos == kb ? 2 : (kb == 1 ? 3 : 4));
-                dcase[cls] += (u64)(n_ - dlast); dcnt[cls] += 1; dlast = n_;
-            }
-            // (5) the rest of the bookkeeping, off the critical path
+            // (5) the bookkeeping, off the critical path
             used_sum += used;
             ++e;
             if (hop) {
+                const u32 hi_ = geo.site(ci), hj_ = geo.site(cj);
                 dP += geo.dx(hi_, hj_);                                  // step 3b: dP = dx
                 const u64 h = hops_start + hc - 1u - log_base;
                 if (lane == 0 && b == 0 && h < p.log_cap) {
                     p.log_a[h] = a_start + used_sum - 1; p.log_i[h] = hi_; p.log_j[h] = hj_;
                 }
             }
-            DXT(4)
         }
-        if (lane == 0) for (int k = 0; k < 5; ++k) { atomicAdd(&p.ctl->dbg[k], dcase[k]); atomicAdd(&p.ctl->dbg[8 + k], dcnt[k]); }
         if (quit) {                       // let the consumers of this CTA go (they see the abort flag in their waits)
             if (lane == 0) *(volatile u32*)&cm->abort = 1u;
             return;
         }
-        // end of the launch: the remaining hops go into the bitmap once every warp is done with it
         asm volatile("bar.sync 1, %0;" ::"r"(THREADS) : "memory");
-        if (CACHED) for (; e_app < e; ++e_app) apply(e_app);
         if (b == 0 && lane == 0) {
             CgCtl* c = p.ctl;
             const u32 ns = n_snaps + ((n_hops & Hm) ? 1u : 0u);
@@ -1016,21 +1025,23 @@ __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 
                 if (metropolis(dE, cuh, cul, p.T, p.inv_T)) best = lab;
             } else tracked = false;
         };
+#ifdef CG_TRACE2
+        bool trl = b == c_first;
+#endif
         for (u32 e = 0;; ++e) {
             const u32 xs = e % CG_XR, e32 = e_start + e;
             // ---- steps 1-2: propose and test on S_e, state untouched
             u32 best = CG_NONE, bi = 0, bj = 0;
+            bool far_ = false;
             if (CACHED) {
+                // A thread whose attempt was consumed takes over its next one when its warp is far from the front of the
+                // window (below, behind the result); only if the new label lies inside the window already - P - used or more,
+                // so hardly ever - it has to happen before the test
+                if (fresh && lab < M) refresh();
                 if (has_label && !fresh) test_mine(best);
                 addterm = false;
+                far_ = __reduce_min_sync(CG_FULL, lab) >= min(CG_FRONT, P >> 2);               // warp-uniform
                 u32 wmin = __reduce_min_sync(CG_FULL, best);
-                // A thread whose attempt was consumed takes over its next one AFTER the warp has handed in its
-                // result: the new label is higher than every other label of the warp (P - used or more), so it
-                // can only matter when it lies inside the window and nothing else in the warp accepts.
-                if (wmin == CG_NONE && __any_sync(CG_FULL, fresh && lab < M)) {
-                    if (fresh) { refresh(); test_mine(best); }
-                    wmin = __reduce_min_sync(CG_FULL, best);
-                }
                 // ---- step 3: lowest accepting label of the warp, for the collector
                 TR(warp, 1);
                 if (wmin == CG_NONE ? lane == 0 : best == wmin) {   // labels are distinct: one lane
@@ -1038,7 +1049,6 @@ __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 
                            ((u64)(sci & mask) << 32) | (u64)(scj & mask));
                 }
                 TR(warp, 2);
-                if (fresh) refresh();
             } else {
                 for (u32 l = lab0 + tid; l < lab1; l += TW) {
                     const Prop q = decode_attempt(tb, p, geo, a0 + l);
@@ -1061,9 +1071,9 @@ __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 
             // issued when it was consumed, behind those of the followed pair); first the decode one attempt ahead
             // (a warp near the front of the window is on the critical path of the next iterations: its decode waits
             // until all of its labels have been consumed and it sits at the far end of the window)
-            if (CACHED) {
-                const bool far = __reduce_min_sync(CG_FULL, lab) >= CG_FRONT;      // warp-uniform
-                if (far && has_label && !nxt_valid) { nxt = decode_attempt(tb, p, geo, a_cur + P); nxt_valid = true; }
+            if (CACHED && far_) {
+                if (fresh) refresh();
+                if (has_label && !nxt_valid) { nxt = decode_attempt(tb, p, geo, a_cur + P); nxt_valid = true; }
             }
             // The slab runs one hop behind: the gathers of the hop consumed last are issued here, behind the result, and
             // were issued one iteration ago for the hop that is finished now - their latency is never waited for, and
@@ -1085,6 +1095,9 @@ __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 
             TR(warp, 3);
             // ---- O_e
             if (!mbar_wait(&cm->full[xs], (e / CG_XR) & 1u, p, cm, 8u)) return;
+#ifdef CG_TRACE2
+            trl = *(volatile u32*)&cm->desc[xs].c_first == b;
+#endif
             { const u32 e_ = e; { const u32 e = e_ + 1u; TR(warp, 0); } }
             const uint4 d = lds128u(&cm->desc[xs]);        // used, flags, ci, cj
             __syncwarp();
@@ -2190,13 +2203,7 @@ extern "C" int cg_get_phase_cycles(cg_sim* s, uint64_t* total, uint64_t* wait, u
     if (update) *update = c.cyc_update;
     if (propose) *propose = c.cyc_propose;
     if (warps) *warps = c.cyc_warps;
-    if (getenv("CG_DBG")) {
-        fprintf(stderr, "dbg:");
-        for (int k = 0; k < 16; ++k) fprintf(stderr, " %llu", (unsigned long long)c.dbg[k]);
-        fprintf(stderr, "\n");
-    }
     if (reset) {
-        for (int k = 0; k < 16; ++k) c.dbg[k] = 0;
         c.cyc_total = c.cyc_wait = c.cyc_update = c.cyc_propose = c.cyc_warps = 0;
         CK(cudaMemcpyAsync(s->d_ctl, &c, sizeof c, cudaMemcpyHostToDevice, s->stream));
         CK(cudaStreamSynchronize(s->stream));
