@@ -470,11 +470,6 @@ struct __align__(16) Comm {
     u32 abort;              // the launch is being abandoned
 };
 
-#ifdef CG_TRACE2
-#define TR(slot, k) do { if (lane == 0 && trl && e - 2000u < 16u) reinterpret_cast<u64*>(p.work)[(((e - 2000u) * 20u + (slot)) * 4u) + (k)] = (u64)clock64(); } while (0)
-#else
-#define TR(slot, k) do { } while (0)
-#endif
 
 struct Waiter {             // watchdog state of one waiting warp
     u64 t0; u32 spins;
@@ -658,9 +653,6 @@ __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 
         for (u32 e = 0;; ++e) {
             const u32 xs = e % CG_XR, e32 = e_start + e;
             const u32 kb = b >= cf ? b - cf : b + nb - cf;
-#ifdef CG_TRACE2
-            const bool trl = kb == 0;
-#endif
             const u32 tail0 = (CACHED && kb == 0) ? per - tr : CG_NONE;
             const u32 w0 = (CACHED && kb == 0) ? tr >> 5 : 0u;
             u32 wr = w0 + (u32)lane; if (wr >= (u32)NW) wr -= NW;
@@ -699,7 +691,6 @@ __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 
                 __nanosleep(CG_POLL_NS);
             }
             if (quit) break;
-            TR(14, 0);
             // post: own[] for the exchange warp, the slot in L2 for the other CTAs, the peers' shared memory
             const u64 s0 = ((u64)e32 << 32) | gmin;
             if (lane == 0) sts128(&cm->own[xs][0], s0, gpay);
@@ -712,10 +703,8 @@ __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 
                 }
                 if (lane == 0) slot_store(my_slot + 2u * ring, s0, s1);
             }
-            TR(14, 1);
             // consume O_e
             if (!mbar_wait(&cm->full[xs], (e / CG_XR) & 1u, p, cm, 3u)) break;
-            TR(14, 2);
             const uint4 d0 = lds128u(&cm->desc[xs]);
             const uint4 d1 = lds128u(&cm->desc[xs].c_first);
             if (CACHED) {
@@ -752,10 +741,6 @@ __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 
         bool quit = false;
         while (hc < n_hops) {
             const u32 xs = e % CG_XR, e32 = e_start + e;
-#ifdef CG_TRACE2
-            const bool trl = b == c_first;
-#endif
-            TR(15, 0);
             // (1) recycle the descriptor slot: every consumer is past iteration e - CG_XR
             if (CACHED && e >= CG_XR && !mbar_wait(&cm->empty[xs], ((e - CG_XR) / CG_XR) & 1u, p, cm, 4u)) { quit = true; break; }
             // (2) gate: every CTA has published the snapshot that covers hop hc + 1 - G
@@ -787,7 +772,6 @@ __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 
                     if (lane == 0) max_release_cta(&cm->ver, need);
                 }
             }
-            TR(15, 1);
             // (3) the first accepting CTA in scan order (step 3).  Position 0 holds the start of
             // the window; a window of scan positions is polled at a time, starting narrow (the winner is nearly
             // always at the first positions), and polling stops at the first accept: posts of later CTAs are
@@ -862,7 +846,6 @@ __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 
                 lo = hi; hi = min(nb, lo + 32u);
             }
             if (quit) break;
-            TR(15, 2);
             if (q == CG_NONE && tlab != CG_NONE) { q = tlab; wp = tpay; }   // only the tail of the window accepted
             // lock step (not CACHED): every warp of this CTA has finished its tests of this iteration before the
             // bitmap changes
@@ -905,7 +888,6 @@ __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 
                 }
                 mbar_arrive(&cm->full[xs]);   // release: the stores above are visible to whoever sees the phase complete
             }
-            TR(15, 3);
             // (5) the bookkeeping, off the critical path
             used_sum += used;
             ++e;
@@ -1025,9 +1007,6 @@ __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 
                 if (metropolis(dE, cuh, cul, p.T, p.inv_T)) best = lab;
             } else tracked = false;
         };
-#ifdef CG_TRACE2
-        bool trl = b == c_first;
-#endif
         for (u32 e = 0;; ++e) {
             const u32 xs = e % CG_XR, e32 = e_start + e;
             // ---- steps 1-2: propose and test on S_e, state untouched
@@ -1043,12 +1022,10 @@ __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 
                 far_ = __reduce_min_sync(CG_FULL, lab) >= min(CG_FRONT, P >> 2);               // warp-uniform
                 u32 wmin = __reduce_min_sync(CG_FULL, best);
                 // ---- step 3: lowest accepting label of the warp, for the collector
-                TR(warp, 1);
                 if (wmin == CG_NONE ? lane == 0 : best == wmin) {   // labels are distinct: one lane
                     sts128(&cm->res[e % (2 * CG_XR)][warp][0], ((u64)e32 << 32) | wmin,
                            ((u64)(sci & mask) << 32) | (u64)(scj & mask));
                 }
-                TR(warp, 2);
             } else {
                 for (u32 l = lab0 + tid; l < lab1; l += TW) {
                     const Prop q = decode_attempt(tb, p, geo, a0 + l);
@@ -1092,13 +1069,8 @@ __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 
             long long t2 = 0;
             if (TIMED) { t2 = clock64(); t_slab += (u64)(t2 - t1); }
             if (last) break;
-            TR(warp, 3);
             // ---- O_e
             if (!mbar_wait(&cm->full[xs], (e / CG_XR) & 1u, p, cm, 8u)) return;
-#ifdef CG_TRACE2
-            trl = *(volatile u32*)&cm->desc[xs].c_first == b;
-#endif
-            { const u32 e_ = e; { const u32 e = e_ + 1u; TR(warp, 0); } }
             const uint4 d = lds128u(&cm->desc[xs]);        // used, flags, ci, cj
             __syncwarp();
             if (lane == 0) mbar_arrive(&cm->empty[xs]);
