@@ -95,9 +95,9 @@ int cg_run(cg_sim* s, uint64_t n_accepted_hops);
  * n_accepted_hops executed hops in ONE persistent launch, every sim on its own
  * CTAs side by side; each chain is exactly the one cg_run would produce.
  * sims[] is a host array of distinct sims that share device, stream and launch
- * shape (544 threads, no clusters, same register tiling and label caching: true for
+ * shape (544 threads, same register tiling and label caching: true for
  * sims of equal L whose M fits their CTAs; see cg_get_launch / cg_set_launch); the sum of
- * their CTA counts must fit on the device at once, else CG_EUNSUPPORTED.
+ * their CTA counts must fit on the device at once, else CG_EUNSUPPORTED; clusters are not used.
  * Asynchronous on that stream; the array is not referenced after the call. */
 int cg_run_many(cg_sim* const* sims, int n_sims, uint64_t n_accepted_hops);
 
@@ -167,8 +167,16 @@ int cg_recompute_eps(cg_sim* s, double* max_abs_dev);
  * oracle and for its bandwidth measurement.  Every hop must satisfy theta_ij
  * (n_i = 1, n_j = 0) at its turn: otherwise CG_EINVAL and nothing is changed.
  * ms (may be NULL) receives the device time of the launch measured with CUDA
- * events on the sim's stream. */
+ * events on the sim's stream.
+ * Two kernels compute the same sums (bit-identical): "staged" keeps whole lattice rows of
+ * eps in shared memory and brings the two table rows every lattice row needs per hop in
+ * with bulk asynchronous copies (cp.async.bulk + mbarrier), three hops ahead; "gathers"
+ * keeps eps in registers and reads the table with per-site loads.  cg_set_update_kernel:
+ * 0 = automatic (the faster one as measured on B200: gathers), 1 = gathers, 2 = staged
+ * (cg_apply_hops then returns CG_EUNSUPPORTED when the rows do not fit shared memory or
+ * L < 32). */
 int cg_apply_hops(cg_sim* s, uint64_t count, const uint32_t* i, const uint32_t* j, float* ms);
+int cg_set_update_kernel(cg_sim* s, int kind);
 
 /* Diagnostics of the one-time set-up (step a0): translation-invariant tables
  * (PAPER.md:80).  K = number of displacements with 0 < r <= L/2 in the order
@@ -187,12 +195,16 @@ int cg_get_phi(cg_sim* s, double* phi /* N */);
 int cg_set_launch(cg_sim* s, int n_ctas, int threads);
 int cg_get_launch(cg_sim* s, int* n_ctas, int* threads, int* smem_bytes);
 
-/* Tuning that never changes results.  snapshot_interval H in {1, 2, 4, 8} (default 4): the
+/* Tuning that never changes results.  snapshot_interval H in {1, 2, 4, 8} (default 8): the
  * eps slabs, kept current in registers after every hop, are written through to memory
- * every H hops (deferred update; PAPER.md:77, 106 W_U); cluster_size in {1, 2, 4, 8, 16}
- * (default 1): CTAs per thread-block cluster, whose members post their results into each
- * other's shared memory instead of through L2.  0 leaves a value as it is.  A new cluster
- * size re-derives the launch shape (CG_EUNSUPPORTED if the device cannot co-schedule it). */
+ * every H hops (deferred update; PAPER.md:77, 106 W_U); cluster_size in {1, 2, 4, 8, 16}:
+ * CTAs per thread-block cluster, whose members post their results into each other's
+ * shared memory instead of through L2; -1 = automatic (the default: clusters of up to 16
+ * when the whole sim fits 96 CTAs, none when it wants every SM - clusters of 8 and 16 leave
+ * SMs of a B200 unused).  0 leaves a value as it is.  A new cluster size re-derives the
+ * launch shape (CG_EUNSUPPORTED if the device cannot co-schedule it).  cg_set_launch with an
+ * explicit CTA count keeps the largest cluster size that divides it; cg_get_tuning reports
+ * the cluster size in use.  cg_run_many launches without clusters. */
 int cg_set_tuning(cg_sim* s, int snapshot_interval, int cluster_size);
 int cg_get_tuning(cg_sim* s, int* snapshot_interval, int* cluster_size);
 

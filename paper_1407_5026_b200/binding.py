@@ -20,7 +20,7 @@ EXPORTS = [
     "cg_run", "cg_run_many", "cg_get_state", "cg_set_state",
     "cg_get_time_stochastic", "cg_get_normals", "cg_get_dos", "cg_get_series", "cg_get_sigma0",
     "cg_get_counters", "cg_enable_hop_log", "cg_get_hops", "cg_recompute_eps", "cg_apply_hops",
-    "cg_get_table_sizes", "cg_get_tables", "cg_get_table_dz", "cg_get_phi", "cg_set_launch", "cg_get_launch",
+    "cg_set_update_kernel", "cg_get_table_sizes", "cg_get_tables", "cg_get_table_dz", "cg_get_phi", "cg_set_launch", "cg_get_launch",
     "cg_set_tuning", "cg_get_tuning", "cg_set_phase_timers", "cg_get_phase_cycles", "cg_bench_l2", "cg_free", "cg_strerror",
     "cg_last_error",
 ]
@@ -65,6 +65,7 @@ def lib():
         "cg_get_series": (ci, [vp, u64, u64, vp, vp]),
         "cg_get_sigma0": (ci, [vp, P(dbl)]),
         "cg_apply_hops": (ci, [vp, u64, vp, vp, P(C.c_float)]),
+        "cg_set_update_kernel": (ci, [vp, ci]),
         "cg_get_table_sizes": (ci, [vp, P(i64), P(i64)]),
         "cg_get_tables": (ci, [vp, vp, vp, vp, vp, P(dbl), P(dbl)]),
         "cg_get_table_dz": (ci, [vp, vp]),
@@ -266,8 +267,10 @@ class CoulombGlass:
             self._check(self._lib.cg_recompute_eps(self._h, C.byref(dev)))
         return dev.value
 
-    def apply_hops(self, i, j):
-        """Scripted hops through the update kernel alone; -> device milliseconds of the launch."""
+    def apply_hops(self, i, j, kernel=None):
+        """Scripted hops through the update kernel alone; -> device milliseconds of the launch.
+        kernel: None/"auto", "gathers" or "staged" (cg_set_update_kernel)."""
+        self._check(self._lib.cg_set_update_kernel(self._h, {None: 0, "auto": 0, "gathers": 1, "staged": 2}[kernel]))
         i = np.ascontiguousarray(i, np.uint32)
         j = np.ascontiguousarray(j, np.uint32)
         assert i.size == j.size

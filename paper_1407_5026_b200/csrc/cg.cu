@@ -241,6 +241,21 @@ __device__ __forceinline__ bool mbar_test(u64* b, u32 parity)    // never suspen
                  : "=r"(ok) : "r"(smem_u32(b)), "r"(parity) : "memory");
     return ok != 0;
 }
+__device__ __forceinline__ void mbar_expect_tx(u64* b, u32 bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.release.cta.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(b)), "r"(bytes) : "memory");
+}
+// bulk asynchronous copy global -> shared memory (TMA engine, 16-byte granularity), completion counted on an mbarrier
+__device__ __forceinline__ void bulk_g2s(void* dst_smem, const void* src_gmem, u32 bytes, u64* bar)
+{
+    asm volatile("cp.async.bulk.shared::cta.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(smem_u32(dst_smem)), "l"(src_gmem), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ bool mbar_spin(u64* b, u32 parity)        // plain wait (kernels without a watchdog)
+{
+    while (!mbar_try(b, parity)) { }
+    return true;
+}
 __device__ __forceinline__ u32 cluster_ctarank()
 {
     u32 r;
@@ -1189,6 +1204,84 @@ cg_update_scripted(const CgParams p, const u32* __restrict__ hop_i, const u32* _
     }
 }
 
+
+// Step a6 alone, staged (include/cg.h: cg_apply_hops).  CTA b owns `rows` whole lattice rows (z, y) and keeps their eps in
+// shared memory.  For an executed hop i -> j the sites of lattice row (z, y) need the table row of the offset
+// ((z - z_j) mod L, (y - y_j) mod L) - L contiguous doubles, 16-byte aligned - read at (x - x_j) mod L, and the same for i:
+// two bulk copies per lattice row (cp.async.bulk, completion counted on an mbarrier) bring them into one of NST stages in
+// shared memory, issued NST - 1 hops ahead by the first warp; every warp then forms eps += 1/r_lj - 1/r_li from shared
+// memory only: no thread waits for a global load, and the load/store units see no gathers at all.  Every table entry of a
+// hop is fetched exactly once by the whole grid (16 N bytes of table traffic per hop, through the copy engine).
+template <int THREADS, int NST>
+__global__ void __launch_bounds__(THREADS)
+cg_update_staged(const CgParams p, const u32* __restrict__ hop_i, const u32* __restrict__ hop_j, u64 count, u32 rows)
+{
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    __shared__ __align__(8) u64 full[NST], empty[NST];
+    const Geo geo = make_geo(p);
+    const u32 L = (u32)p.L, lg = (u32)p.lgL, Lm = L - 1u, mask = p.mask;
+    const u32 total_rows = p.N >> lg;
+    const u32 row0 = blockIdx.x * rows, n_rows = min(rows, total_rows - min(total_rows, row0));
+    const u32 s_lo = row0 << lg, n_s = n_rows << lg;
+    double* const sl = reinterpret_cast<double*>(smem_raw);                  // the slab: rows x L
+    double* const stage = sl + (size_t)rows * L;                             // [NST][2 ends][rows][L]
+    const u32 st_sz = 2u * rows * L;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    double* e = p.eps[p.ctl->cur];
+    if (threadIdx.x == 0)
+        for (int k = 0; k < NST; ++k) { mbar_init(&full[k], 1); mbar_init(&empty[k], THREADS / 32); }
+    for (u32 k = threadIdx.x; k < n_s; k += THREADS) sl[k] = __ldcg(e + s_lo + k);
+    __syncthreads();
+    const double* __restrict__ tf = p.tf;
+    // the table rows of hop h into stage h % NST (first warp)
+    auto fetch = [&](u64 h) {
+        const u32 st = (u32)(h % NST), use = (u32)(h / NST);
+        if (use >= 1u) mbar_spin(&empty[st], (use - 1u) & 1u);
+        if (lane == 0) mbar_expect_tx(&full[st], 2u * n_rows * 8u * L);
+        __syncwarp();
+        const u32 ci = geo.code(__ldg(hop_i + h)), cj = geo.code(__ldg(hop_j + h));
+        const u32 cjr = cj & ~Lm, cir = ci & ~Lm;                            // hop sites with x = 0
+        double* const dj = stage + st * st_sz;
+        double* const di = dj + rows * L;
+        for (u32 r = (u32)lane; r < 2u * n_rows; r += 32u) {
+            const u32 rr = r >> 1, isj = r & 1u;
+            const u32 rc = geo.code((row0 + rr) << lg) | geo.spare;          // first site of the lattice row
+            bulk_g2s((isj ? dj : di) + rr * L, tf + ((rc - (isj ? cjr : cir)) & mask), 8u * L, &full[st]);
+        }
+    };
+    if (n_rows) {
+        if (warp == 0) for (u64 h = 0; h < (u64)(NST - 1) && h < count; ++h) fetch(h);
+        for (u64 h = 0; h < count; ++h) {
+            if (warp == 0 && h + NST - 1 < count) fetch(h + NST - 1);
+            const u32 st = (u32)(h % NST);
+            mbar_spin(&full[st], (u32)(h / NST) & 1u);
+            const double* __restrict__ sj = stage + st * st_sz;
+            const double* __restrict__ si = sj + rows * L;
+            const u32 xi = __ldg(hop_i + h) & Lm, xj = __ldg(hop_j + h) & Lm;
+#pragma unroll 4
+            for (u32 k = threadIdx.x; k < n_s; k += THREADS) {
+                const u32 r = k & ~Lm;                                       // row offset; x = k & Lm
+                sl[k] = __dadd_rn(sl[k], __dsub_rn(sj[r + ((k - xj) & Lm)], si[r + ((k - xi) & Lm)]));
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&empty[st]);
+        }
+        for (u32 k = threadIdx.x; k < n_s; k += THREADS) __stcg(e + s_lo + k, sl[k]);
+    }
+    if (blockIdx.x == 0 && threadIdx.x == 0) {       // occupations and dipole moment, in hop order
+        long long dP = p.ctl->dP; u32 bad = 0;
+        for (u64 h = 0; h < count; ++h) {
+            const u32 i = hop_i[h], j = hop_j[h];
+            const u32 wi = p.nbits[i >> 5], wj = p.nbits[j >> 5];
+            if (!((wi >> (i & 31)) & 1u) || ((wj >> (j & 31)) & 1u)) ++bad;
+            p.nbits[i >> 5] &= ~(1u << (i & 31));
+            p.nbits[j >> 5] |= (1u << (j & 31));
+            dP += geo.dx(i, j);
+        }
+        p.ctl->dP = dP; p.ctl->hops += count; p.ctl->bad_hops += bad;
+    }
+}
+
 // ---- one-time set-up (step a0) --------------------------------------------------------------
 
 // tf from the folded table: entry (dz, dy, dx) of the unfolded index space (fields of width 2L)
@@ -1335,9 +1428,12 @@ struct cg_sim {
     void* d_many = nullptr; size_t many_cap = 0;      // parameter blocks of cg_run_many (owned by its first sim)
     // launch shape and tuning
     int num_sms = 0, n_ctas = 0, threads = 0, smem = 0, rp = 0, pl = 0;   // pl > 0: cached proposals
-    int snap_shift = 2;                   // snapshots every 4 hops
-    int cluster = 1;                      // CTAs per thread-block cluster
+    int snap_shift = 3;                   // snapshots every 8 hops
+    int cluster = 1;                      // CTAs per thread-block cluster in use
+    int cluster_pref = 0;                 // cg_set_tuning: 0 = automatic (clusters when the whole sim fits a few of them)
     bool timers = false;                  // cg_set_phase_timers
+    int update_kernel = 0;                // cg_set_update_kernel: 0 automatic, 1 gathers, 2 staged
+    int smem_optin = 0;
     u64 watchdog_ns = 10ull * 1000 * 1000 * 1000;
     std::string err;
 };
@@ -1607,10 +1703,13 @@ static int max_coresident(cg_sim* s, int threads, int rp, bool cached, int* out)
     persist_fn f = persistent_kernel(threads, rp, cached, false);
     if (!f) return CG_EINVAL;
     CK(cudaFuncSetAttribute((const void*)f, cudaFuncAttributeMaxDynamicSharedMemorySize, s->smem));
-    if (persist_fn ft = threads == 544 ? persistent_kernel(threads, rp, cached, true) : nullptr)
-        CK(cudaFuncSetAttribute((const void*)ft, cudaFuncAttributeMaxDynamicSharedMemorySize, s->smem));
+    persist_fn ft = threads == 544 ? persistent_kernel(threads, rp, cached, true) : nullptr;      // the timed build
+    if (ft) CK(cudaFuncSetAttribute((const void*)ft, cudaFuncAttributeMaxDynamicSharedMemorySize, s->smem));
     if (s->cluster > 1) {
-        if (s->cluster > 8) CK(cudaFuncSetAttribute((const void*)f, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
+        if (s->cluster > 8) {
+            CK(cudaFuncSetAttribute((const void*)f, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
+            if (ft) CK(cudaFuncSetAttribute((const void*)ft, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
+        }
         cudaLaunchConfig_t cfg = {};
         cfg.gridDim = dim3(s->cluster * s->num_sms); cfg.blockDim = dim3(threads); cfg.dynamicSmemBytes = (size_t)s->smem;
         cudaLaunchAttribute at[1];
@@ -1628,7 +1727,7 @@ static int max_coresident(cg_sim* s, int threads, int rp, bool cached, int* out)
     return CG_OK;
 }
 
-static int choose_launch(cg_sim* s, int n_ctas, int threads)
+static int choose_launch_cs(cg_sim* s, int n_ctas, int threads)
 {
     const bool auto_threads = threads == 0;
     if (auto_threads) threads = 544;
@@ -1670,6 +1769,33 @@ static int choose_launch(cg_sim* s, int n_ctas, int threads)
     return CG_EUNSUPPORTED;
 }
 
+// Launch shape for (n_ctas, threads), 0 = heuristic, with the cluster size of cg_set_tuning.  Automatic cluster size
+// (measured): CTAs of one cluster post through shared memory instead of L2, worth 6-8 % when the whole sim
+// sits in one or a few clusters; on B200 clusters of 8 and 16 leave 28 and 36 of the 148 SMs unused, so a sim that
+// wants every SM runs without.  An explicit CTA count keeps the largest cluster size that divides it.
+static int choose_launch(cg_sim* s, int n_ctas, int threads)
+{
+    const int old = s->cluster;
+    int cs = s->cluster_pref;
+    if (cs == 0) {
+        s->cluster = 1;
+        int rc = choose_launch_cs(s, n_ctas, threads);
+        if (rc != CG_OK) { s->cluster = old; return rc; }
+        if (s->n_ctas < 2 || s->n_ctas > 96) return CG_OK;
+        cs = 16;
+        if (n_ctas == 0) while (cs > 1 && cs / 2 >= s->n_ctas) cs /= 2;     // 5 CTAs -> one cluster of 8
+    }
+    if (n_ctas) while (cs > 1 && n_ctas % cs) cs /= 2;
+    for (; cs >= 1; cs /= 2) {
+        s->cluster = cs;
+        const int rc = choose_launch_cs(s, n_ctas, threads);
+        if (rc == CG_OK) return CG_OK;
+        if (s->cluster_pref != 0 || cs == 1) { s->cluster = old; return rc; }
+    }
+    s->cluster = old;
+    return CG_EUNSUPPORTED;
+}
+
 static int init_impl(cg_sim** out, int dim, int L, double W, double xi, double T, double E, uint64_t seed,
                      uint32_t M, void* dev_ws, size_t bytes, void* stream, bool own)
 {
@@ -1700,6 +1826,7 @@ static int init_impl(cg_sim** out, int dim, int L, double W, double xi, double T
     CK(cudaGetDevice(&s->device));
     CK(cudaGetDeviceProperties(&prop, s->device));
     s->num_sms = prop.multiProcessorCount;
+    s->smem_optin = (int)prop.sharedMemPerBlockOptin;
     if (!prop.cooperativeLaunch) { s->err = "device lacks cooperative launch"; return CG_EUNSUPPORTED; }
 
     std::vector<double> tq;
@@ -1810,6 +1937,12 @@ static cudaError_t launch_coop(const void* f, int grid, int threads, int smem, c
     return cudaLaunchKernelExC(&cfg, f, args);
 }
 
+#ifndef CG_UPD_STAGES
+#define CG_UPD_STAGES 6      // hops whose table rows are in flight in the staged update kernel
+#endif
+#ifndef CG_UPD_THREADS
+#define CG_UPD_THREADS 128
+#endif
 #define CG_MAX_LAUNCH_HOPS (1u << 30)     // the kernel counts hops and iterations of one launch in 32 bits
 
 extern "C" int cg_run(cg_sim* s, uint64_t n_hops)
@@ -1841,9 +1974,9 @@ extern "C" int cg_run_many(cg_sim* const* sims, int n_sims, uint64_t n_hops)
         if (!s) return CG_EINVAL;
         for (int m = 0; m < k; ++m) if (sims[m] == s) return CG_EINVAL;       // a sim may appear once
         if (s->device != s0->device || s->stream != s0->stream || s->threads != s0->threads || s->rp != s0->rp
-            || (s->pl > 0) != (s0->pl > 0) || s->cluster != 1) {
+            || (s->pl > 0) != (s0->pl > 0)) {
             s0->err = "cg_run_many: the sims must share device, stream and launch shape (threads, register tiling, "
-                      "cached labels) and use no clusters";
+                      "cached labels)";
             return CG_EINVAL;
         }
         first[(size_t)k + 1] = first[(size_t)k] + (u32)s->n_ctas;
@@ -1869,7 +2002,7 @@ extern "C" int cg_run_many(cg_sim* const* sims, int n_sims, uint64_t n_hops)
     u32* d_first = (u32*)((char*)s0->d_many + ps.size() * sizeof(CgParams));
     while (n_hops) {
         const u32 chunk = (u32)std::min<uint64_t>(n_hops, CG_MAX_LAUNCH_HOPS);
-        for (int k = 0; k < n_sims; ++k) ps[(size_t)k] = make_params(sims[k], chunk);
+        for (int k = 0; k < n_sims; ++k) { ps[(size_t)k] = make_params(sims[k], chunk); ps[(size_t)k].cluster = 1; }   // posts through L2
         // pageable sources: the copies are staged before the calls return
         CK0(s0, cudaMemcpyAsync(d_ps, ps.data(), ps.size() * sizeof(CgParams), cudaMemcpyHostToDevice, s0->stream));
         CK0(s0, cudaMemcpyAsync(d_first, first.data(), first.size() * sizeof(u32), cudaMemcpyHostToDevice, s0->stream));
@@ -2054,8 +2187,20 @@ extern "C" int cg_apply_hops(cg_sim* s, uint64_t count, const uint32_t* i, const
     // one CTA per SM
     const u64 g1 = (s->N / 2 + 127) / 128;
     const int grid = (int)std::max<u64>(1, std::min<u64>((s->N / 2 + 511) / 512, (u64)s->num_sms));
+    // staged kernel: whole lattice rows per CTA, slab + CG_UPD_STAGES stages of two table rows per lattice row in shared memory
+    // (many small CTAs - about 512 sites each, several per SM - keep more table rows in flight per SM than a few large ones)
+    const u32 total_rows = s->N / (u32)s->L;
+    const u32 rows = std::max(1u, 512u / (u32)s->L);
+    const size_t st_smem = (size_t)rows * s->L * 8 * (1 + 2 * CG_UPD_STAGES);
+    // measured on B200: the bulk copies of the rows saturate near 4 TB/s, the gather kernel is twice as fast (DESIGN.md
+    // 6.2): the staged kernel runs only when asked for
+    const bool fits = s->L >= 32 && st_smem + 1024 <= (size_t)s->smem_optin;
+    if (s->update_kernel == 2 && !fits) return CG_EUNSUPPORTED;
+    const bool staged = s->update_kernel == 2;
+    if (staged) CK(cudaFuncSetAttribute((const void*)cg_update_staged<CG_UPD_THREADS, CG_UPD_STAGES>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)st_smem));
     CK(cudaEventRecord(ev.a, s->stream));
-    if (g1 <= (u64)s->num_sms * 12) cg_update_scripted<128, 1><<<(int)g1, 128, 0, s->stream>>>(p, d_ij, d_ij + count, count);
+    if (staged) cg_update_staged<CG_UPD_THREADS, CG_UPD_STAGES><<<(total_rows + rows - 1) / rows, CG_UPD_THREADS, st_smem, s->stream>>>(p, d_ij, d_ij + count, count, rows);
+    else if (g1 <= (u64)s->num_sms * 12) cg_update_scripted<128, 1><<<(int)g1, 128, 0, s->stream>>>(p, d_ij, d_ij + count, count);
     else scripted_kernel(choose_rp(s->N / 2, grid, 512, 8))<<<grid, 512, 0, s->stream>>>(p, d_ij, d_ij + count, count);
     CK(cudaEventRecord(ev.b, s->stream));
     CK(cudaGetLastError());
@@ -2071,6 +2216,13 @@ extern "C" int cg_apply_hops(cg_sim* s, uint64_t count, const uint32_t* i, const
         CK(cudaStreamSynchronize(s->stream));
         return CG_EINVAL;
     }
+    return CG_OK;
+}
+
+extern "C" int cg_set_update_kernel(cg_sim* s, int kind)
+{
+    if (!s || kind < 0 || kind > 2) return CG_EINVAL;
+    s->update_kernel = kind;
     return CG_OK;
 }
 
@@ -2129,21 +2281,21 @@ extern "C" int cg_get_launch(cg_sim* s, int* n_ctas, int* threads, int* smem)
 extern "C" int cg_set_tuning(cg_sim* s, int snapshot_interval, int cluster_size)
 {
     if (!s) return CG_EINVAL;
-    int shift = s->snap_shift, cs = s->cluster;
+    int shift = s->snap_shift, pref = s->cluster_pref;
     if (snapshot_interval) {
         if (snapshot_interval != 1 && snapshot_interval != 2 && snapshot_interval != 4 && snapshot_interval != 8) return CG_EINVAL;
         shift = snapshot_interval == 1 ? 0 : snapshot_interval == 2 ? 1 : snapshot_interval == 4 ? 2 : 3;
     }
     if (cluster_size) {
-        if (cluster_size < 1 || cluster_size > CG_MAX_CLUSTER || (cluster_size & (cluster_size - 1))) return CG_EINVAL;
-        cs = cluster_size;
+        if (cluster_size != -1 && (cluster_size < 1 || cluster_size > CG_MAX_CLUSTER || (cluster_size & (cluster_size - 1)))) return CG_EINVAL;
+        pref = cluster_size == -1 ? 0 : cluster_size;
     }
     CK(cudaStreamSynchronize(s->stream));
-    const int old_shift = s->snap_shift, old_cs = s->cluster;
-    s->snap_shift = shift; s->cluster = cs;
-    if (cs != old_cs) {
+    const int old_pref = s->cluster_pref;
+    s->snap_shift = shift; s->cluster_pref = pref;
+    if (pref != old_pref) {
         const int rc = choose_launch(s, 0, 0);
-        if (rc != CG_OK) { s->snap_shift = old_shift; s->cluster = old_cs; choose_launch(s, 0, 0); return rc; }
+        if (rc != CG_OK) { s->cluster_pref = old_pref; choose_launch(s, 0, 0); return rc; }
     }
     return CG_OK;
 }

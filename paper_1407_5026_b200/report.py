@@ -3,15 +3,19 @@
     python -m paper_1407_5026_b200.report --configs [--hops 200000] [--warm 2000]
     python -m paper_1407_5026_b200.report --replicas [--hops 100000]
     python -m paper_1407_5026_b200.report --observables [--hops 200000]
+    python -m paper_1407_5026_b200.report --l2            # sweep of the L2 roofline probe (cg_bench_l2)
+    python -m paper_1407_5026_b200.report --update        # step a6 alone: gather kernel against bulk-copy staged kernel
+    python -m paper_1407_5026_b200.report --tuning        # snapshot interval H and cluster size at configs 3 and 5
 
 --configs: every workload of BASELINE.json (workloads.CONFIGS), a bounded prefix of its chain, one line each:
 accepted hops/s, window proposals evaluated/s (M per PR iteration), attempts consumed/s
 (m = (p-1)M + q per hop), mean p and mean q (0-based label of the executed proposal),
 acceptance A = hops/attempts over the run and over its last 10 %, the paper's split of the time per hop
- W_U = the eps update alone (`cg_apply_hops` on the hops just executed and their reversal) and
-W_R = time per hop - W_U (in the persistent kernel the two overlap, so W_R is what the update does not
-explain), the update's algorithmic GB/s (16 N bytes per hop) and the drift of the incremental eps against a
-full-sum recomputation.
+ measured inside the persistent kernel that runs (`cg_get_phase_cycles`, timed build of the same
+kernel, a second pass over the same hops): per worker warp of CTA 0 and per iteration, cycles spent testing
+proposals (propose), in its share of the eps update (update = W_U in the loop) and waiting for the outcome
+(wait); W_R = propose + wait; next to it the update alone (`cg_apply_hops`) with its algorithmic GB/s (16 N bytes
+per hop), and the drift of the incremental eps against a full-sum recomputation.
 
 --replicas: independent sims side by side on one GPU: packed into ONE persistent launch (`cg_run_many`), and
 as separate persistent kernels on separate CUDA streams.
@@ -88,12 +92,92 @@ def report_configs(hops, warm):
             us_hop = 1e3 * ms / Hd
             w_u = update_alone_us(kw)
             ln = g.launch()
+            # the paper's split, from the timed build of the same kernel on the next `chunk` hops
+            split = ""
+            if ln["threads"] == 544:
+                g.set_phase_timers(True)
+                g.phase_cycles(reset=True)
+                it0 = g.counters()["iterations"]
+                g.run(chunk)
+                pc = g.phase_cycles()
+                g.set_phase_timers(False)
+                n_it = g.counters()["iterations"] - it0
+                w = max(pc["warps"], 1)
+                split = "  in-loop cycles/iteration: total %.0f = propose %.0f + update %.0f + wait %.0f" % (
+                    pc["total"] / n_it, pc["propose"] / w / n_it, pc["update"] / w / n_it, pc["wait"] / w / n_it)
             print("%-9s T=%-5g M=%-6d %3d CTAs x %d: %7.0f hops/s  %.2e proposals/s  %.2e attempts/s  "
-                  "p=%.3f q=%8.1f  A=%.2e (last 10%%: %.2e)  %5.2f us/hop = W_U %.3f + W_R %.2f  "
-                  "update alone %6.0f GB/s  drift %.1e" % (
+                  "p=%.3f q=%8.1f  A=%.2e (last 10%%: %.2e)  %5.3f us/hop%s  "
+                  "update alone %.3f us/hop = %6.0f GB/s  drift %.1e" % (
                       name, kw["T"], M, ln["n_ctas"], ln["threads"], Hd / ms * 1e3, M * it / ms * 1e3,
-                      at / ms * 1e3, it / Hd, mean_q, A_all, A_last, us_hop, w_u, us_hop - w_u,
+                      at / ms * 1e3, it / Hd, mean_q, A_all, A_last, us_hop, split, w_u,
                       16.0 * N / w_u / 1e3, g.recompute_eps()))
+            sys.stdout.flush()
+
+
+def report_l2():
+    """Sweep of the L2 roofline probe: buffer size, CTAs per SM, threads, access width, mode."""
+    print("# %s: cg_bench_l2, GB/s (read-modify-write counts read + written bytes), best of 5 launches of 500 passes" % (
+        torch.cuda.get_device_name(0)))
+    best = {}
+    for mode in ("rmw", "read", "write"):
+        for mib in (0.5, 2, 4, 16):
+            for cps, thr in ((1, 512), (2, 512), (4, 256), (2, 1024), (8, 128), (4, 512)):
+                for vec in (16, 32):
+                    gb = binding.bench_l2(int(mib * 2**20), reps=500, trials=5, mode=mode, ctas_per_sm=cps,
+                                          threads=thr, vec_bytes=vec)
+                    print("%-5s %4.1f MiB  %d CTAs/SM x %4d threads  %2d-byte accesses: %8.0f GB/s" % (
+                        mode, mib, cps, thr, vec, gb))
+                    if gb > best.get(mode, (0,))[0]:
+                        best[mode] = (gb, mib, cps, thr, vec)
+            sys.stdout.flush()
+    for mode, (gb, mib, cps, thr, vec) in best.items():
+        print("best %-5s: %8.0f GB/s at %.1f MiB, %d CTAs/SM x %d threads, %d-byte accesses" % (mode, gb, mib, cps, thr, vec))
+
+
+def report_update():
+    """Step a6 alone at the headline footprints: the gather kernel against the bulk-copy staged kernel."""
+    print("# %s: cg_apply_hops, 4000 scripted hops (a chain's own hops and their reversal), best of 5" % (
+        torch.cuda.get_device_name(0)))
+    for label, dim, kw in (("2D L=512", 2, dict(L=512, T=0.05, E=0.01, seed=1008, M=65536)),
+                           ("2D L=128", 2, dict(L=128, T=0.05, E=0.01, seed=1005, M=4096)),
+                           ("3D L=64", 3, dict(L=64, T=0.05, E=0.01, seed=64, M=65536))):
+        u = binding.CoulombGlass(hop_log=2000, dim=dim, **kw)
+        u.run(2000)
+        _, hi, hj = u.hops()
+        si = np.concatenate([hi, hj[::-1]])
+        sj = np.concatenate([hj, hi[::-1]])
+        ref = None
+        for kern in ("gathers", "staged"):
+            v = binding.CoulombGlass(dim=dim, **kw)
+            best = min(v.apply_hops(si, sj, kernel=kern) for _ in range(5))
+            eps = v.state()[1]
+            same = "" if ref is None else ("  eps bit-identical to the gather kernel: %s" % np.array_equal(eps, ref))
+            ref = eps if ref is None else ref
+            print("%-9s %-8s %.4f us/hop  %6.0f GB/s algorithmic (16 N bytes per hop)%s" % (
+                label, kern, 1e3 * best / si.size, 16.0 * v.N * si.size / (best * 1e-3) / 1e9, same))
+        sys.stdout.flush()
+
+
+def report_tuning(hops):
+    """cg_set_tuning A/B: snapshot interval H and thread-block clusters (DSMEM posts)."""
+    print("# %s: %d hops after 150000 warm-up hops (relaxed system)" % (torch.cuda.get_device_name(0), hops))
+    for name, idx in (("cfg3_L128", 2), ("cfg5_L512", 0)):
+        kw = workloads.init_args(workloads.CONFIGS[name][idx])
+        for H, cs in ((1, 1), (2, 1), (4, 1), (8, 1), (4, 2), (4, 4), (4, 8), (4, 16)):
+            g = binding.CoulombGlass(**kw)
+            try:
+                g.set_tuning(H, cs)
+            except binding.CgError as e:
+                print("%s H=%d cluster=%d: %s" % (name, H, cs, e))
+                continue
+            g.run(150000)
+            torch.cuda.synchronize()
+            ms = _timed(lambda: g.run(hops))
+            ln = g.launch()
+            print("%-9s H=%d cluster=%-2d %3d CTAs x %4d threads (%s labels): %7.0f hops/s  %.3f us/hop" % (
+                name, H, cs, ln["n_ctas"], ln["threads"],
+                "cached" if kw["M"] <= ln["n_ctas"] * (ln["threads"] - 96) else "recomputed",
+                hops / ms * 1e3, ms * 1e3 / hops))
             sys.stdout.flush()
 
 
@@ -128,7 +212,7 @@ def report_replicas(hops):
                 kw["seed"] += 100 * r
                 g = binding.CoulombGlass(**kw)
                 if n_ctas:
-                    g.set_launch(n_ctas, 512)
+                    g.set_launch(n_ctas, 544)
                 sims.append(g)
         binding.run_many(sims, 1000)
         torch.cuda.synchronize()
@@ -188,6 +272,9 @@ def main():
     ap.add_argument("--configs", action="store_true")
     ap.add_argument("--replicas", action="store_true")
     ap.add_argument("--observables", action="store_true")
+    ap.add_argument("--l2", action="store_true")
+    ap.add_argument("--update", action="store_true")
+    ap.add_argument("--tuning", action="store_true")
     ap.add_argument("--hops", type=int, default=0)
     ap.add_argument("--warm", type=int, default=2000)
     a = ap.parse_args()
@@ -199,6 +286,12 @@ def main():
         report_replicas(a.hops or 100_000)
     if a.observables:
         report_observables(a.hops or 200_000)
+    if a.l2:
+        report_l2()
+    if a.update:
+        report_update()
+    if a.tuning:
+        report_tuning(a.hops or 100_000)
 
 
 if __name__ == "__main__":
