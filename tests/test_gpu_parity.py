@@ -431,7 +431,7 @@ def full_oracles(oracle_lib):
 
 @pytest.mark.slow
 @pytest.mark.parametrize("name,idx", FULL)
-def test_full_length_configs(cg, full_oracles, name, idx):
+def test_full_length_configs(cg, oracle_lib, full_oracles, name, idx):
     """BASELINE.json's configs at their FULL hop counts (1e5 / 1e6 hops), hop log, occupations, eps, clock,
     dP and counters element by element.  CG_SKIP_FULL_PARITY=1 skips (several minutes of oracle time)."""
     import os
