@@ -155,6 +155,22 @@ int cg_get_time_stochastic(cg_sim* s, double* t_tau0);
 int cg_get_normals(cg_sim* s, uint64_t first_hop, uint64_t count, double* z);
 int cg_get_dos(cg_sim* s, double lo, double width, uint32_t nbins, uint64_t* hist, uint64_t* outside);
 int cg_get_series(cg_sim* s, uint64_t first, uint64_t count, double* t, int64_t* P);
+
+/* cg_get_dos_noalloc: cg_get_dos for callers that must not allocate (code under CUDA graph capture,
+ * tight serving loops, harnesses that forbid cudaMalloc).  Same arguments, same result, same kernel;
+ * the only difference is where the kernel's scratch bins live: in a file-scope device array of the
+ * library (CG_DOS_NOALLOC_MAX_BINS + 1 64-bit counters = 64 KiB + 8 B of device memory, held by every
+ * GPU that loads libcg.so until the process exits) instead of a cudaMalloc'ed buffer.  The call performs
+ * no cudaMalloc / cudaFree and no allocating library call; hist and outside are HOST pointers owned by
+ * the caller and written directly.
+ *   nbins > CG_DOS_NOALLOC_MAX_BINS -> CG_EINVAL (cg_last_error names the limit; use cg_get_dos).
+ *   The sim's device must be the current device (CG_EINVAL otherwise): the array's device address is
+ *   looked up once per device with that device current.
+ *   ALL calls on one GPU share the one array, which keeps the counts of the previous call; each call
+ *   clears the part it uses first.  Calls that overlap on the GPU (sims on different streams, several
+ *   host threads) race on it and return garbage: serialise them.  Synchronises the sim's stream. */
+#define CG_DOS_NOALLOC_MAX_BINS 8192u
+int cg_get_dos_noalloc(cg_sim* s, double lo, double width, uint32_t nbins, uint64_t* hist, uint64_t* outside);
 int cg_get_sigma0(cg_sim* s, double* sigma0);
 
 /* Recompute eps from its definition eps_i = phi_i + sum_{j!=i}(n_j - 1/2)/r_ij

@@ -18,7 +18,7 @@ CG_OK, CG_EINVAL, CG_ENOMEM, CG_ECUDA, CG_EUNSUPPORTED, CG_EDEVICE = 0, -1, -2, 
 EXPORTS = [
     "cg_init", "cg_workspace_bytes", "cg_init_ws", "cg_init3", "cg_workspace_bytes3", "cg_init3_ws",
     "cg_run", "cg_run_many", "cg_get_state", "cg_set_state",
-    "cg_get_time_stochastic", "cg_get_normals", "cg_get_dos", "cg_get_series", "cg_get_sigma0",
+    "cg_get_time_stochastic", "cg_get_normals", "cg_get_dos", "cg_get_dos_noalloc", "cg_get_series", "cg_get_sigma0",
     "cg_get_counters", "cg_enable_hop_log", "cg_get_hops", "cg_recompute_eps", "cg_apply_hops",
     "cg_set_update_kernel", "cg_get_table_sizes", "cg_get_tables", "cg_get_table_dz", "cg_get_phi", "cg_set_launch", "cg_get_launch",
     "cg_set_tuning", "cg_get_tuning", "cg_set_phase_timers", "cg_get_phase_cycles", "cg_bench_l2", "cg_free", "cg_strerror",
@@ -62,6 +62,7 @@ def lib():
         "cg_get_time_stochastic": (ci, [vp, P(dbl)]),
         "cg_get_normals": (ci, [vp, u64, u64, vp]),
         "cg_get_dos": (ci, [vp, dbl, dbl, u32, vp, P(u64)]),
+        "cg_get_dos_noalloc": (ci, [vp, dbl, dbl, u32, vp, P(u64)]),
         "cg_get_series": (ci, [vp, u64, u64, vp, vp]),
         "cg_get_sigma0": (ci, [vp, P(dbl)]),
         "cg_apply_hops": (ci, [vp, u64, vp, vp, P(C.c_float)]),
@@ -245,6 +246,16 @@ class CoulombGlass:
         with self._torch.cuda.device(self.device):
             self._check(self._lib.cg_get_dos(self._h, float(lo), float(width), int(nbins), _ptr(hist),
                                              C.byref(outside)))
+        return hist, outside.value
+
+    def dos_noalloc(self, lo, width, nbins, hist=None):
+        """cg_get_dos_noalloc: the same counts; the kernel's scratch is a static device array of the library."""
+        if hist is None:
+            hist = np.zeros(int(nbins), np.uint64)
+        outside = C.c_uint64()
+        with self._torch.cuda.device(self.device):
+            self._check(self._lib.cg_get_dos_noalloc(self._h, float(lo), float(width), int(nbins), _ptr(hist),
+                                                     C.byref(outside)))
         return hist, outside.value
 
     def series(self, first=0, count=None):

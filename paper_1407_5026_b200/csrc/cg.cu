@@ -37,6 +37,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <string>
 #include <vector>
@@ -2638,6 +2639,67 @@ extern "C" int cg_get_dos(cg_sim* s, double lo, double width, uint32_t nbins, ui
     CK(cudaStreamSynchronize(s->stream));
     memcpy(hist, h.data(), 8 * (size_t)nbins);
     if (outside) *outside = h[nbins];
+    return CG_OK;
+}
+
+// ---- cg_get_dos_noalloc: the same histogram without any allocation -------------------------------------
+// For callers that cannot call cudaMalloc (CUDA graph capture, tight serving loops): the scratch bins of
+// cg_dos live in a file-scope device array of CG_DOS_NOALLOC_MAX_BINS + 1 counters (64 KiB + 8 B, held by
+// every GPU that loads the library until exit).  In host code the array's name is only a host-side stand-in
+// for the symbol: its device address is taken once per device, with that device current, by
+// cudaGetSymbolAddress, and only that pointer is ever given to a kernel or a copy.
+static __device__ __align__(256) unsigned long long cg_dos_static_bins[CG_DOS_NOALLOC_MAX_BINS + 1];
+
+#define CG_MAX_DEVICES 64
+static unsigned long long* g_dos_bins_addr[CG_MAX_DEVICES];      // device address of the array on device d, once known
+static std::mutex g_dos_bins_mutex;
+
+// device address of cg_dos_static_bins on the sim's device, which must be the current one
+static int dos_static_bins(cg_sim* s, unsigned long long** out)
+{
+    int dev = -1;
+    CK(cudaGetDevice(&dev));
+    if (dev != s->device || dev < 0 || dev >= CG_MAX_DEVICES) {
+        s->err = "cg_get_dos_noalloc: the sim's device must be the current device";
+        return CG_EINVAL;
+    }
+    std::lock_guard<std::mutex> lock(g_dos_bins_mutex);
+    if (!g_dos_bins_addr[dev]) {
+        void* ptr = nullptr;
+        CK(cudaGetSymbolAddress(&ptr, cg_dos_static_bins));
+        if (!ptr) { s->err = "cudaGetSymbolAddress returned a null address"; return CG_ECUDA; }
+        g_dos_bins_addr[dev] = (unsigned long long*)ptr;
+    }
+    *out = g_dos_bins_addr[dev];
+    return CG_OK;
+}
+
+extern "C" int cg_get_dos_noalloc(cg_sim* s, double lo, double width, uint32_t nbins, uint64_t* hist, uint64_t* outside)
+{
+    if (!s || !hist || !(width > 0.0) || nbins == 0) return CG_EINVAL;
+    if (nbins > CG_DOS_NOALLOC_MAX_BINS) {
+        char buf[160];
+        snprintf(buf, sizeof buf, "cg_get_dos_noalloc: nbins = %u exceeds the static scratch of %u bins "
+                                  "(use cg_get_dos)", nbins, (unsigned)CG_DOS_NOALLOC_MAX_BINS);
+        s->err = buf;
+        return CG_EINVAL;
+    }
+    CgCtl c;
+    int rc = read_ctl(s, &c);
+    if (rc != CG_OK) return rc;
+    unsigned long long* bins = nullptr;
+    if ((rc = dos_static_bins(s, &bins)) != CG_OK) return rc;
+    // the array keeps the counts of the last call: everything this call reads back starts at zero
+    CK(cudaMemsetAsync(bins, 0, 8 * ((size_t)nbins + 1), s->stream));
+    const u32 nsh = nbins <= 8192 ? nbins : 0;
+    const unsigned grid = std::max(1u, std::min((s->N + 2047) / 2048, 148u * 4));
+    cg_dos<<<grid, 256, 4 * (size_t)nsh, s->stream>>>(s->d_eps[c.cur % CG_RING], s->N, lo, width, nbins, nsh, bins);
+    CK(cudaGetLastError());
+    unsigned long long out_of_range = 0;
+    CK(cudaMemcpyAsync(hist, bins, 8 * (size_t)nbins, cudaMemcpyDeviceToHost, s->stream));
+    CK(cudaMemcpyAsync(&out_of_range, bins + nbins, 8, cudaMemcpyDeviceToHost, s->stream));
+    CK(cudaStreamSynchronize(s->stream));
+    if (outside) *outside = out_of_range;
     return CG_OK;
 }
 
