@@ -211,7 +211,8 @@ int cg_get_phi(cg_sim* s, double* phi /* N */);
 int cg_set_launch(cg_sim* s, int n_ctas, int threads);
 int cg_get_launch(cg_sim* s, int* n_ctas, int* threads, int* smem_bytes);
 
-/* Tuning that never changes results.  snapshot_interval H in {1, 2, 4, 8} (default 8): the
+/* Tuning that never changes results.  snapshot_interval H in {1, 2, 4, 8} (default: 8 for N >= 2^18
+ * sites, else 2): the
  * eps slabs, kept current in registers after every hop, are written through to memory
  * every H hops (deferred update; PAPER.md:77, 106 W_U); cluster_size in {1, 2, 4, 8, 16}:
  * CTAs per thread-block cluster, whose members post their results into each other's
@@ -222,6 +223,12 @@ int cg_get_launch(cg_sim* s, int* n_ctas, int* threads, int* smem_bytes);
  * explicit CTA count keeps the largest cluster size that divides it; cg_get_tuning reports
  * the cluster size in use.  cg_run_many launches without clusters. */
 int cg_set_tuning(cg_sim* s, int snapshot_interval, int cluster_size);
+/* How the M labels of an iteration are held in the launch shape in use: *labels_per_thread =
+ * K >= 1: every worker thread keeps K proposals decoded (attempts a, a + P, ..., a + (K-1) P with P = CTAs x
+ * worker threads >= M / K) and only re-tests them in every iteration (K = 1 whenever M <= P; K <= 8, 544-thread
+ * shape, while the extra slots fit shared memory); 0: M is larger than that and every label is decoded and
+ * tested from scratch in every iteration (time linear in M).  Results never depend on it. */
+int cg_get_labels_per_thread(cg_sim* s, int* labels_per_thread);
 int cg_get_tuning(cg_sim* s, int* snapshot_interval, int* cluster_size);
 
 /* The paper's split of the time per hop into rejection and update time (PAPER.md:106:

@@ -70,6 +70,8 @@ typedef unsigned int u32;
 #define CG_KS 2048          // head of the tower kept in shared memory (the rest, hardly ever drawn, stays in L2)
 #define CG_MAX_CLUSTER 16
 #define CG_MAX_SNAP 8       // largest snapshot interval H
+#define CG_KMAX 8           // MULTI: most cached labels per thread
+#define CG_XSLOT_BYTES 40   // MULTI: shared memory per extra label slot and thread
 
 #define CG_F_HOP 1u         // descriptor flags: the iteration executed a hop
 #define CG_F_LAST 2u        //   ... and it was the last one of this launch
@@ -120,6 +122,8 @@ struct CgParams {           // kernel parameter block
     u32 snap_shift;         // snapshots every H = 1 << snap_shift hops
     u32 gate;               // G: hop h waits until every CTA has published the snapshot that covers hop h - G
     u32 cluster;            // CTAs per thread-block cluster (1: none)
+    u32 K;                  // MULTI: cached labels per thread (attempts a, a + P, .., a + (K-1) P); else 1
+    u32 xoff;               // MULTI: byte offset of the extra label slots in dynamic shared memory
     u64 watchdog_ns;        // a wait longer than this aborts the launch (0: never)
 };
 
@@ -460,6 +464,17 @@ __device__ __forceinline__ bool metropolis(double dE, u32 uh, u32 ul, double T, 
 
 #define BIT(sn, s) (((sn)[(s) >> 5] >> ((s) & 31)) & 1u)
 
+// Cached labels: does worker warp wr of the CTA at scan position kb hold a label of the window [0, M)?  Thread t of
+// that CTA holds label (kb per + t - tr) mod P, tr = offset of the window start in the CTA at position 0; the labels of
+// a warp are consecutive (mod P), and only the warp w0 = tr / 32 at position 0 can contain the wrap (label 0).
+__device__ __forceinline__ bool warp_in_window(u32 kb, u32 tr, u32 wr, u32 w0, u32 per, u32 P, u32 M)
+{
+    if (kb == 0u && wr == w0) return true;
+    u32 x = kb * per + 32u * wr + P - tr;       // < 2 P
+    if (x >= P) x -= P;
+    return x < M;
+}
+
 // What the exchange warp publishes about iteration e, in slot e % CG_XR of the descriptor ring.
 struct __align__(16) Desc {
     u32 used;               // attempts consumed: q + 1, or M when the whole window was rejected
@@ -555,9 +570,10 @@ __device__ __forceinline__ bool mbar_wait(u64* b, u32 parity, const CgParams& p,
 //
 // Written as a device function of (parameters, CTA index, CTA count) so that one launch can also hold
 // several sims side by side (cg_pr_persistent_many): nothing in it looks at blockIdx or gridDim.
-template <int NW, int RP, bool CACHED, bool TIMED>
+template <int NW, int RP, bool CACHED, bool TIMED, bool MULTI = false>
 __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 b, const u32 nb)
 {
+    static_assert(!MULTI || CACHED, "MULTI is a variant of the cached-label path");
     constexpr int TW = NW * 32;           // worker threads
     constexpr int THREADS = TW + 96;
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -568,6 +584,16 @@ __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 
     u32* s_disp = reinterpret_cast<u32*>(s_fld + KS);
     u32* s_guide = s_disp + KS;
     u32* s_n = s_guide + CG_GUIDE;
+    // MULTI: label slots 1 .. K-1 of every worker thread (slot 0 lives in registers), [physical slot][thread]
+    const u32 KX = MULTI ? p.K - 1u : 0u;
+    double* x_ei = reinterpret_cast<double*>(smem_raw + (MULTI ? p.xoff : 0u));
+    double* x_ej = x_ei + KX * TW;
+    u32* x_ci = reinterpret_cast<u32*>(x_ej + KX * TW);
+    u32* x_cj = x_ci + KX * TW;
+    u32* x_uh = x_cj + KX * TW;
+    u32* x_ul = x_uh + KX * TW;
+    u32* x_k = x_ul + KX * TW;
+    u32* x_fl = x_k + KX * TW;            // bit 0: n_i, 1: n_j, 2: energies followed, 3: slot decoded
     __shared__ Comm cmem;
     Comm* const cm = &cmem;
     const Tables tb = {s_cdfi, s_invr, s_fld, s_disp, s_guide, p.cdfi, p.invr_k, p.fld_k, p.disp, (u32)KS};
@@ -669,10 +695,13 @@ __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 
         for (u32 e = 0;; ++e) {
             const u32 xs = e % CG_XR, e32 = e_start + e;
             const u32 kb = b >= cf ? b - cf : b + nb - cf;
-            const u32 tail0 = (CACHED && kb == 0) ? per - tr : CG_NONE;
+            // head labels of the CTA at position kb: [kb per - tr, (kb+1) per - tr); anything above (the tail at
+            // position 0; MULTI: the labels of slots 1 .. K-1) ranks after every head label of the grid
+            const u32 tail0 = CACHED ? (kb + 1u) * per - tr : CG_NONE;
             const u32 w0 = (CACHED && kb == 0) ? tr >> 5 : 0u;
             u32 wr = w0 + (u32)lane; if (wr >= (u32)NW) wr -= NW;
-            const bool mine = lane < NW;
+            // CACHED: a warp all of whose labels lie beyond the window (M < P) reports nothing anybody needs
+            const bool mine = lane < NW && (!CACHED || warp_in_window(kb, tr, wr, w0, per, P, M));
             bool ready = !mine; u32 l = CG_NONE, tl = CG_NONE; u64 pay = 0;
             u32 gmin = CG_NONE; u64 gpay = 0;
             wd.reset();
@@ -796,8 +825,10 @@ __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 
             const u32 tail0 = CACHED ? per - t0r : CG_NONE;
             const u32 ring = e32 & (CG_SRING - 1u), e16 = e32 & 0xFFFFu;
             u32 q = CG_NONE; u64 wp = 0;
-            u32 tlab = CG_NONE; u64 tpay = 0;                          // tail accept of position 0
-            u32 lo = 0, hi = min(nb, 4u);
+            u32 tlab = CG_NONE; u64 tpay = 0;                          // lowest late accept among the positions of this lane
+            // positions that hold labels of the window (all of them when it wraps around to position 0)
+            const u32 npos = CACHED ? min(nb, (t0r + M + per - 1u) / per) : nb;
+            u32 lo = 0, hi = min(npos, 4u);
             wd.reset();
             if (CACHED && kb == 0) {
                 // My own workers hold the start of the window: their results, read directly in label order (the
@@ -805,7 +836,7 @@ __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 
                 // A head accept of mine decides the iteration; otherwise the scan below goes on from my own post.
                 const u32 w0 = t0r >> 5;
                 u32 wr = w0 + (u32)lane; if (wr >= (u32)NW) wr -= NW;
-                bool ready = lane >= NW; u32 l = CG_NONE; u64 pay = 0;
+                bool ready = lane >= NW || !warp_in_window(0u, t0r, wr, w0, per, P, M); u32 l = CG_NONE; u64 pay = 0;
                 for (;;) {
                     if (!ready) {
                         u64 q0, q1;
@@ -815,17 +846,18 @@ __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 
                     const u32 racc = __ballot_sync(CG_FULL, ready && l != CG_NONE);
                     const u32 rnot = __ballot_sync(CG_FULL, !ready);
                     const int fa = racc ? __ffs(racc) - 1 : 32, fn = rnot ? __ffs(rnot) - 1 : 32;
-                    if (fa < fn) { q = __shfl_sync(CG_FULL, l, fa); wp = __shfl_sync(CG_FULL, pay, fa); lo = nb; break; }
+                    if (fa < fn) { q = __shfl_sync(CG_FULL, l, fa); wp = __shfl_sync(CG_FULL, pay, fa); lo = npos; break; }
                     if (!rnot) break;                   // no head accept here: the general scan (my tail labels come from own[])
                     if (wait_poll(wd, p, cm, 6u)) { quit = true; break; }
                 }
                 if (quit) break;
             }
-            while (lo < nb) {
+            while (lo < npos) {
                 const u32 k = lo + (u32)lane;
                 const bool mine = k < hi;
                 u32 c = c_first + k; if (c >= nb) c -= nb;
                 const bool local = mine && k != kb && csz > 1 && c - cl0 < csz;
+                const u32 hb = CACHED ? (k + 1u) * per - t0r : CG_NONE;     // head labels of position k lie below this
                 bool ready = !mine; u32 l = CG_NONE; u64 pay = 0;
                 bool found = false;
                 for (;;) {
@@ -842,7 +874,7 @@ __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 
                                 pay = ((q1 >> 24) & 0xFFFFFFull) << 32 | (q1 & 0xFFFFFFull);
                             }
                         }
-                        if (ready && k == 0 && l != CG_NONE && l >= tail0) { tlab = l; tpay = pay; l = CG_NONE; }
+                        if (ready && l != CG_NONE && l >= hb) { if (l < tlab) { tlab = l; tpay = pay; } l = CG_NONE; }
                     }
                     const u32 racc = __ballot_sync(CG_FULL, ready && l != CG_NONE);
                     const u32 rnot = __ballot_sync(CG_FULL, !ready);
@@ -858,11 +890,16 @@ __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 
                     if (wait_poll(wd, p, cm, 6u)) { quit = true; break; }
                 }
                 if (quit || found) break;
-                if (lo == 0) { tlab = __shfl_sync(CG_FULL, tlab, 0); tpay = __shfl_sync(CG_FULL, tpay, 0); }
-                lo = hi; hi = min(nb, lo + 32u);
+                lo = hi; hi = min(npos, lo + 32u);
             }
             if (quit) break;
-            if (q == CG_NONE && tlab != CG_NONE) { q = tlab; wp = tpay; }   // only the tail of the window accepted
+            if (q == CG_NONE) {               // no head label accepted: the lowest of the late ones (labels are distinct)
+                const u32 tmin = __reduce_min_sync(CG_FULL, tlab);
+                if (tmin != CG_NONE) {
+                    const int src = __ffs(__ballot_sync(CG_FULL, tlab == tmin)) - 1;
+                    q = tmin; wp = __shfl_sync(CG_FULL, tpay, src);
+                }
+            }
             // lock step (not CACHED): every warp of this CTA has finished its tests of this iteration before the
             // bitmap changes
             if (!CACHED) {
@@ -884,7 +921,7 @@ __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 
             if (CACHED) {
                 if (t0r + used < per) t0r += used;
                 else {
-                    u32 g0 = c_first * per + t0r + used; if (g0 >= P) g0 -= P;      // used <= M <= P
+                    u32 g0 = c_first * per + t0r + (MULTI ? used % P : used); if (g0 >= P) g0 -= P;      // used <= M (<= P unless MULTI)
                     c_first = g0 / per; t0r = g0 - c_first * per;
                 }
             }
@@ -981,12 +1018,26 @@ __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 
             }
             oi = a; oj = c;
         };
+        // MULTI: logical slot k (1 .. KX) holds attempt a_cur + k P, label lab + k P; it sits in physical slot
+        // (rot + k - 1) mod KX, so that a consumed slot 0 is replaced by rotating (per thread)
+        u32 rot = 0;
+        bool mh = false; u32 mhi = 0, mhj = 0;    // the hop consumed last, not yet applied to slots 1 .. KX
+        auto xidx = [&](u32 k) { u32 ph = rot + k - 1u; if (ph >= KX) ph -= KX; return ph * (u32)TW + (u32)tid; };
+        auto x_decode = [&](u32 k) {              // as of hop hl
+            const Prop q = decode_attempt(tb, p, geo, a_cur + (u64)k * P);
+            const u32 ix = xidx(k);
+            bool oi, oj;
+            read_n(q.ci, q.cj, oi, oj);
+            x_ci[ix] = q.ci | geo.spare; x_cj[ix] = q.cj | geo.spare; x_uh[ix] = q.uh; x_ul[ix] = q.ul; x_k[ix] = q.k;
+            x_fl[ix] = 8u | (oi ? 1u : 0u) | (oj ? 2u : 0u);
+        };
         if (has_label) {
             const u32 g = b * per + (u32)tid, g0 = c_first * per + t0r;
             lab = g >= g0 ? g - g0 : g + P - g0;
             a_cur = a_start + lab;
             take(decode_attempt(tb, p, geo, a_cur));
             read_n(sci & mask, scj & mask, ni, nj);
+            if (MULTI) for (u32 k = 1; k <= KX; ++k) x_decode(k);
         }
 
         Slab<TW, RP> slab;
@@ -1011,16 +1062,21 @@ __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 
             fresh = false;
         };
         // the test of my proposal on the current state (steps 1-2)
+        // A proposal starts to follow its two energies (one snapshot read + the pending hops' terms) while it is
+        // still Mt - M labels away from the window, so that this never happens on the path of an iteration's result
+        const u32 Mt = min(P, max(2u * M, M + 4096u));
         auto test_mine = [&](u32& best) {
-            const bool th = lab < M && ni && !nj;                 // theta_ij, inside the window
+            const bool th = lab < Mt && ni && !nj;                // theta_ij, inside the window or about to enter it
             if (th) {
                 if (!tracked) { read_eps(sci, scj, ei, ej); tracked = true; }
                 else if (addterm) {           // the term of the hop consumed last (gathered when it was consumed)
                     ei = __dadd_rn(ei, __dsub_rn(a_i, b_i)); ej = __dadd_rn(ej, __dsub_rn(a_j, b_j));
                 }
-                // dH_ij = eps_j - eps_i - 1/r_ij - E dx_ij
-                const double dE = __dsub_rn(__dsub_rn(__dsub_rn(ej, ei), c_invr), c_fld);
-                if (metropolis(dE, cuh, cul, p.T, p.inv_T)) best = lab;
+                if (lab < M) {
+                    // dH_ij = eps_j - eps_i - 1/r_ij - E dx_ij
+                    const double dE = __dsub_rn(__dsub_rn(__dsub_rn(ej, ei), c_invr), c_fld);
+                    if (metropolis(dE, cuh, cul, p.T, p.inv_T)) best = lab;
+                }
             } else tracked = false;
         };
         for (u32 e = 0;; ++e) {
@@ -1035,12 +1091,46 @@ __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 
                 if (fresh && lab < M) refresh();
                 if (has_label && !fresh) test_mine(best);
                 addterm = false;
+                bi = sci & mask; bj = scj & mask;
+                if (MULTI && has_label) {
+                    // slots 1 .. KX: the hop consumed last (occupations, followed energies), then the test
+                    const u32 si = mhi | geo.spare, sj = mhj | geo.spare;
+                    for (u32 k = 1; k <= KX; ++k) {
+                        const u32 labk = lab + k * P;
+                        const u32 ix = xidx(k);
+                        u32 fl = x_fl[ix];
+                        if (!(fl & 8u)) {
+                            if (labk >= M) continue;            // decoded later, when the warp is far from the front
+                            x_decode(k); fl = x_fl[ix];
+                        } else if (mh) {
+                            const u32 ci_ = x_ci[ix], cj_ = x_cj[ix];
+                            if (fl & 4u) {
+                                x_ei[ix] = __dadd_rn(x_ei[ix], hop_term(tf, mask, ci_, mhi, mhj));
+                                x_ej[ix] = __dadd_rn(x_ej[ix], hop_term(tf, mask, cj_, mhi, mhj));
+                            }
+                            if (ci_ == si) fl &= ~1u; if (ci_ == sj) fl |= 1u;
+                            if (cj_ == si) fl &= ~2u; if (cj_ == sj) fl |= 2u;
+                        }
+                        if (labk < M && (fl & 3u) == 1u) {     // theta_ij, inside the window
+                            const u32 ci_ = x_ci[ix], cj_ = x_cj[ix];
+                            double vi, vj;
+                            if (!(fl & 4u)) { read_eps(ci_, cj_, vi, vj); x_ei[ix] = vi; x_ej[ix] = vj; fl |= 4u; }
+                            else { vi = x_ei[ix]; vj = x_ej[ix]; }
+                            const u32 kk = x_k[ix];
+                            const double dE = __dsub_rn(__dsub_rn(__dsub_rn(vj, vi), tb.inv(kk)), tb.field(kk));
+                            if (labk < best && metropolis(dE, x_uh[ix], x_ul[ix], p.T, p.inv_T)) {
+                                best = labk; bi = ci_ & mask; bj = cj_ & mask;
+                            }
+                        } else fl &= ~4u;
+                        x_fl[ix] = fl;
+                    }
+                    mh = false;
+                }
                 far_ = __reduce_min_sync(CG_FULL, lab) >= min(CG_FRONT, P >> 2);               // warp-uniform
                 u32 wmin = __reduce_min_sync(CG_FULL, best);
                 // ---- step 3: lowest accepting label of the warp, for the collector
                 if (wmin == CG_NONE ? lane == 0 : best == wmin) {   // labels are distinct: one lane
-                    sts128(&cm->res[e % (2 * CG_XR)][warp][0], ((u64)e32 << 32) | wmin,
-                           ((u64)(sci & mask) << 32) | (u64)(scj & mask));
+                    sts128(&cm->res[e % (2 * CG_XR)][warp][0], ((u64)e32 << 32) | wmin, ((u64)bi << 32) | (u64)bj);
                 }
             } else {
                 for (u32 l = lab0 + tid; l < lab1; l += TW) {
@@ -1066,7 +1156,9 @@ __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 
             // until all of its labels have been consumed and it sits at the far end of the window)
             if (CACHED && far_) {
                 if (fresh) refresh();
-                if (has_label && !nxt_valid) { nxt = decode_attempt(tb, p, geo, a_cur + P); nxt_valid = true; }
+                if (!MULTI && has_label && !nxt_valid) { nxt = decode_attempt(tb, p, geo, a_cur + P); nxt_valid = true; }
+                if (MULTI && has_label)
+                    for (u32 k = 1; k <= KX; ++k) if (!(x_fl[xidx(k)] & 8u)) x_decode(k);
             }
             // The slab runs one hop behind: the gathers of the hop consumed last are issued here, behind the result, and
             // were issued one iteration ago for the hop that is finished now - their latency is never waited for, and
@@ -1093,7 +1185,32 @@ __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 
             if (TIMED) { tprev = clock64(); t_wait += (u64)(tprev - t2); }
             if (d.y & CG_F_ABORT) return;
             last = (d.y & CG_F_LAST) != 0u;
+            if (MULTI && has_label) {
+                // labels first: a consumed slot 0 is replaced by the lowest slot that survives (its state is that of
+                // S_e, like slot 0's), to which the hop of O_e is then applied below like to any slot 0
+                if (lab >= d.x) lab -= d.x;
+                else {
+                    const u32 c = (d.x - lab + P - 1u) / P;        // consumed slots: labels lab + k P < used, 1 <= c <= K
+                    fresh = true; tracked = false; addterm = false;
+                    if (c <= KX) {
+                        const u32 ix = xidx(c);
+                        const u32 fl = x_fl[ix];
+                        if (fl & 8u) {
+                            sci = x_ci[ix]; scj = x_cj[ix]; cuh = x_uh[ix]; cul = x_ul[ix];
+                            const u32 kk = x_k[ix];
+                            c_invr = tb.inv(kk); c_fld = tb.field(kk);
+                            ni = (fl & 1u) != 0u; nj = (fl & 2u) != 0u; tracked = (fl & 4u) != 0u;
+                            if (tracked) { ei = x_ei[ix]; ej = x_ej[ix]; }
+                            fresh = false;
+                        }
+                    }
+                    lab += c * P - d.x; a_cur += (u64)c * P;
+                    rot += c; while (rot >= KX) rot -= KX;
+                    for (u32 k = (c <= KX ? KX + 1u - c : 1u); k <= KX; ++k) x_fl[xidx(k)] = 0u;
+                }
+            }
             if (d.y & CG_F_HOP) {
+                if (MULTI) { mh = true; mhi = d.z; mhj = d.w; }
                 if (CACHED) {
                     // the term of this hop for the pair I follow: the four gathers come first (discarded if my
                     // attempt was consumed or theta_ij turns out to have changed), then the slab's
@@ -1108,7 +1225,7 @@ __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 
                 }
                 ++hl; upd = true; hz = d.z; hw = d.w;
             }
-            if (CACHED) {
+            if (CACHED && !MULTI) {
                 if (has_label) {
                     if (lab >= d.x) lab -= d.x;
                     else {                              // my attempt was consumed: the next one, P attempts later
@@ -1116,7 +1233,7 @@ __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 
                         fresh = true; tracked = false; addterm = false;
                     }
                 }
-            } else a0 += d.x;
+            } else if (!CACHED) a0 += d.x;
         }
         if (inflight) {                   // the last hop of the launch
             const bool snap = (hs & Hm) == 0u;
@@ -1145,10 +1262,10 @@ __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 
     if (csz > 1) cluster_sync_all();
 }
 
-template <int NW, int RP, bool CACHED, bool TIMED>
+template <int NW, int RP, bool CACHED, bool TIMED, bool MULTI = false>
 __global__ void __launch_bounds__(NW * 32 + 96, 1) cg_pr_persistent(const CgParams p)
 {
-    pr_persistent_body<NW, RP, CACHED, TIMED>(p, blockIdx.x, gridDim.x);
+    pr_persistent_body<NW, RP, CACHED, TIMED, MULTI>(p, blockIdx.x, gridDim.x);
 }
 
 // Replica packing (the paper recommends averaging many samples): ONE launch,
@@ -1429,7 +1546,9 @@ struct cg_sim {
     void* d_many = nullptr; size_t many_cap = 0;      // parameter blocks of cg_run_many (owned by its first sim)
     // launch shape and tuning
     int num_sms = 0, n_ctas = 0, threads = 0, smem = 0, rp = 0, pl = 0;   // pl > 0: cached proposals
-    int snap_shift = 3;                   // snapshots every 8 hops
+    int lpt = 1;                          // cached labels per thread (> 1: the MULTI kernel, M > n_ctas * pl)
+    int snap_shift = 3;                   // snapshots every 1 << snap_shift hops
+    bool snap_auto = true;                // not set by cg_set_tuning: chosen from the lattice size at init
     int cluster = 1;                      // CTAs per thread-block cluster in use
     int cluster_pref = 0;                 // cg_set_tuning: 0 = automatic (clusters when the whole sim fits a few of them)
     bool timers = false;                  // cg_set_phase_timers
@@ -1582,10 +1701,16 @@ static void build_tables(cg_sim* s, std::vector<double>& tq)
             }
 }
 
-static size_t smem_bytes(const cg_sim* s)
+static size_t smem_base_bytes(const cg_sim* s)
 {
     const size_t ks = (size_t)std::min<int64_t>(s->Klive, CG_KS);
     return ks * 28 + 4 * CG_GUIDE + 4 * (((size_t)s->N + 31) / 32) + 16;
+}
+// K labels per thread: K - 1 extra slots of CG_XSLOT_BYTES for each of the 448 worker threads, 16-byte aligned
+static size_t smem_xoff(const cg_sim* s) { return (smem_base_bytes(s) + 15) & ~(size_t)15; }
+static size_t smem_bytes(const cg_sim* s, int K)
+{
+    return K > 1 ? smem_xoff(s) + (size_t)(K - 1) * 448 * CG_XSLOT_BYTES : smem_base_bytes(s);
 }
 
 // hops between snapshots -> gate distance G with CG_RING H > 2 G + 2 H - 2 (pr_persistent_body, "Snapshots")
@@ -1620,6 +1745,7 @@ static CgParams make_params(const cg_sim* s, u32 n_hops)
     p.T = s->T; p.E = s->E; p.inv_T = (float)(1.0 / s->T); p.n_hops = n_hops;
     p.snap_shift = (u32)s->snap_shift; p.gate = gate_for(s->snap_shift);
     p.cluster = (u32)s->cluster; p.watchdog_ns = s->watchdog_ns;
+    p.K = (u32)s->lpt; p.xoff = (u32)smem_xoff(s);
     return p;
 }
 
@@ -1646,8 +1772,19 @@ static int workers_of(int threads)
     switch (threads) { case 256: return 5; case 544: return 14; case 608: return 16; case 1024: return 29; }
     return 0;
 }
-static persist_fn persistent_kernel(int threads, int rp, bool cached, bool timed)
+static persist_fn persistent_kernel(int threads, int rp, bool cached, bool timed, bool multi = false)
 {
+    if (multi) {                          // several cached labels per thread: 544-thread shape only, no phase timers
+        if (threads != 544 || !cached) return nullptr;
+        switch (rp) {
+            case 0: return cg_pr_persistent<14, 0, true, false, true>;
+            case 1: return cg_pr_persistent<14, 1, true, false, true>;
+            case 2: return cg_pr_persistent<14, 2, true, false, true>;
+            case 4: return cg_pr_persistent<14, 4, true, false, true>;
+            case 8: return cg_pr_persistent<14, 8, true, false, true>;
+        }
+        return nullptr;
+    }
     switch (workers_of(threads)) {
         case 5: return cached ? persistent_kernel_t<5, true, false>(rp) : persistent_kernel_t<5, false, false>(rp);
         case 14: if (timed) return cached ? persistent_kernel_t<14, true, true>(rp) : persistent_kernel_t<14, false, true>(rp);
@@ -1699,20 +1836,21 @@ static int choose_rp(u64 pairs, int n_ctas, int workers, int cap)
 static int rp_cap(int threads) { return threads == 1024 ? 2 : threads == 608 ? 4 : 8; }
 
 // how many CTAs of this shape can be co-resident (in clusters of s->cluster)
-static int max_coresident(cg_sim* s, int threads, int rp, bool cached, int* out)
+static int max_coresident(cg_sim* s, int threads, int rp, bool cached, int K, int* out)
 {
-    persist_fn f = persistent_kernel(threads, rp, cached, false);
+    const int smem = (int)smem_bytes(s, K);
+    persist_fn f = persistent_kernel(threads, rp, cached, false, K > 1);
     if (!f) return CG_EINVAL;
-    CK(cudaFuncSetAttribute((const void*)f, cudaFuncAttributeMaxDynamicSharedMemorySize, s->smem));
-    persist_fn ft = threads == 544 ? persistent_kernel(threads, rp, cached, true) : nullptr;      // the timed build
-    if (ft) CK(cudaFuncSetAttribute((const void*)ft, cudaFuncAttributeMaxDynamicSharedMemorySize, s->smem));
+    CK(cudaFuncSetAttribute((const void*)f, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+    persist_fn ft = threads == 544 && K == 1 ? persistent_kernel(threads, rp, cached, true) : nullptr;      // the timed build
+    if (ft) CK(cudaFuncSetAttribute((const void*)ft, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
     if (s->cluster > 1) {
         if (s->cluster > 8) {
             CK(cudaFuncSetAttribute((const void*)f, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
             if (ft) CK(cudaFuncSetAttribute((const void*)ft, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
         }
         cudaLaunchConfig_t cfg = {};
-        cfg.gridDim = dim3(s->cluster * s->num_sms); cfg.blockDim = dim3(threads); cfg.dynamicSmemBytes = (size_t)s->smem;
+        cfg.gridDim = dim3(s->cluster * s->num_sms); cfg.blockDim = dim3(threads); cfg.dynamicSmemBytes = (size_t)smem;
         cudaLaunchAttribute at[1];
         at[0].id = cudaLaunchAttributeClusterDimension;
         at[0].val.clusterDim.x = (unsigned)s->cluster; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
@@ -1723,7 +1861,7 @@ static int max_coresident(cg_sim* s, int threads, int rp, bool cached, int* out)
         return CG_OK;
     }
     int per_sm = 0;
-    CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, (const void*)f, threads, s->smem));
+    CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, (const void*)f, threads, smem));
     *out = std::min(per_sm * s->num_sms, CG_MAX_CTAS);
     return CG_OK;
 }
@@ -1746,25 +1884,38 @@ static int choose_launch_cs(cg_sim* s, int n_ctas, int threads)
         }
         if (want < 1 || want > CG_MAX_CTAS || want % cs) return CG_EINVAL;
         int rp = choose_rp(s->N / 2, want, workers, rp_cap(threads));
-        bool cached = s->M <= (u64)want * (u64)workers;
+        // labels cached in the threads: one each when M <= P = CTAs x workers, up to CG_KMAX each (MULTI kernel, 544-thread
+        // shape) while they fit shared memory; beyond that every label is recomputed in every iteration
+        auto labels_per_thread = [&](int ctas) {
+            const u64 Pn = (u64)ctas * (u64)workers;
+            if (s->M <= Pn) return 1;
+            const u64 K = (s->M + Pn - 1) / Pn;
+            if (threads != 544 || K > CG_KMAX) return 0;
+            if (smem_bytes(s, (int)K) + sizeof(Comm) + 1024 > (size_t)s->smem_optin) return 0;
+            return (int)K;
+        };
+        int K = labels_per_thread(want);
+        bool cached = K >= 1;
         int cap = 0;
-        int rc = max_coresident(s, threads, rp, cached, &cap);
+        int rc = max_coresident(s, threads, rp, cached, std::max(K, 1), &cap);
         if (rc != CG_OK) return rc;
         if (cap < cs) { s->err = "persistent kernel does not fit on the device in this cluster size"; return CG_EUNSUPPORTED; }
         if (want > cap) {
             if (!heuristic) return CG_EINVAL;
             want = cap / cs * cs;
             rp = choose_rp(s->N / 2, want, workers, rp_cap(threads));
-            cached = s->M <= (u64)want * (u64)workers;
-            rc = max_coresident(s, threads, rp, cached, &cap);
+            K = labels_per_thread(want);
+            cached = K >= 1;
+            rc = max_coresident(s, threads, rp, cached, std::max(K, 1), &cap);
             if (rc != CG_OK) return rc;
             if (want > cap) return CG_EUNSUPPORTED;
         }
         // clusters strand SMs: if the labels no longer fit the threads, larger CTAs keep them cached
-        if (heuristic && auto_threads && !cached && threads == 544 && s->M <= (u64)want * 512u) { threads = 608; continue; }
+        if (heuristic && auto_threads && K != 1 && threads == 544 && s->M <= (u64)want * 512u) { threads = 608; continue; }
         if (want != s->n_ctas)    // slots of CTAs that no longer exist must not look published
             CK(cudaMemsetAsync(s->d_slots, 0, CG_SLOT_BYTES, s->stream));
         s->n_ctas = want; s->threads = threads; s->rp = rp; s->pl = cached ? workers : 0;
+        s->lpt = std::max(K, 1); s->smem = (int)smem_bytes(s, s->lpt);
         return CG_OK;
     }
     return CG_EUNSUPPORTED;
@@ -1833,7 +1984,7 @@ static int init_impl(cg_sim** out, int dim, int L, double W, double xi, double T
     std::vector<double> tq;
     try { build_tables(s, tq); } catch (const std::bad_alloc&) { return CG_ENOMEM; }
     if (s->Klive > 65535) return CG_EUNSUPPORTED;           // the guide packs k in 16 bits
-    s->smem = (int)smem_bytes(s);
+    s->smem = (int)smem_bytes(s, 1);
     if ((size_t)s->smem + sizeof(Comm) + 1024 > (size_t)prop.sharedMemPerBlockOptin) return CG_EUNSUPPORTED;
 
     const WsLayout w = ws_layout(dim, L);
@@ -1883,6 +2034,9 @@ static int init_impl(cg_sim** out, int dim, int L, double W, double xi, double T
     CK(cudaGetLastError());
     CK(cudaStreamSynchronize(st));                        // host vectors above go out of scope
 
+    // snapshot interval (measured): the 2 MiB of eps at N = 2^18 are worth writing through only every
+    // 8 hops; smaller lattices run best with short pending lists
+    s->snap_shift = s->N >= (1u << 18) ? 3 : 1;
     int rc = choose_launch(s, 0, 0);
     if (rc != CG_OK) return rc;
     guard.s = nullptr;
@@ -1949,7 +2103,7 @@ static cudaError_t launch_coop(const void* f, int grid, int threads, int smem, c
 extern "C" int cg_run(cg_sim* s, uint64_t n_hops)
 {
     if (!s) return CG_EINVAL;
-    persist_fn f = persistent_kernel(s->threads, s->rp, s->pl > 0, s->timers && s->threads == 544);
+    persist_fn f = persistent_kernel(s->threads, s->rp, s->pl > 0, s->timers && s->threads == 544 && s->lpt == 1, s->lpt > 1);
     if (!f) return CG_EINVAL;
     while (n_hops) {
         const u32 chunk = (u32)std::min<uint64_t>(n_hops, CG_MAX_LAUNCH_HOPS);
@@ -1975,7 +2129,7 @@ extern "C" int cg_run_many(cg_sim* const* sims, int n_sims, uint64_t n_hops)
         if (!s) return CG_EINVAL;
         for (int m = 0; m < k; ++m) if (sims[m] == s) return CG_EINVAL;       // a sim may appear once
         if (s->device != s0->device || s->stream != s0->stream || s->threads != s0->threads || s->rp != s0->rp
-            || (s->pl > 0) != (s0->pl > 0)) {
+            || (s->pl > 0 && s->lpt == 1) != (s0->pl > 0 && s0->lpt == 1)) {
             s0->err = "cg_run_many: the sims must share device, stream and launch shape (threads, register tiling, "
                       "cached labels)";
             return CG_EINVAL;
@@ -1983,7 +2137,7 @@ extern "C" int cg_run_many(cg_sim* const* sims, int n_sims, uint64_t n_hops)
         first[(size_t)k + 1] = first[(size_t)k] + (u32)s->n_ctas;
         smem = std::max(smem, s->smem);
     }
-    many_fn f = many_kernel(s0->threads, s0->rp, s0->pl > 0);
+    many_fn f = many_kernel(s0->threads, s0->rp, s0->pl > 0 && s0->lpt == 1);     // several labels per thread: recomputed here
     if (!f) { s0->err = "cg_run_many: only 544-thread launch shapes"; return CG_EUNSUPPORTED; }
     CK0(s0, cudaFuncSetAttribute((const void*)f, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
     int per_sm = 0;
@@ -2003,7 +2157,10 @@ extern "C" int cg_run_many(cg_sim* const* sims, int n_sims, uint64_t n_hops)
     u32* d_first = (u32*)((char*)s0->d_many + ps.size() * sizeof(CgParams));
     while (n_hops) {
         const u32 chunk = (u32)std::min<uint64_t>(n_hops, CG_MAX_LAUNCH_HOPS);
-        for (int k = 0; k < n_sims; ++k) { ps[(size_t)k] = make_params(sims[k], chunk); ps[(size_t)k].cluster = 1; }   // posts through L2
+        for (int k = 0; k < n_sims; ++k) {
+            ps[(size_t)k] = make_params(sims[k], chunk); ps[(size_t)k].cluster = 1;       // posts through L2
+            if (sims[k]->lpt > 1) { ps[(size_t)k].PL = 0; ps[(size_t)k].K = 1; }
+        }
         // pageable sources: the copies are staged before the calls return
         CK0(s0, cudaMemcpyAsync(d_ps, ps.data(), ps.size() * sizeof(CgParams), cudaMemcpyHostToDevice, s0->stream));
         CK0(s0, cudaMemcpyAsync(d_first, first.data(), first.size() * sizeof(u32), cudaMemcpyHostToDevice, s0->stream));
@@ -2286,6 +2443,7 @@ extern "C" int cg_set_tuning(cg_sim* s, int snapshot_interval, int cluster_size)
     if (snapshot_interval) {
         if (snapshot_interval != 1 && snapshot_interval != 2 && snapshot_interval != 4 && snapshot_interval != 8) return CG_EINVAL;
         shift = snapshot_interval == 1 ? 0 : snapshot_interval == 2 ? 1 : snapshot_interval == 4 ? 2 : 3;
+        s->snap_auto = false;
     }
     if (cluster_size) {
         if (cluster_size != -1 && (cluster_size < 1 || cluster_size > CG_MAX_CLUSTER || (cluster_size & (cluster_size - 1)))) return CG_EINVAL;
@@ -2306,6 +2464,13 @@ extern "C" int cg_get_tuning(cg_sim* s, int* snapshot_interval, int* cluster_siz
     if (!s) return CG_EINVAL;
     if (snapshot_interval) *snapshot_interval = 1 << s->snap_shift;
     if (cluster_size) *cluster_size = s->cluster;
+    return CG_OK;
+}
+
+extern "C" int cg_get_labels_per_thread(cg_sim* s, int* labels_per_thread)
+{
+    if (!s || !labels_per_thread) return CG_EINVAL;
+    *labels_per_thread = s->pl > 0 ? s->lpt : 0;
     return CG_OK;
 }
 

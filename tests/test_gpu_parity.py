@@ -201,7 +201,7 @@ def test_launch_shape_may_change_between_runs(cg, oracle_lib):
     assert g.recompute_eps() < 1e-9
 
 
-@pytest.mark.parametrize("n_ctas,threads,M", [(148, 544, 303104), (148, 256, 65536), (20, 1024, 65536), (148, 1024, 65536)])
+@pytest.mark.parametrize("n_ctas,threads,M", [(148, 544, 303104), (30, 544, 303104), (148, 256, 65536), (20, 1024, 65536), (148, 1024, 65536)])
 def test_labels_recomputed_or_cached(cg, oracle_lib, n_ctas, threads, M):
     """M larger than the label-owning threads of the grid takes the path that decodes every label in
     every iteration; otherwise proposals are cached.  Both must give the serial chain."""
@@ -212,6 +212,33 @@ def test_labels_recomputed_or_cached(cg, oracle_lib, n_ctas, threads, M):
     o = oracle_lib.Oracle(**kw)
     o.run(3000)
     _compare(g, o, 3000)
+
+
+@pytest.mark.parametrize("kw,n_ctas,K,hops", [
+    (dict(L=16, T=0.01, E=0.0, seed=6, M=3000), 2, 4, 300),      # cold: whole windows rejected, every slot of a thread consumed at once
+    (dict(L=16, T=0.01, E=0.0, seed=6, M=897), 2, 2, 300),       # one single label in the second slot
+    (dict(L=32, T=5.0, E=0.3, seed=4, M=7168), 2, 8, 20000),     # hot: q = 0 mostly; the most labels per thread, M = K P exactly
+    (dict(L=64, T=0.05, E=0.01, seed=2, M=5000), 3, 4, 20000),   # ragged last slot, three CTAs
+    (dict(L=64, T=0.03, E=0.01, seed=12, M=40000), 37, 3, 20000),
+    (dict(L=16, dim=3, T=0.05, E=0.01, seed=13, M=9000), 8, 3, 6000),
+    (dict(L=32, T=0.08, E=0.01, seed=5, M=4096), 1, 0, 2000),    # more than 8 labels per thread: recomputed
+])
+def test_several_cached_labels_per_thread(cg, oracle_lib, kw, n_ctas, K, hops):
+    """M larger than the label-owning threads P of the grid (M up to the resident threads and beyond):
+    every thread keeps K = ceil(M / P) <= 8 proposals decoded, slot 0 in registers, the others in shared memory;
+    the lowest accepting label over all slots wins (labels of slot k rank after all labels of slot k - 1).  Split
+    runs re-decode the slots; the chain must be the serial one whatever K."""
+    g = cg.CoulombGlass(hop_log=hops, **kw)
+    g.set_launch(n_ctas, 544)
+    assert g.labels_per_thread() == K
+    g.run(hops // 3)
+    g.run(hops - hops // 3)
+    o = oracle_lib.Oracle(**kw)
+    o.run(hops)
+    _compare(g, o, hops)
+    c = g.counters()
+    assert c["proposals_evaluated"] == kw["M"] * c["iterations"]
+    assert g.recompute_eps() < 1e-9
 
 
 def test_config4_M_sweep_is_one_trajectory(cg):
