@@ -171,7 +171,7 @@ def run_reference(args):
     }))
 
 
-CTL_BYTES = 128  # sizeof(CgCtl) in csrc/cg.cu: the control block cg_set_state / cg_get_state move
+CTL_BYTES = 176  # sizeof(CgCtl) in csrc/cg.cu: the control block cg_set_state / cg_get_state move
 
 
 L2_PROBES = [  # the shapes that came out on top of the sweep (profiles/r2_l2_sweep.txt), re-measured live

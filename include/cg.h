@@ -244,6 +244,12 @@ int cg_get_tuning(cg_sim* s, int* snapshot_interval, int* cluster_size);
  * by default: cg_set_phase_timers(s, 1) makes the following cg_run calls use the timed build
  * of the same kernel (544-thread launch shapes only; otherwise nothing is recorded). */
 int cg_set_phase_timers(cg_sim* s, int on);
+/* The select side of W_R (step 3) from the same timed build: cycles6[0..4] = SUMS over the exchange
+ * warps of all CTAs of the cycles spent (0) waiting until the slowest consumer of the CTA has released the
+ * descriptor slot, (1) at the gate on published eps snapshots, (2) at scan position 0: waiting for the CTA's own
+ * workers, (3) scanning the posts of the CTAs in label order, (4) deciding and publishing the outcome;
+ * cycles6[5] = exchange warps that contributed (CTAs x launches).  Reset together with cg_get_phase_cycles. */
+int cg_get_exchange_cycles(cg_sim* s, uint64_t* cycles6);
 int cg_get_phase_cycles(cg_sim* s, uint64_t* total, uint64_t* wait, uint64_t* update,
                         uint64_t* propose, uint64_t* warps, int reset);
 

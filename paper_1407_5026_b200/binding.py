@@ -21,7 +21,7 @@ EXPORTS = [
     "cg_get_time_stochastic", "cg_get_normals", "cg_get_dos", "cg_get_dos_noalloc", "cg_get_series", "cg_get_sigma0",
     "cg_get_counters", "cg_enable_hop_log", "cg_get_hops", "cg_recompute_eps", "cg_apply_hops",
     "cg_set_update_kernel", "cg_get_table_sizes", "cg_get_tables", "cg_get_table_dz", "cg_get_phi", "cg_set_launch", "cg_get_launch",
-    "cg_set_tuning", "cg_get_tuning", "cg_get_labels_per_thread", "cg_set_phase_timers", "cg_get_phase_cycles", "cg_bench_l2", "cg_free", "cg_strerror",
+    "cg_set_tuning", "cg_get_tuning", "cg_get_labels_per_thread", "cg_set_phase_timers", "cg_get_phase_cycles", "cg_get_exchange_cycles", "cg_bench_l2", "cg_free", "cg_strerror",
     "cg_last_error",
 ]
 
@@ -76,6 +76,7 @@ def lib():
         "cg_set_tuning": (ci, [vp, ci, ci]),
         "cg_get_tuning": (ci, [vp, P(ci), P(ci)]),
         "cg_get_labels_per_thread": (ci, [vp, P(ci)]),
+        "cg_get_exchange_cycles": (ci, [vp, vp]),
         "cg_set_phase_timers": (ci, [vp, ci]),
         "cg_get_phase_cycles": (ci, [vp, P(u64), P(u64), P(u64), P(u64), P(u64), ci]),
         "cg_bench_l2": (ci, [sz, ci, ci, ci, ci, ci, ci, P(dbl)]),
@@ -328,6 +329,12 @@ class CoulombGlass:
         a, b = C.c_int(), C.c_int()
         self._check(self._lib.cg_get_tuning(self._h, C.byref(a), C.byref(b)))
         return {"snapshot_interval": a.value, "cluster_size": b.value}
+
+    def exchange_cycles(self):
+        """cg_get_exchange_cycles: where the exchange warps (all CTAs) spent their cycles, timed build."""
+        a = np.zeros(6, np.uint64)
+        self._check(self._lib.cg_get_exchange_cycles(self._h, _ptr(a)))
+        return dict(zip(("recycle", "gate", "own_workers", "scan", "publish", "warps"), (int(v) for v in a)))
 
     def labels_per_thread(self):
         k = C.c_int()

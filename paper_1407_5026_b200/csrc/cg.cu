@@ -95,6 +95,7 @@ struct CgCtl {              // device-resident control block (one per sim)
     u32 abort;              // != 0: the watchdog of the persistent kernel fired (which wait: see cg.h)
     u32 pad;
     u64 cyc_warps;          // worker warps that contributed to cyc_wait/update/propose
+    u64 cyc_x[6];           // exchange warps of all CTAs (cg_get_exchange_cycles): recycle, gate, own workers, scan, publish; CTAs
 };
 
 struct CgParams {           // kernel parameter block
@@ -784,10 +785,14 @@ __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 
         u32 ver = 0;                      // newest snapshot known to be published by every CTA
         Waiter wd;
         bool quit = false;
+        u64 tx[5] = {0, 0, 0, 0, 0};
+        long long xt = TIMED ? clock64() : 0;
+        auto stamp = [&](int k) { if (TIMED) { const long long now = clock64(); tx[k] += (u64)(now - xt); xt = now; } };
         while (hc < n_hops) {
             const u32 xs = e % CG_XR, e32 = e_start + e;
             // (1) recycle the descriptor slot: every consumer is past iteration e - CG_XR
             if (CACHED && e >= CG_XR && !mbar_wait(&cm->empty[xs], ((e - CG_XR) / CG_XR) & 1u, p, cm, 4u)) { quit = true; break; }
+            stamp(0);
             // (2) gate: every CTA has published the snapshot that covers hop hc + 1 - G
             if (nb > 1 && hc + 1u > p.gate) {
                 const u32 need = (hc + 1u - p.gate) >> Hs;
@@ -821,6 +826,7 @@ __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 
             // the window; a window of scan positions is polled at a time, starting narrow (the winner is nearly
             // always at the first positions), and polling stops at the first accept: posts of later CTAs are
             // never waited for, and the CTA at position 0, when it accepts, waits for nobody.
+            stamp(1);
             const u32 kb = b >= c_first ? b - c_first : b + nb - c_first;
             const u32 tail0 = CACHED ? per - t0r : CG_NONE;
             const u32 ring = e32 & (CG_SRING - 1u), e16 = e32 & 0xFFFFu;
@@ -852,6 +858,7 @@ __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 
                 }
                 if (quit) break;
             }
+            stamp(2);
             while (lo < npos) {
                 const u32 k = lo + (u32)lane;
                 const bool mine = k < hi;
@@ -893,6 +900,7 @@ __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 
                 lo = hi; hi = min(npos, lo + 32u);
             }
             if (quit) break;
+            stamp(3);
             if (q == CG_NONE) {               // no head label accepted: the lowest of the late ones (labels are distinct)
                 const u32 tmin = __reduce_min_sync(CG_FULL, tlab);
                 if (tmin != CG_NONE) {
@@ -952,6 +960,7 @@ __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 
                     p.log_a[h] = a_start + used_sum - 1; p.log_i[h] = hi_; p.log_j[h] = hj_;
                 }
             }
+            stamp(4);
         }
         if (quit) {                       // let the consumers of this CTA go (they see the abort flag in their waits)
             if (lane == 0) *(volatile u32*)&cm->abort = 1u;
@@ -966,6 +975,10 @@ __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 
             c->dP += dP; c->cur = (cur0 + ns) % CG_RING; c->epoch += e;
             c->pub_base = pub_base + ns;
             c->cyc_total += (u64)(clock64() - t_begin);
+        }
+        if (TIMED && lane == 0) {
+            for (int k = 0; k < 5; ++k) atomicAdd(&p.ctl->cyc_x[k], tx[k]);
+            atomicAdd(&p.ctl->cyc_x[5], 1ull);
         }
         __syncwarp();
         asm volatile("bar.sync 2, %0;" ::"r"(THREADS) : "memory");
@@ -1095,24 +1108,38 @@ __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 
                 if (MULTI && has_label) {
                     // slots 1 .. KX: the hop consumed last (occupations, followed energies), then the test
                     const u32 si = mhi | geo.spare, sj = mhj | geo.spare;
-                    for (u32 k = 1; k <= KX; ++k) {
+                    // the four table gathers of a followed slot are issued one slot ahead of their use
+                    // (the slots are visited in physical order: the lowest accepting label does not depend on the order)
+                    u32 n_ix = (u32)tid, n_fl = x_fl[n_ix], n_ci = x_ci[n_ix], n_cj = x_cj[n_ix];
+                    u32 k = KX + 1u - rot; if (k > KX) k -= KX;     // logical slot in physical slot 0
+                    double g0 = 0, g1 = 0, g2 = 0, g3 = 0;
+                    auto gather = [&]() {
+                        if (mh && (n_fl & 12u) == 12u) {
+                            g0 = __ldg(tf + ((n_ci - mhj) & mask)); g1 = __ldg(tf + ((n_ci - mhi) & mask));
+                            g2 = __ldg(tf + ((n_cj - mhj) & mask)); g3 = __ldg(tf + ((n_cj - mhi) & mask));
+                        }
+                    };
+                    gather();
+                    for (u32 ph = 0; ph < KX; ++ph, k = (k == KX ? 1u : k + 1u)) {
                         const u32 labk = lab + k * P;
-                        const u32 ix = xidx(k);
-                        u32 fl = x_fl[ix];
+                        const u32 ix = n_ix;
+                        u32 fl = n_fl;
+                        const u32 ci_ = n_ci, cj_ = n_cj;
+                        const double t0 = g0, t1 = g1, t2 = g2, t3 = g3;
+                        if (ph + 1u < KX) { n_ix += (u32)TW; n_fl = x_fl[n_ix]; n_ci = x_ci[n_ix]; n_cj = x_cj[n_ix]; gather(); }
                         if (!(fl & 8u)) {
                             if (labk >= M) continue;            // decoded later, when the warp is far from the front
                             x_decode(k); fl = x_fl[ix];
                         } else if (mh) {
-                            const u32 ci_ = x_ci[ix], cj_ = x_cj[ix];
                             if (fl & 4u) {
-                                x_ei[ix] = __dadd_rn(x_ei[ix], hop_term(tf, mask, ci_, mhi, mhj));
-                                x_ej[ix] = __dadd_rn(x_ej[ix], hop_term(tf, mask, cj_, mhi, mhj));
+                                x_ei[ix] = __dadd_rn(x_ei[ix], __dsub_rn(t0, t1));
+                                x_ej[ix] = __dadd_rn(x_ej[ix], __dsub_rn(t2, t3));
                             }
                             if (ci_ == si) fl &= ~1u; if (ci_ == sj) fl |= 1u;
                             if (cj_ == si) fl &= ~2u; if (cj_ == sj) fl |= 2u;
                         }
                         if (labk < M && (fl & 3u) == 1u) {     // theta_ij, inside the window
-                            const u32 ci_ = x_ci[ix], cj_ = x_cj[ix];
+                            const u32 ci_ = x_ci[ix], cj_ = x_cj[ix];     // (a slot decoded just now: not the values read ahead)
                             double vi, vj;
                             if (!(fl & 4u)) { read_eps(ci_, cj_, vi, vj); x_ei[ix] = vi; x_ej[ix] = vj; fl |= 4u; }
                             else { vi = x_ei[ix]; vj = x_ej[ix]; }
@@ -2467,6 +2494,16 @@ extern "C" int cg_get_tuning(cg_sim* s, int* snapshot_interval, int* cluster_siz
     return CG_OK;
 }
 
+extern "C" int cg_get_exchange_cycles(cg_sim* s, uint64_t* cycles6)
+{
+    if (!s || !cycles6) return CG_EINVAL;
+    CgCtl c;
+    int rc = read_ctl(s, &c);
+    if (rc != CG_OK) return rc;
+    for (int k = 0; k < 6; ++k) cycles6[k] = c.cyc_x[k];
+    return CG_OK;
+}
+
 extern "C" int cg_get_labels_per_thread(cg_sim* s, int* labels_per_thread)
 {
     if (!s || !labels_per_thread) return CG_EINVAL;
@@ -2495,6 +2532,7 @@ extern "C" int cg_get_phase_cycles(cg_sim* s, uint64_t* total, uint64_t* wait, u
     if (warps) *warps = c.cyc_warps;
     if (reset) {
         c.cyc_total = c.cyc_wait = c.cyc_update = c.cyc_propose = c.cyc_warps = 0;
+        for (int k = 0; k < 6; ++k) c.cyc_x[k] = 0;
         CK(cudaMemcpyAsync(s->d_ctl, &c, sizeof c, cudaMemcpyHostToDevice, s->stream));
         CK(cudaStreamSynchronize(s->stream));
     }

@@ -6,6 +6,8 @@
     python -m paper_1407_5026_b200.report --l2            # sweep of the L2 roofline probe (cg_bench_l2)
     python -m paper_1407_5026_b200.report --update        # step a6 alone: gather kernel against bulk-copy staged kernel
     python -m paper_1407_5026_b200.report --tuning        # snapshot interval H and cluster size at configs 3 and 5
+    python -m paper_1407_5026_b200.report --one cfg5_L512 [--hops 20000]    # one config, two launches (ncu target)
+    python -m paper_1407_5026_b200.report --l2-one        # the best L2 probe shape alone (ncu target)
 
 --configs: every workload of BASELINE.json (workloads.CONFIGS), a bounded prefix of its chain, one line each:
 accepted hops/s, window proposals evaluated/s (M per PR iteration), attempts consumed/s
@@ -267,6 +269,27 @@ def report_observables(hops):
         sys.stdout.flush()
 
 
+def report_one(name, idx, hops, warm):
+    """One config, two launches of the persistent kernel (warm-up, then `hops` hops): the target of the ncu captures
+    under profiles/ (`-k regex:cg_pr_persistent --launch-skip 1 --launch-count 1`)."""
+    sms = torch.cuda.get_device_properties(0).multi_processor_count
+    kw = workloads.init_args(workloads.CONFIGS[name][idx], sms * 2048)
+    g = binding.CoulombGlass(**kw)
+    g.run(warm)
+    torch.cuda.synchronize()
+    ms = _timed(lambda: g.run(hops))
+    c = g.counters()
+    print("%s[%d] %s: %d hops after %d warm-up hops: %.0f hops/s, %d iterations in all, launch %s, H=%d, labels/thread %d" % (
+        name, idx, kw, hops, warm, hops / ms * 1e3, c["iterations"], g.launch(), g.tuning()["snapshot_interval"],
+        g.labels_per_thread()))
+
+
+def report_l2_one():
+    """The best read-modify-write shape of the L2 probe sweep, a few launches: the target of its ncu capture."""
+    gb = binding.bench_l2(16 << 20, reps=500, trials=3, mode="rmw", ctas_per_sm=8, threads=128, vec_bytes=16)
+    print("cg_bench_l2 rmw 16 MiB, 8 CTAs/SM x 128 threads, 16-byte accesses: %.0f GB/s" % gb)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--configs", action="store_true")
@@ -275,11 +298,18 @@ def main():
     ap.add_argument("--l2", action="store_true")
     ap.add_argument("--update", action="store_true")
     ap.add_argument("--tuning", action="store_true")
+    ap.add_argument("--one", default="", help="CONFIG[:index], e.g. cfg5_L512 or cfg3_L128:3")
+    ap.add_argument("--l2-one", action="store_true")
     ap.add_argument("--hops", type=int, default=0)
     ap.add_argument("--warm", type=int, default=2000)
     a = ap.parse_args()
     if not torch.cuda.is_available():
         raise SystemExit("report needs a CUDA device: the hot path has no CPU fallback")
+    if a.one:
+        name, _, idx = a.one.partition(":")
+        report_one(name, int(idx or 0), a.hops or 20_000, a.warm)
+    if a.l2_one:
+        report_l2_one()
     if a.configs:
         report_configs(a.hops or 200_000, a.warm)
     if a.replicas:
