@@ -102,7 +102,6 @@ struct CgParams {           // kernel parameter block
     double* eps[CG_RING];   // ring of local-energy snapshot buffers, N each
     double* work;           // RP == 0 only: the CTAs' private working copy of eps
     const double* tf;       // unfolded table 1/r (see site_code)
-    const double* tf1m;     // copy of tf shifted by one entry, minus one: tf1m[o] = tf[o] too, but tf1m + o is 16-byte aligned for ODD o
     const double* tq;       // folded table 1/r, (Lz/2+1) x (L/2+1) x (L/2+1)
     u32* nbits;             // occupations, bit s of word s/32
     const u64* cdfi;        // live tower as integer thresholds: u_d < cdf_k  <=>  m < cdfi_k
@@ -314,9 +313,9 @@ __device__ __forceinline__ double hop_term(const double* __restrict__ tf, u32 ma
 }
 
 // eps slab of one CTA: sites [2 pr0, 2 pr1).  With RP > 0 warp w keeps the blocks of 64 consecutive
-// sites number w, w + TW/32, ... (RP of them) in registers across hops - lane l holds the PAIR of neighbouring
-// sites 2l, 2l + 1 of a block, so that every load and store is a double2 and a warp covers 512 contiguous
-// bytes - and writes the values through to a snapshot buffer when asked to; with RP == 0 the slab lives in the CTA's part
+// sites number w, w + TW/32, ... (RP of them) in registers across hops - lane l holds sites l and
+// 32 + l of a block, so that every load and store of the warp covers 256 contiguous bytes - and writes
+// the values through to a snapshot buffer when asked to; with RP == 0 the slab lives in the CTA's part
 // of a private working buffer in global memory (L2).
 // issue() starts the table gathers of a hop, finish() adds (and stores): the caller puts independent
 // work between the two.
@@ -330,7 +329,10 @@ struct Slab {
     u32 hci, hcj;
     u32 tix;                             // index of this thread among the TW threads that hold the slab
 
-    __device__ __forceinline__ u32 site_a(u32 pr0, int k) const { return 2u * (pr0 + (u32)k * TW + tix); }
+    __device__ __forceinline__ u32 site_a(u32 pr0, int k) const
+    {
+        return 2u * (pr0 + (u32)k * TW + (tix & ~31u)) + (tix & 31u);
+    }
 
     __device__ __forceinline__ void load(const double* src, double* work, u32 pr0, u32 pr1, const Geo& g, u32 t)
     {
@@ -338,31 +340,26 @@ struct Slab {
         if (RP > 0) {
 #pragma unroll
             for (int k = 0; k < RP; ++k) {
-                const u32 sa = site_a(pr0, k);
-                const bool va = sa < 2u * pr1;          // a pair of neighbouring sites (x even, x + 1) is valid as a whole
-                valid |= (va ? 3u : 0u) << (2 * k);
+                const u32 sa = site_a(pr0, k), sb = sa + 32u;
+                const bool va = sa < 2u * pr1, vb = sb < 2u * pr1;
+                valid |= (va ? 1u : 0u) << (2 * k) | (vb ? 1u : 0u) << (2 * k + 1);
                 sca[k] = va ? g.code(sa) | g.spare : g.spare;
-                scb[k] = sca[k] + 1u;
-                const double2 v = va ? __ldcg(reinterpret_cast<const double2*>(src + sa)) : make_double2(0.0, 0.0);
-                ea[k] = v.x; eb[k] = v.y;
+                scb[k] = vb ? g.code(sb) | g.spare : g.spare;
+                ea[k] = va ? __ldcg(src + sa) : 0.0;
+                eb[k] = vb ? __ldcg(src + sb) : 0.0;
             }
         } else if (work != src) {
             for (u32 s = 2u * pr0 + tix; s < 2u * pr1; s += TW) __stcg(work + s, __ldcg(src + s));
         }
     }
 
-    // The two sites of a pair are neighbours along x, so their table entries are adjacent (rows are extended
-    // periodically): ONE 16-byte load per pair and hop end - from tf when the offset is even, from the copy shifted by
-    // one entry when it is odd (north_star item 6: double2 loads and stores).
-    __device__ __forceinline__ void issue(const double* __restrict__ tf, const double* __restrict__ tf1m, u32 mask, u32 ci, u32 cj)
+    __device__ __forceinline__ void issue(const double* __restrict__ tf, u32 mask, u32 ci, u32 cj)
     {
         hci = ci; hcj = cj;
 #pragma unroll
         for (int k = 0; k < RP; ++k) {
-            const u32 oj = (sca[k] - cj) & mask, oi = (sca[k] - ci) & mask;
-            const double2 vj = __ldg(reinterpret_cast<const double2*>(((oj & 1u) ? tf1m : tf) + oj));
-            const double2 vi = __ldg(reinterpret_cast<const double2*>(((oi & 1u) ? tf1m : tf) + oi));
-            ja[k] = vj.x; jb[k] = vj.y; ia[k] = vi.x; ib[k] = vi.y;
+            ja[k] = __ldg(tf + ((sca[k] - cj) & mask)); ia[k] = __ldg(tf + ((sca[k] - ci) & mask));
+            jb[k] = __ldg(tf + ((scb[k] - cj) & mask)); ib[k] = __ldg(tf + ((scb[k] - ci) & mask));
         }
     }
 
@@ -395,7 +392,8 @@ struct Slab {
 #pragma unroll
             for (int k = 0; k < RP; ++k) {
                 const u32 sa = site_a(pr0, k);
-                if ((valid >> (2 * k)) & 1u) __stcg(reinterpret_cast<double2*>(snap + sa), make_double2(ea[k], eb[k]));
+                if ((valid >> (2 * k)) & 1u) __stcg(snap + sa, ea[k]);
+                if ((valid >> (2 * k + 1)) & 1u) __stcg(snap + sa + 32u, eb[k]);
             }
         } else {
             for (u32 s = 2u * pr0 + tix; s < 2u * pr1; s += TW) __stcg(snap + s, __ldcg(work + s));
@@ -1202,7 +1200,7 @@ __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 
                 }
                 inflight = false;
             }
-            if (upd) { slab.issue(tf, p.tf1m, mask, hz, hw); hs = hl; inflight = true; upd = false; }
+            if (upd) { slab.issue(tf, mask, hz, hw); hs = hl; inflight = true; upd = false; }
             long long t2 = 0;
             if (TIMED) { t2 = clock64(); t_slab += (u64)(t2 - t1); }
             if (last) break;
@@ -1334,7 +1332,7 @@ cg_update_scripted(const CgParams p, const u32* __restrict__ hop_i, const u32* _
     Slab<THREADS, RP> slab;
     slab.load(e, e, pr0, pr1, geo, threadIdx.x);
     for (u64 h = 0; h < count; ++h) {
-        slab.issue(p.tf, p.tf1m, p.mask, geo.code(__ldg(hop_i + h)), geo.code(__ldg(hop_j + h)));
+        slab.issue(p.tf, p.mask, geo.code(__ldg(hop_i + h)), geo.code(__ldg(hop_j + h)));
         slab.finish(p.tf, p.mask, geo, e, e, pr0, pr1);
     }
     if (b == 0 && threadIdx.x == 0) {       // occupations and dipole moment, in hop order
@@ -1436,17 +1434,12 @@ __global__ void cg_build_tf(const double* __restrict__ tq, double* __restrict__ 
 {
     for (u32 idx = blockIdx.x * blockDim.x + threadIdx.x; idx < total; idx += gridDim.x * blockDim.x) {
         const int dx = idx & (2 * L - 1), dy = (idx >> (lg + 1)) & (2 * L - 1), dz = idx >> (2 * lg + 2);
-        // entries L .. 2L-1 of a row repeat entries 0 .. L-1: the x offsets d, d+1 of two neighbouring sites are then
-        // adjacent entries also when d+1 wraps around (d = L-1), so that one 16-byte load fetches both
-        const int px = dx & (L - 1);
         double v = 0.0;
-        if (dy < L && dz < Lz) {
-            const int fx = min(px, L - px), fy = min(dy, L - dy), fz = min(dz, Lz - dz);
+        if (dx < L && dy < L && dz < Lz) {
+            const int fx = min(dx, L - dx), fy = min(dy, L - dy), fz = min(dz, Lz - dz);
             v = tq[((size_t)fz * pitch + fy) * pitch + fx];
         }
         tf[idx] = v;
-        if (idx) tf[(size_t)total + idx - 1] = v;     // the copy shifted by one entry: tf1[i] = tf[i + 1]
-        if (idx == total - 1) tf[(size_t)total + idx] = 0.0;
     }
 }
 
@@ -1632,7 +1625,7 @@ static WsLayout ws_layout(int dim, int L)
     w.phi = o; o += align256(8 * N);
     w.nbits = o; o += align256(N / 8 + 4);
     w.tq = o; o += align256(8 * hz * h * h);
-    w.tf = o; o += align256(8 * 2 * tf_len);            // the table and its copy shifted by one entry
+    w.tf = o; o += align256(8 * tf_len);
     w.cdfi = o; o += align256(8 * kcap);
     w.invr_k = o; o += align256(8 * kcap);
     w.fld_k = o; o += align256(8 * kcap);
@@ -1764,7 +1757,7 @@ static CgParams make_params(const cg_sim* s, u32 n_hops)
     CgParams p;
     for (int k = 0; k < CG_RING; ++k) p.eps[k] = s->d_eps[k];
     p.work = s->d_work;
-    p.tf = s->d_tf; p.tf1m = s->d_tf + s->tf_len - 1; p.tq = s->d_tq; p.nbits = s->d_nbits;
+    p.tf = s->d_tf; p.tq = s->d_tq; p.nbits = s->d_nbits;
     p.cdfi = s->d_cdfi; p.invr_k = s->d_invr_k; p.fld_k = s->d_fld_k; p.disp = s->d_disp;
     p.guide = s->d_guide;
     p.slots = s->d_slots; p.ctl = s->d_ctl;
