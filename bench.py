@@ -346,12 +346,15 @@ def run_ours(args):
         it0 = warm.counters()["iterations"]
         warm.run(20000)
         pc = warm.phase_cycles()
+        xc = warm.exchange_cycles()
         warm.set_phase_timers(False)
         n_it = warm.counters()["iterations"] - it0
         w = max(pc["warps"], 1)
         out["in_loop_cycles_per_iteration"] = {
             "total": pc["total"] / n_it, "propose": pc["propose"] / w / n_it, "update_W_U": pc["update"] / w / n_it,
-            "wait": pc["wait"] / w / n_it, "what": "CTA 0, mean over its worker warps; timed build of the same kernel, 20000 hops"}
+            "wait": pc["wait"] / w / n_it, "what": "CTA 0, mean over its worker warps; timed build of the same kernel, 20000 hops",
+            "exchange_warp": {k: xc[k] / max(xc["warps"], 1) / n_it for k in ("recycle", "gate", "own_workers", "scan", "publish")},
+            "exchange_warp_what": "mean over the exchange warps of all CTAs (cg_get_exchange_cycles)"}
     # the update kernel alone on scripted hops (forward log + its reversal = back to the start state)
     warm_kw = reps[0]["warm_kw"]
     u = pkg.CoulombGlass(device=devices[0], hop_log=2000, **warm_kw)

@@ -96,21 +96,27 @@ def report_configs(hops, warm):
             ln = g.launch()
             # the paper's split, from the timed build of the same kernel on the next `chunk` hops
             split = ""
-            if ln["threads"] == 544:
+            if ln["threads"] == 544 and g.labels_per_thread() <= 1:
                 g.set_phase_timers(True)
                 g.phase_cycles(reset=True)
                 it0 = g.counters()["iterations"]
                 g.run(chunk)
                 pc = g.phase_cycles()
+                xc = g.exchange_cycles()
                 g.set_phase_timers(False)
                 n_it = g.counters()["iterations"] - it0
                 w = max(pc["warps"], 1)
-                split = "  in-loop cycles/iteration: total %.0f = propose %.0f + update %.0f + wait %.0f" % (
-                    pc["total"] / n_it, pc["propose"] / w / n_it, pc["update"] / w / n_it, pc["wait"] / w / n_it)
-            print("%-9s T=%-5g M=%-6d %3d CTAs x %d: %7.0f hops/s  %.2e proposals/s  %.2e attempts/s  "
+                xw = max(xc["warps"], 1)
+                split = ("  in-loop cycles/iteration: total %.0f = propose %.0f + update %.0f + wait %.0f; exchange warps (mean of "
+                         "%d CTAs): recycle %.0f gate %.0f own workers %.0f scan %.0f publish %.0f" % (
+                             pc["total"] / n_it, pc["propose"] / w / n_it, pc["update"] / w / n_it, pc["wait"] / w / n_it, xw,
+                             xc["recycle"] / xw / n_it, xc["gate"] / xw / n_it, xc["own_workers"] / xw / n_it,
+                             xc["scan"] / xw / n_it, xc["publish"] / xw / n_it))
+            print("%-9s T=%-5g M=%-6d %3d CTAs x %d, H=%d, %d label(s)/thread: %7.0f hops/s  %.2e proposals/s  %.2e attempts/s  "
                   "p=%.3f q=%8.1f  A=%.2e (last 10%%: %.2e)  %5.3f us/hop%s  "
                   "update alone %.3f us/hop = %6.0f GB/s  drift %.1e" % (
-                      name, kw["T"], M, ln["n_ctas"], ln["threads"], Hd / ms * 1e3, M * it / ms * 1e3,
+                      name, kw["T"], M, ln["n_ctas"], ln["threads"], g.tuning()["snapshot_interval"], g.labels_per_thread(),
+                      Hd / ms * 1e3, M * it / ms * 1e3,
                       at / ms * 1e3, it / Hd, mean_q, A_all, A_last, us_hop, split, w_u,
                       16.0 * N / w_u / 1e3, g.recompute_eps()))
             sys.stdout.flush()
@@ -228,7 +234,7 @@ def report_replicas(hops):
     packed("cfg3_L128", [0, 1, 2, 3], 2, n_ctas=sms // 8)
     packed("cfg1_L16", [0], 32)
     packed("cfg1_L16", [0], sms)
-    packed("cfg2_L64", [0], sms // 5)
+    packed("cfg2_L64", [0], sms // 5, n_ctas=5)
     run("cfg3_L128", [0, 1, 2, 3], 1)     # the temperature sweep of config 3 as one replica set
     run("cfg3_L128", [0, 1, 2, 3], 2)
     run("cfg1_L16", [0], 1)
