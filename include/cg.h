@@ -217,7 +217,7 @@ int cg_get_launch(cg_sim* s, int* n_ctas, int* threads, int* smem_bytes);
  * every H hops (deferred update; PAPER.md:77, 106 W_U); cluster_size in {1, 2, 4, 8, 16}:
  * CTAs per thread-block cluster, whose members post their results into each other's
  * shared memory instead of through L2; -1 = automatic (the default: clusters of up to 16
- * when the whole sim fits 96 CTAs, none when it wants every SM - clusters of 8 and 16 leave
+ * when the whole sim fits 96 CTAs, pairs when it wants every SM - clusters of 8 and 16 leave
  * SMs of a B200 unused).  0 leaves a value as it is.  A new cluster size re-derives the
  * launch shape (CG_EUNSUPPORTED if the device cannot co-schedule it).  cg_set_launch with an
  * explicit CTA count keeps the largest cluster size that divides it; cg_get_tuning reports

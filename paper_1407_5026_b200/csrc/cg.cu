@@ -1957,7 +1957,7 @@ static int choose_launch_cs(cg_sim* s, int n_ctas, int threads)
 // Launch shape for (n_ctas, threads), 0 = heuristic, with the cluster size of cg_set_tuning.  Automatic cluster size
 // (measured): CTAs of one cluster post through shared memory instead of L2, worth 6-8 % when the whole sim
 // sits in one or a few clusters; on B200 clusters of 8 and 16 leave 28 and 36 of the 148 SMs unused, so a sim that
-// wants every SM runs without.  An explicit CTA count keeps the largest cluster size that divides it.
+// wants every SM runs in pairs (+2 % at config 5, +15 % at config 4 with M = 65536).  An explicit CTA count keeps the largest cluster size that divides it.
 static int choose_launch(cg_sim* s, int n_ctas, int threads)
 {
     const int old = s->cluster;
@@ -1966,9 +1966,12 @@ static int choose_launch(cg_sim* s, int n_ctas, int threads)
         s->cluster = 1;
         int rc = choose_launch_cs(s, n_ctas, threads);
         if (rc != CG_OK) { s->cluster = old; return rc; }
-        if (s->n_ctas < 2 || s->n_ctas > 96) return CG_OK;
-        cs = 16;
-        if (n_ctas == 0) while (cs > 1 && cs / 2 >= s->n_ctas) cs /= 2;     // 5 CTAs -> one cluster of 8
+        if (s->n_ctas < 2) return CG_OK;
+        if (s->n_ctas > 96) cs = 2;       // pairs pack the 148 SMs exactly: half of the changes of decider stay inside a cluster
+        else {
+            cs = 16;
+            if (n_ctas == 0) while (cs > 1 && cs / 2 >= s->n_ctas) cs /= 2;     // 5 CTAs -> one cluster of 8
+        }
     }
     if (n_ctas) while (cs > 1 && n_ctas % cs) cs /= 2;
     for (; cs >= 1; cs /= 2) {
