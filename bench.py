@@ -227,6 +227,9 @@ def run_ours(args):
             warm=pkg.CoulombGlass(device=dev, **warm_kw),     # warm-up replica: same shape, other seed
             g=pkg.CoulombGlass(device=dev, **kw),             # the timed workload starts at hop 0
             flush=torch.zeros(512 << 20, dtype=torch.uint8, device="cuda:%d" % dev)))   # > 126 MB L2
+        if args.cluster:
+            reps[-1]["warm"].set_tuning(0, args.cluster)
+            reps[-1]["g"].set_tuning(0, args.cluster)
         if args.ctas or args.threads:
             reps[-1]["warm"].set_launch(args.ctas, args.threads)
             reps[-1]["g"].set_launch(args.ctas, args.threads)
@@ -395,6 +398,8 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--ctas", type=int, default=0)
     ap.add_argument("--threads", type=int, default=0)
+    ap.add_argument("--cluster", type=int, default=0,
+                    help="thread-block cluster size (0: automatic; 1 for runs under ncu, which cannot replay cooperative cluster launches)")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)

@@ -275,19 +275,21 @@ def report_observables(hops):
         sys.stdout.flush()
 
 
-def report_one(name, idx, hops, warm):
+def report_one(name, idx, hops, warm, cluster=0):
     """One config, two launches of the persistent kernel (warm-up, then `hops` hops): the target of the ncu captures
     under profiles/ (`-k regex:cg_pr_persistent --launch-skip 1 --launch-count 1`)."""
     sms = torch.cuda.get_device_properties(0).multi_processor_count
     kw = workloads.init_args(workloads.CONFIGS[name][idx], sms * 2048)
     g = binding.CoulombGlass(**kw)
+    if cluster:
+        g.set_tuning(0, cluster)          # ncu cannot replay cooperative launches with a cluster dimension: --cluster 1 there
     g.run(warm)
     torch.cuda.synchronize()
     ms = _timed(lambda: g.run(hops))
     c = g.counters()
     print("%s[%d] %s: %d hops after %d warm-up hops: %.0f hops/s, %d iterations in all, launch %s, H=%d, labels/thread %d" % (
         name, idx, kw, hops, warm, hops / ms * 1e3, c["iterations"], g.launch(), g.tuning()["snapshot_interval"],
-        g.labels_per_thread()))
+        g.labels_per_thread()) + ", cluster %d" % g.tuning()["cluster_size"])
 
 
 def report_l2_one():
@@ -306,6 +308,7 @@ def main():
     ap.add_argument("--tuning", action="store_true")
     ap.add_argument("--one", default="", help="CONFIG[:index], e.g. cfg5_L512 or cfg3_L128:3")
     ap.add_argument("--l2-one", action="store_true")
+    ap.add_argument("--cluster", type=int, default=0, help="cluster size for --one (0: automatic)")
     ap.add_argument("--hops", type=int, default=0)
     ap.add_argument("--warm", type=int, default=2000)
     a = ap.parse_args()
@@ -313,7 +316,7 @@ def main():
         raise SystemExit("report needs a CUDA device: the hot path has no CPU fallback")
     if a.one:
         name, _, idx = a.one.partition(":")
-        report_one(name, int(idx or 0), a.hops or 20_000, a.warm)
+        report_one(name, int(idx or 0), a.hops or 20_000, a.warm, a.cluster)
     if a.l2_one:
         report_l2_one()
     if a.configs:
