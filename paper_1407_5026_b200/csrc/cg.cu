@@ -1319,6 +1319,122 @@ cg_pr_persistent_many(const CgParams* __restrict__ ps, const u32* __restrict__ f
     pr_persistent_body<NW, RP, CACHED, false>(sp, s_b, s_nb);
 }
 
+// ---- a sim that fits ONE CTA: everything in shared memory, two CTA barriers per iteration ------------------------
+// Small lattices (the paper recommends averaging many samples) have no exchange between CTAs to hide, so
+// the dataflow between role warps above only costs them hand-overs.  Here all CG_ST threads are workers.  Thread t owns
+// the attempts a = t (mod CG_ST) and keeps its proposal decoded; eps and the occupation bitmap live in shared memory,
+// so a test (steps 1-2) reads eps_i, eps_j and n_i, n_j afresh (no followed energies, no pending
+// terms), the lowest accepting label (step 3) is ONE 64-bit shared-memory atomicMin of (label, thread), and after the
+// barrier every thread adds the hop's term to its sites of eps (step 3b: the same single rounded add per
+// site and hop as everywhere else).  Second barrier, next iteration.
+#define CG_ST 512           // threads (= labels held) of the single-CTA kernel
+#define CG_SINGLE_MAX_N 8192u   // eps in shared memory: 64 KiB
+__device__ __forceinline__ void pr_single_body(const CgParams& p)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int KS = p.Ksm;
+    u64* s_cdfi = reinterpret_cast<u64*>(smem_raw);
+    double* s_invr = reinterpret_cast<double*>(s_cdfi + KS);
+    double* s_fld = s_invr + KS;
+    double* s_eps = s_fld + KS;
+    u32* s_disp = reinterpret_cast<u32*>(s_eps + p.N);
+    u32* s_guide = s_disp + KS;
+    u32* s_n = s_guide + CG_GUIDE;
+    __shared__ u64 s_key[3];               // (label << 32 | thread) of the lowest accept of iterations e, e+1, e+2 (mod 3)
+    __shared__ u32 s_sites[2][CG_ST][2];   // coded sites of every thread's proposal, by iteration parity
+    const Tables tb = {s_cdfi, s_invr, s_fld, s_disp, s_guide, p.cdfi, p.invr_k, p.fld_k, p.disp, (u32)KS};
+    const Geo geo = {p.hi1, p.hi2, p.spare, p.mask, (u32)(p.L - 1), p.lgL};
+    const int tid = threadIdx.x, lane = tid & 31;
+    const u32 N = p.N, M = p.M, mask = p.mask, P = CG_ST;
+    const double* __restrict__ tf = p.tf;
+    CgCtl* const ctl = p.ctl;
+    double* const g_eps = p.eps[ctl->cur];
+
+    for (int k = tid; k < KS; k += CG_ST) {
+        s_cdfi[k] = p.cdfi[k]; s_invr[k] = p.invr_k[k]; s_fld[k] = p.fld_k[k]; s_disp[k] = p.disp[k];
+    }
+    for (int k = tid; k < CG_GUIDE; k += CG_ST) s_guide[k] = p.guide[k];
+    for (u32 w = tid; w < (N + 31) / 32; w += CG_ST) s_n[w] = p.nbits[w];
+    for (u32 k = tid; k < N; k += CG_ST) s_eps[k] = __ldcg(g_eps + k);
+    if (tid < 3) s_key[tid] = ~0ull;
+    const u64 a_start = ctl->attempts, hops_start = ctl->hops, log_base = ctl->log_base;
+    const u32 n_hops = p.n_hops;
+    __syncthreads();
+
+    // my attempt and the one after it (a proposal is a pure function of seed and attempt index)
+    const u32 g0 = (u32)(a_start % P);
+    u32 lab = (u32)tid >= g0 ? (u32)tid - g0 : (u32)tid + P - g0;
+    u64 a_cur = a_start + lab;
+    Prop cur = decode_attempt(tb, p, geo, a_cur), nxt = decode_attempt(tb, p, geo, a_cur + P);
+    double c_invr = tb.inv(cur.k), c_fld = tb.field(cur.k);
+    u32 hc = 0, e = 0;
+    u64 used_sum = 0;
+    long long dP = 0;
+    while (hc < n_hops) {
+        // ---- steps 1-2: test my proposal on the current state
+        sts64u(&s_sites[e & 1u][tid][0], cur.ci, cur.cj);
+        u32 best = CG_NONE;
+        if (lab < M) {
+            const u32 si = geo.site(cur.ci), sj = geo.site(cur.cj);
+            if (BIT(s_n, si) && !BIT(s_n, sj)) {                          // theta_ij
+                // dH_ij = eps_j - eps_i - 1/r_ij - E dx_ij
+                const double dE = __dsub_rn(__dsub_rn(__dsub_rn(s_eps[sj], s_eps[si]), c_invr), c_fld);
+                if (metropolis(dE, cur.uh, cur.ul, p.T, p.inv_T)) best = lab;
+            }
+        }
+        // ---- step 3: the lowest accepting label; labels are distinct
+        const u32 wmin = __reduce_min_sync(CG_FULL, best);
+        if (best != CG_NONE && best == wmin) atomicMin(&s_key[e % 3u], ((u64)best << 32) | (u64)tid);
+        if (tid == 0) s_key[(e + 1u) % 3u] = ~0ull;                        // last read before the previous barrier pair
+        __syncthreads();
+        const u64 key = s_key[e % 3u];
+        const bool hop = key != ~0ull;
+        const u32 used = hop ? (u32)(key >> 32) + 1u : M;                 // m = (p-1) M + q
+        if (hop) {
+            const uint2 w = lds64u(&s_sites[e & 1u][(u32)key][0]);        // coded sites of the executed hop
+            // step 3b: eps_l += 1/r_lj - 1/r_li, difference first, then ONE add
+            for (u32 l = tid; l < N; l += CG_ST)
+                s_eps[l] = __dadd_rn(s_eps[l], hop_term(tf, mask, geo.code(l) | geo.spare, w.x, w.y));
+            ++hc;
+            if (tid == 0) {                                                // step 3a, dP, hop log
+                const u32 hi_ = geo.site(w.x), hj_ = geo.site(w.y);
+                s_n[hi_ >> 5] &= ~(1u << (hi_ & 31));
+                s_n[hj_ >> 5] |= 1u << (hj_ & 31);
+                dP += geo.dx(hi_, hj_);
+                const u64 h = hops_start + hc - 1u - log_base;
+                if (h < p.log_cap) { p.log_a[h] = a_start + used_sum + used - 1; p.log_i[h] = hi_; p.log_j[h] = hj_; }
+            }
+        }
+        used_sum += used;
+        ++e;
+        if (lab >= used) lab -= used;
+        else {                                                             // consumed: my next attempt, P attempts later
+            lab += P - used; a_cur += P;
+            cur = nxt; c_invr = tb.inv(cur.k); c_fld = tb.field(cur.k);
+            nxt = decode_attempt(tb, p, geo, a_cur + P);
+        }
+        __syncthreads();
+    }
+    for (u32 k = tid; k < N; k += CG_ST) __stcg(g_eps + k, s_eps[k]);
+    for (u32 w = tid; w < (N + 31) / 32; w += CG_ST) p.nbits[w] = s_n[w];
+    if (tid == 0) {
+        ctl->attempts = a_start + used_sum; ctl->hops = hops_start + hc;
+        ctl->iterations += e; ctl->proposals += (u64)M * e;
+        ctl->dP += dP; ctl->epoch += e;
+    }
+}
+
+__global__ void __launch_bounds__(CG_ST, 1) cg_pr_single(const CgParams p) { pr_single_body(p); }
+
+// many single-CTA sims in one launch: CTA s runs sim s
+__global__ void __launch_bounds__(CG_ST, 1) cg_pr_single_many(const CgParams* __restrict__ ps)
+{
+    __shared__ CgParams sp;
+    if (threadIdx.x == 0) sp = ps[blockIdx.x];
+    __syncthreads();
+    pr_single_body(sp);
+}
+
 __device__ __forceinline__ Geo make_geo(const CgParams& p)
 {
     const Geo g = {p.hi1, p.hi2, p.spare, p.mask, (u32)(p.L - 1), p.lgL};
@@ -1580,6 +1696,7 @@ struct cg_sim {
     // launch shape and tuning
     int num_sms = 0, n_ctas = 0, threads = 0, smem = 0, rp = 0, pl = 0;   // pl > 0: cached proposals
     int lpt = 1;                          // cached labels per thread (> 1: the MULTI kernel, M > n_ctas * pl)
+    bool single = false;                  // the single-CTA kernel (cg_pr_single): 1 CTA x CG_ST threads, state in shared memory
     int snap_shift = 3;                   // snapshots every 1 << snap_shift hops
     bool snap_auto = true;                // not set by cg_set_tuning: chosen from the lattice size at init
     int cluster = 1;                      // CTAs per thread-block cluster in use
@@ -1958,8 +2075,29 @@ static int choose_launch_cs(cg_sim* s, int n_ctas, int threads)
 // (measured): CTAs of one cluster post through shared memory instead of L2, worth 6-8 % when the whole sim
 // sits in one or a few clusters; on B200 clusters of 8 and 16 leave 28 and 36 of the 148 SMs unused, so a sim that
 // wants every SM runs in pairs (+2 % at config 5, +15 % at config 4 with M = 65536).  An explicit CTA count keeps the largest cluster size that divides it.
+// shared memory of the single-CTA kernel: tower head, guide, bitmap and eps
+static size_t smem_single_bytes(const cg_sim* s) { return smem_base_bytes(s) + 8 * (size_t)s->N + 16; }
+
 static int choose_launch(cg_sim* s, int n_ctas, int threads)
 {
+    // A sim whose labels and sites fit one CTA runs in the single-CTA kernel (everything in shared memory): chosen
+    // automatically, or asked for as (1 CTA, CG_ST threads); any other explicit shape keeps the dataflow kernel.
+    {
+        const bool fits = s->M <= CG_ST && s->N <= CG_SINGLE_MAX_N
+                          && smem_single_bytes(s) + 12 * 1024 <= (size_t)s->smem_optin;
+        const bool asked = threads == CG_ST && n_ctas <= 1;
+        const bool automatic = threads == 0 && n_ctas == 0 && s->cluster_pref == 0 && std::max<u64>(s->M, s->N / 2) <= CG_ST;
+        if (asked && !fits) return CG_EINVAL;
+        if (fits && (asked || automatic)) {
+            const int smem = (int)smem_single_bytes(s);
+            CK(cudaFuncSetAttribute((const void*)cg_pr_single, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+            CK(cudaFuncSetAttribute((const void*)cg_pr_single_many, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+            s->single = true; s->n_ctas = 1; s->threads = CG_ST; s->rp = 0; s->pl = CG_ST; s->lpt = 1; s->smem = smem;
+            s->cluster = 1;
+            return CG_OK;
+        }
+        s->single = false;
+    }
     const int old = s->cluster;
     int cs = s->cluster_pref;
     if (cs == 0) {
@@ -2139,6 +2277,16 @@ static cudaError_t launch_coop(const void* f, int grid, int threads, int smem, c
 extern "C" int cg_run(cg_sim* s, uint64_t n_hops)
 {
     if (!s) return CG_EINVAL;
+    if (s->single) {
+        while (n_hops) {
+            const u32 chunk = (u32)std::min<uint64_t>(n_hops, CG_MAX_LAUNCH_HOPS);
+            const CgParams p = make_params(s, chunk);
+            cg_pr_single<<<1, CG_ST, (size_t)s->smem, s->stream>>>(p);
+            CK(cudaGetLastError());
+            n_hops -= chunk;
+        }
+        return CG_OK;
+    }
     persist_fn f = persistent_kernel(s->threads, s->rp, s->pl > 0, s->timers && s->threads == 544 && s->lpt == 1, s->lpt > 1);
     if (!f) return CG_EINVAL;
     while (n_hops) {
@@ -2173,15 +2321,20 @@ extern "C" int cg_run_many(cg_sim* const* sims, int n_sims, uint64_t n_hops)
         first[(size_t)k + 1] = first[(size_t)k] + (u32)s->n_ctas;
         smem = std::max(smem, s->smem);
     }
-    many_fn f = many_kernel(s0->threads, s0->rp, s0->pl > 0 && s0->lpt == 1);     // several labels per thread: recomputed here
-    if (!f) { s0->err = "cg_run_many: only 544-thread launch shapes"; return CG_EUNSUPPORTED; }
-    CK0(s0, cudaFuncSetAttribute((const void*)f, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-    int per_sm = 0;
-    CK0(s0, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, (const void*)f, s0->threads, smem));
+    const bool single = s0->single;       // threads == CG_ST everywhere: single-CTA sims, which need not be co-resident
+    many_fn f = single ? nullptr : many_kernel(s0->threads, s0->rp, s0->pl > 0 && s0->lpt == 1);     // several labels per thread: recomputed here
+    if (!single && !f) { s0->err = "cg_run_many: only 544-thread launch shapes"; return CG_EUNSUPPORTED; }
     const u32 total = first[(size_t)n_sims];
-    if (total > (u32)(per_sm * s0->num_sms)) {     // every CTA of every sim must be resident: they wait for each other
-        s0->err = "cg_run_many: the sims' CTAs do not fit on the device together";
-        return CG_EUNSUPPORTED;
+    if (single) {
+        CK0(s0, cudaFuncSetAttribute((const void*)cg_pr_single_many, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+    } else {
+        CK0(s0, cudaFuncSetAttribute((const void*)f, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+        int per_sm = 0;
+        CK0(s0, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, (const void*)f, s0->threads, smem));
+        if (total > (u32)(per_sm * s0->num_sms)) {     // every CTA of every sim must be resident: they wait for each other
+            s0->err = "cg_run_many: the sims' CTAs do not fit on the device together";
+            return CG_EUNSUPPORTED;
+        }
     }
     const size_t need = ps.size() * sizeof(CgParams) + first.size() * sizeof(u32);
     if (s0->many_cap < need) {
@@ -2202,6 +2355,10 @@ extern "C" int cg_run_many(cg_sim* const* sims, int n_sims, uint64_t n_hops)
         CK0(s0, cudaMemcpyAsync(d_first, first.data(), first.size() * sizeof(u32), cudaMemcpyHostToDevice, s0->stream));
         u32 n = (u32)n_sims;
         void* args[] = {&d_ps, &d_first, &n};
+        if (single) {
+            cg_pr_single_many<<<(unsigned)n_sims, CG_ST, (size_t)smem, s0->stream>>>(d_ps);
+            CK0(s0, cudaGetLastError());
+        } else
         CK0(s0, launch_coop((const void*)f, (int)total, s0->threads, smem, s0->stream, 1, args));
         n_hops -= chunk;
     }

@@ -241,6 +241,52 @@ def test_several_cached_labels_per_thread(cg, oracle_lib, kw, n_ctas, K, hops):
     assert g.recompute_eps() < 1e-9
 
 
+@pytest.mark.parametrize("kw,explicit,hops", [
+    (dict(L=16, T=0.1, E=0.0, seed=1, M=256), False, 30000),             # config 1: chosen automatically
+    (dict(L=4, T=0.5, E=0.0, seed=3, M=12), False, 5000),
+    (dict(L=16, T=0.01, E=0.0, seed=6, M=512), False, 300),              # cold: whole windows rejected
+    (dict(L=8, T=5.0, E=0.3, seed=4, M=5), False, 20000),                # hot: q = 0 mostly
+    (dict(L=32, T=0.08, E=0.01, seed=5, M=500), False, 6000),            # N/2 = 512 sites per thread pair, ragged M
+    (dict(L=64, T=0.05, E=0.01, seed=2, M=512), True, 6000),             # 8 sites per thread, asked for
+    (dict(L=8, dim=3, T=0.05, E=0.01, seed=13, M=384), False, 6000),     # cubic lattice
+    (dict(L=16, dim=3, T=0.1, E=-0.02, seed=14, M=100), True, 4000),
+])
+def test_single_cta_kernel(cg, oracle_lib, kw, explicit, hops):
+    """A sim whose labels and sites fit one CTA runs in cg_pr_single (512 threads, eps and occupations in shared
+    memory, two CTA barriers per iteration); the chain must be the serial one, also across launches."""
+    g = cg.CoulombGlass(hop_log=hops, **kw)
+    if explicit:
+        g.set_launch(1, 512)
+    assert g.launch()["n_ctas"] == 1 and g.launch()["threads"] == 512 and g.labels_per_thread() == 1
+    g.run(hops // 3)
+    g.run(hops - hops // 3)
+    o = oracle_lib.Oracle(**kw)
+    o.run(hops)
+    _compare(g, o, hops)
+    assert g.recompute_eps() < 1e-9
+    # the same chain goes on in the dataflow kernel and back
+    g.set_launch(1, 544)
+    g2 = cg.CoulombGlass(hop_log=hops + 600, **kw)
+    g2.set_launch(3 if kw["L"] >= 8 else 1, 544)
+    g2.run(hops)
+    g2.set_launch(1, 512)
+    g2.run(300)
+    g2.set_launch(2 if kw["L"] >= 8 else 1, 544)
+    g2.run(300)
+    o.run(600)
+    _compare(g2, o, hops + 600)
+
+
+def test_single_cta_kernel_refuses_what_does_not_fit(cg):
+    g = cg.CoulombGlass(L=16, T=0.1, M=4096)
+    assert g.launch()["threads"] == 544                # M beyond 512 labels: the dataflow kernel
+    with pytest.raises(cg.CgError):
+        g.set_launch(1, 512)
+    g = cg.CoulombGlass(L=128, T=0.1, M=256)
+    with pytest.raises(cg.CgError):
+        g.set_launch(1, 512)                           # eps does not fit shared memory
+
+
 def test_config4_M_sweep_is_one_trajectory(cg):
     """Config 4 of BASELINE.json (L=256, T=0.02): the hop log must be the same for every M (reading G8),
     including M = resident threads of the chip; only iterations and proposals differ."""
