@@ -435,15 +435,28 @@ __device__ __forceinline__ u32 tower_search(const Tables& t, u64 m)
 
 // Attempt a -> proposal (reading G9): one Philox block, i = (w0 N) >> 32,
 // displacement from 43 bits, acceptance uniform from the remaining 53.
-__device__ __forceinline__ Prop decode_attempt(const Tables& t, const CgParams& p, const Geo& g, u64 a)
+// in two halves, for callers that spread the work: the random words (Philox), then the tower search
+__device__ __forceinline__ Prop decode_words(const CgParams& p, const Geo& g, u64 a, u64& m)
 {
     u32 w0, w1, w2, w3;
     philox4x32_10((u32)a, (u32)(a >> 32), 0u, 0u, p.seed_lo, p.seed_hi, w0, w1, w2, w3);
     Prop r;
     r.ci = g.code(__umulhi(w0, p.N));
-    r.k = tower_search(t, ((u64)w1 << 11) | (u64)(w2 >> 21));
-    r.cj = (r.ci + t.dcode(r.k)) & g.mask;
+    m = ((u64)w1 << 11) | (u64)(w2 >> 21);
+    r.k = 0; r.cj = 0;
     r.uh = w2 & 0x1FFFFFu; r.ul = w3;
+    return r;
+}
+__device__ __forceinline__ void decode_finish(const Tables& t, const Geo& g, Prop& r, u64 m)
+{
+    r.k = tower_search(t, m);
+    r.cj = (r.ci + t.dcode(r.k)) & g.mask;
+}
+__device__ __forceinline__ Prop decode_attempt(const Tables& t, const CgParams& p, const Geo& g, u64 a)
+{
+    u64 m;
+    Prop r = decode_words(p, g, a, m);
+    decode_finish(t, g, r, m);
     return r;
 }
 
@@ -1340,8 +1353,8 @@ __device__ __forceinline__ void pr_single_body(const CgParams& p)
     u32* s_disp = reinterpret_cast<u32*>(s_eps + p.N);
     u32* s_guide = s_disp + KS;
     u32* s_n = s_guide + CG_GUIDE;
-    __shared__ u64 s_key[3];               // (label << 32 | thread) of the lowest accept of iterations e, e+1, e+2 (mod 3)
-    __shared__ u32 s_sites[2][CG_ST][2];   // coded sites of every thread's proposal, by iteration parity
+    __shared__ u32 s_key[3];               // lowest accepting label of iterations e, e+1, e+2 (mod 3); thread = (label + g0) mod CG_ST
+    __shared__ __align__(8) u32 s_sites[2][CG_ST][2];   // coded sites of every thread's proposal, by iteration parity
     const Tables tb = {s_cdfi, s_invr, s_fld, s_disp, s_guide, p.cdfi, p.invr_k, p.fld_k, p.disp, (u32)KS};
     const Geo geo = {p.hi1, p.hi2, p.spare, p.mask, (u32)(p.L - 1), p.lgL};
     const int tid = threadIdx.x, lane = tid & 31;
@@ -1356,17 +1369,21 @@ __device__ __forceinline__ void pr_single_body(const CgParams& p)
     for (int k = tid; k < CG_GUIDE; k += CG_ST) s_guide[k] = p.guide[k];
     for (u32 w = tid; w < (N + 31) / 32; w += CG_ST) s_n[w] = p.nbits[w];
     for (u32 k = tid; k < N; k += CG_ST) s_eps[k] = __ldcg(g_eps + k);
-    if (tid < 3) s_key[tid] = ~0ull;
+    if (tid < 3) s_key[tid] = CG_NONE;
     const u64 a_start = ctl->attempts, hops_start = ctl->hops, log_base = ctl->log_base;
     const u32 n_hops = p.n_hops;
     __syncthreads();
 
     // my attempt and the one after it (a proposal is a pure function of seed and attempt index)
-    const u32 g0 = (u32)(a_start % P);
-    u32 lab = (u32)tid >= g0 ? (u32)tid - g0 : (u32)tid + P - g0;
+    u32 g0 = (u32)(a_start % P);          // the thread that holds the first label of the window
+    u32 lab = ((u32)tid - g0) & (P - 1u);
     u64 a_cur = a_start + lab;
+    // the attempt after mine is decoded in two halves while my label lies outside the window (nothing to test then):
+    // stage 0 = nothing yet, 1 = random words drawn, 2 = complete
     Prop cur = decode_attempt(tb, p, geo, a_cur), nxt = decode_attempt(tb, p, geo, a_cur + P);
+    u32 stage = 2; u64 nxt_m = 0;
     double c_invr = tb.inv(cur.k), c_fld = tb.field(cur.k);
+    u32 c_si = geo.site(cur.ci), c_sj = geo.site(cur.cj);
     u32 hc = 0, e = 0;
     u64 used_sum = 0;
     long long dP = 0;
@@ -1375,28 +1392,28 @@ __device__ __forceinline__ void pr_single_body(const CgParams& p)
         sts64u(&s_sites[e & 1u][tid][0], cur.ci, cur.cj);
         u32 best = CG_NONE;
         if (lab < M) {
-            const u32 si = geo.site(cur.ci), sj = geo.site(cur.cj);
-            if (BIT(s_n, si) && !BIT(s_n, sj)) {                          // theta_ij
+            if (BIT(s_n, c_si) && !BIT(s_n, c_sj)) {                      // theta_ij
                 // dH_ij = eps_j - eps_i - 1/r_ij - E dx_ij
-                const double dE = __dsub_rn(__dsub_rn(__dsub_rn(s_eps[sj], s_eps[si]), c_invr), c_fld);
+                const double dE = __dsub_rn(__dsub_rn(__dsub_rn(s_eps[c_sj], s_eps[c_si]), c_invr), c_fld);
                 if (metropolis(dE, cur.uh, cur.ul, p.T, p.inv_T)) best = lab;
             }
-        }
+        } else if (stage == 0u) { nxt = decode_words(p, geo, a_cur + P, nxt_m); stage = 1u; }
+        else if (stage == 1u) { decode_finish(tb, geo, nxt, nxt_m); stage = 2u; }
         // ---- step 3: the lowest accepting label; labels are distinct
         const u32 wmin = __reduce_min_sync(CG_FULL, best);
-        if (best != CG_NONE && best == wmin) atomicMin(&s_key[e % 3u], ((u64)best << 32) | (u64)tid);
-        if (tid == 0) s_key[(e + 1u) % 3u] = ~0ull;                        // last read before the previous barrier pair
+        if (wmin != CG_NONE && lane == 0) atomicMin(&s_key[e % 3u], wmin);
+        if (tid == 0) s_key[(e + 1u) % 3u] = CG_NONE;                      // last read before the previous barrier pair
         __syncthreads();
-        const u64 key = s_key[e % 3u];
-        const bool hop = key != ~0ull;
-        const u32 used = hop ? (u32)(key >> 32) + 1u : M;                 // m = (p-1) M + q
+        const u32 key = s_key[e % 3u];
+        const bool hop = key != CG_NONE;
+        const u32 used = hop ? key + 1u : M;                               // m = (p-1) M + q
         if (hop) {
-            const uint2 w = lds64u(&s_sites[e & 1u][(u32)key][0]);        // coded sites of the executed hop
+            const uint2 w = lds64u(&s_sites[e & 1u][(key + g0) & (P - 1u)][0]);      // coded sites of the executed hop
             // step 3b: eps_l += 1/r_lj - 1/r_li, difference first, then ONE add
             for (u32 l = tid; l < N; l += CG_ST)
                 s_eps[l] = __dadd_rn(s_eps[l], hop_term(tf, mask, geo.code(l) | geo.spare, w.x, w.y));
             ++hc;
-            if (tid == 0) {                                                // step 3a, dP, hop log
+            if (tid == CG_ST - 1) {                                        // step 3a, dP, hop log (a thread with few sites)
                 const u32 hi_ = geo.site(w.x), hj_ = geo.site(w.y);
                 s_n[hi_ >> 5] &= ~(1u << (hi_ & 31));
                 s_n[hj_ >> 5] |= 1u << (hj_ & 31);
@@ -1406,18 +1423,22 @@ __device__ __forceinline__ void pr_single_body(const CgParams& p)
             }
         }
         used_sum += used;
+        g0 = (g0 + used) & (P - 1u);
         ++e;
         if (lab >= used) lab -= used;
         else {                                                             // consumed: my next attempt, P attempts later
+            if (stage == 0u) nxt = decode_words(p, geo, a_cur + P, nxt_m);       // (M close to P: no idle iterations)
+            if (stage != 2u) decode_finish(tb, geo, nxt, nxt_m);
             lab += P - used; a_cur += P;
             cur = nxt; c_invr = tb.inv(cur.k); c_fld = tb.field(cur.k);
-            nxt = decode_attempt(tb, p, geo, a_cur + P);
+            c_si = geo.site(cur.ci); c_sj = geo.site(cur.cj);
+            stage = 0u;
         }
         __syncthreads();
     }
     for (u32 k = tid; k < N; k += CG_ST) __stcg(g_eps + k, s_eps[k]);
     for (u32 w = tid; w < (N + 31) / 32; w += CG_ST) p.nbits[w] = s_n[w];
-    if (tid == 0) {
+    if (tid == CG_ST - 1) {
         ctl->attempts = a_start + used_sum; ctl->hops = hops_start + hc;
         ctl->iterations += e; ctl->proposals += (u64)M * e;
         ctl->dP += dP; ctl->epoch += e;
