@@ -95,7 +95,8 @@ int cg_run(cg_sim* s, uint64_t n_accepted_hops);
  * n_accepted_hops executed hops in ONE persistent launch, every sim on its own
  * CTAs side by side; each chain is exactly the one cg_run would produce.
  * sims[] is a host array of distinct sims that share device, stream and launch
- * shape (544 threads, same register tiling and label caching: true for
+ * shape (either all single-CTA sims - 512 threads, any number of them, one CTA each -
+ * or 544 threads with the same register tiling and label caching: true for
  * sims of equal L whose M fits their CTAs; see cg_get_launch / cg_set_launch); the sum of
  * their CTA counts must fit on the device at once, else CG_EUNSUPPORTED; clusters are not used.
  * Asynchronous on that stream; the array is not referenced after the call. */
@@ -207,7 +208,10 @@ int cg_get_phi(cg_sim* s, double* phi /* N */);
 /* Launch shape of the persistent kernel: n_ctas in [1, co-resident maximum] (a multiple
  * of the cluster size), threads in {256, 544, 608, 1024} = 32 x (5, 14, 16 or 29 worker
  * warps + 3 service warps); 0 keeps the heuristic.  Results never depend on it.
- * cg_get_launch reports the shape in use. */
+ * (1, 512) is the single-CTA kernel: 512 worker threads, eps and occupations in shared
+ * memory, two CTA barriers per iteration - for sims with M <= 512 labels and N <= 8192
+ * sites (CG_EINVAL otherwise); the heuristic picks it whenever max(M, N/2) <= 512 and no
+ * cluster size was asked for.  cg_get_launch reports the shape in use. */
 int cg_set_launch(cg_sim* s, int n_ctas, int threads);
 int cg_get_launch(cg_sim* s, int* n_ctas, int* threads, int* smem_bytes);
 

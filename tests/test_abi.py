@@ -77,6 +77,8 @@ def test_diagnostic_entry_points_validate_arguments(cg):
     assert lib.cg_get_phase_cycles(None, None, None, None, None, None, 0) == cg.binding.CG_EINVAL
     assert lib.cg_set_launch(None, 0, 0) == cg.binding.CG_EINVAL
     assert lib.cg_get_counters(None, None, None, None, None) == cg.binding.CG_EINVAL
+    assert lib.cg_get_exchange_cycles(None, None) == cg.binding.CG_EINVAL
+    assert lib.cg_get_labels_per_thread(None, None) == cg.binding.CG_EINVAL
     out = C.c_double()
     assert lib.cg_bench_l2(100, 1, 1, 0, 2, 512, 16, C.byref(out)) == cg.binding.CG_EINVAL       # too small a buffer
     assert lib.cg_bench_l2(1 << 20, 1, 1, 3, 2, 512, 16, C.byref(out)) == cg.binding.CG_EINVAL   # no such mode
@@ -92,5 +94,6 @@ def test_observable_entry_points_validate_arguments(cg):
     assert lib.cg_get_time_stochastic(None, C.byref(d)) == E
     assert lib.cg_get_normals(None, 0, 1, None) == E
     assert lib.cg_get_dos(None, 0.0, 1.0, 4, None, C.byref(u)) == E
+    assert lib.cg_get_dos_noalloc(None, 0.0, 1.0, 4, None, C.byref(u)) == E
     assert lib.cg_get_series(None, 0, 0, None, None) == E
     assert lib.cg_get_sigma0(None, C.byref(d)) == E
