@@ -210,10 +210,15 @@ int cg_get_phi(cg_sim* s, double* phi /* N */);
  * warps + 3 service warps); 0 keeps the heuristic.  Results never depend on it.
  * (1, 512) is the single-CTA kernel: 512 worker threads, eps and occupations in shared
  * memory, two CTA barriers per iteration - for sims with M <= 512 labels and N <= 8192
- * sites (CG_EINVAL otherwise); the heuristic picks it whenever max(M, N/2) <= 512 and no
- * cluster size was asked for.  cg_get_launch reports the shape in use. */
+ * sites (CG_EINVAL otherwise); (1, 1024) is the same kernel with 1024 threads when
+ * 512 < M <= 1024 and N <= 8192 (otherwise the dataflow shape of that size).  The heuristic
+ * picks the single-CTA kernel whenever M <= 1024, N <= 1024 and no cluster size was asked
+ * for.  cg_get_launch reports the shape in use, cg_get_kernel which kernel it belongs to. */
 int cg_set_launch(cg_sim* s, int n_ctas, int threads);
 int cg_get_launch(cg_sim* s, int* n_ctas, int* threads, int* smem_bytes);
+/* Which kernel cg_run launches in the shape in use: *kind = 0 the dataflow kernel cg_pr_persistent, 1 the
+ * single-CTA kernel cg_pr_single (512 threads for M <= 512, 1024 threads for M <= 1024). */
+int cg_get_kernel(cg_sim* s, int* kind);
 
 /* Tuning that never changes results.  snapshot_interval H in {1, 2, 4, 8} (default: 8 for N >= 2^18
  * sites, else 2): the

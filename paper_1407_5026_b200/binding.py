@@ -20,7 +20,7 @@ EXPORTS = [
     "cg_run", "cg_run_many", "cg_get_state", "cg_set_state",
     "cg_get_time_stochastic", "cg_get_normals", "cg_get_dos", "cg_get_dos_noalloc", "cg_get_series", "cg_get_sigma0",
     "cg_get_counters", "cg_enable_hop_log", "cg_get_hops", "cg_recompute_eps", "cg_apply_hops",
-    "cg_set_update_kernel", "cg_get_table_sizes", "cg_get_tables", "cg_get_table_dz", "cg_get_phi", "cg_set_launch", "cg_get_launch",
+    "cg_set_update_kernel", "cg_get_table_sizes", "cg_get_tables", "cg_get_table_dz", "cg_get_phi", "cg_set_launch", "cg_get_launch", "cg_get_kernel",
     "cg_set_tuning", "cg_get_tuning", "cg_get_labels_per_thread", "cg_set_phase_timers", "cg_get_phase_cycles", "cg_get_exchange_cycles", "cg_bench_l2", "cg_free", "cg_strerror",
     "cg_last_error",
 ]
@@ -73,6 +73,7 @@ def lib():
         "cg_get_phi": (ci, [vp, vp]),
         "cg_set_launch": (ci, [vp, ci, ci]),
         "cg_get_launch": (ci, [vp, P(ci), P(ci), P(ci)]),
+        "cg_get_kernel": (ci, [vp, P(ci)]),
         "cg_set_tuning": (ci, [vp, ci, ci]),
         "cg_get_tuning": (ci, [vp, P(ci), P(ci)]),
         "cg_get_labels_per_thread": (ci, [vp, P(ci)]),
@@ -335,6 +336,12 @@ class CoulombGlass:
         a = np.zeros(6, np.uint64)
         self._check(self._lib.cg_get_exchange_cycles(self._h, _ptr(a)))
         return dict(zip(("recycle", "gate", "own_workers", "scan", "publish", "warps"), (int(v) for v in a)))
+
+    def kernel(self):
+        """'single' (cg_pr_single: one CTA, state in shared memory) or 'dataflow' (cg_pr_persistent)."""
+        k = C.c_int()
+        self._check(self._lib.cg_get_kernel(self._h, C.byref(k)))
+        return "single" if k.value == 1 else "dataflow"
 
     def labels_per_thread(self):
         k = C.c_int()

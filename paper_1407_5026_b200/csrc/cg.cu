@@ -1340,8 +1340,9 @@ cg_pr_persistent_many(const CgParams* __restrict__ ps, const u32* __restrict__ f
 // terms), the lowest accepting label (step 3) is ONE 64-bit shared-memory atomicMin of (label, thread), and after the
 // barrier every thread adds the hop's term to its sites of eps (step 3b: the same single rounded add per
 // site and hop as everywhere else).  Second barrier, next iteration.
-#define CG_ST 512           // threads (= labels held) of the single-CTA kernel
+#define CG_ST 512           // threads (= labels held) of the single-CTA kernel; 1024 for 512 < M <= 1024
 #define CG_SINGLE_MAX_N 8192u   // eps in shared memory: 64 KiB
+template <int ST>
 __device__ __forceinline__ void pr_single_body(const CgParams& p)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -1353,22 +1354,22 @@ __device__ __forceinline__ void pr_single_body(const CgParams& p)
     u32* s_disp = reinterpret_cast<u32*>(s_eps + p.N);
     u32* s_guide = s_disp + KS;
     u32* s_n = s_guide + CG_GUIDE;
-    __shared__ u32 s_key[3];               // lowest accepting label of iterations e, e+1, e+2 (mod 3); thread = (label + g0) mod CG_ST
-    __shared__ __align__(8) u32 s_sites[2][CG_ST][2];   // coded sites of every thread's proposal, by iteration parity
+    __shared__ u32 s_key[3];               // lowest accepting label of iterations e, e+1, e+2 (mod 3); thread = (label + g0) mod ST
+    __shared__ __align__(8) u32 s_sites[2][ST][2];   // coded sites of every thread's proposal, by iteration parity
     const Tables tb = {s_cdfi, s_invr, s_fld, s_disp, s_guide, p.cdfi, p.invr_k, p.fld_k, p.disp, (u32)KS};
     const Geo geo = {p.hi1, p.hi2, p.spare, p.mask, (u32)(p.L - 1), p.lgL};
     const int tid = threadIdx.x, lane = tid & 31;
-    const u32 N = p.N, M = p.M, mask = p.mask, P = CG_ST;
+    const u32 N = p.N, M = p.M, mask = p.mask, P = ST;
     const double* __restrict__ tf = p.tf;
     CgCtl* const ctl = p.ctl;
     double* const g_eps = p.eps[ctl->cur];
 
-    for (int k = tid; k < KS; k += CG_ST) {
+    for (int k = tid; k < KS; k += ST) {
         s_cdfi[k] = p.cdfi[k]; s_invr[k] = p.invr_k[k]; s_fld[k] = p.fld_k[k]; s_disp[k] = p.disp[k];
     }
-    for (int k = tid; k < CG_GUIDE; k += CG_ST) s_guide[k] = p.guide[k];
-    for (u32 w = tid; w < (N + 31) / 32; w += CG_ST) s_n[w] = p.nbits[w];
-    for (u32 k = tid; k < N; k += CG_ST) s_eps[k] = __ldcg(g_eps + k);
+    for (int k = tid; k < CG_GUIDE; k += ST) s_guide[k] = p.guide[k];
+    for (u32 w = tid; w < (N + 31) / 32; w += ST) s_n[w] = p.nbits[w];
+    for (u32 k = tid; k < N; k += ST) s_eps[k] = __ldcg(g_eps + k);
     if (tid < 3) s_key[tid] = CG_NONE;
     const u64 a_start = ctl->attempts, hops_start = ctl->hops, log_base = ctl->log_base;
     const u32 n_hops = p.n_hops;
@@ -1415,10 +1416,10 @@ __device__ __forceinline__ void pr_single_body(const CgParams& p)
         if (hop) {
             const uint2 w = lds64u(&s_sites[e & 1u][(key + g0) & (P - 1u)][0]);      // coded sites of the executed hop
             // step 3b: eps_l += 1/r_lj - 1/r_li, difference first, then ONE add
-            for (u32 l = tid; l < N; l += CG_ST)
+            for (u32 l = tid; l < N; l += ST)
                 s_eps[l] = __dadd_rn(s_eps[l], hop_term(tf, mask, geo.code(l) | geo.spare, w.x, w.y));
             ++hc;
-            if (tid == CG_ST - 1) {                                        // step 3a, dP, hop log (a thread with few sites)
+            if (tid == ST - 1) {                                        // step 3a, dP, hop log (a thread with few sites)
                 const u32 hi_ = geo.site(w.x), hj_ = geo.site(w.y);
                 s_n[hi_ >> 5] &= ~(1u << (hi_ & 31));
                 s_n[hj_ >> 5] |= 1u << (hj_ & 31);
@@ -1441,24 +1442,26 @@ __device__ __forceinline__ void pr_single_body(const CgParams& p)
         }
         __syncthreads();
     }
-    for (u32 k = tid; k < N; k += CG_ST) __stcg(g_eps + k, s_eps[k]);
-    for (u32 w = tid; w < (N + 31) / 32; w += CG_ST) p.nbits[w] = s_n[w];
-    if (tid == CG_ST - 1) {
+    for (u32 k = tid; k < N; k += ST) __stcg(g_eps + k, s_eps[k]);
+    for (u32 w = tid; w < (N + 31) / 32; w += ST) p.nbits[w] = s_n[w];
+    if (tid == ST - 1) {
         ctl->attempts = a_start + used_sum; ctl->hops = hops_start + hc;
         ctl->iterations += e; ctl->proposals += (u64)M * e;
         ctl->dP += dP; ctl->epoch += e;
     }
 }
 
-__global__ void __launch_bounds__(CG_ST, 1) cg_pr_single(const CgParams p) { pr_single_body(p); }
+template <int ST>
+__global__ void __launch_bounds__(ST, 1) cg_pr_single(const CgParams p) { pr_single_body<ST>(p); }
 
 // many single-CTA sims in one launch: CTA s runs sim s
-__global__ void __launch_bounds__(CG_ST, 1) cg_pr_single_many(const CgParams* __restrict__ ps)
+template <int ST>
+__global__ void __launch_bounds__(ST, 1) cg_pr_single_many(const CgParams* __restrict__ ps)
 {
     __shared__ CgParams sp;
     if (threadIdx.x == 0) sp = ps[blockIdx.x];
     __syncthreads();
-    pr_single_body(sp);
+    pr_single_body<ST>(sp);
 }
 
 __device__ __forceinline__ Geo make_geo(const CgParams& p)
@@ -2109,16 +2112,24 @@ static int choose_launch(cg_sim* s, int n_ctas, int threads)
     // A sim whose labels and sites fit one CTA runs in the single-CTA kernel (everything in shared memory): chosen
     // automatically, or asked for as (1 CTA, CG_ST threads); any other explicit shape keeps the dataflow kernel.
     {
-        const bool fits = s->M <= CG_ST && s->N <= CG_SINGLE_MAX_N
+        // CG_ST threads hold up to CG_ST labels; 2 CG_ST threads (registers: 64 each) hold up to 2 CG_ST
+        const int st = s->M <= CG_ST ? CG_ST : 2 * CG_ST;
+        const bool fits = s->M <= 2 * CG_ST && s->N <= CG_SINGLE_MAX_N
                           && smem_single_bytes(s) + 12 * 1024 <= (size_t)s->smem_optin;
+        // asked for: (1 CTA, 512 threads), or (1 CTA, 1024 threads) when 512 < M <= 1024 fits (else that is a dataflow shape);
+        // automatic: up to 1024 sites (measured: at L = 64 the dataflow kernel on 8 CTAs is the faster one for a single sim,
+        // 662 k against 508 k hops/s at M = 1024, but the single-CTA kernel takes one SM instead of eight: replica packing)
         const bool asked = threads == CG_ST && n_ctas <= 1;
-        const bool automatic = threads == 0 && n_ctas == 0 && s->cluster_pref == 0 && std::max<u64>(s->M, s->N / 2) <= CG_ST;
-        if (asked && !fits) return CG_EINVAL;
-        if (fits && (asked || automatic)) {
+        const bool asked2 = threads == 2 * CG_ST && n_ctas == 1 && fits && st == 2 * CG_ST;
+        const bool automatic = threads == 0 && n_ctas == 0 && s->cluster_pref == 0 && s->N <= 2 * CG_ST && s->M <= 2 * CG_ST;
+        if (asked && (!fits || st != CG_ST)) return CG_EINVAL;
+        if (fits && (asked || asked2 || automatic)) {
             const int smem = (int)smem_single_bytes(s);
-            CK(cudaFuncSetAttribute((const void*)cg_pr_single, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-            CK(cudaFuncSetAttribute((const void*)cg_pr_single_many, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-            s->single = true; s->n_ctas = 1; s->threads = CG_ST; s->rp = 0; s->pl = CG_ST; s->lpt = 1; s->smem = smem;
+            CK(cudaFuncSetAttribute((const void*)cg_pr_single<CG_ST>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+            CK(cudaFuncSetAttribute((const void*)cg_pr_single_many<CG_ST>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+            CK(cudaFuncSetAttribute((const void*)cg_pr_single<2 * CG_ST>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+            CK(cudaFuncSetAttribute((const void*)cg_pr_single_many<2 * CG_ST>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+            s->single = true; s->n_ctas = 1; s->threads = st; s->rp = 0; s->pl = st; s->lpt = 1; s->smem = smem;
             s->cluster = 1;
             return CG_OK;
         }
@@ -2307,7 +2318,8 @@ extern "C" int cg_run(cg_sim* s, uint64_t n_hops)
         while (n_hops) {
             const u32 chunk = (u32)std::min<uint64_t>(n_hops, CG_MAX_LAUNCH_HOPS);
             const CgParams p = make_params(s, chunk);
-            cg_pr_single<<<1, CG_ST, (size_t)s->smem, s->stream>>>(p);
+            if (s->threads == CG_ST) cg_pr_single<CG_ST><<<1, CG_ST, (size_t)s->smem, s->stream>>>(p);
+            else cg_pr_single<2 * CG_ST><<<1, 2 * CG_ST, (size_t)s->smem, s->stream>>>(p);
             CK(cudaGetLastError());
             n_hops -= chunk;
         }
@@ -2339,7 +2351,7 @@ extern "C" int cg_run_many(cg_sim* const* sims, int n_sims, uint64_t n_hops)
         if (!s) return CG_EINVAL;
         for (int m = 0; m < k; ++m) if (sims[m] == s) return CG_EINVAL;       // a sim may appear once
         if (s->device != s0->device || s->stream != s0->stream || s->threads != s0->threads || s->rp != s0->rp
-            || (s->pl > 0 && s->lpt == 1) != (s0->pl > 0 && s0->lpt == 1)) {
+            || (s->pl > 0 && s->lpt == 1) != (s0->pl > 0 && s0->lpt == 1) || s->single != s0->single) {
             s0->err = "cg_run_many: the sims must share device, stream and launch shape (threads, register tiling, "
                       "cached labels)";
             return CG_EINVAL;
@@ -2352,7 +2364,8 @@ extern "C" int cg_run_many(cg_sim* const* sims, int n_sims, uint64_t n_hops)
     if (!single && !f) { s0->err = "cg_run_many: only 544-thread launch shapes"; return CG_EUNSUPPORTED; }
     const u32 total = first[(size_t)n_sims];
     if (single) {
-        CK0(s0, cudaFuncSetAttribute((const void*)cg_pr_single_many, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+        CK0(s0, cudaFuncSetAttribute((const void*)cg_pr_single_many<CG_ST>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+        CK0(s0, cudaFuncSetAttribute((const void*)cg_pr_single_many<2 * CG_ST>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
     } else {
         CK0(s0, cudaFuncSetAttribute((const void*)f, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
         int per_sm = 0;
@@ -2382,7 +2395,8 @@ extern "C" int cg_run_many(cg_sim* const* sims, int n_sims, uint64_t n_hops)
         u32 n = (u32)n_sims;
         void* args[] = {&d_ps, &d_first, &n};
         if (single) {
-            cg_pr_single_many<<<(unsigned)n_sims, CG_ST, (size_t)smem, s0->stream>>>(d_ps);
+            if (s0->threads == CG_ST) cg_pr_single_many<CG_ST><<<(unsigned)n_sims, CG_ST, (size_t)smem, s0->stream>>>(d_ps);
+            else cg_pr_single_many<2 * CG_ST><<<(unsigned)n_sims, 2 * CG_ST, (size_t)smem, s0->stream>>>(d_ps);
             CK0(s0, cudaGetLastError());
         } else
         CK0(s0, launch_coop((const void*)f, (int)total, s0->threads, smem, s0->stream, 1, args));
@@ -2693,6 +2707,13 @@ extern "C" int cg_get_exchange_cycles(cg_sim* s, uint64_t* cycles6)
     int rc = read_ctl(s, &c);
     if (rc != CG_OK) return rc;
     for (int k = 0; k < 6; ++k) cycles6[k] = c.cyc_x[k];
+    return CG_OK;
+}
+
+extern "C" int cg_get_kernel(cg_sim* s, int* kind)
+{
+    if (!s || !kind) return CG_EINVAL;
+    *kind = s->single ? 1 : 0;
     return CG_OK;
 }
 

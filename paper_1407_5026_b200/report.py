@@ -211,7 +211,7 @@ def report_replicas(hops):
             name, len(sims), sims[0].launch()["n_ctas"], len(sims) * hops / ms * 1e3, hops / ms * 1e3))
         sys.stdout.flush()
 
-    def packed(name, idxs, copies, n_ctas=0):
+    def packed(name, idxs, copies, n_ctas=0, threads=544):
         """The same replica sets through cg_run_many: one launch, every sim on its own CTAs."""
         sims = []
         for r in range(copies):
@@ -220,13 +220,14 @@ def report_replicas(hops):
                 kw["seed"] += 100 * r
                 g = binding.CoulombGlass(**kw)
                 if n_ctas:
-                    g.set_launch(n_ctas, 544)
+                    g.set_launch(n_ctas, threads)
                 sims.append(g)
         binding.run_many(sims, 1000)
         torch.cuda.synchronize()
         ms = _timed(lambda: binding.run_many(sims, hops))
-        print("%s x%d replicas packed into one launch (%d CTAs each): %.0f hops/s aggregate, %.0f per replica" % (
-            name, len(sims), sims[0].launch()["n_ctas"], len(sims) * hops / ms * 1e3, hops / ms * 1e3))
+        print("%s x%d replicas packed into one launch (%d CTAs x %d threads each, %s kernel): %.0f hops/s aggregate, %.0f per replica" % (
+            name, len(sims), sims[0].launch()["n_ctas"], sims[0].launch()["threads"], sims[0].kernel(),
+            len(sims) * hops / ms * 1e3, hops / ms * 1e3))
         sys.stdout.flush()
 
     sms = torch.cuda.get_device_properties(0).multi_processor_count
@@ -235,6 +236,7 @@ def report_replicas(hops):
     packed("cfg1_L16", [0], 32)
     packed("cfg1_L16", [0], sms)
     packed("cfg2_L64", [0], sms // 5, n_ctas=5)
+    packed("cfg2_L64", [0], sms, n_ctas=1, threads=1024)        # config 2 on ONE SM each: the single-CTA kernel
     run("cfg3_L128", [0, 1, 2, 3], 1)     # the temperature sweep of config 3 as one replica set
     run("cfg3_L128", [0, 1, 2, 3], 2)
     run("cfg1_L16", [0], 1)

@@ -257,7 +257,7 @@ def test_single_cta_kernel(cg, oracle_lib, kw, explicit, hops):
     g = cg.CoulombGlass(hop_log=hops, **kw)
     if explicit:
         g.set_launch(1, 512)
-    assert g.launch()["n_ctas"] == 1 and g.launch()["threads"] == 512 and g.labels_per_thread() == 1
+    assert g.launch()["n_ctas"] == 1 and g.launch()["threads"] == 512 and g.labels_per_thread() == 1 and g.kernel() == "single"
     g.run(hops // 3)
     g.run(hops - hops // 3)
     o = oracle_lib.Oracle(**kw)
@@ -277,9 +277,29 @@ def test_single_cta_kernel(cg, oracle_lib, kw, explicit, hops):
     _compare(g2, o, hops + 600)
 
 
+@pytest.mark.parametrize("kw,shape,hops", [
+    (dict(L=32, T=0.08, E=0.01, seed=5, M=1024), None, 6000),            # automatic: M = the threads of the CTA, no idle lanes
+    (dict(L=32, T=0.08, E=0.01, seed=5, M=700), None, 6000),
+    (dict(L=64, T=0.05, E=0.0, seed=2, M=1024), (1, 1024), 6000),        # config 2 on one SM (replica packing)
+    (dict(L=16, dim=3, T=0.05, E=0.01, seed=13, M=1000), (1, 1024), 4000),
+    (dict(L=16, T=0.01, E=0.0, seed=6, M=1024), None, 300),              # cold: whole windows rejected
+])
+def test_single_cta_kernel_with_1024_threads(cg, oracle_lib, kw, shape, hops):
+    g = cg.CoulombGlass(hop_log=hops, **kw)
+    if shape:
+        g.set_launch(*shape)
+    assert g.kernel() == "single" and g.launch()["n_ctas"] == 1 and g.launch()["threads"] == 1024
+    g.run(hops // 2)
+    g.run(hops - hops // 2)
+    o = oracle_lib.Oracle(**kw)
+    o.run(hops)
+    _compare(g, o, hops)
+    assert g.recompute_eps() < 1e-9
+
+
 def test_single_cta_kernel_refuses_what_does_not_fit(cg):
     g = cg.CoulombGlass(L=16, T=0.1, M=4096)
-    assert g.launch()["threads"] == 544                # M beyond 512 labels: the dataflow kernel
+    assert g.launch()["threads"] == 544 and g.kernel() == "dataflow"      # M beyond 1024 labels: the dataflow kernel
     with pytest.raises(cg.CgError):
         g.set_launch(1, 512)
     g = cg.CoulombGlass(L=128, T=0.1, M=256)
