@@ -794,7 +794,8 @@ __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 
         const u64 log_base = p.ctl->log_base, hops_start = p.ctl->hops;
         u64 used_sum = 0;                 // attempts consumed in this launch
         long long dP = 0;
-        u32 e = 0, hc = 0;                // iterations and hops decided in this launch
+        u32 e = 0, hc = 0;                // iterations (mod 2^32: ring positions and epoch tags only) and hops decided in this launch
+        u64 its = 0;                      // iterations of this launch (a cold system runs many more iterations than hops)
         u32 ver = 0;                      // newest snapshot known to be published by every CTA
         Waiter wd;
         bool quit = false;
@@ -970,7 +971,7 @@ __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 
             }
             // (5) the bookkeeping, off the critical path
             used_sum += used;
-            ++e;
+            ++e; ++its;
             if (hop) {
                 const u32 hi_ = geo.site(ci), hj_ = geo.site(cj);
                 dP += geo.dx(hi_, hj_);                                  // step 3b: dP = dx
@@ -990,8 +991,8 @@ __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 
             CgCtl* c = p.ctl;
             const u32 ns = n_snaps + ((n_hops & Hm) ? 1u : 0u);
             c->attempts = a_start + used_sum; c->hops = hops_start + hc;
-            c->iterations += e; c->proposals += (u64)M * e;
-            c->dP += dP; c->cur = (cur0 + ns) % CG_RING; c->epoch += e;
+            c->iterations += its; c->proposals += (u64)M * its;
+            c->dP += dP; c->cur = (cur0 + ns) % CG_RING; c->epoch += its;
             c->pub_base = pub_base + ns;
             c->cyc_total += (u64)(clock64() - t_begin);
         }
@@ -1385,7 +1386,8 @@ __device__ __forceinline__ void pr_single_body(const CgParams& p)
     u32 stage = 2; u64 nxt_m = 0;
     double c_invr = tb.inv(cur.k), c_fld = tb.field(cur.k);
     u32 c_si = geo.site(cur.ci), c_sj = geo.site(cur.cj);
-    u32 hc = 0, e = 0;
+    u32 hc = 0, e = 0, k3 = 0;             // e: iterations mod 2^32 (parity of the site buffers only), k3 = iterations mod 3
+    u64 its = 0;
     u64 used_sum = 0;
     long long dP = 0;
     while (hc < n_hops) {
@@ -1407,10 +1409,12 @@ __device__ __forceinline__ void pr_single_body(const CgParams& p)
         }
         // ---- step 3: the lowest accepting label; labels are distinct
         const u32 wmin = __reduce_min_sync(CG_FULL, best);
-        if (wmin != CG_NONE && lane == 0) atomicMin(&s_key[e % 3u], wmin);
-        if (tid == 0) s_key[(e + 1u) % 3u] = CG_NONE;                      // last read before the previous barrier pair
+        const u32 k3n = k3 == 2u ? 0u : k3 + 1u;
+        if (wmin != CG_NONE && lane == 0) atomicMin(&s_key[k3], wmin);
+        if (tid == 0) s_key[k3n] = CG_NONE;                                // last read before the previous barrier pair
         __syncthreads();
-        const u32 key = s_key[e % 3u];
+        const u32 key = s_key[k3];
+        k3 = k3n;
         const bool hop = key != CG_NONE;
         const u32 used = hop ? key + 1u : M;                               // m = (p-1) M + q
         if (hop) {
@@ -1430,7 +1434,7 @@ __device__ __forceinline__ void pr_single_body(const CgParams& p)
         }
         used_sum += used;
         g0 = (g0 + used) & (P - 1u);
-        ++e;
+        ++e; ++its;
         if (lab >= used) lab -= used;
         else {                                                             // consumed: my next attempt, P attempts later
             if (stage == 0u) nxt = decode_words(p, geo, a_cur + P, nxt_m);       // (M close to P: no idle iterations)
@@ -1446,8 +1450,8 @@ __device__ __forceinline__ void pr_single_body(const CgParams& p)
     for (u32 w = tid; w < (N + 31) / 32; w += ST) p.nbits[w] = s_n[w];
     if (tid == ST - 1) {
         ctl->attempts = a_start + used_sum; ctl->hops = hops_start + hc;
-        ctl->iterations += e; ctl->proposals += (u64)M * e;
-        ctl->dP += dP; ctl->epoch += e;
+        ctl->iterations += its; ctl->proposals += (u64)M * its;
+        ctl->dP += dP; ctl->epoch += its;
     }
 }
 
