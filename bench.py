@@ -267,29 +267,41 @@ def run_ours(args):
     c = g.counters()
     assert all(r["g"].counters()["hops"] == K * H for r in reps)
 
-    # ---- end to end through the C ABI with pinned HOST buffers (restore -> run -> read back), every replica
+    # ---- end to end through the C ABI with pinned HOST buffers (restore -> run -> read back), every replica: the SAME
+    # workload as above (a fresh sim of the same seed, hops 1..K*H), its state living in host memory between the steps
     for r in reps:
+        with torch.cuda.device(r["dev"]):
+            r["e"] = pkg.CoulombGlass(device=r["dev"], **r["kw"])
+            if args.cluster:
+                r["e"].set_tuning(0, args.cluster)
+            if args.ctas or args.threads:
+                r["e"].set_launch(args.ctas, args.threads)
         r["n_host"] = torch.empty(N, dtype=torch.int8).pin_memory().numpy()
         r["eps_host"] = torch.empty(N, dtype=torch.float64).pin_memory().numpy()
-        _, r["dP"] = r["warm"].state_into(r["n_host"], r["eps_host"])
-        r["wc"] = r["warm"].counters()
+        with torch.cuda.device(r["dev"]):
+            _, r["dP"] = r["e"].state_into(r["n_host"], r["eps_host"])
+            r["wc"] = r["e"].counters()
     barrier()
     t0 = time.perf_counter()
     for _ in range(K):
         for r in reps:
-            r["warm"].set_state(r["n_host"], r["eps_host"], r["wc"]["attempts"], r["wc"]["hops"], r["dP"])    # H2D
-            r["warm"].run(H)
+            with torch.cuda.device(r["dev"]):
+                r["e"].set_state(r["n_host"], r["eps_host"], r["wc"]["attempts"], r["wc"]["hops"], r["dP"])    # H2D
+                r["e"].run(H)
         for r in reps:
-            _, r["dP"] = r["warm"].state_into(r["n_host"], r["eps_host"])                                   # D2H, syncs
-            r["wc"] = r["warm"].counters()
+            with torch.cuda.device(r["dev"]):
+                _, r["dP"] = r["e"].state_into(r["n_host"], r["eps_host"])                               # D2H, syncs
+                r["wc"] = r["e"].counters()
     barrier()
+    assert all(r["wc"]["hops"] == K * H and r["wc"]["attempts"] == r["g"].counters()["attempts"] for r in reps)   # the same chain
     e2e_ms, e2e_hops = reduce_over_ranks(1e3 * (time.perf_counter() - t0), K * H * len(reps),
                                          dist if world > 1 else None)
     bitmap = 4 * ((N + 31) // 32)
     e2e = {"value": e2e_hops / (e2e_ms * 1e-3), "unit": UNIT,
            "h2d_bytes_per_step": 8 * N + bitmap + CTL_BYTES,
            "d2h_bytes_per_step": 8 * N + bitmap + 3 * CTL_BYTES,
-           "what": "cg_set_state(host n, eps) + cg_run + cg_get_state(host n, eps) + cg_get_counters per step and replica"}
+           "what": "the same workload (fresh sim, same seed, hops 1..steps*hops_per_step): cg_set_state(host n, eps) + cg_run + "
+                   "cg_get_state(host n, eps) + cg_get_counters per step and replica; wall clock"}
 
     if rank != 0:
         return
