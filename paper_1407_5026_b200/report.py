@@ -6,6 +6,7 @@
     python -m paper_1407_5026_b200.report --l2            # sweep of the L2 roofline probe (cg_bench_l2)
     python -m paper_1407_5026_b200.report --update        # step a6 alone: gather kernel against bulk-copy staged kernel
     python -m paper_1407_5026_b200.report --tuning        # snapshot interval H and cluster size at configs 3 and 5
+    python -m paper_1407_5026_b200.report --cubic         # 3D cubic lattices (64^3 = the headline footprint)
     python -m paper_1407_5026_b200.report --one cfg5_L512 [--hops 20000]    # one config, two launches (ncu target)
     python -m paper_1407_5026_b200.report --l2-one        # the best L2 probe shape alone (ncu target)
 
@@ -120,6 +121,24 @@ def report_configs(hops, warm):
                       at / ms * 1e3, it / Hd, mean_q, A_all, A_last, us_hop, split, w_u,
                       16.0 * N / w_u / 1e3, g.recompute_eps()))
             sys.stdout.flush()
+
+
+def report_3d(hops):
+    """The cubic lattice at the headline footprint N = 64^3 = 2^18 and at 32^3."""
+    print("# %s: 3D cubic lattices, %d hops after 2000 warm-up hops" % (torch.cuda.get_device_name(0), hops))
+    for kw in (dict(L=64, T=0.05, E=0.01, seed=64, M=65536), dict(L=32, T=0.05, E=0.01, seed=32, M=8192),
+               dict(L=16, T=0.1, E=0.01, seed=16, M=1024), dict(L=8, T=0.1, E=0.0, seed=8, M=256)):
+        g = binding.CoulombGlass(dim=3, **kw)
+        g.run(2000)
+        torch.cuda.synchronize()
+        c0 = g.counters()
+        ms = _timed(lambda: g.run(hops))
+        c = g.counters()
+        ln = g.launch()
+        print("3D L=%-3d N=%-7d T=%-5g M=%-6d %3d CTAs x %4d (%s kernel): %7.0f hops/s  %.3f us/hop  A=%.2e  q=%.1f  drift %.1e" % (
+            kw["L"], g.N, kw["T"], kw["M"], ln["n_ctas"], ln["threads"], g.kernel(), hops / ms * 1e3, ms * 1e3 / hops,
+            hops / (c["attempts"] - c0["attempts"]), (c["attempts"] - c0["attempts"]) / hops - 1.0, g.recompute_eps()))
+        sys.stdout.flush()
 
 
 def report_l2():
@@ -308,6 +327,7 @@ def main():
     ap.add_argument("--l2", action="store_true")
     ap.add_argument("--update", action="store_true")
     ap.add_argument("--tuning", action="store_true")
+    ap.add_argument("--cubic", action="store_true", help="throughput on 3D cubic lattices")
     ap.add_argument("--one", default="", help="CONFIG[:index], e.g. cfg5_L512 or cfg3_L128:3")
     ap.add_argument("--l2-one", action="store_true")
     ap.add_argument("--cluster", type=int, default=0, help="cluster size for --one (0: automatic)")
@@ -333,6 +353,8 @@ def main():
         report_update()
     if a.tuning:
         report_tuning(a.hops or 100_000)
+    if a.cubic:
+        report_3d(a.hops or 50_000)
 
 
 if __name__ == "__main__":
