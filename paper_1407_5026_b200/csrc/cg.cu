@@ -559,8 +559,8 @@ __device__ __forceinline__ bool mbar_wait(u64* b, u32 parity, const CgParams& p,
 // Otherwise (M > P) CTA b evaluates labels [b per, (b+1) per) from scratch in every iteration, with the
 // warps of the CTA in lock step (the occupation bitmap is then always current).
 //
-// Roles: warp 0 the collector (C), 1 the exchange warp (X), 2 the service warp (S), warps 3 .. NW+2 the
-// workers.  Iteration e ("exchange"), state S_e before it, outcome O_e:
+// Roles: warp 0 the service warp (S), warps 1 .. NW the workers, warp NW+1 the collector (C), NW+2 the exchange warp (X):
+// the warp arbiter prefers high warp ids, and C and X sit on the path of every hand-over.  Iteration e ("exchange"), state S_e before it, outcome O_e:
 //   worker:  test own label on S_e -> res[e][warp]; slab update of the hop of O_{e-1}; wait for O_e (mbarrier
 //            full[e]); consume it (labels, occupations of the followed pair, followed energies); arrive empty[e]
 //   C:       reduce res[e][*] in label order, stopping at the first accept -> own[e], the CTA's slot in L2
@@ -613,9 +613,11 @@ __device__ __forceinline__ void pr_persistent_body(const CgParams& p, const u32 
     const Tables tb = {s_cdfi, s_invr, s_fld, s_disp, s_guide, p.cdfi, p.invr_k, p.fld_k, p.disp, (u32)KS};
     const Geo geo = {p.hi1, p.hi2, p.spare, p.mask, (u32)(p.L - 1), p.lgL};
 
-    // the three role warps come first: the warp arbiter prefers high warp ids, and the pollers must not
-    // take issue slots from the workers of their sub-partition
-    const int lane = threadIdx.x & 31, role = threadIdx.x >> 5, warp = role - 3, tid = (int)threadIdx.x - 96;
+    // warp 0 = service warp, warps 1 .. NW = workers, then the collector and the exchange warp: the warp arbiter prefers high
+    // warp ids, and those two sit on the path of every hand-over between CTAs (measured: +2-3 % at configs 2 and 3, nothing
+    // lost at config 5; the service warp mostly sleeps on its mbarrier)
+    const int wid = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int role = wid == 0 ? 2 : wid == NW + 1 ? 0 : wid == NW + 2 ? 1 : 3, warp = wid - 1, tid = (int)threadIdx.x - 32;
     const int atid = threadIdx.x;         // index among all threads (set-up loops)
     const u32 N = p.N, M = p.M, mask = p.mask;
     const double* __restrict__ tf = p.tf;
