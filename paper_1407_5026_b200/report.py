@@ -7,6 +7,7 @@
     python -m paper_1407_5026_b200.report --update        # step a6 alone: gather kernel against bulk-copy staged kernel
     python -m paper_1407_5026_b200.report --tuning        # snapshot interval H and cluster size at configs 3 and 5
     python -m paper_1407_5026_b200.report --cubic         # 3D cubic lattices (64^3 = the headline footprint)
+    python -m paper_1407_5026_b200.report --soak          # 34 M hops: different shapes / kernels give the same chain
     python -m paper_1407_5026_b200.report --one cfg5_L512 [--hops 20000]    # one config, two launches (ncu target)
     python -m paper_1407_5026_b200.report --l2-one        # the best L2 probe shape alone (ncu target)
 
@@ -139,6 +140,59 @@ def report_3d(hops):
             kw["L"], g.N, kw["T"], kw["M"], ln["n_ctas"], ln["threads"], g.kernel(), hops / ms * 1e3, ms * 1e3 / hops,
             hops / (c["attempts"] - c0["attempts"]), (c["attempts"] - c0["attempts"]) / hops - 1.0, g.recompute_eps()))
         sys.stdout.flush()
+
+
+def report_soak():
+    """Long chains of every config in two or three different launch shapes / kernels / tunings: they must be the SAME
+    chain (final occupations, eps bit for bit, clock, dP, attempts, the whole hop log) - a soak for rare races."""
+    import time
+
+    def run(kw, hops, shape=None, tuning=None, chunks=1):
+        g = binding.CoulombGlass(hop_log=hops, **kw)
+        if tuning:
+            g.set_tuning(*tuning)
+        if shape:
+            g.set_launch(*shape)
+        t0 = time.time()
+        for _ in range(chunks):
+            g.run(hops // chunks)
+        if hops % chunks:
+            g.run(hops % chunks)
+        torch.cuda.synchronize()
+        dt = time.time() - t0
+        n, eps, t, dP = g.state()
+        return dict(n=n, eps=eps, t=t, dP=dP, c=g.counters(), h=g.hops(0, hops), dt=dt, launch=g.launch(), kernel=g.kernel(),
+                    tun=g.tuning(), drift=g.recompute_eps())
+
+    def same(a, b):
+        return (np.array_equal(a["n"], b["n"]) and np.array_equal(a["eps"], b["eps"]) and a["t"] == b["t"] and a["dP"] == b["dP"]
+                and a["c"]["attempts"] == b["c"]["attempts"] and a["c"]["hops"] == b["c"]["hops"]
+                and all(np.array_equal(x, y) for x, y in zip(a["h"], b["h"])))
+
+    sms = torch.cuda.get_device_properties(0).multi_processor_count
+    cases = [
+        ("cfg5_L512", 0, 4_000_000, [dict(), dict(shape=(sms, 544), tuning=(2, 1)), dict(shape=(100, 608), tuning=(4, 2), chunks=7)]),
+        ("cfg3_L128", 3, 6_000_000, [dict(), dict(shape=(19, 544), tuning=(1, 1)), dict(shape=(48, 544), tuning=(8, 16), chunks=5)]),
+        ("cfg4_L256", 3, 400_000, [dict(), dict(shape=(sms, 544), tuning=(1, 1)), dict(shape=(74, 544), tuning=(4, 2))]),
+        ("cfg4_L256", 0, 3_000_000, [dict(), dict(shape=(37, 1024), tuning=(2, 1))]),
+        ("cfg2_L64", 0, 6_000_000, [dict(), dict(shape=(1, 1024)), dict(shape=(5, 544), tuning=(8, 1), chunks=3)]),
+        ("cfg1_L16", 0, 10_000_000, [dict(), dict(shape=(1, 544), tuning=(2, 1)), dict(shape=(3, 256), chunks=4)]),
+    ]
+    print("# %s: soak - every line below the reference must say identical: True" % torch.cuda.get_device_name(0))
+    for name, idx, hops, variants in cases:
+        kw = workloads.init_args(workloads.CONFIGS[name][idx], sms * 2048)
+        ref = None
+        for v in variants:
+            r = run(kw, hops, **v)
+            tag = "%s kernel %s, H=%d cluster=%d" % (
+                r["kernel"], r["launch"], r["tun"]["snapshot_interval"], r["tun"]["cluster_size"])
+            if ref is None:
+                ref = r
+                print("%s[%d] M=%d, %d hops: reference %s: %.1f s, %d attempts, drift %.1e" % (
+                    name, idx, kw["M"], hops, tag, r["dt"], r["c"]["attempts"], r["drift"]))
+            else:
+                print("    %s: %.1f s, identical: %s, drift %.1e" % (tag, r["dt"], same(ref, r), r["drift"]))
+            sys.stdout.flush()
 
 
 def report_l2():
@@ -328,6 +382,7 @@ def main():
     ap.add_argument("--update", action="store_true")
     ap.add_argument("--tuning", action="store_true")
     ap.add_argument("--cubic", action="store_true", help="throughput on 3D cubic lattices")
+    ap.add_argument("--soak", action="store_true", help="long chains in different shapes and kernels must be identical")
     ap.add_argument("--one", default="", help="CONFIG[:index], e.g. cfg5_L512 or cfg3_L128:3")
     ap.add_argument("--l2-one", action="store_true")
     ap.add_argument("--cluster", type=int, default=0, help="cluster size for --one (0: automatic)")
@@ -355,6 +410,8 @@ def main():
         report_tuning(a.hops or 100_000)
     if a.cubic:
         report_3d(a.hops or 50_000)
+    if a.soak:
+        report_soak()
 
 
 if __name__ == "__main__":
