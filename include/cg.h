@@ -211,7 +211,9 @@ int cg_get_phi(cg_sim* s, double* phi /* N */);
  * (1, 512) is the single-CTA kernel: 512 worker threads, eps and occupations in shared
  * memory, two CTA barriers per iteration - for sims with M <= 512 labels and N <= 8192
  * sites (CG_EINVAL otherwise); (1, 1024) is the same kernel with 1024 threads when
- * 512 < M <= 1024 and N <= 8192 (otherwise the dataflow shape of that size).  The heuristic
+ * 512 < M <= 1024 and N <= 8192 (otherwise the dataflow shape of that size); (1, 512) with
+ * M > 512 or N > 8192 is the variant with 2, 4 or 8 labels per thread (M <= 4096,
+ * N <= 16384: a lattice of L = 128 on one SM, for replica packing).  The heuristic
  * picks the single-CTA kernel whenever M <= 1024, N <= 1024 and no cluster size was asked
  * for.  cg_get_launch reports the shape in use, cg_get_kernel which kernel it belongs to. */
 int cg_set_launch(cg_sim* s, int n_ctas, int threads);

@@ -1470,6 +1470,137 @@ __global__ void __launch_bounds__(ST, 1) cg_pr_single_many(const CgParams* __res
     pr_single_body<ST>(sp);
 }
 
+// ---- the single-CTA kernel with KL labels per thread: lattices up to N = 16384 on ONE SM (replica packing) --------
+// Same idea as cg_pr_single (eps, occupations and tower in shared memory, two CTA barriers per iteration), for
+// M <= KL x 512 labels: thread t holds the attempts a, a + 512, .., a + (KL-1) 512 (labels lab + j 512) in registers
+// and tests all of them in every iteration.  The lowest accepting label and its two coded sites travel in ONE 64-bit
+// shared-memory atomicMin (label << 42 | c_i << 21 | c_j).  A consumed slot 0 is replaced by shifting the slots down and
+// decoding a new top one.  Slower per sim than the dataflow kernel on 8-32 SMs, but it takes one SM: 148 lattices of
+// L = 128 run side by side (cg_run_many).
+#define CG_SK_MAX_N 16384u
+template <int KL>
+__device__ __forceinline__ void pr_singlek_body(const CgParams& p)
+{
+    constexpr int ST = CG_ST;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int KS = p.Ksm;
+    u64* s_cdfi = reinterpret_cast<u64*>(smem_raw);
+    double* s_invr = reinterpret_cast<double*>(s_cdfi + KS);
+    double* s_fld = s_invr + KS;
+    double* s_eps = s_fld + KS;
+    u32* s_disp = reinterpret_cast<u32*>(s_eps + p.N);
+    u32* s_guide = s_disp + KS;
+    u32* s_n = s_guide + CG_GUIDE;
+    __shared__ u64 s_key[3];
+    const Tables tb = {s_cdfi, s_invr, s_fld, s_disp, s_guide, p.cdfi, p.invr_k, p.fld_k, p.disp, (u32)KS};
+    const Geo geo = {p.hi1, p.hi2, p.spare, p.mask, (u32)(p.L - 1), p.lgL};
+    const int tid = threadIdx.x, lane = tid & 31;
+    const u32 N = p.N, M = p.M, mask = p.mask, P = ST;
+    const double* __restrict__ tf = p.tf;
+    CgCtl* const ctl = p.ctl;
+    double* const g_eps = p.eps[ctl->cur];
+
+    for (int k = tid; k < KS; k += ST) {
+        s_cdfi[k] = p.cdfi[k]; s_invr[k] = p.invr_k[k]; s_fld[k] = p.fld_k[k]; s_disp[k] = p.disp[k];
+    }
+    for (int k = tid; k < CG_GUIDE; k += ST) s_guide[k] = p.guide[k];
+    for (u32 w = tid; w < (N + 31) / 32; w += ST) s_n[w] = p.nbits[w];
+    for (u32 k = tid; k < N; k += ST) s_eps[k] = __ldcg(g_eps + k);
+    if (tid < 3) s_key[tid] = ~0ull;
+    const u64 a_start = ctl->attempts, hops_start = ctl->hops, log_base = ctl->log_base;
+    const u32 n_hops = p.n_hops;
+    __syncthreads();
+
+    const u32 g0 = (u32)(a_start % P);
+    u32 lab = ((u32)tid - g0) & (P - 1u);          // label of slot 0; slot j holds label lab + j P
+    u64 a_cur = a_start + lab;
+    u32 cci[KL], ccj[KL], cuh[KL], cul[KL], ck[KL];
+#pragma unroll
+    for (int j = 0; j < KL; ++j) {
+        const Prop q = decode_attempt(tb, p, geo, a_cur + (u64)j * P);
+        cci[j] = q.ci; ccj[j] = q.cj; cuh[j] = q.uh; cul[j] = q.ul; ck[j] = q.k;
+    }
+    u32 hc = 0, k3 = 0;
+    u64 its = 0, used_sum = 0;
+    long long dP = 0;
+    while (hc < n_hops) {
+        // ---- steps 1-2 for my KL labels, step 3: lowest accepting label
+        u64 best = ~0ull;
+#pragma unroll
+        for (int j = 0; j < KL; ++j) {
+            const u32 labj = lab + (u32)j * P;
+            if (labj < M) {
+                const u32 si = geo.site(cci[j]), sj = geo.site(ccj[j]);
+                if (BIT(s_n, si) && !BIT(s_n, sj)) {
+                    const double dE = __dsub_rn(__dsub_rn(__dsub_rn(s_eps[sj], s_eps[si]), tb.inv(ck[j])), tb.field(ck[j]));
+                    if (metropolis(dE, cuh[j], cul[j], p.T, p.inv_T))
+                        best = min(best, ((u64)labj << 42) | ((u64)cci[j] << 21) | (u64)ccj[j]);
+                }
+            }
+        }
+        const u32 blab = (u32)(best >> 42);            // 0x3FFFFF when nothing accepted
+        const u32 wmin = __reduce_min_sync(CG_FULL, blab);
+        const u32 k3n = k3 == 2u ? 0u : k3 + 1u;
+        if (best != ~0ull && blab == wmin) atomicMin(&s_key[k3], best);
+        if (tid == 0) s_key[k3n] = ~0ull;
+        __syncthreads();
+        const u64 key = s_key[k3];
+        k3 = k3n;
+        const bool hop = key != ~0ull;
+        const u32 used = hop ? (u32)(key >> 42) + 1u : M;
+        if (hop) {
+            const u32 wci = (u32)(key >> 21) & 0x1FFFFFu, wcj = (u32)key & 0x1FFFFFu;
+            // step 3b: eps_l += 1/r_lj - 1/r_li, difference first, then ONE add.  (The folded table in shared
+            // memory instead of the unfolded one through L1/L2 was measured slower, 22.1 M against 24.2 M hops/s for 148 sims of
+            // L = 128: the update is bound by its instruction count, 16384 sites on one SM, not by the table traffic.)
+            for (u32 l = tid; l < N; l += ST)
+                s_eps[l] = __dadd_rn(s_eps[l], hop_term(tf, mask, geo.code(l) | geo.spare, wci, wcj));
+            ++hc;
+            if (tid == ST - 1) {
+                const u32 hi_ = geo.site(wci), hj_ = geo.site(wcj);
+                s_n[hi_ >> 5] &= ~(1u << (hi_ & 31));
+                s_n[hj_ >> 5] |= 1u << (hj_ & 31);
+                dP += geo.dx(hi_, hj_);
+                const u64 h = hops_start + hc - 1u - log_base;
+                if (h < p.log_cap) { p.log_a[h] = a_start + used_sum + used - 1; p.log_i[h] = hi_; p.log_j[h] = hj_; }
+            }
+        }
+        used_sum += used;
+        ++its;
+        if (lab >= used) lab -= used;
+        else {
+            // slots whose labels are consumed: lab + j P < used, j < c; the others move down, new ones are decoded at the top
+            const u32 c = (used - lab + P - 1u) / P;      // 1 <= c <= KL
+            for (u32 r = 0; r < c; ++r) {
+#pragma unroll
+                for (int j = 0; j + 1 < KL; ++j) { cci[j] = cci[j + 1]; ccj[j] = ccj[j + 1]; cuh[j] = cuh[j + 1]; cul[j] = cul[j + 1]; ck[j] = ck[j + 1]; }
+                const Prop q = decode_attempt(tb, p, geo, a_cur + (u64)(KL + r) * P);
+                cci[KL - 1] = q.ci; ccj[KL - 1] = q.cj; cuh[KL - 1] = q.uh; cul[KL - 1] = q.ul; ck[KL - 1] = q.k;
+            }
+            lab += c * P - used; a_cur += (u64)c * P;
+        }
+        __syncthreads();
+    }
+    for (u32 k = tid; k < N; k += ST) __stcg(g_eps + k, s_eps[k]);
+    for (u32 w = tid; w < (N + 31) / 32; w += ST) p.nbits[w] = s_n[w];
+    if (tid == ST - 1) {
+        ctl->attempts = a_start + used_sum; ctl->hops = hops_start + hc;
+        ctl->iterations += its; ctl->proposals += (u64)M * its;
+        ctl->dP += dP; ctl->epoch += its;
+    }
+}
+
+template <int KL>
+__global__ void __launch_bounds__(CG_ST, 1) cg_pr_singlek(const CgParams p) { pr_singlek_body<KL>(p); }
+template <int KL>
+__global__ void __launch_bounds__(CG_ST, 1) cg_pr_singlek_many(const CgParams* __restrict__ ps)
+{
+    __shared__ CgParams sp;
+    if (threadIdx.x == 0) sp = ps[blockIdx.x];
+    __syncthreads();
+    pr_singlek_body<KL>(sp);
+}
+
 __device__ __forceinline__ Geo make_geo(const CgParams& p)
 {
     const Geo g = {p.hi1, p.hi2, p.spare, p.mask, (u32)(p.L - 1), p.lgL};
@@ -2128,7 +2259,22 @@ static int choose_launch(cg_sim* s, int n_ctas, int threads)
         const bool asked = threads == CG_ST && n_ctas <= 1;
         const bool asked2 = threads == 2 * CG_ST && n_ctas == 1 && fits && st == 2 * CG_ST;
         const bool automatic = threads == 0 && n_ctas == 0 && s->cluster_pref == 0 && s->N <= 2 * CG_ST && s->M <= 2 * CG_ST;
-        if (asked && (!fits || st != CG_ST)) return CG_EINVAL;
+        if (asked && (st != CG_ST || s->N > CG_SINGLE_MAX_N)) {
+            // more than 512 labels on 512 threads: the variant with 2, 4 or 8 labels per thread (lattices up to N = 16384 on one SM)
+            const int kl = s->M <= 2 * CG_ST ? 2 : s->M <= 4 * CG_ST ? 4 : 8;
+            const int smem = (int)(smem_base_bytes(s) + 8 * (size_t)s->N + 16);
+            if (s->M > 8 * CG_ST || s->N > CG_SK_MAX_N || (size_t)smem + 4 * 1024 > (size_t)s->smem_optin) return CG_EINVAL;
+            CK(cudaFuncSetAttribute((const void*)cg_pr_singlek<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+            CK(cudaFuncSetAttribute((const void*)cg_pr_singlek<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+            CK(cudaFuncSetAttribute((const void*)cg_pr_singlek<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+            CK(cudaFuncSetAttribute((const void*)cg_pr_singlek_many<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+            CK(cudaFuncSetAttribute((const void*)cg_pr_singlek_many<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+            CK(cudaFuncSetAttribute((const void*)cg_pr_singlek_many<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+            s->single = true; s->n_ctas = 1; s->threads = CG_ST; s->rp = 0; s->pl = CG_ST; s->lpt = kl; s->smem = smem;
+            s->cluster = 1;
+            return CG_OK;
+        }
+        if (asked && !fits) return CG_EINVAL;
         if (fits && (asked || asked2 || automatic)) {
             const int smem = (int)smem_single_bytes(s);
             CK(cudaFuncSetAttribute((const void*)cg_pr_single<CG_ST>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
@@ -2324,7 +2470,10 @@ extern "C" int cg_run(cg_sim* s, uint64_t n_hops)
         while (n_hops) {
             const u32 chunk = (u32)std::min<uint64_t>(n_hops, CG_MAX_LAUNCH_HOPS);
             const CgParams p = make_params(s, chunk);
-            if (s->threads == CG_ST) cg_pr_single<CG_ST><<<1, CG_ST, (size_t)s->smem, s->stream>>>(p);
+            if (s->lpt == 2) cg_pr_singlek<2><<<1, CG_ST, (size_t)s->smem, s->stream>>>(p);
+            else if (s->lpt == 4) cg_pr_singlek<4><<<1, CG_ST, (size_t)s->smem, s->stream>>>(p);
+            else if (s->lpt == 8) cg_pr_singlek<8><<<1, CG_ST, (size_t)s->smem, s->stream>>>(p);
+            else if (s->threads == CG_ST) cg_pr_single<CG_ST><<<1, CG_ST, (size_t)s->smem, s->stream>>>(p);
             else cg_pr_single<2 * CG_ST><<<1, 2 * CG_ST, (size_t)s->smem, s->stream>>>(p);
             CK(cudaGetLastError());
             n_hops -= chunk;
@@ -2357,7 +2506,7 @@ extern "C" int cg_run_many(cg_sim* const* sims, int n_sims, uint64_t n_hops)
         if (!s) return CG_EINVAL;
         for (int m = 0; m < k; ++m) if (sims[m] == s) return CG_EINVAL;       // a sim may appear once
         if (s->device != s0->device || s->stream != s0->stream || s->threads != s0->threads || s->rp != s0->rp
-            || (s->pl > 0 && s->lpt == 1) != (s0->pl > 0 && s0->lpt == 1) || s->single != s0->single) {
+            || (s->pl > 0 && s->lpt == 1) != (s0->pl > 0 && s0->lpt == 1) || s->single != s0->single || (s->single && s->lpt != s0->lpt)) {
             s0->err = "cg_run_many: the sims must share device, stream and launch shape (threads, register tiling, "
                       "cached labels)";
             return CG_EINVAL;
@@ -2372,6 +2521,9 @@ extern "C" int cg_run_many(cg_sim* const* sims, int n_sims, uint64_t n_hops)
     if (single) {
         CK0(s0, cudaFuncSetAttribute((const void*)cg_pr_single_many<CG_ST>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
         CK0(s0, cudaFuncSetAttribute((const void*)cg_pr_single_many<2 * CG_ST>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+        CK0(s0, cudaFuncSetAttribute((const void*)cg_pr_singlek_many<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+        CK0(s0, cudaFuncSetAttribute((const void*)cg_pr_singlek_many<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+        CK0(s0, cudaFuncSetAttribute((const void*)cg_pr_singlek_many<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
     } else {
         CK0(s0, cudaFuncSetAttribute((const void*)f, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
         int per_sm = 0;
@@ -2401,7 +2553,10 @@ extern "C" int cg_run_many(cg_sim* const* sims, int n_sims, uint64_t n_hops)
         u32 n = (u32)n_sims;
         void* args[] = {&d_ps, &d_first, &n};
         if (single) {
-            if (s0->threads == CG_ST) cg_pr_single_many<CG_ST><<<(unsigned)n_sims, CG_ST, (size_t)smem, s0->stream>>>(d_ps);
+            if (s0->lpt == 2) cg_pr_singlek_many<2><<<(unsigned)n_sims, CG_ST, (size_t)smem, s0->stream>>>(d_ps);
+            else if (s0->lpt == 4) cg_pr_singlek_many<4><<<(unsigned)n_sims, CG_ST, (size_t)smem, s0->stream>>>(d_ps);
+            else if (s0->lpt == 8) cg_pr_singlek_many<8><<<(unsigned)n_sims, CG_ST, (size_t)smem, s0->stream>>>(d_ps);
+            else if (s0->threads == CG_ST) cg_pr_single_many<CG_ST><<<(unsigned)n_sims, CG_ST, (size_t)smem, s0->stream>>>(d_ps);
             else cg_pr_single_many<2 * CG_ST><<<(unsigned)n_sims, 2 * CG_ST, (size_t)smem, s0->stream>>>(d_ps);
             CK0(s0, cudaGetLastError());
         } else

@@ -310,6 +310,7 @@ def report_replicas(hops):
     packed("cfg1_L16", [0], sms)
     packed("cfg2_L64", [0], sms // 5, n_ctas=5)
     packed("cfg2_L64", [0], sms, n_ctas=1, threads=1024)        # config 2 on ONE SM each: the single-CTA kernel
+    packed("cfg3_L128", [0, 1, 2, 3], sms // 4, n_ctas=1, threads=512)   # config 3 (its four temperatures) on ONE SM each: 8 labels per thread
     run("cfg3_L128", [0, 1, 2, 3], 1)     # the temperature sweep of config 3 as one replica set
     run("cfg3_L128", [0, 1, 2, 3], 2)
     run("cfg1_L16", [0], 1)

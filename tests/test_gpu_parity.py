@@ -297,12 +297,38 @@ def test_single_cta_kernel_with_1024_threads(cg, oracle_lib, kw, shape, hops):
     assert g.recompute_eps() < 1e-9
 
 
+@pytest.mark.parametrize("kw,K,hops", [
+    (dict(L=128, T=0.2, E=0.01, seed=3, M=4096), 8, 4000),               # config 3 on ONE SM (replica packing)
+    (dict(L=128, T=0.03, E=0.01, seed=6, M=4096), 8, 3000),
+    (dict(L=64, T=0.05, E=0.0, seed=2, M=2000), 4, 6000),                # ragged M: labels beyond M are not tested
+    (dict(L=64, T=0.05, E=0.0, seed=2, M=1024), 2, 6000),
+    (dict(L=16, T=0.01, E=0.0, seed=6, M=4096), 8, 300),                 # cold: whole windows rejected, all 8 slots consumed at once
+    (dict(L=16, dim=3, T=0.05, E=0.01, seed=13, M=3000), 8, 4000),
+    (dict(L=128, T=0.1, E=0.01, seed=4, M=256), 2, 3000),                # few labels, eps beyond the 64 KiB of the one-label kernel
+])
+def test_single_cta_kernel_with_several_labels_per_thread(cg, oracle_lib, kw, K, hops):
+    """(1 CTA, 512 threads) for M > 512 or N > 8192: cg_pr_singlek, K = 2, 4 or 8 labels per thread in registers, the lowest
+    accepting label and its sites in one 64-bit shared atomicMin.  Must be the serial chain; split runs re-decode the slots."""
+    g = cg.CoulombGlass(hop_log=hops, **kw)
+    g.set_launch(1, 512)
+    assert g.kernel() == "single" and g.launch()["threads"] == 512 and g.labels_per_thread() == K
+    g.run(hops // 3)
+    g.run(hops - hops // 3)
+    o = oracle_lib.Oracle(**kw)
+    o.run(hops)
+    _compare(g, o, hops)
+    c = g.counters()
+    assert c["proposals_evaluated"] == kw["M"] * c["iterations"]
+    assert g.recompute_eps() < 1e-9
+
+
 def test_single_cta_kernel_refuses_what_does_not_fit(cg):
     g = cg.CoulombGlass(L=16, T=0.1, M=4096)
-    assert g.launch()["threads"] == 544 and g.kernel() == "dataflow"      # M beyond 1024 labels: the dataflow kernel
+    assert g.launch()["threads"] == 544 and g.kernel() == "dataflow"      # M beyond 1024 labels: the dataflow kernel by default
+    g = cg.CoulombGlass(L=16, T=0.1, M=4097)
     with pytest.raises(cg.CgError):
-        g.set_launch(1, 512)
-    g = cg.CoulombGlass(L=128, T=0.1, M=256)
+        g.set_launch(1, 512)                           # more than 8 labels per thread
+    g = cg.CoulombGlass(L=256, T=0.1, M=256)
     with pytest.raises(cg.CgError):
         g.set_launch(1, 512)                           # eps does not fit shared memory
 
