@@ -178,9 +178,19 @@ def report_soak():
         ("cfg2_L64", 0, 6_000_000, [dict(), dict(shape=(1, 1024)), dict(shape=(5, 544), tuning=(8, 1), chunks=3)]),
         ("cfg1_L16", 0, 10_000_000, [dict(), dict(shape=(1, 544), tuning=(2, 1)), dict(shape=(3, 256), chunks=4)]),
     ]
+    # the single-CTA kernels (512 and 1024 threads, 2/4/8 labels per thread) against the dataflow kernel, 2D and 3D, hot and cold
+    extra = [
+        ("L=32 M=1024", dict(L=32, T=0.08, E=0.01, seed=5, M=1024), 4_000_000, [dict(), dict(shape=(3, 544), tuning=(2, 1))]),
+        ("L=64 M=2000", dict(L=64, T=0.05, E=0.01, seed=2, M=2000), 2_000_000, [dict(shape=(1, 512)), dict(shape=(5, 544))]),
+        ("L=128 M=4096", dict(L=128, T=0.05, E=0.01, seed=5, M=4096), 1_000_000, [dict(shape=(1, 512)), dict(), dict(shape=(19, 544), tuning=(4, 1))]),
+        ("3D L=8 M=256", dict(L=8, dim=3, T=0.1, E=0.01, seed=8, M=256), 4_000_000, [dict(), dict(shape=(2, 544))]),
+        ("3D L=16 M=3000", dict(L=16, dim=3, T=0.05, E=0.01, seed=13, M=3000), 1_000_000, [dict(shape=(1, 512)), dict()]),
+        ("cold L=16 M=4096", dict(L=16, T=0.01, E=0.0, seed=6, M=4096), 20_000, [dict(shape=(1, 512)), dict(), dict(shape=(2, 544))]),
+    ]
     print("# %s: soak - every line below the reference must say identical: True" % torch.cuda.get_device_name(0))
-    for name, idx, hops, variants in cases:
-        kw = workloads.init_args(workloads.CONFIGS[name][idx], sms * 2048)
+    for name, idx, hops, variants in cases + [(n, k, h, v) for n, k, h, v in extra]:
+        kw = idx if isinstance(idx, dict) else workloads.init_args(workloads.CONFIGS[name][idx], sms * 2048)
+        idx = 0 if isinstance(idx, dict) else idx
         ref = None
         for v in variants:
             r = run(kw, hops, **v)
