@@ -27,6 +27,9 @@
 //     readers replay the newest hops), next to the head of the tower (PAPER.md:71,
 //     80) and its guide table; 1/r comes from an unfolded table in L2 indexed with
 //     one subtraction and one mask (2D and 3D lattices share the code).
+//   * a sim that fits ONE CTA (M <= 1024 labels, or up to 8 labels per thread on request; N <= 16384 sites)
+//     runs in a kernel of its own (cg_pr_single, cg_pr_singlek): every thread a worker, eps, occupations and
+//     the tower in shared memory, two CTA barriers per iteration; cg_run_many packs such sims one per SM.
 // Nothing in this file is shared with oracle/ (the CPU reference).
 #include "cg.h"
 
